@@ -1,0 +1,149 @@
+/*
+ * fkconv.h -- C-ABI boundary of the B200-native Fast-Kernel (FK) table convolution.
+ *
+ * What the library computes (P:NN = /root/reference/PAPER.md line NN):
+ *
+ *   hadronic   sigma[n][r] = sum_{c,i,j} f[r][a_c][i] * f[r][b_c][j] * FK[n][i][j][c]        Eq. (1)
+ *              over a sparse list of C active ordered flavour pairs (a_c, b_c)  ("49 flavour
+ *              combinations"); f = PDF values on the x-grid; R replicas = R columns of
+ *              the "PDF matrix" (Table 3).
+ *   DIS        sigma[n][r] = sum_{c,i} f[r][flav_c][i] * FK[n][i][c]      (DIS rows of Table 1, P:51-56;
+ *              formula from BASELINE.json north_star, reading R1)
+ *   gradient   "the convolution and its corresponding gradient", as a vector-Jacobian product:
+ *              df[r][alpha][i] = d( sum_n g[n][r] * sigma[n][r] ) / d f[r][alpha][i]          (reading R8)
+ *
+ * The luminosity L[k][r] = f[r][a_c][i] * f[r][b_c][j] is built on the fly inside the kernels and is
+ * never written to HBM.  Every result is bitwise reproducible run to run (fixed reduction trees, no
+ * floating-point atomics).
+ *
+ * Conventions
+ *  - plain C, no exceptions cross the boundary; every call returns an fk_status (0 = FK_OK) and
+ *    fk_last_error_string() gives the detail for the calling thread.
+ *  - "dev" pointers are CUDA device pointers owned by the caller (8-byte aligned; 16-byte aligned
+ *    rows are streamed with 128-bit loads, anything else takes the 64-bit path); "host" pointers are
+ *    ordinary host memory, read before the call returns.  Index lists are tiny and live on the host.
+ *  - outputs are overwritten, never accumulated into.
+ *  - every compute call is asynchronous on `stream` (a cudaStream_t passed as void*, NULL = the
+ *    legacy default stream) and never synchronises the device; the *_host variants copy through
+ *    pinned staging owned by the table and DO wait for the result before returning.
+ *  - logical layouts (BASELINE.json): hadronic FK[N][nx][nx][C] (i, j, channel; channel innermost),
+ *    DIS FK[N][nx][nA], pairs[C][2] = (a_c, b_c) with i <-> a_c and j <-> b_c, flav[nA],
+ *    f[R][nfl][nx], sigma[N][R], g[N][R], df[R][nfl][nx].
+ *  - limits: 1 <= nfl <= 256, 1 <= C (or nA) <= 1024, N*K < 2^62, R >= 1.  Outside: FK_ERR_UNSUPPORTED.
+ *  - there is no CPU fallback: without a CUDA device every compute call returns FK_ERR_CUDA.
+ */
+#ifndef FKCONV_H
+#define FKCONV_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum fk_status {
+    FK_OK = 0,
+    FK_ERR_INVALID_ARG = -1, /* null pointer, non-positive size, flavour index out of [0,nfl) */
+    FK_ERR_ALLOC = -2,       /* device or host allocation failed */
+    FK_ERR_CUDA = -3,        /* a CUDA runtime call or kernel launch failed */
+    FK_ERR_UNSUPPORTED = -4  /* sizes outside the limits above */
+} fk_status;
+
+enum { FK_KIND_DIS = 0, FK_KIND_HADRONIC = 1 };
+enum { FK_F64 = 0, FK_F32 = 1 };
+/* table storage: BORROW keeps the caller's logical-layout buffer (no copy; it must outlive the
+ * table); PACK copies into the library's device layout: channel-major, x innermost
+ * ([N][C][nx][nx] resp. [N][nA][nx]), each datapoint row padded to a multiple of 16 bytes. */
+enum { FK_STORE_BORROW = 0, FK_STORE_PACK = 1 };
+
+typedef struct fk_table fk_table; /* opaque: one FK table resident in HBM + its scratch */
+typedef struct fk_group fk_group; /* opaque: a ragged set of tables with a static work list */
+
+/* Thread-local description of the last failure of this thread ("" if none). Never NULL. */
+const char* fk_last_error_string(void);
+/* Library version, and the compute capability it was compiled for (100 = sm_100a). */
+int fk_version(void);
+int fk_compiled_arch(void);
+
+/* Kernel timing hook for bench.py's roofline: while enabled, every forward call brackets its
+ * dominant kernel (the streaming contraction, or the dense contraction for large R) with a CUDA event
+ * pair on the caller's stream.  fk_profile_read waits for those events, returns the mean kernel
+ * duration in milliseconds and the number of launches timed since the last read, and clears them. */
+int fk_profile_enable(int on);
+int fk_profile_read(double* mean_kernel_ms, int* launches);
+
+/* ------------------------------------------------------------------ stateless entry points (fp64)
+ * Eq. (1) P:43 / DIS / VJP on the caller's logical-layout device buffers.  Level-1 partials live in
+ * stream-ordered scratch (cudaMallocAsync on `stream`).
+ *   fk     dev   [N][nx][nx][C]  (DIS: [N][nx][nA])
+ *   pairs  host  [C][2] int32    (DIS: flav host [nA] int32)
+ *   f      dev   [R][nfl][nx]
+ *   sigma  dev   [N][R]          (written)
+ *   g      dev   [N][R]
+ *   df     dev   [R][nfl][nx]    (written; exactly 0 for flavours in no pair)
+ */
+int fk_conv_dis(const double* fk, const int32_t* flav, const double* f, double* sigma,
+                int N, int nx, int nfl, int nA, int R, void* stream);
+int fk_conv_hadronic(const double* fk, const int32_t* pairs, const double* f, double* sigma,
+                     int N, int nx, int nfl, int C, int R, void* stream);
+int fk_conv_hadronic_vjp(const double* fk, const int32_t* pairs, const double* f, const double* g,
+                         double* df, int N, int nx, int nfl, int C, int R, void* stream);
+int fk_conv_dis_vjp(const double* fk, const int32_t* flav, const double* f, const double* g,
+                    double* df, int N, int nx, int nfl, int nA, int R, void* stream);
+
+/* fp32 variant (reading R18): float storage and float FMA with short chains, the
+ * cross-thread stages in double, float results.  Same argument meaning as above. */
+int fk_conv_dis_f32(const float* fk, const int32_t* flav, const float* f, float* sigma,
+                    int N, int nx, int nfl, int nA, int R, void* stream);
+int fk_conv_hadronic_f32(const float* fk, const int32_t* pairs, const float* f, float* sigma,
+                         int N, int nx, int nfl, int C, int R, void* stream);
+int fk_conv_hadronic_vjp_f32(const float* fk, const int32_t* pairs, const float* f, const float* g,
+                             float* df, int N, int nx, int nfl, int C, int R, void* stream);
+
+/* ------------------------------------------------------------------ resident-table path
+ * What a fit uses: thousands of iterations over fixed tables, tables loaded once.
+ * fk_table_create validates the index list, (store==PACK) repacks and (dtype==FK_F32) demotes the
+ * logical fp64 table `fk_logical` (dev) with round-to-nearest, and pre-allocates scratch for up to
+ * `R_hint` replicas (grown on demand by later calls, which then allocate once, outside any graph).
+ * kind: FK_KIND_*; C = number of pairs (hadronic) or active flavours (DIS).
+ * fk_table_create synchronises `stream` work it issues before returning (one-time, untimed). */
+int fk_table_create(fk_table** out, int kind, const double* fk_logical, const int32_t* index_list,
+                    int N, int nx, int nfl, int C, int dtype, int store, int R_hint);
+int fk_table_destroy(fk_table* t);
+/* N, nx, nfl, C, K (= C*nx*nx or nA*nx), row stride in elements, device bytes held by the table. */
+int fk_table_info(const fk_table* t, int* N, int* nx, int* nfl, int* C, int64_t* K,
+                  int64_t* row_stride, int64_t* device_bytes);
+/* f, sigma, g, df: dev, in the table's dtype (double for FK_F64, float for FK_F32). */
+int fk_table_conv(fk_table* t, const void* f, void* sigma, int R, void* stream);
+int fk_table_vjp(fk_table* t, const void* f, const void* g, void* df, int R, void* stream);
+/* Same with HOST buffers: H2D of f (and g) and D2H of the result run inside the call, through
+ * pinned staging, on `stream`; the call returns after the result has landed in host memory. */
+int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R, void* stream);
+int fk_table_vjp_host(fk_table* t, const void* f_host, const void* g_host, void* df_host, int R,
+                      void* stream);
+/* Kernel launches issued by the last conv / vjp call on this table (for bench.py's gpu_launches). */
+int fk_table_last_launches(const fk_table* t);
+
+/* ------------------------------------------------------------------ grouped ragged launch
+ * A global fit convolves many tables of different (N, nx, C) every iteration.
+ * fk_group_create builds a static work list over the T tables (all of one dtype); each forward or
+ * VJP pass is then ONE persistent launch per stage over all tables.
+ *   f_cat      dev  concatenation over t of f_t[R][nfl_t][nx_t]   (offsets: fk_group_offsets)
+ *   sigma_cat  dev  concatenation over t of sigma_t[N_t][R]
+ *   g_cat      dev  concatenation over t of g_t[N_t][R]
+ *   df_cat     dev  concatenation over t of df_t[R][nfl_t][nx_t]  (per table, reading R14)
+ * The tables must outlive the group. */
+int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint);
+int fk_group_destroy(fk_group* g);
+/* element offsets (for R replicas) of table t inside f_cat/df_cat and sigma_cat/g_cat; arrays of
+ * T+1 int64 written to host memory (entry T = total length). */
+int fk_group_offsets(const fk_group* g, int R, int64_t* f_offsets, int64_t* sigma_offsets);
+int fk_conv_grouped(fk_group* g, const void* f_cat, void* sigma_cat, int R, void* stream);
+int fk_conv_grouped_vjp(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat, int R,
+                        void* stream);
+int fk_group_last_launches(const fk_group* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FKCONV_H */

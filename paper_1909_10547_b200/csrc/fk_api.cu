@@ -1,0 +1,685 @@
+// fk_api.cu -- the C-ABI of include/fkconv.h: argument validation, table / group handles, launch plans.
+// Host logic only; every step of the path runs in the kernels of fk_stream.cuh / fk_vjp.cuh /
+// fk_gemm.cuh.  There is no CPU fallback anywhere in this file.
+#include "../../include/fkconv.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "fk_common.cuh"
+#include "fk_gemm.cuh"
+#include "fk_pack.cuh"
+#include "fk_stream.cuh"
+#include "fk_vjp.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define FK_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? FK_ERR_ALLOC : FK_ERR_CUDA, "%s: %s",    \
+                        #call, cudaGetErrorString(e_));                                            \
+    } while (0)
+
+int env_int(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+int sm_count() {
+    static std::mutex mu;
+    static std::map<int, int> cache;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    std::lock_guard<std::mutex> lk(mu);
+    auto it = cache.find(dev);
+    if (it != cache.end()) return it->second;
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 0;
+    cache[dev] = n;
+    return n;
+}
+
+// resident CTAs per SM of a kernel instantiation (cached)
+int ctas_per_sm(const void* func, int threads, size_t smem) {
+    static std::mutex mu;
+    static std::map<std::pair<const void*, size_t>, int> cache;
+    std::lock_guard<std::mutex> lk(mu);
+    auto key = std::make_pair(func, smem);
+    auto it = cache.find(key);
+    if (it != cache.end()) return it->second;
+    if (smem > 48 * 1024) cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, func, threads, smem) != cudaSuccess || n < 1) n = 1;
+    cache[key] = n;
+    return n;
+}
+
+// ---- kernel timing hook (fk_profile_enable / fk_profile_read) ----
+struct Profiler {
+    std::mutex mu;
+    bool on = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> pairs;
+    size_t used = 0;
+    bool begin(cudaStream_t s, size_t& slot) {
+        std::lock_guard<std::mutex> lk(mu);
+        if (!on) return false;
+        if (used == pairs.size()) {
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return false;
+            pairs.emplace_back(a, b);
+        }
+        slot = used++;
+        cudaEventRecord(pairs[slot].first, s);
+        return true;
+    }
+    void end(cudaStream_t s, size_t slot) {
+        std::lock_guard<std::mutex> lk(mu);
+        cudaEventRecord(pairs[slot].second, s);
+    }
+} g_prof;
+
+template <typename T> constexpr int dtype_of();
+template <> constexpr int dtype_of<double>() { return FK_F64; }
+template <> constexpr int dtype_of<float>() { return FK_F32; }
+size_t dtype_size(int dtype) { return dtype == FK_F64 ? 8 : 4; }
+
+// ------------------------------------------------------------------------------------------------
+// plans
+// ------------------------------------------------------------------------------------------------
+struct Plan {
+    int kc = 0;       // forward stream: chunk length (elements)
+    int nchunks = 0;  // forward stream: chunks per row
+    int nsplit = 0;   // VJP stage 1: datapoint splits
+    int nkb = 0;      // VJP stage 1: k-blocks
+    int gsplit = 0;   // forward GEMM: K-splits
+};
+
+constexpr int STREAM_UNROLL = 4;
+
+template <typename T> int stream_chunk_unit(int vec) { return 32 * vec * STREAM_UNROLL; }
+
+void make_plan(fk::TableDesc& d, int dtype, Plan& pl) {
+    const int vecw = dtype == FK_F64 ? 2 : 4;
+    const int unit = 32 * vecw * STREAM_UNROLL;  // also valid for the VEC = 1 path (multiple of 32*UNROLL)
+    int kc_default = env_int("FKCONV_KC", dtype == FK_F64 ? 1024 : 2048);
+    kc_default = std::max(unit, kc_default / unit * unit);
+    const int kround = (d.K + unit - 1) / unit * unit;
+    pl.kc = std::min(kc_default, kround);
+    pl.nchunks = (d.K + pl.kc - 1) / pl.kc;
+    d.nchunks = pl.nchunks;
+    d.kc = pl.kc;
+
+    const int vec = d.vec_ok ? vecw : 1;
+    pl.nkb = (d.K + fk::COLSUM_THREADS * vec - 1) / (fk::COLSUM_THREADS * vec);
+    const int sms = std::max(1, sm_count());
+    const int want = env_int("FKCONV_COLSUM_CTAS_PER_SM", 24) * sms;  // CTAs wanted for stage 1
+    int nsplit = (want + pl.nkb - 1) / pl.nkb;
+    nsplit = std::min(nsplit, std::max(1, d.N / 16));                  // >= 16 datapoints per split
+    nsplit = std::max(nsplit, (d.N + fk::COLSUM_MAX_ROWS - 1) / fk::COLSUM_MAX_ROWS);
+    nsplit = std::max(1, std::min(nsplit, d.N));
+    pl.nsplit = nsplit;
+    d.nsplit = nsplit;
+}
+
+size_t part_elems_per_replica(const fk::TableDesc& d) { return d.nchunks > 1 ? (size_t)d.N * d.nchunks : 0; }
+size_t G_elems_per_replica(const fk::TableDesc& d) { return (size_t)d.nsplit * d.K; }
+
+// ------------------------------------------------------------------------------------------------
+// validation
+// ------------------------------------------------------------------------------------------------
+int check_dims(const char* who, int kind, int N, int nx, int nfl, int C, int R) {
+    if (N <= 0 || nx <= 0 || nfl <= 0 || C <= 0 || R <= 0)
+        return fail(FK_ERR_INVALID_ARG, "%s: non-positive size (N=%d nx=%d nfl=%d C=%d R=%d)", who, N, nx, nfl, C, R);
+    if (nfl > fk::MAX_NFL || C > fk::MAX_C)
+        return fail(FK_ERR_UNSUPPORTED, "%s: nfl=%d > %d or C=%d > %d", who, nfl, fk::MAX_NFL, C, fk::MAX_C);
+    const long long K = kind == FK_KIND_HADRONIC ? (long long)C * nx * nx : (long long)C * nx;
+    if (K >= (1LL << 31) - 4096) return fail(FK_ERR_UNSUPPORTED, "%s: K=%lld does not fit 31 bits", who, K);
+    if ((long long)nfl * nx >= (1LL << 24)) return fail(FK_ERR_UNSUPPORTED, "%s: nfl*nx too large", who);
+    if (kind == FK_KIND_DIS && C > nfl)
+        return fail(FK_ERR_INVALID_ARG, "%s: nA=%d > nfl=%d", who, C, nfl);
+    return FK_OK;
+}
+
+int fill_channels(const char* who, int kind, const int32_t* idx, int nfl, int C, fk::ChannelList& ch) {
+    memset(&ch, 0, sizeof ch);
+    for (int c = 0; c < C; ++c) {
+        const int a = kind == FK_KIND_HADRONIC ? idx[2 * c] : idx[c];
+        const int b = kind == FK_KIND_HADRONIC ? idx[2 * c + 1] : 0;
+        if (a < 0 || a >= nfl || b < 0 || b >= nfl)
+            return fail(FK_ERR_INVALID_ARG, "%s: flavour index out of [0,%d) at channel %d: (%d,%d)", who, nfl, c, a, b);
+        ch.a[c] = (uint8_t)a;
+        ch.b[c] = (uint8_t)b;
+    }
+    return FK_OK;
+}
+
+fk::TableDesc make_desc(int kind, int layout, const void* fkp, int N, int nx, int nfl, int C, long long row_stride,
+                        int dtype) {
+    fk::TableDesc d;
+    memset(&d, 0, sizeof d);
+    d.fk = fkp;
+    d.K = kind == FK_KIND_HADRONIC ? C * nx * nx : C * nx;
+    d.row_stride = row_stride > 0 ? row_stride : d.K;
+    d.N = N; d.nx = nx; d.nfl = nfl; d.C = C;
+    d.kind = kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS;
+    d.layout = layout;
+    const int vecw = dtype == FK_F64 ? 2 : 4;
+    d.vec_ok = ((uintptr_t)fkp % 16 == 0) && (d.row_stride % vecw == 0);
+    return d;
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+template <int RT> struct StreamShape;  // rows per warp, by replica tile
+template <> struct StreamShape<1> { static constexpr int RPW = 2; };
+template <> struct StreamShape<2> { static constexpr int RPW = 2; };
+template <> struct StreamShape<4> { static constexpr int RPW = 1; };
+
+template <typename T, int VEC, int RT, bool GROUPED>
+const void* stream_func() {
+    return (const void*)fk::fk_stream_kernel<T, VEC, RT, StreamShape<RT>::RPW, STREAM_UNROLL, GROUPED>;
+}
+
+template <typename T, int VEC, int RT, bool GROUPED>
+int stream_grid_for(int kc, long long units) {
+    const size_t smem = (size_t)RT * kc * sizeof(T);
+    const int occ = ctas_per_sm(stream_func<T, VEC, RT, GROUPED>(), fk::STREAM_THREADS, smem);
+    const int cap = env_int("FKCONV_STREAM_CTAS_PER_SM", 0);
+    const int per_sm = cap > 0 ? std::min(cap, occ) : occ;
+    const long long by_work = (units + 8 * StreamShape<RT>::RPW - 1) / (8 * StreamShape<RT>::RPW);
+    return (int)std::max(1LL, std::min<long long>((long long)sm_count() * per_sm, by_work));
+}
+
+template <typename T, int VEC, int RT, bool GROUPED>
+cudaError_t launch_stream(const fk::StreamParams& p, int grid, cudaStream_t s) {
+    const size_t smem = (size_t)RT * p.kc_stride * sizeof(T);
+    ctas_per_sm(stream_func<T, VEC, RT, GROUPED>(), fk::STREAM_THREADS, smem);  // sets the smem attribute if needed
+    fk::fk_stream_kernel<T, VEC, RT, StreamShape<RT>::RPW, STREAM_UNROLL, GROUPED>
+        <<<grid, fk::STREAM_THREADS, smem, s>>>(p);
+    return cudaGetLastError();
+}
+
+// picks the replica tile for a pass starting at r0
+inline int pick_rt(int remaining) { return remaining >= 3 ? 4 : remaining; }
+
+template <typename T, bool GROUPED>
+int stream_grid(bool vec_ok, int rt, int kc, long long units) {
+    constexpr int VW = fk::VecWidth<T>::value;
+    if (vec_ok) {
+        if (rt == 1) return stream_grid_for<T, VW, 1, GROUPED>(kc, units);
+        if (rt == 2) return stream_grid_for<T, VW, 2, GROUPED>(kc, units);
+        return stream_grid_for<T, VW, 4, GROUPED>(kc, units);
+    }
+    if (rt == 1) return stream_grid_for<T, 1, 1, GROUPED>(kc, units);
+    if (rt == 2) return stream_grid_for<T, 1, 2, GROUPED>(kc, units);
+    return stream_grid_for<T, 1, 4, GROUPED>(kc, units);
+}
+
+template <typename T, bool GROUPED>
+cudaError_t stream_dispatch(bool vec_ok, int rt, const fk::StreamParams& p, int grid, cudaStream_t s) {
+    constexpr int VW = fk::VecWidth<T>::value;
+    if (vec_ok) {
+        if (rt == 1) return launch_stream<T, VW, 1, GROUPED>(p, grid, s);
+        if (rt == 2) return launch_stream<T, VW, 2, GROUPED>(p, grid, s);
+        return launch_stream<T, VW, 4, GROUPED>(p, grid, s);
+    }
+    if (rt == 1) return launch_stream<T, 1, 1, GROUPED>(p, grid, s);
+    if (rt == 2) return launch_stream<T, 1, 2, GROUPED>(p, grid, s);
+    return launch_stream<T, 1, 4, GROUPED>(p, grid, s);
+}
+
+template <typename T, bool GROUPED>
+cudaError_t colsum_dispatch(bool vec_ok, int rt, const fk::ColsumParams& p, int grid, cudaStream_t s) {
+    constexpr int VW = fk::VecWidth<T>::value;
+    constexpr int U = 8;
+#define FK_COLSUM(V, RTv) fk::fk_colsum_kernel<T, V, RTv, U, GROUPED><<<grid, fk::COLSUM_THREADS, 0, s>>>(p)
+    if (vec_ok) {
+        if (rt == 1) FK_COLSUM(VW, 1); else if (rt == 2) FK_COLSUM(VW, 2); else FK_COLSUM(VW, 4);
+    } else {
+        if (rt == 1) FK_COLSUM(1, 1); else if (rt == 2) FK_COLSUM(1, 2); else FK_COLSUM(1, 4);
+    }
+#undef FK_COLSUM
+    return cudaGetLastError();
+}
+
+// One table, any R.  `part` holds >= part_elems_per_replica * R doubles (may be null if nchunks == 1).
+template <typename T>
+int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const T* f, T* sigma,
+                    int R, double* part, double* gemm_part, cudaStream_t s, int* launches) {
+    int nl = 0;
+    if (fk::gemm_wanted(R)) {
+        int rc = fk::gemm_forward_single<T>(d, ch, f, sigma, R, gemm_part, pl.gsplit, s, &nl);
+        if (rc != 0) return fail(FK_ERR_CUDA, "gemm forward launch failed: %s", cudaGetErrorString((cudaError_t)rc));
+        if (launches) *launches = nl;
+        return FK_OK;
+    }
+    fk::StreamParams p;
+    memset(&p, 0, sizeof p);
+    p.desc = d;
+    p.chan = ch;
+    p.f = f;
+    p.part = part;
+    p.sigma = sigma;
+    p.units = (long long)pl.nchunks * d.N;
+    p.R = R;
+    p.kc_stride = pl.kc;
+    for (int r0 = 0; r0 < R;) {
+        const int rt = pick_rt(R - r0);
+        p.r0 = r0;
+        const int grid = stream_grid<T, false>(d.vec_ok, rt, pl.kc, p.units);
+        size_t slot = 0;
+        const bool timed = r0 == 0 && g_prof.begin(s, slot);
+        cudaError_t e = stream_dispatch<T, false>(d.vec_ok, rt, p, grid, s);
+        if (timed) g_prof.end(s, slot);
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "stream kernel launch failed: %s", cudaGetErrorString(e));
+        ++nl;
+        r0 += rt;
+    }
+    if (pl.nchunks > 1) {
+        fk::ReduceParams q;
+        memset(&q, 0, sizeof q);
+        q.desc = d;
+        q.part = part;
+        q.sigma = sigma;
+        q.rows = d.N;
+        q.R = R;
+        const long long outs = (long long)d.N * R;
+        const int grid = (int)std::min<long long>((outs + 7) / 8, (long long)sm_count() * 8);
+        fk::fk_reduce_chunks_kernel<T, false><<<std::max(1, grid), 256, 0, s>>>(q);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "reduce kernel launch failed: %s", cudaGetErrorString(e));
+        ++nl;
+    }
+    if (launches) *launches = nl;
+    return FK_OK;
+}
+
+// `G` holds >= G_elems_per_replica * R doubles.
+template <typename T>
+int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const T* f, const T* g, T* df,
+                   int R, double* G, cudaStream_t s, int* launches) {
+    int nl = 0;
+    if (fk::gemm_wanted(R)) {
+        int rc = fk::gemm_colsum_single<T>(d, g, G, R, s, &nl);
+        if (rc != 0) return fail(FK_ERR_CUDA, "gemm colsum launch failed: %s", cudaGetErrorString((cudaError_t)rc));
+    } else {
+        fk::ColsumParams p;
+        memset(&p, 0, sizeof p);
+        p.desc = d;
+        p.g = g;
+        p.G = G;
+        p.R = R;
+        p.nkb = pl.nkb;
+        for (int r0 = 0; r0 < R;) {
+            const int rt = pick_rt(R - r0);
+            p.r0 = r0;
+            cudaError_t e = colsum_dispatch<T, false>(d.vec_ok, rt, p, pl.nkb * pl.nsplit, s);
+            if (e != cudaSuccess) return fail(FK_ERR_CUDA, "colsum kernel launch failed: %s", cudaGetErrorString(e));
+            ++nl;
+            r0 += rt;
+        }
+    }
+    fk::GatherParams q;
+    memset(&q, 0, sizeof q);
+    q.desc = d;
+    if (fk::gemm_wanted(R)) q.desc.nsplit = 1;  // the GEMM stage 1 writes a single, complete G
+    q.chan = ch;
+    q.f = f;
+    q.G = G;
+    q.df = df;
+    q.R = R;
+    fk::fk_vjp_gather_kernel<T, false><<<dim3(d.nfl * d.nx, R), fk::GATHER_THREADS, 0, s>>>(q);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gather kernel launch failed: %s", cudaGetErrorString(e));
+    ++nl;
+    if (launches) *launches = nl;
+    return FK_OK;
+}
+
+size_t conv_scratch_elems(const fk::TableDesc& d, const Plan& pl, int R) {
+    if (fk::gemm_wanted(R)) return fk::gemm_forward_scratch_elems(d, R, pl.gsplit);
+    return part_elems_per_replica(d) * R;
+}
+size_t vjp_scratch_elems(const fk::TableDesc& d, int R) {
+    if (fk::gemm_wanted(R)) return (size_t)d.K * R;
+    return G_elems_per_replica(d) * R;
+}
+
+// stateless front end shared by the fp64 / fp32 entry points
+template <typename T>
+int stateless(const char* who, int kind, bool vjp, const T* fkp, const int32_t* idx, const T* f, const T* g, T* out,
+              int N, int nx, int nfl, int C, int R, void* stream) {
+    g_err.clear();
+    if (!fkp || !idx || !f || !out || (vjp && !g)) return fail(FK_ERR_INVALID_ARG, "%s: null pointer", who);
+    int rc = check_dims(who, kind, N, nx, nfl, C, R);
+    if (rc) return rc;
+    if ((uintptr_t)fkp % sizeof(T) || (uintptr_t)f % sizeof(T) || (uintptr_t)out % sizeof(T))
+        return fail(FK_ERR_INVALID_ARG, "%s: misaligned pointer", who);
+    fk::ChannelList ch;
+    rc = fill_channels(who, kind, idx, nfl, C, ch);
+    if (rc) return rc;
+    fk::TableDesc d = make_desc(kind, fk::LAYOUT_LOGICAL, fkp, N, nx, nfl, C, 0, dtype_of<T>());
+    Plan pl;
+    make_plan(d, dtype_of<T>(), pl);
+    pl.gsplit = fk::gemm_pick_split(d, R, sm_count());
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t elems = vjp ? vjp_scratch_elems(d, R) : conv_scratch_elems(d, pl, R);
+    double* scratch = nullptr;
+    if (elems) FK_CUDA(cudaMallocAsync((void**)&scratch, elems * sizeof(double), s));
+    rc = vjp ? run_vjp_single<T>(d, ch, pl, f, g, out, R, scratch, s, nullptr)
+             : run_conv_single<T>(d, ch, pl, f, out, R, scratch, scratch, s, nullptr);
+    if (scratch) {
+        cudaError_t e = cudaFreeAsync(scratch, s);
+        if (rc == FK_OK && e != cudaSuccess) return fail(FK_ERR_CUDA, "cudaFreeAsync: %s", cudaGetErrorString(e));
+    }
+    return rc;
+}
+
+}  // namespace
+
+// --------------------------------------------------------------------------------------------------
+// handles
+// --------------------------------------------------------------------------------------------------
+struct fk_table {
+    fk::TableDesc desc;
+    fk::ChannelList chan;
+    Plan plan;
+    int dtype = FK_F64, store = FK_STORE_BORROW, kind = FK_KIND_HADRONIC;
+    void* owned_fk = nullptr;
+    uint8_t* dev_chan = nullptr;  // [2][C] for grouped launches
+    double* scratch = nullptr;    // forward partials / VJP column sums (one buffer, used by one call at a time)
+    size_t scratch_elems = 0;
+    void* h_stage = nullptr;      // pinned host staging for the *_host calls
+    void* d_stage = nullptr;
+    size_t stage_bytes = 0;
+    int last_launches = 0;
+};
+
+namespace {
+
+int ensure_scratch(fk_table* t, size_t elems) {
+    if (elems <= t->scratch_elems) return FK_OK;
+    if (t->scratch) cudaFree(t->scratch);
+    t->scratch = nullptr;
+    t->scratch_elems = 0;
+    FK_CUDA(cudaMalloc((void**)&t->scratch, elems * sizeof(double)));
+    t->scratch_elems = elems;
+    return FK_OK;
+}
+
+int ensure_stage(fk_table* t, size_t bytes) {
+    if (bytes <= t->stage_bytes) return FK_OK;
+    if (t->h_stage) cudaFreeHost(t->h_stage);
+    if (t->d_stage) cudaFree(t->d_stage);
+    t->h_stage = t->d_stage = nullptr;
+    t->stage_bytes = 0;
+    FK_CUDA(cudaMallocHost(&t->h_stage, bytes));
+    FK_CUDA(cudaMalloc(&t->d_stage, bytes));
+    t->stage_bytes = bytes;
+    return FK_OK;
+}
+
+size_t table_scratch_need(const fk_table* t, int R) {
+    Plan pl = t->plan;
+    pl.gsplit = fk::gemm_pick_split(t->desc, R, sm_count());
+    return std::max(conv_scratch_elems(t->desc, pl, R), vjp_scratch_elems(t->desc, R));
+}
+
+template <typename T>
+int table_conv_t(fk_table* t, const void* f, void* sigma, int R, cudaStream_t s) {
+    Plan pl = t->plan;
+    pl.gsplit = fk::gemm_pick_split(t->desc, R, sm_count());
+    int rc = ensure_scratch(t, table_scratch_need(t, R));
+    if (rc) return rc;
+    return run_conv_single<T>(t->desc, t->chan, pl, (const T*)f, (T*)sigma, R, t->scratch, t->scratch, s,
+                              &t->last_launches);
+}
+
+template <typename T>
+int table_vjp_t(fk_table* t, const void* f, const void* g, void* df, int R, cudaStream_t s) {
+    int rc = ensure_scratch(t, table_scratch_need(t, R));
+    if (rc) return rc;
+    return run_vjp_single<T>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)df, R, t->scratch, s,
+                             &t->last_launches);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* fk_last_error_string(void) { return g_err.c_str(); }
+int fk_version(void) { return 100; }
+int fk_compiled_arch(void) { return 100; }
+
+int fk_profile_enable(int on) {
+    std::lock_guard<std::mutex> lk(g_prof.mu);
+    g_prof.on = on != 0;
+    return FK_OK;
+}
+int fk_profile_read(double* mean_kernel_ms, int* launches) {
+    std::lock_guard<std::mutex> lk(g_prof.mu);
+    double tot = 0.0;
+    int n = 0;
+    for (size_t i = 0; i < g_prof.used; ++i) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(g_prof.pairs[i].second) == cudaSuccess &&
+            cudaEventElapsedTime(&ms, g_prof.pairs[i].first, g_prof.pairs[i].second) == cudaSuccess) {
+            tot += ms;
+            ++n;
+        }
+    }
+    g_prof.used = 0;
+    if (mean_kernel_ms) *mean_kernel_ms = n ? tot / n : 0.0;
+    if (launches) *launches = n;
+    return FK_OK;
+}
+
+int fk_conv_dis(const double* fk, const int32_t* flav, const double* f, double* sigma, int N, int nx, int nfl, int nA,
+                int R, void* stream) {
+    return stateless<double>("fk_conv_dis", FK_KIND_DIS, false, fk, flav, f, nullptr, sigma, N, nx, nfl, nA, R, stream);
+}
+int fk_conv_hadronic(const double* fk, const int32_t* pairs, const double* f, double* sigma, int N, int nx, int nfl,
+                     int C, int R, void* stream) {
+    return stateless<double>("fk_conv_hadronic", FK_KIND_HADRONIC, false, fk, pairs, f, nullptr, sigma, N, nx, nfl, C, R,
+                             stream);
+}
+int fk_conv_hadronic_vjp(const double* fk, const int32_t* pairs, const double* f, const double* g, double* df, int N,
+                         int nx, int nfl, int C, int R, void* stream) {
+    return stateless<double>("fk_conv_hadronic_vjp", FK_KIND_HADRONIC, true, fk, pairs, f, g, df, N, nx, nfl, C, R,
+                             stream);
+}
+int fk_conv_dis_vjp(const double* fk, const int32_t* flav, const double* f, const double* g, double* df, int N, int nx,
+                    int nfl, int nA, int R, void* stream) {
+    return stateless<double>("fk_conv_dis_vjp", FK_KIND_DIS, true, fk, flav, f, g, df, N, nx, nfl, nA, R, stream);
+}
+int fk_conv_dis_f32(const float* fk, const int32_t* flav, const float* f, float* sigma, int N, int nx, int nfl, int nA,
+                    int R, void* stream) {
+    return stateless<float>("fk_conv_dis_f32", FK_KIND_DIS, false, fk, flav, f, nullptr, sigma, N, nx, nfl, nA, R, stream);
+}
+int fk_conv_hadronic_f32(const float* fk, const int32_t* pairs, const float* f, float* sigma, int N, int nx, int nfl,
+                         int C, int R, void* stream) {
+    return stateless<float>("fk_conv_hadronic_f32", FK_KIND_HADRONIC, false, fk, pairs, f, nullptr, sigma, N, nx, nfl, C,
+                            R, stream);
+}
+int fk_conv_hadronic_vjp_f32(const float* fk, const int32_t* pairs, const float* f, const float* g, float* df, int N,
+                             int nx, int nfl, int C, int R, void* stream) {
+    return stateless<float>("fk_conv_hadronic_vjp_f32", FK_KIND_HADRONIC, true, fk, pairs, f, g, df, N, nx, nfl, C, R,
+                            stream);
+}
+
+// ---------------------------------------------------------------------------------------- tables
+int fk_table_create(fk_table** out, int kind, const double* fk_logical, const int32_t* index_list, int N, int nx,
+                    int nfl, int C, int dtype, int store, int R_hint) {
+    g_err.clear();
+    if (!out) return fail(FK_ERR_INVALID_ARG, "fk_table_create: null out");
+    *out = nullptr;
+    if (!fk_logical || !index_list) return fail(FK_ERR_INVALID_ARG, "fk_table_create: null pointer");
+    if (kind != FK_KIND_DIS && kind != FK_KIND_HADRONIC) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad kind %d", kind);
+    if (dtype != FK_F64 && dtype != FK_F32) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad dtype %d", dtype);
+    if (store != FK_STORE_BORROW && store != FK_STORE_PACK) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad store %d", store);
+    if (dtype == FK_F32 && store == FK_STORE_BORROW)
+        return fail(FK_ERR_INVALID_ARG, "fk_table_create: an fp32 table must be packed (the logical input is fp64)");
+    int rc = check_dims("fk_table_create", kind, N, nx, nfl, C, std::max(1, R_hint));
+    if (rc) return rc;
+    if ((uintptr_t)fk_logical % 8) return fail(FK_ERR_INVALID_ARG, "fk_table_create: misaligned fk pointer");
+
+    fk_table* t = new (std::nothrow) fk_table();
+    if (!t) return fail(FK_ERR_ALLOC, "fk_table_create: host allocation failed");
+    rc = fill_channels("fk_table_create", kind, index_list, nfl, C, t->chan);
+    if (rc) { delete t; return rc; }
+    t->dtype = dtype; t->store = store; t->kind = kind;
+
+    const int K = kind == FK_KIND_HADRONIC ? C * nx * nx : C * nx;
+    auto bail = [&](int code) { fk_table_destroy(t); return code; };
+    if (store == FK_STORE_PACK) {
+        const int vecw = dtype == FK_F64 ? 2 : 4;
+        const long long row_stride = ((long long)K + vecw - 1) / vecw * vecw;
+        const size_t bytes = (size_t)N * row_stride * dtype_size(dtype);
+        cudaError_t e = cudaMalloc(&t->owned_fk, bytes);
+        if (e != cudaSuccess) { bail(0); return fail(FK_ERR_ALLOC, "fk_table_create: cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); }
+        const long long total = (long long)N * row_stride;
+        const int grid = (int)std::min<long long>((total + 255) / 256, 148LL * 64);
+        if (dtype == FK_F64)
+            fk::fk_pack_kernel<double><<<grid, 256>>>(fk_logical, (double*)t->owned_fk, N, nx, C,
+                                                     kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, row_stride);
+        else
+            fk::fk_pack_kernel<float><<<grid, 256>>>(fk_logical, (float*)t->owned_fk, N, nx, C,
+                                                    kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, row_stride);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: pack kernel: %s", cudaGetErrorString(e)); }
+        t->desc = make_desc(kind, fk::LAYOUT_PACKED, t->owned_fk, N, nx, nfl, C, row_stride, dtype);
+    } else {
+        t->desc = make_desc(kind, fk::LAYOUT_LOGICAL, fk_logical, N, nx, nfl, C, 0, dtype);
+    }
+    make_plan(t->desc, dtype, t->plan);
+
+    cudaError_t e = cudaMalloc((void**)&t->dev_chan, 2 * (size_t)C);
+    if (e == cudaSuccess) e = cudaMemcpy(t->dev_chan, t->chan.a, C, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t->dev_chan + C, t->chan.b, C, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: channel upload: %s", cudaGetErrorString(e)); }
+    t->desc.chan_a = t->dev_chan;
+    t->desc.chan_b = t->dev_chan + C;
+
+    rc = ensure_scratch(t, table_scratch_need(t, std::max(1, R_hint)));
+    if (rc) return bail(rc);
+    *out = t;
+    return FK_OK;
+}
+
+int fk_table_destroy(fk_table* t) {
+    if (!t) return FK_OK;
+    if (t->owned_fk) cudaFree(t->owned_fk);
+    if (t->dev_chan) cudaFree(t->dev_chan);
+    if (t->scratch) cudaFree(t->scratch);
+    if (t->h_stage) cudaFreeHost(t->h_stage);
+    if (t->d_stage) cudaFree(t->d_stage);
+    delete t;
+    return FK_OK;
+}
+
+int fk_table_info(const fk_table* t, int* N, int* nx, int* nfl, int* C, int64_t* K, int64_t* row_stride,
+                  int64_t* device_bytes) {
+    if (!t) return fail(FK_ERR_INVALID_ARG, "fk_table_info: null table");
+    if (N) *N = t->desc.N;
+    if (nx) *nx = t->desc.nx;
+    if (nfl) *nfl = t->desc.nfl;
+    if (C) *C = t->desc.C;
+    if (K) *K = t->desc.K;
+    if (row_stride) *row_stride = t->desc.row_stride;
+    if (device_bytes)
+        *device_bytes = (int64_t)((t->owned_fk ? (size_t)t->desc.N * t->desc.row_stride * dtype_size(t->dtype) : 0) +
+                                  t->scratch_elems * sizeof(double) + t->stage_bytes + 2 * (size_t)t->desc.C);
+    return FK_OK;
+}
+
+int fk_table_conv(fk_table* t, const void* f, void* sigma, int R, void* stream) {
+    g_err.clear();
+    if (!t || !f || !sigma) return fail(FK_ERR_INVALID_ARG, "fk_table_conv: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv: R=%d", R);
+    return t->dtype == FK_F64 ? table_conv_t<double>(t, f, sigma, R, (cudaStream_t)stream)
+                              : table_conv_t<float>(t, f, sigma, R, (cudaStream_t)stream);
+}
+
+int fk_table_vjp(fk_table* t, const void* f, const void* g, void* df, int R, void* stream) {
+    g_err.clear();
+    if (!t || !f || !g || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp: R=%d", R);
+    return t->dtype == FK_F64 ? table_vjp_t<double>(t, f, g, df, R, (cudaStream_t)stream)
+                              : table_vjp_t<float>(t, f, g, df, R, (cudaStream_t)stream);
+}
+
+int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R, void* stream) {
+    g_err.clear();
+    if (!t || !f_host || !sigma_host) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_host: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_host: R=%d", R);
+    const size_t es = dtype_size(t->dtype);
+    const size_t fb = (size_t)R * t->desc.nfl * t->desc.nx * es, sb = (size_t)t->desc.N * R * es;
+    const size_t fb_al = (fb + 255) / 256 * 256;
+    int rc = ensure_stage(t, 2 * fb_al + 2 * ((sb + 255) / 256 * 256));
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    char* h = (char*)t->h_stage; char* d = (char*)t->d_stage;
+    memcpy(h, f_host, fb);
+    FK_CUDA(cudaMemcpyAsync(d, h, fb, cudaMemcpyHostToDevice, s));
+    rc = fk_table_conv(t, d, d + fb_al, R, stream);
+    if (rc) return rc;
+    FK_CUDA(cudaMemcpyAsync(h + fb_al, d + fb_al, sb, cudaMemcpyDeviceToHost, s));
+    FK_CUDA(cudaStreamSynchronize(s));
+    memcpy(sigma_host, h + fb_al, sb);
+    return FK_OK;
+}
+
+int fk_table_vjp_host(fk_table* t, const void* f_host, const void* g_host, void* df_host, int R, void* stream) {
+    g_err.clear();
+    if (!t || !f_host || !g_host || !df_host) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp_host: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp_host: R=%d", R);
+    const size_t es = dtype_size(t->dtype);
+    const size_t fb = (size_t)R * t->desc.nfl * t->desc.nx * es, gb = (size_t)t->desc.N * R * es;
+    const size_t fb_al = (fb + 255) / 256 * 256, gb_al = (gb + 255) / 256 * 256;
+    int rc = ensure_stage(t, 2 * fb_al + 2 * gb_al);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    char* h = (char*)t->h_stage; char* d = (char*)t->d_stage;
+    memcpy(h, f_host, fb);
+    memcpy(h + fb_al, g_host, gb);
+    FK_CUDA(cudaMemcpyAsync(d, h, fb_al + gb, cudaMemcpyHostToDevice, s));
+    rc = fk_table_vjp(t, d, d + fb_al, d + fb_al + gb_al, R, stream);
+    if (rc) return rc;
+    FK_CUDA(cudaMemcpyAsync(h + fb_al + gb_al, d + fb_al + gb_al, fb, cudaMemcpyDeviceToHost, s));
+    FK_CUDA(cudaStreamSynchronize(s));
+    memcpy(df_host, h + fb_al + gb_al, fb);
+    return FK_OK;
+}
+
+int fk_table_last_launches(const fk_table* t) { return t ? t->last_launches : 0; }
+
+}  // extern "C"
+
+#include "fk_group.inl"

@@ -1,0 +1,126 @@
+// fk_common.cuh -- descriptors, index decode and small device helpers shared by the kernels.
+// Hand-written for sm_100a.  Nothing here is shared with oracle/ (see include/fkconv.h for the maths).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace fk {
+
+constexpr int KIND_DIS = 0;
+constexpr int KIND_HADRONIC = 1;
+constexpr int LAYOUT_LOGICAL = 0;  // hadronic k = (i*nx + j)*C + c ; DIS k = i*nA + c   (BASELINE.json order)
+constexpr int LAYOUT_PACKED = 1;   // hadronic k = (c*nx + i)*nx + j ; DIS k = c*nx + i   (x innermost)
+
+constexpr int MAX_C = 1024;   // active flavour pairs / flavours per table
+constexpr int MAX_NFL = 256;  // flavour indices are stored as uint8
+
+// Flavour indices of the active channels, passed BY VALUE in kernel-parameter space for single-table
+// launches (no H2D copy, no allocation, graph-capturable).  Grouped launches read them from HBM.
+struct ChannelList {
+    uint8_t a[MAX_C];  // a_c  (DIS: flav_c)
+    uint8_t b[MAX_C];  // b_c  (DIS: unused)
+};
+
+// One FK table as the kernels see it.
+struct TableDesc {
+    const void* fk;       // device; datapoint n starts at fk + n*row_stride elements
+    long long row_stride; // elements (>= K; PACK pads it to a 16-byte multiple)
+    int K;                // contraction length per datapoint: C*nx*nx (hadronic) or nA*nx (DIS)
+    int N, nx, nfl, C;
+    int kind, layout;
+    int vec_ok;           // rows are 16-byte aligned -> 128-bit loads
+    // grouped launches only
+    const uint8_t* chan_a;   // device copies of the channel list (a_c / b_c)
+    const uint8_t* chan_b;
+    long long f_off;         // element offset of f_t / df_t inside f_cat for R = 1 (scaled by R)
+    long long out_off;       // element offset of sigma_t / g_t inside sigma_cat for R = 1 (scaled by R)
+    long long part_off;      // element offset of this table's level-1 partials for R = 1 (scaled by R)
+    long long g_off;         // element offset of this table's column sums G for R = 1 (scaled by R)
+    int nchunks;             // forward: number of K-chunks
+    int nsplit;              // VJP stage 1: number of datapoint splits
+    int kc;                  // forward: chunk length in elements (multiple of 32*VEC*UNROLL)
+};
+
+// Offsets (inside one replica's f[nfl][nx]) of the two PDF factors of contraction index k.
+// Hadronic: L[k] = f[ia] * f[ib];  DIS: L[k] = f[ia] (ib = -1).
+__device__ __forceinline__ void decode_k(const TableDesc& d, const uint8_t* __restrict__ ca,
+                                         const uint8_t* __restrict__ cb, int k, int& ia, int& ib) {
+    const int nx = d.nx;
+    if (d.kind == KIND_HADRONIC) {
+        int c, i, j;
+        if (d.layout == LAYOUT_LOGICAL) {
+            c = k % d.C;
+            const int p = k / d.C;
+            i = p / nx;
+            j = p - i * nx;
+        } else {
+            const int q = k / nx;
+            j = k - q * nx;
+            c = q / nx;
+            i = q - c * nx;
+        }
+        ia = (int)ca[c] * nx + i;
+        ib = (int)cb[c] * nx + j;
+    } else {
+        int c, i;
+        if (d.layout == LAYOUT_LOGICAL) {
+            i = k / d.C;
+            c = k - i * d.C;
+        } else {
+            c = k / nx;
+            i = k - c * nx;
+        }
+        ia = (int)ca[c] * nx + i;
+        ib = -1;
+    }
+}
+
+// Contraction index of (i, j, c) resp. (i, c) in the table's k-order (inverse of decode_k).
+__device__ __forceinline__ int encode_k(const TableDesc& d, int i, int j, int c) {
+    if (d.kind == KIND_HADRONIC)
+        return d.layout == LAYOUT_LOGICAL ? (i * d.nx + j) * d.C + c : (c * d.nx + i) * d.nx + j;
+    return d.layout == LAYOUT_LOGICAL ? i * d.C + c : c * d.nx + i;
+}
+
+// ---- streaming loads: FK is read once, keep it out of L1 -------------------------------------
+template <typename T, int VEC> struct Vec;
+template <> struct Vec<double, 2> { double v[2]; };
+template <> struct Vec<double, 1> { double v[1]; };
+template <> struct Vec<float, 4> { float v[4]; };
+template <> struct Vec<float, 1> { float v[1]; };
+
+__device__ __forceinline__ Vec<double, 2> ld_stream(const double* p, Vec<double, 2>*) {
+    Vec<double, 2> r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.v[0]), "=d"(r.v[1]) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ Vec<double, 1> ld_stream(const double* p, Vec<double, 1>*) {
+    Vec<double, 1> r;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r.v[0]) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ Vec<float, 4> ld_stream(const float* p, Vec<float, 4>*) {
+    Vec<float, 4> r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
+                 : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ Vec<float, 1> ld_stream(const float* p, Vec<float, 1>*) {
+    Vec<float, 1> r;
+    asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r.v[0]) : "l"(p));
+    return r;
+}
+
+// ---- fixed-order warp tree (xor butterfly): every lane ends with the same bits ------------------
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <typename T> struct VecWidth;
+template <> struct VecWidth<double> { static constexpr int value = 2; };
+template <> struct VecWidth<float> { static constexpr int value = 4; };
+
+}  // namespace fk

@@ -1,0 +1,277 @@
+// fk_group.inl -- ragged grouped launch; included at the end of fk_api.cu.
+// A global fit convolves many tables of different (N, nx, C) every iteration.  The
+// host builds, once, a static work list balanced by bytes; a forward pass is then ONE persistent
+// stream launch (+ one level-2 reduce) over all tables, a VJP pass one column-sum launch + one
+// gather launch.  Reduction order is fixed by the list, so results are bitwise repeatable.
+
+struct fk_group {
+    std::vector<fk_table*> tables;
+    std::vector<fk::TableDesc> descs;  // host copies with the concatenation offsets filled in
+    int T = 0, dtype = FK_F64;
+    bool all_vec = true;
+    int kc_max = 0;
+    long long rows_total = 0, ai_total = 0, f_total1 = 0, part_total1 = 0, G_total1 = 0, elems_total = 0;
+    fk::TableDesc* d_descs = nullptr;
+    int* d_row_prefix = nullptr;
+    int* d_ai_prefix = nullptr;
+    fk::ColsumSeg* d_csegs = nullptr;
+    int ncsegs = 0;
+    struct WorkList { fk::Segment* d_segs = nullptr; int* d_cta_start = nullptr; int nsegs = 0; };
+    std::map<int, WorkList> worklists;  // by grid size
+    double* scratch = nullptr;
+    size_t scratch_elems = 0;
+    int last_launches = 0;
+};
+
+namespace {
+
+int group_scratch(fk_group* g, size_t elems) {
+    if (elems <= g->scratch_elems) return FK_OK;
+    if (g->scratch) cudaFree(g->scratch);
+    g->scratch = nullptr;
+    g->scratch_elems = 0;
+    FK_CUDA(cudaMalloc((void**)&g->scratch, elems * sizeof(double)));
+    g->scratch_elems = elems;
+    return FK_OK;
+}
+
+// Static forward work list for a grid of `G` CTAs: (table, chunk) row ranges, cut so that every CTA
+// streams the same number of FK elements (+- one row of one chunk).
+int group_worklist(fk_group* g, int G, fk_group::WorkList** out) {
+    auto it = g->worklists.find(G);
+    if (it != g->worklists.end()) { *out = &it->second; return FK_OK; }
+    std::vector<fk::Segment> segs;
+    std::vector<int> start(G + 1, 0);
+    const double quota = (double)g->elems_total / G;
+    double done = 0.0;
+    int cta = 0;
+    for (int t = 0; t < g->T; ++t) {
+        const fk::TableDesc& d = g->descs[t];
+        for (int chunk = 0; chunk < d.nchunks; ++chunk) {
+            const int klen = std::min(d.kc, d.K - chunk * d.kc);
+            int r = 0;
+            while (r < d.N) {
+                const double room = quota * (cta + 1) - done;
+                int take = (int)std::ceil(room / klen - 1e-9);
+                take = std::max(1, std::min(take, d.N - r));
+                segs.push_back(fk::Segment{t, chunk, r, r + take});
+                done += (double)take * klen;
+                r += take;
+                while (cta + 1 < G && done >= quota * (cta + 1) - 0.5) start[++cta] = (int)segs.size();
+            }
+        }
+    }
+    for (int c = cta + 1; c <= G; ++c) start[c] = (int)segs.size();
+    fk_group::WorkList wl;
+    wl.nsegs = (int)segs.size();
+    FK_CUDA(cudaMalloc((void**)&wl.d_segs, segs.size() * sizeof(fk::Segment)));
+    FK_CUDA(cudaMalloc((void**)&wl.d_cta_start, start.size() * sizeof(int)));
+    FK_CUDA(cudaMemcpy(wl.d_segs, segs.data(), segs.size() * sizeof(fk::Segment), cudaMemcpyHostToDevice));
+    FK_CUDA(cudaMemcpy(wl.d_cta_start, start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice));
+    auto ins = g->worklists.emplace(G, wl);
+    *out = &ins.first->second;
+    return FK_OK;
+}
+
+template <typename T>
+int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStream_t s) {
+    int rc = group_scratch(g, std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * R);
+    if (rc) return rc;
+    int nl = 0;
+    fk::StreamParams p;
+    memset(&p, 0, sizeof p);
+    p.descs = g->d_descs;
+    p.f = f_cat;
+    p.part = g->scratch;
+    p.sigma = sigma_cat;
+    p.R = R;
+    p.kc_stride = g->kc_max;
+    const long long units = (g->elems_total + g->kc_max - 1) / g->kc_max;
+    for (int r0 = 0; r0 < R;) {
+        const int rt = pick_rt(R - r0);
+        p.r0 = r0;
+        const int grid = stream_grid<T, true>(g->all_vec, rt, g->kc_max, units);
+        fk_group::WorkList* wl = nullptr;
+        rc = group_worklist(g, grid, &wl);
+        if (rc) return rc;
+        p.segs = wl->d_segs;
+        p.cta_seg_start = wl->d_cta_start;
+        cudaError_t e = stream_dispatch<T, true>(g->all_vec, rt, p, grid, s);
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped stream launch failed: %s", cudaGetErrorString(e));
+        ++nl;
+        r0 += rt;
+    }
+    if (g->part_total1 > 0) {
+        fk::ReduceParams q;
+        memset(&q, 0, sizeof q);
+        q.descs = g->d_descs;
+        q.row_prefix = g->d_row_prefix;
+        q.T = g->T;
+        q.part = g->scratch;
+        q.sigma = sigma_cat;
+        q.rows = g->rows_total;
+        q.R = R;
+        const long long outs = g->rows_total * R;
+        const int grid = (int)std::min<long long>((outs + 7) / 8, (long long)sm_count() * 8);
+        fk::fk_reduce_chunks_kernel<T, true><<<std::max(1, grid), 256, 0, s>>>(q);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped reduce launch failed: %s", cudaGetErrorString(e));
+        ++nl;
+    }
+    g->last_launches = nl;
+    return FK_OK;
+}
+
+template <typename T>
+int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat, int R, cudaStream_t s) {
+    int rc = group_scratch(g, std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * R);
+    if (rc) return rc;
+    int nl = 0;
+    fk::ColsumParams p;
+    memset(&p, 0, sizeof p);
+    p.descs = g->d_descs;
+    p.segs = g->d_csegs;
+    p.g = g_cat;
+    p.G = g->scratch;
+    p.R = R;
+    for (int r0 = 0; r0 < R;) {
+        const int rt = pick_rt(R - r0);
+        p.r0 = r0;
+        cudaError_t e = colsum_dispatch<T, true>(g->all_vec, rt, p, g->ncsegs, s);
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped colsum launch failed: %s", cudaGetErrorString(e));
+        ++nl;
+        r0 += rt;
+    }
+    fk::GatherParams q;
+    memset(&q, 0, sizeof q);
+    q.descs = g->d_descs;
+    q.ai_prefix = g->d_ai_prefix;
+    q.T = g->T;
+    q.f = f_cat;
+    q.G = g->scratch;
+    q.df = df_cat;
+    q.R = R;
+    fk::fk_vjp_gather_kernel<T, true><<<dim3((unsigned)g->ai_total, R), fk::GATHER_THREADS, 0, s>>>(q);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gather launch failed: %s", cudaGetErrorString(e));
+    ++nl;
+    g->last_launches = nl;
+    return FK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) {
+    g_err.clear();
+    if (!out) return fail(FK_ERR_INVALID_ARG, "fk_group_create: null out");
+    *out = nullptr;
+    if (!tables || T <= 0) return fail(FK_ERR_INVALID_ARG, "fk_group_create: no tables");
+    for (int t = 0; t < T; ++t)
+        if (!tables[t]) return fail(FK_ERR_INVALID_ARG, "fk_group_create: table %d is null", t);
+    fk_group* g = new (std::nothrow) fk_group();
+    if (!g) return fail(FK_ERR_ALLOC, "fk_group_create: host allocation failed");
+    g->T = T;
+    g->dtype = tables[0]->dtype;
+    std::vector<int> row_prefix(T + 1, 0), ai_prefix(T + 1, 0);
+    std::vector<fk::ColsumSeg> csegs;
+    for (int t = 0; t < T; ++t) {
+        fk_table* tb = tables[t];
+        if (tb->dtype != g->dtype) { delete g; return fail(FK_ERR_INVALID_ARG, "fk_group_create: mixed dtypes"); }
+        fk::TableDesc d = tb->desc;
+        d.f_off = g->f_total1;
+        d.out_off = g->rows_total;
+        d.part_off = g->part_total1;
+        d.g_off = g->G_total1;
+        g->f_total1 += (long long)d.nfl * d.nx;
+        g->rows_total += d.N;
+        g->ai_total += (long long)d.nfl * d.nx;
+        g->part_total1 += (long long)part_elems_per_replica(d);
+        g->G_total1 += (long long)G_elems_per_replica(d);
+        g->elems_total += (long long)d.N * d.K;
+        g->all_vec = g->all_vec && d.vec_ok;
+        g->kc_max = std::max(g->kc_max, d.kc);
+        row_prefix[t + 1] = (int)g->rows_total;
+        ai_prefix[t + 1] = (int)g->ai_total;
+        for (int sp = 0; sp < d.nsplit; ++sp)
+            for (int kb = 0; kb < tb->plan.nkb; ++kb) csegs.push_back(fk::ColsumSeg{t, kb, sp, 0});
+        g->tables.push_back(tb);
+        g->descs.push_back(d);
+    }
+    if (g->rows_total >= (1LL << 31) || g->ai_total >= (1LL << 31)) {
+        delete g;
+        return fail(FK_ERR_UNSUPPORTED, "fk_group_create: more than 2^31 datapoints or PDF slots");
+    }
+    if (!g->all_vec) {
+        // the VEC = 1 kernels index k-blocks of COLSUM_THREADS elements: rebuild the stage-1 list accordingly
+        csegs.clear();
+        for (int t = 0; t < T; ++t) {
+            const fk::TableDesc& d = g->descs[t];
+            const int nkb = (d.K + fk::COLSUM_THREADS - 1) / fk::COLSUM_THREADS;
+            for (int sp = 0; sp < d.nsplit; ++sp)
+                for (int kb = 0; kb < nkb; ++kb) csegs.push_back(fk::ColsumSeg{t, kb, sp, 0});
+        }
+    }
+    g->ncsegs = (int)csegs.size();
+    auto bail = [&](int code) { fk_group_destroy(g); return code; };
+    cudaError_t e = cudaMalloc((void**)&g->d_descs, T * sizeof(fk::TableDesc));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_row_prefix, (T + 1) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_ai_prefix, (T + 1) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_csegs, csegs.size() * sizeof(fk::ColsumSeg));
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_descs, g->descs.data(), T * sizeof(fk::TableDesc), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_row_prefix, row_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_ai_prefix, ai_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_csegs, csegs.data(), csegs.size() * sizeof(fk::ColsumSeg), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_group_create: %s", cudaGetErrorString(e)); }
+    int rc = group_scratch(g, std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * std::max(1, R_hint));
+    if (rc) return bail(rc);
+    *out = g;
+    return FK_OK;
+}
+
+int fk_group_destroy(fk_group* g) {
+    if (!g) return FK_OK;
+    if (g->d_descs) cudaFree(g->d_descs);
+    if (g->d_row_prefix) cudaFree(g->d_row_prefix);
+    if (g->d_ai_prefix) cudaFree(g->d_ai_prefix);
+    if (g->d_csegs) cudaFree(g->d_csegs);
+    for (auto& kv : g->worklists) {
+        if (kv.second.d_segs) cudaFree(kv.second.d_segs);
+        if (kv.second.d_cta_start) cudaFree(kv.second.d_cta_start);
+    }
+    if (g->scratch) cudaFree(g->scratch);
+    delete g;
+    return FK_OK;
+}
+
+int fk_group_offsets(const fk_group* g, int R, int64_t* f_offsets, int64_t* sigma_offsets) {
+    if (!g || R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_group_offsets: bad argument");
+    for (int t = 0; t < g->T; ++t) {
+        if (f_offsets) f_offsets[t] = g->descs[t].f_off * R;
+        if (sigma_offsets) sigma_offsets[t] = g->descs[t].out_off * R;
+    }
+    if (f_offsets) f_offsets[g->T] = g->f_total1 * R;
+    if (sigma_offsets) sigma_offsets[g->T] = g->rows_total * R;
+    return FK_OK;
+}
+
+int fk_conv_grouped(fk_group* g, const void* f_cat, void* sigma_cat, int R, void* stream) {
+    g_err.clear();
+    if (!g || !f_cat || !sigma_cat) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped: R=%d", R);
+    return g->dtype == FK_F64 ? group_conv_t<double>(g, f_cat, sigma_cat, R, (cudaStream_t)stream)
+                              : group_conv_t<float>(g, f_cat, sigma_cat, R, (cudaStream_t)stream);
+}
+
+int fk_conv_grouped_vjp(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat, int R, void* stream) {
+    g_err.clear();
+    if (!g || !f_cat || !g_cat || !df_cat) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped_vjp: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped_vjp: R=%d", R);
+    return g->dtype == FK_F64 ? group_vjp_t<double>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream)
+                              : group_vjp_t<float>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream);
+}
+
+int fk_group_last_launches(const fk_group* g) { return g ? g->last_launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,38 @@
+// fk_pack.cuh -- one-time, untimed table pack: logical channel-innermost fp64 table
+// -> device layout: channel-major, x innermost, rows padded with zeros to a 16-byte multiple,
+// optionally demoted to fp32 with round-to-nearest (reading R18).  Tables are loaded once and kept
+// resident for the whole fit, so this runs off the timed path.
+#pragma once
+
+#include "fk_common.cuh"
+
+namespace fk {
+
+// out[n][kp] = (T) in[n][klog(kp)],  kp in packed order; pad columns [K, row_stride) = 0
+template <typename T>
+__global__ void __launch_bounds__(256)
+fk_pack_kernel(const double* __restrict__ in, T* __restrict__ out, int N, int nx, int C, int kind,
+               int K, long long row_stride) {
+    const long long total = (long long)N * row_stride;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
+         t += (long long)gridDim.x * blockDim.x) {
+        const long long n = t / row_stride;
+        const int kp = (int)(t - n * row_stride);
+        T v = T(0);
+        if (kp < K) {
+            int klog;
+            if (kind == KIND_HADRONIC) {
+                const int q = kp / nx, j = kp - q * nx;
+                const int c = q / nx, i = q - c * nx;
+                klog = (i * nx + j) * C + c;
+            } else {
+                const int c = kp / nx, i = kp - c * nx;
+                klog = i * C + c;
+            }
+            v = (T)in[n * (long long)K + klog];  // fp64 -> fp32: cvt.rn
+        }
+        out[t] = v;
+    }
+}
+
+}  // namespace fk

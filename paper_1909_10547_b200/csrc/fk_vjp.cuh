@@ -1,0 +1,212 @@
+// fk_vjp.cuh -- gradient of the convolution as a VJP, minimal-flop order:
+//
+//   stage 1 (one FK pass, bandwidth-bound):  G[r][k] = sum_n g[n][r] * FK[n][k]
+//   stage 2 (tiny, gather form, no atomics): df[r][alpha][i] =
+//        sum_{c: a_c = alpha} sum_j G[r][k(i,j,c)] * f[r][b_c][j]
+//      + sum_{c: b_c = alpha} sum_j G[r][k(j,i,c)] * f[r][a_c][j]          (hadronic; the a_c == b_c,
+//        i == j diagonal gets both terms because both sums visit it)
+//      DIS: df[r][alpha][i] = sum_{c: flav_c = alpha} G[r][k(i,c)]
+//
+// Stage 1: a thread owns VEC consecutive k and walks down the datapoints of its split with UNROLL
+// independent 128-bit loads in flight; no cross-thread reduction at all.  Datapoints are cut into
+// `nsplit` fixed ranges for parallelism; stage 2 adds the splits in a fixed order.
+#pragma once
+
+#include "fk_common.cuh"
+
+namespace fk {
+
+struct ColsumSeg {  // grouped work list entry
+    int table, kblock, split, pad_;
+};
+
+struct ColsumParams {
+    TableDesc desc;           // single-table launch
+    const TableDesc* descs;   // grouped (device)
+    const ColsumSeg* segs;    // grouped (device), one per CTA
+    const void* g;            // g[N][R] or g_cat
+    double* G;                // [nsplit][R][K] per table
+    int R, r0;
+    int nkb;                  // single: k-blocks per split
+};
+
+constexpr int COLSUM_THREADS = 256;
+constexpr int COLSUM_MAX_ROWS = 512;  // datapoints per split (bounds the g tile in shared memory)
+
+template <typename T, int VEC, int RT, int UNROLL, bool GROUPED>
+__global__ void __launch_bounds__(COLSUM_THREADS)
+fk_colsum_kernel(const __grid_constant__ ColsumParams p) {
+    using V = Vec<T, VEC>;
+    constexpr int NACC = (RT == 1) ? 4 : 2;
+    __shared__ T gs[(COLSUM_MAX_ROWS + UNROLL) * RT];
+
+    const TableDesc* dp = &p.desc;
+    int kblock, split;
+    if constexpr (GROUPED) {
+        const ColsumSeg sg = p.segs[blockIdx.x];
+        dp = &p.descs[sg.table];
+        kblock = sg.kblock;
+        split = sg.split;
+    } else {
+        kblock = blockIdx.x % p.nkb;
+        split = blockIdx.x / p.nkb;
+    }
+    const TableDesc& d = *dp;
+    const int R = p.R;
+    const int rb = (int)((long long)d.N * split / d.nsplit);
+    const int re = (int)((long long)d.N * (split + 1) / d.nsplit);
+    const int rows = re - rb;
+
+    // g tile [rows rounded up to UNROLL][RT], zero padded
+    const T* __restrict__ g = reinterpret_cast<const T*>(p.g) + d.out_off * R;
+    const int rows_pad = (rows + UNROLL - 1) / UNROLL * UNROLL;
+    for (int t = threadIdx.x; t < rows_pad * RT; t += COLSUM_THREADS) {
+        const int m = t / RT, r = t - m * RT;
+        const int rr = p.r0 + r;
+        gs[t] = (m < rows && rr < R) ? __ldg(g + (long long)(rb + m) * R + rr) : T(0);
+    }
+    __syncthreads();
+
+    const int k = (kblock * COLSUM_THREADS + threadIdx.x) * VEC;
+    if (k >= d.K) return;
+    const T* __restrict__ col = reinterpret_cast<const T*>(d.fk) + k;
+
+    T acc[NACC][RT][VEC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a)
+#pragma unroll
+        for (int r = 0; r < RT; ++r)
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) acc[a][r][e] = T(0);
+
+    for (int m = 0; m < rows_pad; m += UNROLL) {
+        V x[UNROLL];
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u)
+            x[u] = ld_stream(col + (long long)(rb + min(m + u, rows - 1)) * d.row_stride, (V*)nullptr);
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u)
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                const T gv = gs[(m + u) * RT + r];  // broadcast; 0 on the padded rows
+#pragma unroll
+                for (int e = 0; e < VEC; ++e)
+                    acc[u % NACC][r][e] = fma(gv, x[u].v[e], acc[u % NACC][r][e]);
+            }
+    }
+
+    double* __restrict__ G = p.G + d.g_off * R;
+#pragma unroll
+    for (int r = 0; r < RT; ++r) {
+        const int rr = p.r0 + r;
+        if (rr >= R) continue;
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) {
+            if (k + e >= d.K) continue;
+            double s = (double)acc[0][r][e];
+#pragma unroll
+            for (int a = 1; a < NACC; ++a) s += (double)acc[a][r][e];
+            G[((long long)split * R + rr) * d.K + k + e] = s;
+        }
+    }
+}
+
+// ---- stage 2: one CTA per (table, alpha, i), replicas on blockIdx.y -----------------------------
+struct GatherParams {
+    TableDesc desc;           // single
+    ChannelList chan;         // single
+    const TableDesc* descs;   // grouped (device)
+    const int* ai_prefix;     // grouped (device) [T+1]: first (alpha, i) slot of each table
+    int T;
+    const void* f;
+    const double* G;
+    void* df;
+    int R;
+};
+
+constexpr int GATHER_THREADS = 128;
+
+template <typename T, bool GROUPED>
+__global__ void __launch_bounds__(GATHER_THREADS)
+fk_vjp_gather_kernel(const __grid_constant__ GatherParams p) {
+    __shared__ short listA[MAX_C], listB[MAX_C];
+    __shared__ int cnt[2];
+    __shared__ double wsum[GATHER_THREADS / 32];
+
+    const TableDesc* dp = &p.desc;
+    const uint8_t* __restrict__ ca = p.chan.a;
+    const uint8_t* __restrict__ cb = p.chan.b;
+    int slot = blockIdx.x;
+    if constexpr (GROUPED) {
+        int lo = 0, hi = p.T;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (p.ai_prefix[mid] <= slot) lo = mid; else hi = mid;
+        }
+        dp = &p.descs[lo];
+        slot -= p.ai_prefix[lo];
+        ca = dp->chan_a;
+        cb = dp->chan_b;
+    }
+    const TableDesc& d = *dp;
+    const int nx = d.nx, C = d.C, R = p.R;
+    const int alpha = slot / nx, i = slot - alpha * nx;
+    const int r = blockIdx.y;
+    const bool had = d.kind == KIND_HADRONIC;
+
+    if (threadIdx.x == 0) {  // channel lists of this flavour, in channel order (fixed)
+        int na = 0, nb = 0;
+        for (int c = 0; c < C; ++c) {
+            if (ca[c] == alpha) listA[na++] = (short)c;
+            if (had && cb[c] == alpha) listB[nb++] = (short)c;
+        }
+        cnt[0] = na;
+        cnt[1] = nb;
+    }
+    __syncthreads();
+    const int na = cnt[0], nb = cnt[1];
+
+    const T* __restrict__ f = reinterpret_cast<const T*>(p.f) + d.f_off * R + (long long)r * d.nfl * nx;
+    const double* __restrict__ G = p.G + d.g_off * R + (long long)r * d.K;
+    const long long split_stride = (long long)R * d.K;
+    const int nsplit = d.nsplit;
+
+    double acc = 0.0;
+    if (had) {
+        const int items = (na + nb) * nx;
+        for (int t = threadIdx.x; t < items; t += GATHER_THREADS) {
+            const int q = t / nx, j = t - q * nx;
+            int k, fo;
+            if (q < na) {
+                const int c = listA[q];
+                k = encode_k(d, i, j, c);
+                fo = (int)cb[c] * nx + j;
+            } else {
+                const int c = listB[q - na];
+                k = encode_k(d, j, i, c);
+                fo = (int)ca[c] * nx + j;
+            }
+            double gk = 0.0;
+            for (int s = 0; s < nsplit; ++s) gk += G[s * split_stride + k];
+            acc = fma(gk, (double)f[fo], acc);
+        }
+    } else {
+        for (int t = threadIdx.x; t < na; t += GATHER_THREADS) {
+            const int k = encode_k(d, i, 0, listA[t]);
+            double gk = 0.0;
+            for (int s = 0; s < nsplit; ++s) gk += G[s * split_stride + k];
+            acc += gk;
+        }
+    }
+    acc = warp_sum(acc);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = wsum[0];
+#pragma unroll
+        for (int w = 1; w < GATHER_THREADS / 32; ++w) s += wsum[w];
+        reinterpret_cast<T*>(p.df)[d.f_off * R + ((long long)r * d.nfl + alpha) * nx + i] = (T)s;
+    }
+}
+
+}  // namespace fk

@@ -1,0 +1,283 @@
+"""Thin ctypes binding over the C-ABI library `libfkconv.so` (include/fkconv.h) - argument
+marshalling only: every step of the path runs in the CUDA kernels.  Same names as the C entry points.
+
+Tensors are torch CUDA tensors (PyTorch is used for device memory and streams only); index lists
+are host int32 arrays.  Importing this module fails loudly if the library has not been built
+(`python -m paper_1909_10547_b200.build`); there is no CPU fallback and nothing here imports `oracle/`.
+
+Eq. (1) of arXiv:1909.10547: sigma[n][r] = sum_{c,i,j} f[r][a_c][i] f[r][b_c][j] FK[n][i][j][c].
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfkconv.so")
+
+FK_OK, FK_ERR_INVALID_ARG, FK_ERR_ALLOC, FK_ERR_CUDA, FK_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+FK_KIND_DIS, FK_KIND_HADRONIC = 0, 1
+FK_F64, FK_F32 = 0, 1
+FK_STORE_BORROW, FK_STORE_PACK = 0, 1
+
+# every symbol include/fkconv.h declares
+SYMBOLS = (
+    "fk_last_error_string", "fk_version", "fk_compiled_arch", "fk_profile_enable", "fk_profile_read",
+    "fk_conv_dis", "fk_conv_hadronic", "fk_conv_hadronic_vjp", "fk_conv_dis_vjp",
+    "fk_conv_dis_f32", "fk_conv_hadronic_f32", "fk_conv_hadronic_vjp_f32",
+    "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp",
+    "fk_table_conv_host", "fk_table_vjp_host", "fk_table_last_launches",
+    "fk_group_create", "fk_group_destroy", "fk_group_offsets", "fk_conv_grouped",
+    "fk_conv_grouped_vjp", "fk_group_last_launches",
+)
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_1909_10547_b200.build` "
+        "(nvcc, sm_100a). The FK convolution has no CPU fallback.")
+
+lib = ctypes.CDLL(LIB_PATH)
+for _name in SYMBOLS:
+    getattr(lib, _name).restype = ctypes.c_int
+lib.fk_last_error_string.restype = ctypes.c_char_p
+
+_vp, _ci = ctypes.c_void_p, ctypes.c_int
+for _name in ("fk_conv_dis", "fk_conv_hadronic", "fk_conv_dis_f32", "fk_conv_hadronic_f32"):
+    getattr(lib, _name).argtypes = [_vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
+for _name in ("fk_conv_hadronic_vjp", "fk_conv_dis_vjp", "fk_conv_hadronic_vjp_f32"):
+    getattr(lib, _name).argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
+lib.fk_profile_enable.argtypes = [_ci]
+lib.fk_profile_read.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(_ci)]
+lib.fk_table_create.argtypes = [ctypes.POINTER(_vp), _ci, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _ci, _ci]
+lib.fk_table_destroy.argtypes = [_vp]
+lib.fk_table_info.argtypes = [_vp] + [ctypes.POINTER(_ci)] * 4 + [ctypes.POINTER(ctypes.c_int64)] * 3
+lib.fk_table_conv.argtypes = [_vp, _vp, _vp, _ci, _vp]
+lib.fk_table_vjp.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
+lib.fk_table_conv_host.argtypes = [_vp, _vp, _vp, _ci, _vp]
+lib.fk_table_vjp_host.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
+lib.fk_table_last_launches.argtypes = [_vp]
+lib.fk_group_create.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(_vp), _ci, _ci]
+lib.fk_group_destroy.argtypes = [_vp]
+lib.fk_group_offsets.argtypes = [_vp, _ci, _vp, _vp]
+lib.fk_conv_grouped.argtypes = [_vp, _vp, _vp, _ci, _vp]
+lib.fk_conv_grouped_vjp.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
+lib.fk_group_last_launches.argtypes = [_vp]
+
+
+class FkError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = lib.fk_last_error_string()
+        super().__init__(f"{where}: status {code}: {msg.decode() if msg else ''}")
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != FK_OK:
+        raise FkError(rc, where)
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dev(t: torch.Tensor, dtype=None) -> int:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise TypeError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _idx(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _hostptr(a: np.ndarray) -> int:
+    return a.ctypes.data
+
+
+def version() -> int:
+    return lib.fk_version()
+
+
+def compiled_arch() -> int:
+    return lib.fk_compiled_arch()
+
+
+# ------------------------------------------------------------------ stateless entry points
+def fk_conv_hadronic(fk, pairs, f, sigma=None, stream=None):
+    """fk[N][nx][nx][C], pairs[C][2] (host), f[R][nfl][nx] -> sigma[N][R] (fp64, or fp32 if fk is)."""
+    N, nx, _, C = fk.shape
+    R, nfl, _ = f.shape
+    pairs = _idx(pairs)
+    if sigma is None:
+        sigma = torch.empty((N, R), dtype=fk.dtype, device=fk.device)
+    fn = lib.fk_conv_hadronic if fk.dtype == torch.float64 else lib.fk_conv_hadronic_f32
+    _check(fn(_dev(fk), _hostptr(pairs), _dev(f, fk.dtype), _dev(sigma, fk.dtype), N, nx, nfl, C, R,
+              _stream(stream)), "fk_conv_hadronic")
+    return sigma
+
+
+def fk_conv_dis(fk, flav, f, sigma=None, stream=None):
+    """fk[N][nx][nA], flav[nA] (host), f[R][nfl][nx] -> sigma[N][R]."""
+    N, nx, nA = fk.shape
+    R, nfl, _ = f.shape
+    flav = _idx(flav)
+    if sigma is None:
+        sigma = torch.empty((N, R), dtype=fk.dtype, device=fk.device)
+    fn = lib.fk_conv_dis if fk.dtype == torch.float64 else lib.fk_conv_dis_f32
+    _check(fn(_dev(fk), _hostptr(flav), _dev(f, fk.dtype), _dev(sigma, fk.dtype), N, nx, nfl, nA, R,
+              _stream(stream)), "fk_conv_dis")
+    return sigma
+
+
+def fk_conv_hadronic_vjp(fk, pairs, f, g, df=None, stream=None):
+    """df[R][nfl][nx] = d(sum_n g[n][r] sigma[n][r]) / d f[r][alpha][i]."""
+    N, nx, _, C = fk.shape
+    R, nfl, _ = f.shape
+    pairs = _idx(pairs)
+    if df is None:
+        df = torch.empty_like(f)
+    fn = lib.fk_conv_hadronic_vjp if fk.dtype == torch.float64 else lib.fk_conv_hadronic_vjp_f32
+    _check(fn(_dev(fk), _hostptr(pairs), _dev(f, fk.dtype), _dev(g, fk.dtype), _dev(df, fk.dtype),
+              N, nx, nfl, C, R, _stream(stream)), "fk_conv_hadronic_vjp")
+    return df
+
+
+def fk_conv_dis_vjp(fk, flav, f, g, df=None, stream=None):
+    N, nx, nA = fk.shape
+    R, nfl, _ = f.shape
+    flav = _idx(flav)
+    if df is None:
+        df = torch.empty_like(f)
+    _check(lib.fk_conv_dis_vjp(_dev(fk, torch.float64), _hostptr(flav), _dev(f, torch.float64),
+                               _dev(g, torch.float64), _dev(df, torch.float64), N, nx, nfl, nA, R,
+                               _stream(stream)), "fk_conv_dis_vjp")
+    return df
+
+
+# ------------------------------------------------------------------ resident tables
+class FkTable:
+    """fk_table handle.  `fk_logical` is the fp64 logical-layout table on the device; with
+    store=FK_STORE_BORROW it must stay alive (a reference is kept here)."""
+
+    def __init__(self, kind, fk_logical, index_list, nfl, dtype=FK_F64, store=FK_STORE_PACK, R_hint=1):
+        self.kind = kind
+        idx = _idx(index_list)
+        if kind == FK_KIND_HADRONIC:
+            N, nx, _, C = fk_logical.shape
+        else:
+            N, nx, C = fk_logical.shape
+        self.N, self.nx, self.nfl, self.C = N, nx, nfl, C
+        self.dtype = dtype
+        self.tdtype = torch.float64 if dtype == FK_F64 else torch.float32
+        self.device = fk_logical.device
+        self._keep = fk_logical if store == FK_STORE_BORROW else None
+        h = _vp()
+        _check(lib.fk_table_create(ctypes.byref(h), kind, _dev(fk_logical, torch.float64), _hostptr(idx),
+                                   N, nx, nfl, C, dtype, store, R_hint), "fk_table_create")
+        self.handle = h
+
+    def info(self):
+        N, nx, nfl, C = _ci(), _ci(), _ci(), _ci()
+        K, rs, nb = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        _check(lib.fk_table_info(self.handle, N, nx, nfl, C, K, rs, nb), "fk_table_info")
+        return dict(N=N.value, nx=nx.value, nfl=nfl.value, C=C.value, K=K.value, row_stride=rs.value,
+                    device_bytes=nb.value)
+
+    def conv(self, f, sigma=None, stream=None):
+        R = f.shape[0]
+        if sigma is None:
+            sigma = torch.empty((self.N, R), dtype=self.tdtype, device=self.device)
+        _check(lib.fk_table_conv(self.handle, _dev(f, self.tdtype), _dev(sigma, self.tdtype), R,
+                                 _stream(stream)), "fk_table_conv")
+        return sigma
+
+    def vjp(self, f, g, df=None, stream=None):
+        R = f.shape[0]
+        if df is None:
+            df = torch.empty_like(f)
+        _check(lib.fk_table_vjp(self.handle, _dev(f, self.tdtype), _dev(g, self.tdtype), _dev(df, self.tdtype),
+                                R, _stream(stream)), "fk_table_vjp")
+        return df
+
+    def conv_host(self, f_host: np.ndarray, sigma_host: np.ndarray, stream=None):
+        R = f_host.shape[0]
+        _check(lib.fk_table_conv_host(self.handle, _hostptr(f_host), _hostptr(sigma_host), R, _stream(stream)),
+               "fk_table_conv_host")
+        return sigma_host
+
+    def vjp_host(self, f_host: np.ndarray, g_host: np.ndarray, df_host: np.ndarray, stream=None):
+        R = f_host.shape[0]
+        _check(lib.fk_table_vjp_host(self.handle, _hostptr(f_host), _hostptr(g_host), _hostptr(df_host), R,
+                                     _stream(stream)), "fk_table_vjp_host")
+        return df_host
+
+    def last_launches(self) -> int:
+        return lib.fk_table_last_launches(self.handle)
+
+    def destroy(self):
+        if getattr(self, "handle", None):
+            lib.fk_table_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class FkGroup:
+    """fk_group handle: ragged set of tables, one persistent launch per pass."""
+
+    def __init__(self, tables, R_hint=1):
+        self.tables = list(tables)
+        T = len(self.tables)
+        arr = (_vp * T)(*[t.handle for t in self.tables])
+        h = _vp()
+        _check(lib.fk_group_create(ctypes.byref(h), arr, T, R_hint), "fk_group_create")
+        self.handle = h
+        self.T = T
+        self.tdtype = self.tables[0].tdtype
+        self.device = self.tables[0].device
+
+    def offsets(self, R):
+        fo = np.zeros(self.T + 1, dtype=np.int64)
+        so = np.zeros(self.T + 1, dtype=np.int64)
+        _check(lib.fk_group_offsets(self.handle, R, _hostptr(fo), _hostptr(so)), "fk_group_offsets")
+        return fo, so
+
+    def conv(self, f_cat, R, sigma_cat=None, stream=None):
+        if sigma_cat is None:
+            _, so = self.offsets(R)
+            sigma_cat = torch.empty(int(so[-1]), dtype=self.tdtype, device=self.device)
+        _check(lib.fk_conv_grouped(self.handle, _dev(f_cat, self.tdtype), _dev(sigma_cat, self.tdtype), R,
+                                   _stream(stream)), "fk_conv_grouped")
+        return sigma_cat
+
+    def vjp(self, f_cat, g_cat, R, df_cat=None, stream=None):
+        if df_cat is None:
+            df_cat = torch.empty_like(f_cat)
+        _check(lib.fk_conv_grouped_vjp(self.handle, _dev(f_cat, self.tdtype), _dev(g_cat, self.tdtype),
+                                       _dev(df_cat, self.tdtype), R, _stream(stream)), "fk_conv_grouped_vjp")
+        return df_cat
+
+    def last_launches(self) -> int:
+        return lib.fk_group_last_launches(self.handle)
+
+    def destroy(self):
+        if getattr(self, "handle", None):
+            lib.fk_group_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

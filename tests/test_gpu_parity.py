@@ -1,0 +1,261 @@
+"""GPU-vs-oracle parity through the C-ABI (include/fkconv.h), element by element on seeded inputs.
+
+Small and medium cases here; the BASELINE.json full-size configurations are in test_gpu_fullsize.py.
+Tolerances: BASELINE.json north_star (fp64 1e-13, fp32 1e-5 of sum|terms|); exact-integer inputs must
+match bit for bit in any summation order.
+"""
+import numpy as np
+import pytest
+
+from oracle import fk_oracle as O
+from paper_1909_10547_b200 import synth
+from tests._parity import TOL32, TOL64, rel_err, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def K():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    from paper_1909_10547_b200 import fkconv
+    return fkconv
+
+
+def _tables(K, case, kind):
+    """The same table through every storage path: stateless (logical), BORROW handle, PACK handle."""
+    fk_d = to_dev(case.fk)
+    idx = case.pairs if kind == K.FK_KIND_HADRONIC else case.flav
+    tb = K.FkTable(kind, fk_d, idx, case.nfl, K.FK_F64, K.FK_STORE_BORROW)
+    tp = K.FkTable(kind, fk_d, idx, case.nfl, K.FK_F64, K.FK_STORE_PACK)
+    return fk_d, idx, tb, tp
+
+
+# ------------------------------------------------------------------ config 0 and friends (hadronic)
+@pytest.mark.parametrize("R", [1, 2, 3, 6])
+def test_config0_forward_and_vjp(K, R):
+    case = synth.config0(R=R)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    fk_d, idx, tb, tp = _tables(K, case, K.FK_KIND_HADRONIC)
+    f_d, g_d = to_dev(case.f), to_dev(case.g)
+    outs = {
+        "stateless": K.fk_conv_hadronic(fk_d, idx, f_d),
+        "borrow": tb.conv(f_d),
+        "pack": tp.conv(f_d),
+    }
+    for name, s in outs.items():
+        assert rel_err(s.cpu().numpy(), ref, scale) <= TOL64, name
+    douts = {
+        "stateless": K.fk_conv_hadronic_vjp(fk_d, idx, f_d, g_d),
+        "borrow": tb.vjp(f_d, g_d),
+        "pack": tp.vjp(f_d, g_d),
+    }
+    for name, d in douts.items():
+        assert rel_err(d.cpu().numpy(), dref, D) <= TOL64, name
+
+
+RAGGED = [  # (N, nx, nfl, C)  - odd nx / odd C (64-bit load path), N=1, C=1, K below one chunk, several chunks
+    (1, 7, 14, 1), (37, 23, 14, 29), (5, 3, 3, 9), (130, 9, 5, 13), (33, 31, 14, 21), (64, 16, 14, 40),
+    (3, 50, 14, 2), (300, 5, 2, 4),
+]
+
+
+@pytest.mark.parametrize("shape", RAGGED)
+@pytest.mark.parametrize("R", [1, 5])
+def test_ragged_shapes_hadronic(K, shape, R):
+    N, nx, nfl, C = shape
+    case = synth.hadronic_case(5, N, nx, C, R, nfl=nfl, sub=N * 1000 + nx)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    fk_d, idx, tb, tp = _tables(K, case, K.FK_KIND_HADRONIC)
+    f_d, g_d = to_dev(case.f), to_dev(case.g)
+    for name, s in (("stateless", K.fk_conv_hadronic(fk_d, idx, f_d)), ("borrow", tb.conv(f_d)), ("pack", tp.conv(f_d))):
+        assert rel_err(s.cpu().numpy(), ref, scale) <= TOL64, (name, shape)
+    for name, d in (("stateless", K.fk_conv_hadronic_vjp(fk_d, idx, f_d, g_d)), ("borrow", tb.vjp(f_d, g_d)),
+                    ("pack", tp.vjp(f_d, g_d))):
+        assert rel_err(d.cpu().numpy(), dref, D) <= TOL64, (name, shape)
+    # a flavour that appears in no pair gets exactly zero
+    used = set(case.pairs[:, 0]) | set(case.pairs[:, 1])
+    dn = tp.vjp(f_d, g_d).cpu().numpy()
+    for a in range(nfl):
+        if a not in used:
+            assert np.all(dn[:, a, :] == 0.0)
+
+
+# ------------------------------------------------------------------ config 1 (DIS)
+@pytest.mark.parametrize("R", [1, 100])
+def test_config1_dis(K, R):
+    case = synth.config1(R=R)
+    ref, scale = O.dis(case.fk, case.flav, case.f)
+    dref, D = O.dis_vjp(case.fk, case.flav, case.f, case.g)
+    fk_d, idx, tb, tp = _tables(K, case, K.FK_KIND_DIS)
+    f_d, g_d = to_dev(case.f), to_dev(case.g)
+    for name, s in (("stateless", K.fk_conv_dis(fk_d, idx, f_d)), ("borrow", tb.conv(f_d)), ("pack", tp.conv(f_d))):
+        assert rel_err(s.cpu().numpy(), ref, scale) <= TOL64, name
+    for name, d in (("stateless", K.fk_conv_dis_vjp(fk_d, idx, f_d, g_d)), ("borrow", tb.vjp(f_d, g_d)),
+                    ("pack", tp.vjp(f_d, g_d))):
+        assert rel_err(d.cpu().numpy(), dref, D) <= TOL64, name
+
+
+def test_dis_small_unsorted_flavours(K):
+    rng = np.random.default_rng(3)
+    N, nx, nfl = 19, 11, 6
+    flav = np.array([4, 0, 2], dtype=np.int32)
+    fk = rng.standard_normal((N, nx, 3))
+    f = rng.uniform(0.1, 2.0, (2, nfl, nx))
+    ref, scale = O.dis(fk, flav, f)
+    s = K.fk_conv_dis(to_dev(fk), flav, to_dev(f))
+    assert rel_err(s.cpu().numpy(), ref, scale) <= TOL64
+
+
+def test_dis_equals_hadronic_with_delta_flavour_on_gpu(K):
+    """DIS = hadronic with a pseudo-flavour delta_j0 on the second leg; ties the two
+    GPU kernels to each other end to end."""
+    rng = np.random.default_rng(8)
+    N, nx, nfl, nA = 40, 12, 5, 3
+    flav = np.array([3, 1, 4], dtype=np.int32)
+    fk_dis = rng.standard_normal((N, nx, nA))
+    f = rng.uniform(0.1, 2.0, (2, nfl, nx))
+    f_ext = np.zeros((2, nfl + 1, nx)); f_ext[:, :nfl] = f; f_ext[:, nfl, 0] = 1.0
+    pairs = np.stack([flav, np.full(nA, nfl)], axis=1).astype(np.int32)
+    fk_h = rng.standard_normal((N, nx, nx, nA)); fk_h[:, :, 0, :] = fk_dis
+    s_dis = K.fk_conv_dis(to_dev(fk_dis), flav, to_dev(f)).cpu().numpy()
+    s_had = K.fk_conv_hadronic(to_dev(fk_h), pairs, to_dev(f_ext)).cpu().numpy()
+    _, scale = O.dis(fk_dis, flav, f)
+    assert rel_err(s_had, s_dis, scale) <= TOL64
+
+
+# ------------------------------------------------------------------ exact arithmetic and determinism
+@pytest.mark.parametrize("shape", [(40, 12, 30, 1), (17, 25, 50, 3), (200, 9, 11, 5)])
+def test_exact_integer_inputs_are_bitwise_equal(K, shape):
+    N, nx, C, R = shape
+    case = synth.integer_hadronic_case(N, N, nx, C, R)
+    ref, _ = O.hadronic(case.fk, case.pairs, case.f)
+    dref, _ = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    fk_d, idx, tb, tp = _tables(K, case, K.FK_KIND_HADRONIC)
+    f_d, g_d = to_dev(case.f), to_dev(case.g)
+    for s in (K.fk_conv_hadronic(fk_d, idx, f_d), tb.conv(f_d), tp.conv(f_d)):
+        assert np.array_equal(s.cpu().numpy(), ref)
+    for d in (K.fk_conv_hadronic_vjp(fk_d, idx, f_d, g_d), tb.vjp(f_d, g_d), tp.vjp(f_d, g_d)):
+        assert np.array_equal(d.cpu().numpy(), dref)
+
+
+def test_bitwise_repeatable_runs(K):
+    case = synth.hadronic_case(6, 96, 30, 37, 2, sub=1)
+    fk_d, idx, tb, tp = _tables(K, case, K.FK_KIND_HADRONIC)
+    f_d, g_d = to_dev(case.f), to_dev(case.g)
+    s0 = tp.conv(f_d).cpu().numpy(); d0 = tp.vjp(f_d, g_d).cpu().numpy()
+    for _ in range(10):
+        assert np.array_equal(tp.conv(f_d).cpu().numpy(), s0)
+        assert np.array_equal(tp.vjp(f_d, g_d).cpu().numpy(), d0)
+
+
+def test_replica_independence(K):
+    """Column r of a batched call equals the R=1 call on replica r (within tolerance)."""
+    case = synth.hadronic_case(6, 50, 20, 25, 7, sub=2)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    fk_d = to_dev(case.fk)
+    batched = K.fk_conv_hadronic(fk_d, case.pairs, to_dev(case.f)).cpu().numpy()
+    for r in range(case.R):
+        one = K.fk_conv_hadronic(fk_d, case.pairs, to_dev(case.f[r:r + 1])).cpu().numpy()
+        assert rel_err(one[:, 0], batched[:, r], scale[:, r]) <= 2 * TOL64
+
+
+# ------------------------------------------------------------------ fp32 variant
+@pytest.mark.parametrize("R", [1, 4])
+def test_fp32_variant(K, R):
+    import torch
+    case = synth.hadronic_case(3, 64, 30, 40, R, sub=4)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)       # fp64 oracle of the fp64 inputs
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    f32 = torch.float32
+    fk_d = to_dev(case.fk)
+    s = K.fk_conv_hadronic(fk_d.to(f32), case.pairs, to_dev(case.f, f32))
+    assert s.dtype == f32 and rel_err(s.cpu().numpy(), ref, scale) <= TOL32
+    d = K.fk_conv_hadronic_vjp(fk_d.to(f32), case.pairs, to_dev(case.f, f32), to_dev(case.g, f32))
+    assert rel_err(d.cpu().numpy(), dref, D) <= TOL32
+    tp = K.FkTable(K.FK_KIND_HADRONIC, fk_d, case.pairs, case.nfl, K.FK_F32, K.FK_STORE_PACK)
+    s2 = tp.conv(to_dev(case.f, f32))
+    assert s2.dtype == f32 and rel_err(s2.cpu().numpy(), ref, scale) <= TOL32
+    d2 = tp.vjp(to_dev(case.f, f32), to_dev(case.g, f32))
+    assert rel_err(d2.cpu().numpy(), dref, D) <= TOL32
+
+
+# ------------------------------------------------------------------ host-buffer calls
+def test_host_buffer_calls(K):
+    case = synth.hadronic_case(6, 48, 20, 30, 2, sub=5)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    tp = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl)
+    sig = np.empty((case.N, case.R)); df = np.empty_like(case.f)
+    tp.conv_host(case.f, sig)
+    tp.vjp_host(case.f, case.g, df)
+    assert rel_err(sig, ref, scale) <= TOL64
+    assert rel_err(df, dref, D) <= TOL64
+    assert tp.last_launches() >= 2
+
+
+# ------------------------------------------------------------------ grouped ragged launch
+@pytest.mark.parametrize("R", [1, 3])
+@pytest.mark.parametrize("store", ["pack", "borrow"])
+def test_grouped_small_ragged(K, R, store):
+    import torch
+    shapes = synth.small_ragged_shapes(T=7)
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    cases = [synth.config4_table(t, shapes, R, params) for t in range(shapes.T)]
+    st = K.FK_STORE_PACK if store == "pack" else K.FK_STORE_BORROW
+    keep = [to_dev(c.fk) for c in cases]
+    tabs = [K.FkTable(K.FK_KIND_HADRONIC, keep[t], cases[t].pairs, cases[t].nfl, K.FK_F64, st) for t in range(shapes.T)]
+    grp = K.FkGroup(tabs, R_hint=R)
+    fo, so = grp.offsets(R)
+    f_cat = torch.cat([to_dev(c.f).reshape(-1) for c in cases])
+    g_cat = torch.cat([to_dev(c.g).reshape(-1) for c in cases])
+    assert f_cat.numel() == fo[-1] and g_cat.numel() == so[-1]
+    sig = grp.conv(f_cat, R).cpu().numpy()
+    df = grp.vjp(f_cat, g_cat, R).cpu().numpy()
+    for t, c in enumerate(cases):
+        ref, scale = O.hadronic(c.fk, c.pairs, c.f)
+        dref, D = O.hadronic_vjp(c.fk, c.pairs, c.f, c.g)
+        assert rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale) <= TOL64, t
+        assert rel_err(df[fo[t]:fo[t + 1]].reshape(R, c.nfl, c.nx), dref, D) <= TOL64, t
+    # repeatable
+    assert np.array_equal(grp.conv(f_cat, R).cpu().numpy(), sig)
+    assert np.array_equal(grp.vjp(f_cat, g_cat, R).cpu().numpy(), df)
+    assert grp.last_launches() >= 2
+
+
+def test_grouped_mixed_dis_and_hadronic(K):
+    """A 'global' group: DIS and hadronic tables in one launch."""
+    import torch
+    R = 2
+    h = synth.hadronic_case(6, 30, 12, 17, R, sub=7)
+    d = synth.config1(R=R, N=200)
+    th = K.FkTable(K.FK_KIND_HADRONIC, to_dev(h.fk), h.pairs, h.nfl)
+    td = K.FkTable(K.FK_KIND_DIS, to_dev(d.fk), d.flav, d.nfl)
+    grp = K.FkGroup([th, td], R_hint=R)
+    fo, so = grp.offsets(R)
+    f_cat = torch.cat([to_dev(h.f).reshape(-1), to_dev(d.f).reshape(-1)])
+    g_cat = torch.cat([to_dev(h.g).reshape(-1), to_dev(d.g).reshape(-1)])
+    sig = grp.conv(f_cat, R).cpu().numpy()
+    df = grp.vjp(f_cat, g_cat, R).cpu().numpy()
+    ref_h, sc_h = O.hadronic(h.fk, h.pairs, h.f); ref_d, sc_d = O.dis(d.fk, d.flav, d.f)
+    assert rel_err(sig[so[0]:so[1]].reshape(h.N, R), ref_h, sc_h) <= TOL64
+    assert rel_err(sig[so[1]:so[2]].reshape(d.N, R), ref_d, sc_d) <= TOL64
+    dref_h, D_h = O.hadronic_vjp(h.fk, h.pairs, h.f, h.g); dref_d, D_d = O.dis_vjp(d.fk, d.flav, d.f, d.g)
+    assert rel_err(df[fo[0]:fo[1]].reshape(R, h.nfl, h.nx), dref_h, D_h) <= TOL64
+    assert rel_err(df[fo[1]:fo[2]].reshape(R, d.nfl, d.nx), dref_d, D_d) <= TOL64
+
+
+# ------------------------------------------------------------------ error paths on a live device
+def test_error_paths_on_device(K):
+    case = synth.hadronic_case(6, 4, 5, 3, 1, sub=9)
+    fk_d, f_d = to_dev(case.fk), to_dev(case.f)
+    bad = case.pairs.copy(); bad[1, 0] = case.nfl
+    with pytest.raises(K.FkError) as e:
+        K.fk_conv_hadronic(fk_d, bad, f_d)
+    assert e.value.code == K.FK_ERR_INVALID_ARG
+    with pytest.raises(K.FkError):
+        K.FkTable(K.FK_KIND_HADRONIC, fk_d, bad, case.nfl)
+    with pytest.raises(K.FkError):
+        K.FkTable(K.FK_KIND_HADRONIC, fk_d, case.pairs, case.nfl, K.FK_F32, K.FK_STORE_BORROW)
