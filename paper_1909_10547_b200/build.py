@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfkconv.so")
 SOURCES = ["fk_api.cu"]
-DEPS = ["fk_api.cu", "fk_group.inl", "fk_common.cuh", "fk_stream.cuh", "fk_vjp.cuh", "fk_gemm.cuh", "fk_pack.cuh"]
+DEPS = ["fk_api.cu", "fk_group.inl", "fk_common.cuh", "fk_fwd.cuh", "fk_vjp.cuh", "fk_gemm.cuh", "fk_pack.cuh"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -47,6 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [_nvcc(), *NVCC_FLAGS]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("FKCONV_NVCC_FLAGS", "").split()  # e.g. -DFK_BULK_DEPTH=4 for tuning builds
     cmd += ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd, cwd=CSRC)
     os.replace(tmp, LIB)

@@ -20,7 +20,7 @@
 #include "fk_common.cuh"
 #include "fk_gemm.cuh"
 #include "fk_pack.cuh"
-#include "fk_stream.cuh"
+#include "fk_fwd.cuh"
 #include "fk_vjp.cuh"
 
 namespace {
@@ -64,21 +64,6 @@ int sm_count() {
     return n;
 }
 
-// resident CTAs per SM of a kernel instantiation (cached)
-int ctas_per_sm(const void* func, int threads, size_t smem) {
-    static std::mutex mu;
-    static std::map<std::pair<const void*, size_t>, int> cache;
-    std::lock_guard<std::mutex> lk(mu);
-    auto key = std::make_pair(func, smem);
-    auto it = cache.find(key);
-    if (it != cache.end()) return it->second;
-    if (smem > 48 * 1024) cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, func, threads, smem) != cudaSuccess || n < 1) n = 1;
-    cache[key] = n;
-    return n;
-}
-
 // ---- kernel timing hook (fk_profile_enable / fk_profile_read) ----
 struct Profiler {
     std::mutex mu;
@@ -111,39 +96,42 @@ size_t dtype_size(int dtype) { return dtype == FK_F64 ? 8 : 4; }
 // ------------------------------------------------------------------------------------------------
 // plans
 // ------------------------------------------------------------------------------------------------
+// Both bandwidth-bound kernels (forward, VJP stage 1) cut a table into CTAs of one k-block
+// (256 * VEC consecutive k: 4 KB of every row) times one datapoint range.
 struct Plan {
-    int kc = 0;       // forward stream: chunk length (elements)
-    int nchunks = 0;  // forward stream: chunks per row
-    int nsplit = 0;   // VJP stage 1: datapoint splits
-    int nkb = 0;      // VJP stage 1: k-blocks
+    int nkb = 0;      // k-blocks per row
+    int fsplit = 0;   // forward: datapoint ranges
+    int nsplit = 0;   // VJP stage 1: datapoint ranges
     int gsplit = 0;   // forward GEMM: K-splits
 };
 
-constexpr int STREAM_UNROLL = 4;
-
-template <typename T> int stream_chunk_unit(int vec) { return 32 * vec * STREAM_UNROLL; }
+constexpr int FWD_U = 8;  // rows in flight per thread of the forward column kernel
 
 void make_plan(fk::TableDesc& d, int dtype, Plan& pl) {
     const int vecw = dtype == FK_F64 ? 2 : 4;
-    const int unit = 32 * vecw * STREAM_UNROLL;  // also valid for the VEC = 1 path (multiple of 32*UNROLL)
-    int kc_default = env_int("FKCONV_KC", dtype == FK_F64 ? 1024 : 2048);
-    kc_default = std::max(unit, kc_default / unit * unit);
-    const int kround = (d.K + unit - 1) / unit * unit;
-    pl.kc = std::min(kc_default, kround);
-    pl.nchunks = (d.K + pl.kc - 1) / pl.kc;
-    d.nchunks = pl.nchunks;
-    d.kc = pl.kc;
-
     const int vec = d.vec_ok ? vecw : 1;
-    pl.nkb = (d.K + fk::COLSUM_THREADS * vec - 1) / (fk::COLSUM_THREADS * vec);
+    pl.nkb = (d.K + fk::FWD_THREADS * vec - 1) / (fk::FWD_THREADS * vec);
     const int sms = std::max(1, sm_count());
+
+    // forward: ~32 datapoints per CTA (finer for small tables so that the grid still covers the GPU a few
+    // times over), never fewer than one batch of FWD_U rows
+    int rows = env_int("FKCONV_FWD_ROWS", 32);
+    const long long want_f = (long long)env_int("FKCONV_FWD_MIN_CTAS_PER_SM", 8) * sms;
+    while (rows > FWD_U && (long long)pl.nkb * ((d.N + rows - 1) / rows) < want_f) rows /= 2;
+    rows = std::max(rows, 1);
+    pl.fsplit = std::max(1, std::min(d.N, (d.N + rows - 1) / rows));
+
+    // VJP stage 1: fewer, longer ranges (every range writes K column sums that stage 2 adds up)
     const int want = env_int("FKCONV_COLSUM_CTAS_PER_SM", 24) * sms;  // CTAs wanted for stage 1
     int nsplit = (want + pl.nkb - 1) / pl.nkb;
     nsplit = std::min(nsplit, std::max(1, d.N / 16));                  // >= 16 datapoints per split
     nsplit = std::max(nsplit, (d.N + fk::COLSUM_MAX_ROWS - 1) / fk::COLSUM_MAX_ROWS);
     nsplit = std::max(1, std::min(nsplit, d.N));
     pl.nsplit = nsplit;
-    d.nsplit = nsplit;
+
+    d.nchunks = pl.nkb;
+    d.fsplit = pl.fsplit;
+    d.nsplit = pl.nsplit;
 }
 
 size_t part_elems_per_replica(const fk::TableDesc& d) { return d.nchunks > 1 ? (size_t)d.N * d.nchunks : 0; }
@@ -196,62 +184,20 @@ fk::TableDesc make_desc(int kind, int layout, const void* fkp, int N, int nx, in
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
-template <int RT> struct StreamShape;  // rows per warp, by replica tile
-template <> struct StreamShape<1> { static constexpr int RPW = 2; };
-template <> struct StreamShape<2> { static constexpr int RPW = 2; };
-template <> struct StreamShape<4> { static constexpr int RPW = 1; };
-
-template <typename T, int VEC, int RT, bool GROUPED>
-const void* stream_func() {
-    return (const void*)fk::fk_stream_kernel<T, VEC, RT, StreamShape<RT>::RPW, STREAM_UNROLL, GROUPED>;
-}
-
-template <typename T, int VEC, int RT, bool GROUPED>
-int stream_grid_for(int kc, long long units) {
-    const size_t smem = (size_t)RT * kc * sizeof(T);
-    const int occ = ctas_per_sm(stream_func<T, VEC, RT, GROUPED>(), fk::STREAM_THREADS, smem);
-    const int cap = env_int("FKCONV_STREAM_CTAS_PER_SM", 0);
-    const int per_sm = cap > 0 ? std::min(cap, occ) : occ;
-    const long long by_work = (units + 8 * StreamShape<RT>::RPW - 1) / (8 * StreamShape<RT>::RPW);
-    return (int)std::max(1LL, std::min<long long>((long long)sm_count() * per_sm, by_work));
-}
-
-template <typename T, int VEC, int RT, bool GROUPED>
-cudaError_t launch_stream(const fk::StreamParams& p, int grid, cudaStream_t s) {
-    const size_t smem = (size_t)RT * p.kc_stride * sizeof(T);
-    ctas_per_sm(stream_func<T, VEC, RT, GROUPED>(), fk::STREAM_THREADS, smem);  // sets the smem attribute if needed
-    fk::fk_stream_kernel<T, VEC, RT, StreamShape<RT>::RPW, STREAM_UNROLL, GROUPED>
-        <<<grid, fk::STREAM_THREADS, smem, s>>>(p);
-    return cudaGetLastError();
-}
-
 // picks the replica tile for a pass starting at r0
 inline int pick_rt(int remaining) { return remaining >= 3 ? 4 : remaining; }
 
 template <typename T, bool GROUPED>
-int stream_grid(bool vec_ok, int rt, int kc, long long units) {
+cudaError_t fwd_dispatch(bool vec_ok, int rt, const fk::FwdParams& p, int grid, cudaStream_t s) {
     constexpr int VW = fk::VecWidth<T>::value;
+#define FK_FWD(V, RTv) fk::fk_fwd_column_kernel<T, V, RTv, FWD_U, GROUPED><<<grid, fk::FWD_THREADS, 0, s>>>(p)
     if (vec_ok) {
-        if (rt == 1) return stream_grid_for<T, VW, 1, GROUPED>(kc, units);
-        if (rt == 2) return stream_grid_for<T, VW, 2, GROUPED>(kc, units);
-        return stream_grid_for<T, VW, 4, GROUPED>(kc, units);
+        if (rt == 1) FK_FWD(VW, 1); else if (rt == 2) FK_FWD(VW, 2); else FK_FWD(VW, 4);
+    } else {
+        if (rt == 1) FK_FWD(1, 1); else if (rt == 2) FK_FWD(1, 2); else FK_FWD(1, 4);
     }
-    if (rt == 1) return stream_grid_for<T, 1, 1, GROUPED>(kc, units);
-    if (rt == 2) return stream_grid_for<T, 1, 2, GROUPED>(kc, units);
-    return stream_grid_for<T, 1, 4, GROUPED>(kc, units);
-}
-
-template <typename T, bool GROUPED>
-cudaError_t stream_dispatch(bool vec_ok, int rt, const fk::StreamParams& p, int grid, cudaStream_t s) {
-    constexpr int VW = fk::VecWidth<T>::value;
-    if (vec_ok) {
-        if (rt == 1) return launch_stream<T, VW, 1, GROUPED>(p, grid, s);
-        if (rt == 2) return launch_stream<T, VW, 2, GROUPED>(p, grid, s);
-        return launch_stream<T, VW, 4, GROUPED>(p, grid, s);
-    }
-    if (rt == 1) return launch_stream<T, 1, 1, GROUPED>(p, grid, s);
-    if (rt == 2) return launch_stream<T, 1, 2, GROUPED>(p, grid, s);
-    return launch_stream<T, 1, 4, GROUPED>(p, grid, s);
+#undef FK_FWD
+    return cudaGetLastError();
 }
 
 template <typename T, bool GROUPED>
@@ -279,29 +225,27 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
         if (launches) *launches = nl;
         return FK_OK;
     }
-    fk::StreamParams p;
+    fk::FwdParams p;
     memset(&p, 0, sizeof p);
     p.desc = d;
     p.chan = ch;
     p.f = f;
     p.part = part;
     p.sigma = sigma;
-    p.units = (long long)pl.nchunks * d.N;
     p.R = R;
-    p.kc_stride = pl.kc;
+    const int fgrid = pl.nkb * pl.fsplit;
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
-        const int grid = stream_grid<T, false>(d.vec_ok, rt, pl.kc, p.units);
         size_t slot = 0;
         const bool timed = r0 == 0 && g_prof.begin(s, slot);
-        cudaError_t e = stream_dispatch<T, false>(d.vec_ok, rt, p, grid, s);
+        cudaError_t e = fwd_dispatch<T, false>(d.vec_ok, rt, p, fgrid, s);
         if (timed) g_prof.end(s, slot);
-        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "stream kernel launch failed: %s", cudaGetErrorString(e));
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "forward kernel launch failed: %s", cudaGetErrorString(e));
         ++nl;
         r0 += rt;
     }
-    if (pl.nchunks > 1) {
+    if (pl.nkb > 1) {
         fk::ReduceParams q;
         memset(&q, 0, sizeof q);
         q.desc = d;

@@ -37,9 +37,14 @@ struct TableDesc {
     long long out_off;       // element offset of sigma_t / g_t inside sigma_cat for R = 1 (scaled by R)
     long long part_off;      // element offset of this table's level-1 partials for R = 1 (scaled by R)
     long long g_off;         // element offset of this table's column sums G for R = 1 (scaled by R)
-    int nchunks;             // forward: number of K-chunks
-    int nsplit;              // VJP stage 1: number of datapoint splits
-    int kc;                  // forward: chunk length in elements (multiple of 32*VEC*UNROLL)
+    int nchunks;             // forward: number of k-blocks (= level-1 partials per row)
+    int fsplit;              // forward: number of datapoint ranges per k-block
+    int nsplit;              // VJP stage 1: number of datapoint ranges per k-block
+};
+
+// Work list entry of the column kernels (forward and VJP stage 1): one CTA = one (k-block, datapoint range).
+struct ColSeg {
+    int table, kblock, split, pad_;
 };
 
 // Offsets (inside one replica's f[nfl][nx]) of the two PDF factors of contraction index k.

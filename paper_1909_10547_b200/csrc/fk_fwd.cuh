@@ -1,0 +1,196 @@
+// fk_fwd.cuh -- bandwidth-bound forward path (R <= 4 per pass).
+//
+//   sigma[n][r] = sum_k FK[n][k] * L[k][r],   L[k][r] = f[r][a_c][i] * f[r][b_c][j]      Eq. (1)
+//
+// "Column" decomposition, chosen from the read-pattern measurements in profiles/r01_read_patterns.md:
+// a CTA owns a block of FWD_THREADS * VEC consecutive k (4 KB of every row) and a range of datapoints.
+//   a1  each thread keeps the luminosity of ITS k (VEC values per replica) in registers for the whole
+//       CTA: the luminosity is built once per CTA straight from f and never touches HBM;
+//   a2  the CTA walks down its datapoints U rows at a time: U independent, fully coalesced 128-bit
+//       no-allocate loads per thread are in flight (the CTA reads U x 4 KB contiguous pieces), each
+//       FK element is multiplied by the thread's L values -- per-thread chains are VEC FMAs long;
+//   a3  level 1: the U row sums of a warp are folded together in one multi-value xor-butterfly
+//       (U-1 + log2(32/U) shuffles for U rows), the 8 warp results are added in a fixed order through
+//       shared memory -> ONE partial per (row, k-block); level 2: fk_reduce_chunks_kernel adds the
+//       k-blocks of a row in a fixed order.  No atomics anywhere: results are bitwise repeatable.
+// The grid is the list of (k-block, datapoint range) pairs -- for a grouped launch the host-built list
+// over all tables -- several waves of small CTAs that the hardware scheduler balances.
+#pragma once
+
+#include "fk_common.cuh"
+
+namespace fk {
+
+struct FwdParams {
+    TableDesc desc;           // single-table launch
+    ChannelList chan;         // single-table launch
+    const TableDesc* descs;   // grouped launch (device)
+    const ColSeg* segs;       // grouped launch (device), one per CTA
+    const void* f;            // f[R][nfl][nx] or f_cat
+    double* part;             // level-1 partials [row][replica][k-block]
+    void* sigma;              // direct output for tables with a single k-block
+    int R, r0;                // replicas, first replica of this pass
+};
+
+constexpr int FWD_THREADS = 256;
+constexpr int FWD_WARPS = FWD_THREADS / 32;
+
+// Folds U per-lane values (one per row) across the warp: afterwards lane l holds the warp total of
+// row l >> (5 - log2 U).  Fixed tree; a+b and b+a give the same bits, so every lane agrees.
+template <int U>
+__device__ __forceinline__ double fold_rows(double (&p)[U], int lane) {
+    int off = 16;
+#pragma unroll
+    for (int n = U; n > 1; n >>= 1, off >>= 1) {
+        const bool hi = (lane & off) != 0;
+#pragma unroll
+        for (int i = 0; i < n / 2; ++i) {
+            const double send = hi ? p[i] : p[i + n / 2];
+            const double keep = hi ? p[i + n / 2] : p[i];
+            p[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+        }
+    }
+    double s = p[0];
+#pragma unroll
+    for (; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    return s;
+}
+
+template <typename T, int VEC, int RT, int U, bool GROUPED>
+__global__ void __launch_bounds__(FWD_THREADS)
+fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
+    using V = Vec<T, VEC>;
+    constexpr int LPR = 32 / U;  // lanes that end up holding the same row
+    __shared__ double red[2][FWD_WARPS][U][RT];
+
+    const TableDesc* dp = &p.desc;
+    const uint8_t* __restrict__ ca = p.chan.a;
+    const uint8_t* __restrict__ cb = p.chan.b;
+    int kblock, split;
+    if constexpr (GROUPED) {
+        const ColSeg sg = p.segs[blockIdx.x];
+        dp = &p.descs[sg.table];
+        ca = dp->chan_a;
+        cb = dp->chan_b;
+        kblock = sg.kblock;
+        split = sg.split;
+    } else {
+        kblock = blockIdx.x % p.desc.nchunks;
+        split = blockIdx.x / p.desc.nchunks;
+    }
+    const TableDesc& d = *dp;
+    const int R = p.R;
+    const int rb = (int)((long long)d.N * split / d.fsplit);
+    const int re = (int)((long long)d.N * (split + 1) / d.fsplit);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    // a1: this thread's luminosity values
+    const int k = (kblock * FWD_THREADS + threadIdx.x) * VEC;
+    const bool kin = k < d.K;  // VEC > 1: rows are padded to a multiple of VEC, so the whole vector is readable
+    T L[RT][VEC];
+    {
+        const int fstride = d.nfl * d.nx;
+        const T* __restrict__ f = reinterpret_cast<const T*>(p.f) + d.f_off * R;
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) {
+            int ia = 0, ib = -1;
+            const bool in = k + e < d.K;
+            if (in) decode_k(d, ca, cb, k + e, ia, ib);
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                const int rr = p.r0 + r;
+                T l = T(0);
+                if (in && rr < R) {
+                    l = __ldg(f + (long long)rr * fstride + ia);
+                    if (ib >= 0) l *= __ldg(f + (long long)rr * fstride + ib);
+                }
+                L[r][e] = l;
+            }
+        }
+    }
+    const T* __restrict__ col = reinterpret_cast<const T*>(d.fk) + (kin ? k : 0);
+
+    int buf = 0;
+    for (int m = rb; m < re; m += U, buf ^= 1) {
+        // a2: U rows in flight
+        V x[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) x[u] = ld_stream(col + (long long)min(m + u, re - 1) * d.row_stride, (V*)nullptr);
+        double pr[RT][U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const bool live = kin && (m + u < re);
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                T s = x[u].v[0] * L[r][0];
+#pragma unroll
+                for (int e = 1; e < VEC; ++e) s = fma(x[u].v[e], L[r][e], s);
+                pr[r][u] = live ? (double)s : 0.0;
+            }
+        }
+        // a3 level 1: warp fold, then the 8 warps in a fixed order
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const double s = fold_rows<U>(pr[r], lane);
+            if ((lane & (LPR - 1)) == 0) red[buf][warp][lane / LPR][r] = s;
+        }
+        __syncthreads();
+        if (threadIdx.x < U * RT) {
+            const int u = threadIdx.x / RT, r = threadIdx.x - u * RT;
+            double s = red[buf][0][u][r];
+#pragma unroll
+            for (int w = 1; w < FWD_WARPS; ++w) s += red[buf][w][u][r];
+            const int n = m + u, rr = p.r0 + r;
+            if (n < re && rr < R) {
+                if (d.nchunks == 1)
+                    reinterpret_cast<T*>(p.sigma)[d.out_off * R + (long long)n * R + rr] = (T)s;
+                else
+                    p.part[d.part_off * R + ((long long)n * R + rr) * d.nchunks + kblock] = s;
+            }
+        }
+    }
+}
+
+// ---- a3 level 2: sigma[n][r] = sum over k-blocks, fixed order (lane-strided chains + butterfly) ----
+struct ReduceParams {
+    TableDesc desc;           // single
+    const TableDesc* descs;   // grouped (device)
+    const int* row_prefix;    // grouped (device) [T+1]: first global row of each table
+    int T;
+    const double* part;
+    void* sigma;
+    long long rows;           // total rows (single: N)
+    int R;
+};
+
+template <typename T, bool GROUPED>
+__global__ void __launch_bounds__(256) fk_reduce_chunks_kernel(const __grid_constant__ ReduceParams p) {
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    const long long total = p.rows * p.R;
+    for (long long o = warp0; o < total; o += nwarps) {
+        const long long grow = o / p.R;
+        const int r = (int)(o - grow * p.R);
+        const TableDesc* d = &p.desc;
+        long long n = grow;
+        if constexpr (GROUPED) {
+            int lo = 0, hi = p.T;  // last table with row_prefix[t] <= grow
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (p.row_prefix[mid] <= grow) lo = mid; else hi = mid;
+            }
+            d = &p.descs[lo];
+            n = grow - p.row_prefix[lo];
+        }
+        const int nch = d->nchunks;
+        if (nch == 1) continue;  // written directly by the column kernel
+        const double* src = p.part + d->part_off * p.R + (n * p.R + r) * nch;
+        double s = 0.0;
+        for (int c = lane; c < nch; c += 32) s += src[c];
+        s = warp_sum(s);
+        if (lane == 0) reinterpret_cast<T*>(p.sigma)[d->out_off * p.R + n * p.R + r] = (T)s;
+    }
+}
+
+}  // namespace fk

@@ -1,23 +1,23 @@
 // fk_group.inl -- ragged grouped launch; included at the end of fk_api.cu.
 // A global fit convolves many tables of different (N, nx, C) every iteration.  The
-// host builds, once, a static work list balanced by bytes; a forward pass is then ONE persistent
-// stream launch (+ one level-2 reduce) over all tables, a VJP pass one column-sum launch + one
-// gather launch.  Reduction order is fixed by the list, so results are bitwise repeatable.
+// host builds, once, static work lists of (table, k-block, datapoint range) CTAs; a forward pass is
+// then ONE column-kernel launch (+ one level-2 reduce) over all tables, a VJP pass one column-sum
+// launch + one gather launch; the hardware CTA scheduler balances the ragged list.  Every partial has
+// a fixed slot and every sum a fixed order, so results are bitwise repeatable.
 
 struct fk_group {
     std::vector<fk_table*> tables;
     std::vector<fk::TableDesc> descs;  // host copies with the concatenation offsets filled in
     int T = 0, dtype = FK_F64;
     bool all_vec = true;
-    int kc_max = 0;
     long long rows_total = 0, ai_total = 0, f_total1 = 0, part_total1 = 0, G_total1 = 0, elems_total = 0;
     fk::TableDesc* d_descs = nullptr;
     int* d_row_prefix = nullptr;
     int* d_ai_prefix = nullptr;
-    fk::ColsumSeg* d_csegs = nullptr;
+    fk::ColSeg* d_fsegs = nullptr;  // forward CTAs: (table, k-block, datapoint range)
+    int nfsegs = 0;
+    fk::ColSeg* d_csegs = nullptr;  // VJP stage-1 CTAs
     int ncsegs = 0;
-    struct WorkList { fk::Segment* d_segs = nullptr; int* d_cta_start = nullptr; int nsegs = 0; };
-    std::map<int, WorkList> worklists;  // by grid size
     double* scratch = nullptr;
     size_t scratch_elems = 0;
     int last_launches = 0;
@@ -35,69 +35,24 @@ int group_scratch(fk_group* g, size_t elems) {
     return FK_OK;
 }
 
-// Static forward work list for a grid of `G` CTAs: (table, chunk) row ranges, cut so that every CTA
-// streams the same number of FK elements (+- one row of one chunk).
-int group_worklist(fk_group* g, int G, fk_group::WorkList** out) {
-    auto it = g->worklists.find(G);
-    if (it != g->worklists.end()) { *out = &it->second; return FK_OK; }
-    std::vector<fk::Segment> segs;
-    std::vector<int> start(G + 1, 0);
-    const double quota = (double)g->elems_total / G;
-    double done = 0.0;
-    int cta = 0;
-    for (int t = 0; t < g->T; ++t) {
-        const fk::TableDesc& d = g->descs[t];
-        for (int chunk = 0; chunk < d.nchunks; ++chunk) {
-            const int klen = std::min(d.kc, d.K - chunk * d.kc);
-            int r = 0;
-            while (r < d.N) {
-                const double room = quota * (cta + 1) - done;
-                int take = (int)std::ceil(room / klen - 1e-9);
-                take = std::max(1, std::min(take, d.N - r));
-                segs.push_back(fk::Segment{t, chunk, r, r + take});
-                done += (double)take * klen;
-                r += take;
-                while (cta + 1 < G && done >= quota * (cta + 1) - 0.5) start[++cta] = (int)segs.size();
-            }
-        }
-    }
-    for (int c = cta + 1; c <= G; ++c) start[c] = (int)segs.size();
-    fk_group::WorkList wl;
-    wl.nsegs = (int)segs.size();
-    FK_CUDA(cudaMalloc((void**)&wl.d_segs, segs.size() * sizeof(fk::Segment)));
-    FK_CUDA(cudaMalloc((void**)&wl.d_cta_start, start.size() * sizeof(int)));
-    FK_CUDA(cudaMemcpy(wl.d_segs, segs.data(), segs.size() * sizeof(fk::Segment), cudaMemcpyHostToDevice));
-    FK_CUDA(cudaMemcpy(wl.d_cta_start, start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice));
-    auto ins = g->worklists.emplace(G, wl);
-    *out = &ins.first->second;
-    return FK_OK;
-}
-
 template <typename T>
 int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStream_t s) {
     int rc = group_scratch(g, std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * R);
     if (rc) return rc;
     int nl = 0;
-    fk::StreamParams p;
+    fk::FwdParams p;
     memset(&p, 0, sizeof p);
     p.descs = g->d_descs;
+    p.segs = g->d_fsegs;
     p.f = f_cat;
     p.part = g->scratch;
     p.sigma = sigma_cat;
     p.R = R;
-    p.kc_stride = g->kc_max;
-    const long long units = (g->elems_total + g->kc_max - 1) / g->kc_max;
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
-        const int grid = stream_grid<T, true>(g->all_vec, rt, g->kc_max, units);
-        fk_group::WorkList* wl = nullptr;
-        rc = group_worklist(g, grid, &wl);
-        if (rc) return rc;
-        p.segs = wl->d_segs;
-        p.cta_seg_start = wl->d_cta_start;
-        cudaError_t e = stream_dispatch<T, true>(g->all_vec, rt, p, grid, s);
-        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped stream launch failed: %s", cudaGetErrorString(e));
+        cudaError_t e = fwd_dispatch<T, true>(g->all_vec, rt, p, g->nfsegs, s);
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped forward launch failed: %s", cudaGetErrorString(e));
         ++nl;
         r0 += rt;
     }
@@ -175,11 +130,20 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     g->T = T;
     g->dtype = tables[0]->dtype;
     std::vector<int> row_prefix(T + 1, 0), ai_prefix(T + 1, 0);
-    std::vector<fk::ColsumSeg> csegs;
     for (int t = 0; t < T; ++t) {
         fk_table* tb = tables[t];
         if (tb->dtype != g->dtype) { delete g; return fail(FK_ERR_INVALID_ARG, "fk_group_create: mixed dtypes"); }
+        g->all_vec = g->all_vec && tb->desc.vec_ok;
+    }
+    std::vector<fk::ColSeg> fsegs, csegs;
+    for (int t = 0; t < T; ++t) {
+        fk_table* tb = tables[t];
         fk::TableDesc d = tb->desc;
+        if (!g->all_vec && d.vec_ok) {  // one kernel instantiation per launch: the whole group takes the 64-bit path
+            d.vec_ok = 0;
+            Plan pl;
+            make_plan(d, g->dtype, pl);
+        }
         d.f_off = g->f_total1;
         d.out_off = g->rows_total;
         d.part_off = g->part_total1;
@@ -190,12 +154,12 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
         g->part_total1 += (long long)part_elems_per_replica(d);
         g->G_total1 += (long long)G_elems_per_replica(d);
         g->elems_total += (long long)d.N * d.K;
-        g->all_vec = g->all_vec && d.vec_ok;
-        g->kc_max = std::max(g->kc_max, d.kc);
         row_prefix[t + 1] = (int)g->rows_total;
         ai_prefix[t + 1] = (int)g->ai_total;
+        for (int sp = 0; sp < d.fsplit; ++sp)
+            for (int kb = 0; kb < d.nchunks; ++kb) fsegs.push_back(fk::ColSeg{t, kb, sp, 0});
         for (int sp = 0; sp < d.nsplit; ++sp)
-            for (int kb = 0; kb < tb->plan.nkb; ++kb) csegs.push_back(fk::ColsumSeg{t, kb, sp, 0});
+            for (int kb = 0; kb < d.nchunks; ++kb) csegs.push_back(fk::ColSeg{t, kb, sp, 0});
         g->tables.push_back(tb);
         g->descs.push_back(d);
     }
@@ -203,26 +167,19 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
         delete g;
         return fail(FK_ERR_UNSUPPORTED, "fk_group_create: more than 2^31 datapoints or PDF slots");
     }
-    if (!g->all_vec) {
-        // the VEC = 1 kernels index k-blocks of COLSUM_THREADS elements: rebuild the stage-1 list accordingly
-        csegs.clear();
-        for (int t = 0; t < T; ++t) {
-            const fk::TableDesc& d = g->descs[t];
-            const int nkb = (d.K + fk::COLSUM_THREADS - 1) / fk::COLSUM_THREADS;
-            for (int sp = 0; sp < d.nsplit; ++sp)
-                for (int kb = 0; kb < nkb; ++kb) csegs.push_back(fk::ColsumSeg{t, kb, sp, 0});
-        }
-    }
+    g->nfsegs = (int)fsegs.size();
     g->ncsegs = (int)csegs.size();
     auto bail = [&](int code) { fk_group_destroy(g); return code; };
     cudaError_t e = cudaMalloc((void**)&g->d_descs, T * sizeof(fk::TableDesc));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_row_prefix, (T + 1) * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_ai_prefix, (T + 1) * sizeof(int));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_csegs, csegs.size() * sizeof(fk::ColsumSeg));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_csegs, csegs.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_fsegs, fsegs.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_fsegs, fsegs.data(), fsegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_descs, g->descs.data(), T * sizeof(fk::TableDesc), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_row_prefix, row_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_ai_prefix, ai_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(g->d_csegs, csegs.data(), csegs.size() * sizeof(fk::ColsumSeg), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_csegs, csegs.data(), csegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_group_create: %s", cudaGetErrorString(e)); }
     int rc = group_scratch(g, std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * std::max(1, R_hint));
     if (rc) return bail(rc);
@@ -236,10 +193,7 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_row_prefix) cudaFree(g->d_row_prefix);
     if (g->d_ai_prefix) cudaFree(g->d_ai_prefix);
     if (g->d_csegs) cudaFree(g->d_csegs);
-    for (auto& kv : g->worklists) {
-        if (kv.second.d_segs) cudaFree(kv.second.d_segs);
-        if (kv.second.d_cta_start) cudaFree(kv.second.d_cta_start);
-    }
+    if (g->d_fsegs) cudaFree(g->d_fsegs);
     if (g->scratch) cudaFree(g->scratch);
     delete g;
     return FK_OK;

@@ -16,14 +16,10 @@
 
 namespace fk {
 
-struct ColsumSeg {  // grouped work list entry
-    int table, kblock, split, pad_;
-};
-
 struct ColsumParams {
     TableDesc desc;           // single-table launch
     const TableDesc* descs;   // grouped (device)
-    const ColsumSeg* segs;    // grouped (device), one per CTA
+    const ColSeg* segs;    // grouped (device), one per CTA
     const void* g;            // g[N][R] or g_cat
     double* G;                // [nsplit][R][K] per table
     int R, r0;
@@ -43,7 +39,7 @@ fk_colsum_kernel(const __grid_constant__ ColsumParams p) {
     const TableDesc* dp = &p.desc;
     int kblock, split;
     if constexpr (GROUPED) {
-        const ColsumSeg sg = p.segs[blockIdx.x];
+        const ColSeg sg = p.segs[blockIdx.x];
         dp = &p.descs[sg.table];
         kblock = sg.kblock;
         split = sg.split;
