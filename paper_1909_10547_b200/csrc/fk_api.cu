@@ -15,6 +15,7 @@
 #include <mutex>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "fk_common.cuh"
@@ -102,7 +103,6 @@ struct Plan {
     int nkb = 0;      // k-blocks per row
     int fsplit = 0;   // forward: datapoint ranges
     int nsplit = 0;   // VJP stage 1: datapoint ranges
-    int gsplit = 0;   // forward GEMM: K-splits
 };
 
 constexpr int FWD_U = 8;  // rows in flight per thread of the forward column kernel
@@ -214,16 +214,91 @@ cudaError_t colsum_dispatch(bool vec_ok, int rt, const fk::ColsumParams& p, int 
     return cudaGetLastError();
 }
 
+// ---- R >> 1: FP64 tensor-core contraction (fk_gemm.cuh) ---------------------------------------------
+struct GemmPlan {
+    int ksplit, kper, RPmax;
+};
+
+template <typename T>
+bool gemm_wanted(const fk::TableDesc& d, int R) {
+    if (dtype_of<T>() != FK_F64) return false;  // the fp32 variant stays on the FFMA column kernel (reading R18)
+    if ((long long)d.nfl * d.nx >= (long long)fk::KDEC_NONE) return false;
+    return R >= env_int("FKCONV_GEMM_MIN_R", 5);
+}
+
+GemmPlan gemm_plan(const fk::TableDesc& d, int R) {
+    GemmPlan gp;
+    const int mtiles = (d.N + fk::GEMM_BM - 1) / fk::GEMM_BM;
+    const int target = std::max(1, sm_count()) * std::max(1, env_int("FKCONV_GEMM_WAVES", 1));
+    int ksplit = std::max(1, target / mtiles);
+    gp.kper = ((d.K + ksplit - 1) / ksplit + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT;
+    gp.ksplit = (d.K + gp.kper - 1) / gp.kper;
+    gp.RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    return gp;
+}
+
+// doubles: fT [slots][RPmax] + level-1 partials [ksplit][N][RPmax] (+ k codes when the caller has none)
+size_t gemm_fwd_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
+    const GemmPlan gp = gemm_plan(d, R);
+    return (size_t)d.nfl * d.nx * gp.RPmax + (size_t)gp.ksplit * d.N * gp.RPmax + (with_kdec ? ((size_t)d.K + 1) / 2 : 0);
+}
+
+int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint32_t* kdec, const double* f,
+                  double* sigma, int R, double* scratch, cudaStream_t s, int* launches) {
+    const GemmPlan gp = gemm_plan(d, R);
+    const int slots = d.nfl * d.nx;
+    double* fT = scratch;
+    double* gpart = fT + (size_t)slots * gp.RPmax;
+    int nl = 0;
+    if (!kdec) {
+        uint32_t* kd = reinterpret_cast<uint32_t*>(gpart + (size_t)gp.ksplit * d.N * gp.RPmax);
+        fk::fk_kdec_kernel<<<std::min(1024, (d.K + 255) / 256), 256, 0, s>>>(d, ch, kd);
+        ++nl;
+        kdec = kd;
+    }
+    static const bool attr_ok = [] {
+        return cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess &&
+               cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess;
+    }();
+    if (!attr_ok) return fail(FK_ERR_CUDA, "gemm: cannot reserve %d bytes of shared memory", fk::GEMM_SMEM_BYTES);
+    const int mtiles = (d.N + fk::GEMM_BM - 1) / fk::GEMM_BM;
+    for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
+        fk::GemmFwdParams p;
+        memset(&p, 0, sizeof p);
+        p.desc = d;
+        p.kdec = kdec;
+        p.fT = fT;
+        p.gpart = gpart;
+        p.RP = (std::min(fk::GEMM_BN, R - r0) + 7) / 8 * 8;
+        p.nfrag = p.RP / 8;
+        p.nfw = (p.nfrag + 1) / 2;
+        p.ksplit = gp.ksplit;
+        p.kper = gp.kper;
+        const long long tot = (long long)slots * p.RP;
+        fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
+        size_t slot = 0;
+        const bool timed = r0 == 0 && g_prof.begin(s, slot);
+        if (d.vec_ok) fk::fk_gemm_fwd_kernel<2><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        else fk::fk_gemm_fwd_kernel<1><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        if (timed) g_prof.end(s, slot);
+        const long long outs = (long long)d.N * p.RP;
+        fk::fk_gemm_reduce_kernel<double><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
+            gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, gp.ksplit);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm forward launch failed: %s", cudaGetErrorString(e));
+        nl += 3;
+    }
+    if (launches) *launches = nl;
+    return FK_OK;
+}
+
 // One table, any R.  `part` holds >= part_elems_per_replica * R doubles (may be null if nchunks == 1).
 template <typename T>
-int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const T* f, T* sigma,
-                    int R, double* part, double* gemm_part, cudaStream_t s, int* launches) {
+int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const uint32_t* kdec,
+                    const T* f, T* sigma, int R, double* part, cudaStream_t s, int* launches) {
     int nl = 0;
-    if (fk::gemm_wanted(R)) {
-        int rc = fk::gemm_forward_single<T>(d, ch, f, sigma, R, gemm_part, pl.gsplit, s, &nl);
-        if (rc != 0) return fail(FK_ERR_CUDA, "gemm forward launch failed: %s", cudaGetErrorString((cudaError_t)rc));
-        if (launches) *launches = nl;
-        return FK_OK;
+    if constexpr (std::is_same<T, double>::value) {
+        if (gemm_wanted<T>(d, R)) return run_conv_gemm(d, ch, kdec, f, sigma, R, part, s, launches);
     }
     fk::FwdParams p;
     memset(&p, 0, sizeof p);
@@ -269,10 +344,7 @@ template <typename T>
 int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const T* f, const T* g, T* df,
                    int R, double* G, cudaStream_t s, int* launches) {
     int nl = 0;
-    if (fk::gemm_wanted(R)) {
-        int rc = fk::gemm_colsum_single<T>(d, g, G, R, s, &nl);
-        if (rc != 0) return fail(FK_ERR_CUDA, "gemm colsum launch failed: %s", cudaGetErrorString((cudaError_t)rc));
-    } else {
+    {
         fk::ColsumParams p;
         memset(&p, 0, sizeof p);
         p.desc = d;
@@ -292,7 +364,6 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
     fk::GatherParams q;
     memset(&q, 0, sizeof q);
     q.desc = d;
-    if (fk::gemm_wanted(R)) q.desc.nsplit = 1;  // the GEMM stage 1 writes a single, complete G
     q.chan = ch;
     q.f = f;
     q.G = G;
@@ -306,14 +377,12 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
     return FK_OK;
 }
 
-size_t conv_scratch_elems(const fk::TableDesc& d, const Plan& pl, int R) {
-    if (fk::gemm_wanted(R)) return fk::gemm_forward_scratch_elems(d, R, pl.gsplit);
+template <typename T>
+size_t conv_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
+    if (gemm_wanted<T>(d, R)) return gemm_fwd_scratch_elems(d, R, with_kdec);
     return part_elems_per_replica(d) * R;
 }
-size_t vjp_scratch_elems(const fk::TableDesc& d, int R) {
-    if (fk::gemm_wanted(R)) return (size_t)d.K * R;
-    return G_elems_per_replica(d) * R;
-}
+size_t vjp_scratch_elems(const fk::TableDesc& d, int R) { return G_elems_per_replica(d) * R; }
 
 // stateless front end shared by the fp64 / fp32 entry points
 template <typename T>
@@ -331,13 +400,12 @@ int stateless(const char* who, int kind, bool vjp, const T* fkp, const int32_t* 
     fk::TableDesc d = make_desc(kind, fk::LAYOUT_LOGICAL, fkp, N, nx, nfl, C, 0, dtype_of<T>());
     Plan pl;
     make_plan(d, dtype_of<T>(), pl);
-    pl.gsplit = fk::gemm_pick_split(d, R, sm_count());
     cudaStream_t s = (cudaStream_t)stream;
-    const size_t elems = vjp ? vjp_scratch_elems(d, R) : conv_scratch_elems(d, pl, R);
+    const size_t elems = vjp ? vjp_scratch_elems(d, R) : conv_scratch_elems<T>(d, R, true);
     double* scratch = nullptr;
     if (elems) FK_CUDA(cudaMallocAsync((void**)&scratch, elems * sizeof(double), s));
     rc = vjp ? run_vjp_single<T>(d, ch, pl, f, g, out, R, scratch, s, nullptr)
-             : run_conv_single<T>(d, ch, pl, f, out, R, scratch, scratch, s, nullptr);
+             : run_conv_single<T>(d, ch, pl, nullptr, f, out, R, scratch, s, nullptr);
     if (scratch) {
         cudaError_t e = cudaFreeAsync(scratch, s);
         if (rc == FK_OK && e != cudaSuccess) return fail(FK_ERR_CUDA, "cudaFreeAsync: %s", cudaGetErrorString(e));
@@ -357,6 +425,7 @@ struct fk_table {
     int dtype = FK_F64, store = FK_STORE_BORROW, kind = FK_KIND_HADRONIC;
     void* owned_fk = nullptr;
     uint8_t* dev_chan = nullptr;  // [2][C] for grouped launches
+    uint32_t* kdec = nullptr;     // [K] k -> (slot a, slot b) codes for the R >> 1 contraction
     double* scratch = nullptr;    // forward partials / VJP column sums (one buffer, used by one call at a time)
     size_t scratch_elems = 0;
     void* h_stage = nullptr;      // pinned host staging for the *_host calls
@@ -390,18 +459,16 @@ int ensure_stage(fk_table* t, size_t bytes) {
 }
 
 size_t table_scratch_need(const fk_table* t, int R) {
-    Plan pl = t->plan;
-    pl.gsplit = fk::gemm_pick_split(t->desc, R, sm_count());
-    return std::max(conv_scratch_elems(t->desc, pl, R), vjp_scratch_elems(t->desc, R));
+    const size_t conv = t->dtype == FK_F64 ? conv_scratch_elems<double>(t->desc, R, t->kdec == nullptr)
+                                           : conv_scratch_elems<float>(t->desc, R, true);
+    return std::max(conv, vjp_scratch_elems(t->desc, R));
 }
 
 template <typename T>
 int table_conv_t(fk_table* t, const void* f, void* sigma, int R, cudaStream_t s) {
-    Plan pl = t->plan;
-    pl.gsplit = fk::gemm_pick_split(t->desc, R, sm_count());
     int rc = ensure_scratch(t, table_scratch_need(t, R));
     if (rc) return rc;
-    return run_conv_single<T>(t->desc, t->chan, pl, (const T*)f, (T*)sigma, R, t->scratch, t->scratch, s,
+    return run_conv_single<T>(t->desc, t->chan, t->plan, t->kdec, (const T*)f, (T*)sigma, R, t->scratch, s,
                               &t->last_launches);
 }
 
@@ -530,6 +597,15 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
     if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: channel upload: %s", cudaGetErrorString(e)); }
     t->desc.chan_a = t->dev_chan;
     t->desc.chan_b = t->dev_chan + C;
+    if (dtype == FK_F64 && (long long)nfl * nx < (long long)fk::KDEC_NONE) {
+        e = cudaMalloc((void**)&t->kdec, (size_t)K * sizeof(uint32_t));
+        if (e == cudaSuccess) {
+            fk::fk_kdec_kernel<<<std::min(1024, (K + 255) / 256), 256>>>(t->desc, t->chan, t->kdec);
+            e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        }
+        if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: k codes: %s", cudaGetErrorString(e)); }
+    }
 
     rc = ensure_scratch(t, table_scratch_need(t, std::max(1, R_hint)));
     if (rc) return bail(rc);
@@ -541,6 +617,7 @@ int fk_table_destroy(fk_table* t) {
     if (!t) return FK_OK;
     if (t->owned_fk) cudaFree(t->owned_fk);
     if (t->dev_chan) cudaFree(t->dev_chan);
+    if (t->kdec) cudaFree(t->kdec);
     if (t->scratch) cudaFree(t->scratch);
     if (t->h_stage) cudaFreeHost(t->h_stage);
     if (t->d_stage) cudaFree(t->d_stage);

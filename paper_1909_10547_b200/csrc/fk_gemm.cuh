@@ -1,22 +1,219 @@
-// fk_gemm.cuh -- R >> 1 dense contraction -- placeholder until the FP64 split-K
-// kernel lands: gemm_wanted() is false, so every R runs through replica tiles of the stream kernel.
+// fk_gemm.cuh -- R >> 1 dense contraction (the paper's flat view FK[N x K] . PDF[K x R],
+// PAPER.md:83-100) on the FP64 tensor-core path (mma.sync.m8n8k4.f64 = DMMA.8x8x4), fp64 only.
+//
+//   Sigma[n][r] = sum_k FK[n][k] * L[k][r],   L[k][r] = f[r][a_c][i] * f[r][b_c][j]     Eq. (1)
+//
+// The output is tiny (N x R) and K is huge, so all parallelism is split-K: CTA = (128-datapoint tile,
+// K range).  Per K-tile of 32:
+//   * the FK tile [128 n][32 k] streams global -> shared with 16-byte cp.async, 3 stages deep
+//     (FK is read exactly once: every (n, k) belongs to one CTA);
+//   * the luminosity tile L[32 k][<=128 r] is BUILT ON THE FLY from the replica-innermost copy fT of f
+//     (gathered through the table's k -> (slot a, slot b) codes), one K-tile ahead in registers, and put
+//     in shared memory; it never exists in HBM (the custom operator's memory saving);
+//   * 8 warps (4 along n x 2 along r) run DMMA on 32 x (8..64) warp tiles; the +4 padding of both
+//     shared tiles makes every fragment load conflict-free.
+// Level 1 writes one partial tile per K range; fk_gemm_reduce_kernel adds the ranges in a fixed order:
+// no atomics, bitwise repeatable.  B200 has the same FP64 peak on DFMA and DMMA (37.2 TFLOP/s,
+// profiles/r01_fp64_peak.md); DMMA is used because it needs 8x fewer issue slots and 4x less
+// shared-memory operand traffic than a DFMA register tile.  tcgen05 has no f64 kind.
 #pragma once
 
 #include "fk_common.cuh"
 
 namespace fk {
 
-inline bool gemm_wanted(int) { return false; }
-inline int gemm_pick_split(const TableDesc&, int, int) { return 1; }
-inline size_t gemm_forward_scratch_elems(const TableDesc&, int, int) { return 0; }
+constexpr int GEMM_THREADS = 256;
+constexpr int GEMM_BM = 128;               // datapoints per CTA tile
+constexpr int GEMM_KT = 32;                // k per pipeline stage
+constexpr int GEMM_SA = GEMM_KT + 4;       // shared row stride of the FK tile (doubles): conflict-free A fragments
+constexpr int GEMM_BN = 128;               // replicas per pass
+constexpr int GEMM_SB = GEMM_BN + 4;       // shared row stride of the L tile
+constexpr int GEMM_STAGES = 3;
+constexpr int GEMM_SMEM_BYTES = (GEMM_STAGES * GEMM_BM * GEMM_SA + 2 * GEMM_KT * GEMM_SB) * 8;
+constexpr uint32_t KDEC_NONE = 0xffffu;    // DIS: no second factor
 
-template <typename T>
-int gemm_forward_single(const TableDesc&, const ChannelList&, const T*, T*, int, double*, int, cudaStream_t, int*) {
-    return (int)cudaErrorNotSupported;
+struct GemmFwdParams {
+    TableDesc desc;
+    const uint32_t* kdec;  // [K]: slot_a | slot_b << 16, slot = flavour * nx + x  (slot_b = KDEC_NONE for DIS)
+    const double* fT;      // [nfl*nx][RP]: f transposed, replica innermost, zero padded to RP
+    double* gpart;         // [ksplit][N][RP] level-1 partials
+    int RP;                // padded replicas of this pass = 8 * nfrag
+    int nfrag;             // 8-replica fragments in use (<= 16)
+    int nfw;               // fragments per warp column (2 warp columns; <= 8)
+    int ksplit, kper;      // K ranges and their length (multiple of GEMM_KT)
+};
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32_t src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
 }
+__device__ __forceinline__ void cp_async8(uint32_t dst, const void* src, uint32_t src_bytes) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// k -> (slot a, slot b) codes of a table, built once per table (or per stateless call)
+__global__ void __launch_bounds__(256) fk_kdec_kernel(TableDesc d, ChannelList chan, uint32_t* __restrict__ kdec) {
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < d.K; k += gridDim.x * blockDim.x) {
+        int ia, ib;
+        decode_k(d, chan.a, chan.b, k, ia, ib);
+        kdec[k] = (uint32_t)ia | ((ib >= 0 ? (uint32_t)ib : KDEC_NONE) << 16);
+    }
+}
+
+// fT[slot][r - r0] = f[r][slot] for r in [r0, r0 + RP), zero beyond R
 template <typename T>
-int gemm_colsum_single(const TableDesc&, const T*, double*, int, cudaStream_t, int*) {
-    return (int)cudaErrorNotSupported;
+__global__ void __launch_bounds__(256) fk_transpose_f_kernel(const T* __restrict__ f, double* __restrict__ fT, int slots,
+                                                              int R, int r0, int RP) {
+    const long long total = (long long)slots * RP;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const int s = (int)(t / RP), c = (int)(t - (long long)s * RP);
+        const int r = r0 + c;
+        fT[t] = r < R ? (double)f[(long long)r * slots + s] : 0.0;
+    }
+}
+
+template <int VEC>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
+    extern __shared__ __align__(16) unsigned char fk_smem[];
+    double* As = reinterpret_cast<double*>(fk_smem);                  // [STAGES][BM][SA]
+    double* Ls = As + GEMM_STAGES * GEMM_BM * GEMM_SA;                 // [2][KT][SB]
+    const uint32_t As_s = (uint32_t)__cvta_generic_to_shared(As);
+
+    const TableDesc& d = p.desc;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int mtiles = (d.N + GEMM_BM - 1) / GEMM_BM;
+    const int mt = blockIdx.x % mtiles, ks = blockIdx.x / mtiles;
+    const int m0 = mt * GEMM_BM;
+    const int kbeg = ks * p.kper;
+    const int kend = min(d.K, kbeg + p.kper);
+    const int nk = kend > kbeg ? (kend - kbeg + GEMM_KT - 1) / GEMM_KT : 0;
+    const bool had = d.kind == KIND_HADRONIC;
+
+    // ---- producers -------------------------------------------------------------------------------
+    auto load_fk = [&](int t) {  // FK tile of K-tile t -> stage t % STAGES (zero filled outside the table)
+        const int slot = t % GEMM_STAGES;
+        const int kt0 = kbeg + t * GEMM_KT;
+        constexpr int CH = GEMM_KT / VEC;  // chunks per row
+#pragma unroll
+        for (int j = 0; j < GEMM_BM * CH / GEMM_THREADS; ++j) {
+            const int q = tid + j * GEMM_THREADS;
+            const int row = q / CH, cc = q - row * CH;
+            const int n = m0 + row, k = kt0 + cc * VEC;
+            const bool ok = n < d.N && k < kend;
+            const double* src = reinterpret_cast<const double*>(d.fk) + (long long)(ok ? n : 0) * d.row_stride + (ok ? k : 0);
+            const uint32_t dst = As_s + (uint32_t)(((slot * GEMM_BM + row) * GEMM_SA + cc * VEC) * 8);
+            if constexpr (VEC == 2) cp_async16(dst, src, ok ? 16u : 0u);
+            else cp_async8(dst, src, ok ? 8u : 0u);
+        }
+    };
+    // luminosity: thread owns the replica pair (2*c2, 2*c2+1) of K-tile rows kq, kq+4, ..., kq+28
+    const int c2 = tid & 63, kq = tid >> 6;
+    const bool ccol = 2 * c2 < p.RP;
+    double2 la[GEMM_KT / 4], lb[GEMM_KT / 4];
+    auto load_L = [&](int t) {
+        const int kt0 = kbeg + t * GEMM_KT;
+#pragma unroll
+        for (int j = 0; j < GEMM_KT / 4; ++j) {
+            const int k = kt0 + kq + 4 * j;
+            la[j] = make_double2(0.0, 0.0);
+            lb[j] = make_double2(1.0, 1.0);
+            if (ccol && k < kend) {
+                const uint32_t code = __ldg(p.kdec + k);
+                la[j] = __ldg(reinterpret_cast<const double2*>(p.fT + (long long)(code & 0xffffu) * p.RP) + c2);
+                if (had) lb[j] = __ldg(reinterpret_cast<const double2*>(p.fT + (long long)(code >> 16) * p.RP) + c2);
+            }
+        }
+    };
+    auto store_L = [&](int t) {
+        double* Lb = Ls + (t & 1) * GEMM_KT * GEMM_SB;
+        if (ccol) {
+#pragma unroll
+            for (int j = 0; j < GEMM_KT / 4; ++j)
+                *reinterpret_cast<double2*>(Lb + (kq + 4 * j) * GEMM_SB + 2 * c2) =
+                    make_double2(la[j].x * lb[j].x, la[j].y * lb[j].y);
+        }
+    };
+
+    // ---- consumers: warp tile 32 datapoints x (8 * nfw) replicas --------------------------------------
+    const int wm = warp & 3, wn = warp >> 2;
+    const int nfw = min(p.nfw, max(0, p.nfrag - wn * p.nfw));  // fragments of this warp column
+    const int cb = wn * p.nfw * 8;
+    double acc[4][8][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+#pragma unroll
+    for (int s = 0; s < GEMM_STAGES - 1; ++s) {
+        if (s < nk) load_fk(s);
+        cp_async_commit();
+    }
+    if (nk > 0) {
+        load_L(0);
+        store_L(0);
+    }
+    for (int t = 0; t < nk; ++t) {
+        cp_async_wait<GEMM_STAGES - 2>();
+        __syncthreads();  // stage t has landed and L tile t is stored; everyone is done with K-tile t-1
+        if (t + GEMM_STAGES - 1 < nk) load_fk(t + GEMM_STAGES - 1);
+        cp_async_commit();
+        if (t + 1 < nk) load_L(t + 1);
+
+        const double* At = As + ((t % GEMM_STAGES) * GEMM_BM + wm * 32 + (lane >> 2)) * GEMM_SA + (lane & 3);
+        const double* Bt = Ls + (t & 1) * GEMM_KT * GEMM_SB + (lane & 3) * GEMM_SB + cb + (lane >> 2);
+#pragma unroll
+        for (int k4 = 0; k4 < GEMM_KT / 4; ++k4) {
+            double a[4], b[8];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = At[i * 8 * GEMM_SA + k4 * 4];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) b[j] = j < nfw ? Bt[k4 * 4 * GEMM_SB + j * 8] : 0.0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (j < nfw) {
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                }
+        }
+        if (t + 1 < nk) store_L(t + 1);
+    }
+
+    // ---- level-1 partial tile -> gpart[ks][n][c] -------------------------------------------------
+    double* out = p.gpart + (long long)ks * d.N * p.RP;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int n = m0 + wm * 32 + i * 8 + (lane >> 2);
+        if (n >= d.N) continue;
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (j < nfw) {
+                const int c = cb + j * 8 + 2 * (lane & 3);
+                *reinterpret_cast<double2*>(out + (long long)n * p.RP + c) = make_double2(acc[i][j][0], acc[i][j][1]);
+            }
+    }
+}
+
+// level 2: sigma[n][r0 + c] = sum over K ranges, fixed order
+template <typename T>
+__global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const double* __restrict__ gpart, T* __restrict__ sigma,
+                                                              long long out_off, int N, int R, int r0, int RP, int ksplit) {
+    const long long total = (long long)N * RP;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const int n = (int)(t / RP), c = (int)(t - (long long)n * RP);
+        if (r0 + c >= R) continue;
+        double s = 0.0;
+        for (int ks = 0; ks < ksplit; ++ks) s += gpart[(long long)ks * total + t];
+        sigma[out_off + (long long)n * R + r0 + c] = (T)s;
+    }
 }
 
 }  // namespace fk
