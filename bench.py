@@ -32,6 +32,7 @@ if ROOT not in sys.path:
 
 from paper_1909_10547_b200 import synth  # noqa: E402  (seeded inputs only; no method arithmetic)
 
+FP64_PEAK_TFLOPS = 37.2  # 148 SM x 64 FMA/clk x 2 x 1.965 GHz (probe: profiles/r01_fp64_peak.md)
 METRIC = "fk_convolution_achieved_hbm_bandwidth"
 UNIT = "GB/s"
 WORKLOAD = "config2: hadronic FK N=512 nx=50 nfl=14 C=100 R=1 fp64 (1.024 GB), forward + VJP per step"
@@ -241,7 +242,11 @@ def run_extras(K, torch, level, table2, case2, peak):
     ms = _bench_call(lambda: table2.conv(f3, s3), stream, steps=5, warmup=2)
     flops = 2.0 * case2.N * case2.fk[0].size * R
     out["cfg3_forward_R128"] = {"ms": ms, "TFLOPs": flops / ms / 1e9, "replica_evals_per_s": R / ms * 1e3,
-                                "predictions_per_s": case2.N * R / ms * 1e3}
+                                "predictions_per_s": case2.N * R / ms * 1e3, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS}
+    g3 = torch.from_numpy(np.ascontiguousarray(np.broadcast_to(case2.g, (case2.N, R)))).cuda()
+    d3 = torch.empty_like(f3)
+    ms = _bench_call(lambda: table2.vjp(f3, g3, d3), stream, steps=5, warmup=2)
+    out["cfg3_vjp_R128"] = {"ms": ms, "TFLOPs": flops / ms / 1e9, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS}
     if level == "all":
         out.update(run_config4(K, torch, peak))
     return out

@@ -292,6 +292,60 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
     return FK_OK;
 }
 
+// doubles: fT [slots][RPmax] + gP [N][RPmax] + G [K][RPmax]
+size_t gemm_vjp_scratch_elems(const fk::TableDesc& d, int R) {
+    const size_t RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    return ((size_t)d.nfl * d.nx + (size_t)d.N + (size_t)d.K) * RPmax;
+}
+
+int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double* f, const double* g, double* df,
+                 int R, double* scratch, cudaStream_t s, int* launches) {
+    const int RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    const int slots = d.nfl * d.nx;
+    double* fT = scratch;
+    double* gP = fT + (size_t)slots * RPmax;
+    double* G = gP + (size_t)d.N * RPmax;
+    static const bool attr_ok = [] {
+        return cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess &&
+               cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess;
+    }();
+    if (!attr_ok) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
+    int nl = 0;
+    for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
+        const int RP = (std::min(fk::GEMM_BN, R - r0) + 7) / 8 * 8;
+        const long long tf = (long long)slots * RP, tg = (long long)d.N * RP;
+        fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tf + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, RP);
+        fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(2048, (tg + 255) / 256), 256, 0, s>>>(g + d.out_off * R, gP, d.N, R, r0, RP);
+        fk::GemmVjpParams p;
+        memset(&p, 0, sizeof p);
+        p.desc = d;
+        p.gP = gP;
+        p.G = G;
+        p.RP = RP;
+        p.nfrag = RP / 8;
+        p.nfw = (p.nfrag + 1) / 2;
+        const int grid = (d.K + fk::GEMMV_BK - 1) / fk::GEMMV_BK;
+        if (d.vec_ok) fk::fk_gemm_vjp_kernel<2><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        else fk::fk_gemm_vjp_kernel<1><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        fk::GatherRParams q;
+        memset(&q, 0, sizeof q);
+        q.desc = d;
+        q.chan = ch;
+        q.fT = fT;
+        q.G = G;
+        q.df = df;
+        q.R = R;
+        q.r0 = r0;
+        q.RP = RP;
+        fk::fk_vjp_gather_r_kernel<double><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm vjp launch failed: %s", cudaGetErrorString(e));
+        nl += 4;
+    }
+    if (launches) *launches = nl;
+    return FK_OK;
+}
+
 // One table, any R.  `part` holds >= part_elems_per_replica * R doubles (may be null if nchunks == 1).
 template <typename T>
 int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const uint32_t* kdec,
@@ -344,6 +398,9 @@ template <typename T>
 int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const T* f, const T* g, T* df,
                    int R, double* G, cudaStream_t s, int* launches) {
     int nl = 0;
+    if constexpr (std::is_same<T, double>::value) {
+        if (gemm_wanted<T>(d, R)) return run_vjp_gemm(d, ch, f, g, df, R, G, s, launches);
+    }
     {
         fk::ColsumParams p;
         memset(&p, 0, sizeof p);
@@ -382,7 +439,11 @@ size_t conv_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
     if (gemm_wanted<T>(d, R)) return gemm_fwd_scratch_elems(d, R, with_kdec);
     return part_elems_per_replica(d) * R;
 }
-size_t vjp_scratch_elems(const fk::TableDesc& d, int R) { return G_elems_per_replica(d) * R; }
+template <typename T>
+size_t vjp_scratch_elems(const fk::TableDesc& d, int R) {
+    if (gemm_wanted<T>(d, R)) return gemm_vjp_scratch_elems(d, R);
+    return G_elems_per_replica(d) * R;
+}
 
 // stateless front end shared by the fp64 / fp32 entry points
 template <typename T>
@@ -401,7 +462,7 @@ int stateless(const char* who, int kind, bool vjp, const T* fkp, const int32_t* 
     Plan pl;
     make_plan(d, dtype_of<T>(), pl);
     cudaStream_t s = (cudaStream_t)stream;
-    const size_t elems = vjp ? vjp_scratch_elems(d, R) : conv_scratch_elems<T>(d, R, true);
+    const size_t elems = vjp ? vjp_scratch_elems<T>(d, R) : conv_scratch_elems<T>(d, R, true);
     double* scratch = nullptr;
     if (elems) FK_CUDA(cudaMallocAsync((void**)&scratch, elems * sizeof(double), s));
     rc = vjp ? run_vjp_single<T>(d, ch, pl, f, g, out, R, scratch, s, nullptr)
@@ -461,7 +522,8 @@ int ensure_stage(fk_table* t, size_t bytes) {
 size_t table_scratch_need(const fk_table* t, int R) {
     const size_t conv = t->dtype == FK_F64 ? conv_scratch_elems<double>(t->desc, R, t->kdec == nullptr)
                                            : conv_scratch_elems<float>(t->desc, R, true);
-    return std::max(conv, vjp_scratch_elems(t->desc, R));
+    const size_t vjp = t->dtype == FK_F64 ? vjp_scratch_elems<double>(t->desc, R) : vjp_scratch_elems<float>(t->desc, R);
+    return std::max(conv, vjp);
 }
 
 template <typename T>

@@ -216,4 +216,185 @@ __global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const double* __res
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// VJP stage 1 for R >> 1 (minimal-flop order): G[k][c] = sum_n FK[n][k] * g[n][r0 + c].
+// Same machinery with the FK tile used transposed: CTA = 128 consecutive k (1 KB of every row), the
+// contraction runs over ALL datapoints in steps of 32 (no split: one CTA owns its G tile, fixed order),
+// both operands arrive by cp.async (FK tile [32 n][128 k], upstream-gradient tile [32 n][RP]).
+struct GemmVjpParams {
+    TableDesc desc;
+    const double* gP;   // [N][RP]: g of this pass, replica innermost, zero padded
+    double* G;          // [K][RP] column sums, replica innermost
+    int RP, nfrag, nfw;
+};
+
+constexpr int GEMMV_BK = 128;                // k per CTA tile (the M dimension of the MMA)
+constexpr int GEMMV_NT = 32;                 // datapoints per pipeline stage
+constexpr int GEMMV_S = GEMMV_BK + 4;        // shared row stride of both tiles
+constexpr int GEMMV_STAGES = 3;
+constexpr int GEMMV_SMEM_BYTES = GEMMV_STAGES * 2 * GEMMV_NT * GEMMV_S * 8;
+
+template <int VEC>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+fk_gemm_vjp_kernel(const __grid_constant__ GemmVjpParams p) {
+    extern __shared__ __align__(16) unsigned char fk_smem[];
+    double* As = reinterpret_cast<double*>(fk_smem);            // [STAGES][NT][S]  FK tile, k innermost
+    double* Bs = As + GEMMV_STAGES * GEMMV_NT * GEMMV_S;         // [STAGES][NT][S]  g tile, replica innermost
+    const uint32_t As_s = (uint32_t)__cvta_generic_to_shared(As), Bs_s = (uint32_t)__cvta_generic_to_shared(Bs);
+
+    const TableDesc& d = p.desc;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int k0 = blockIdx.x * GEMMV_BK;
+    const int nt = (d.N + GEMMV_NT - 1) / GEMMV_NT;
+
+    auto load_stage = [&](int t) {
+        const int slot = t % GEMMV_STAGES;
+        const int n0 = t * GEMMV_NT;
+        {   // FK tile: NT rows x BK k
+            constexpr int CH = GEMMV_BK / VEC;
+#pragma unroll
+            for (int j = 0; j < GEMMV_NT * CH / GEMM_THREADS; ++j) {
+                const int q = tid + j * GEMM_THREADS;
+                const int row = q / CH, cc = q - row * CH;
+                const int n = n0 + row, k = k0 + cc * VEC;
+                const bool ok = n < d.N && k < d.K;
+                const double* src = reinterpret_cast<const double*>(d.fk) + (long long)(ok ? n : 0) * d.row_stride + (ok ? k : 0);
+                const uint32_t dst = As_s + (uint32_t)(((slot * GEMMV_NT + row) * GEMMV_S + cc * VEC) * 8);
+                if constexpr (VEC == 2) cp_async16(dst, src, ok ? 16u : 0u);
+                else cp_async8(dst, src, ok ? 8u : 0u);
+            }
+        }
+        {   // g tile: NT rows x RP replicas (RP is a multiple of 8: 16-byte chunks)
+            const int CH = p.RP / 2;
+            for (int q = tid; q < GEMMV_NT * CH; q += GEMM_THREADS) {
+                const int row = q / CH, cc = q - row * CH;
+                const int n = n0 + row;
+                const bool ok = n < d.N;
+                const double* src = p.gP + (long long)(ok ? n : 0) * p.RP + cc * 2;
+                cp_async16(Bs_s + (uint32_t)(((slot * GEMMV_NT + row) * GEMMV_S + cc * 2) * 8), src, ok ? 16u : 0u);
+            }
+        }
+    };
+
+    const int wm = warp & 3, wn = warp >> 2;
+    const int nfw = min(p.nfw, max(0, p.nfrag - wn * p.nfw));
+    const int cb = wn * p.nfw * 8;
+    double acc[4][8][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+#pragma unroll
+    for (int s = 0; s < GEMMV_STAGES - 1; ++s) {
+        if (s < nt) load_stage(s);
+        cp_async_commit();
+    }
+    for (int t = 0; t < nt; ++t) {
+        cp_async_wait<GEMMV_STAGES - 2>();
+        __syncthreads();
+        if (t + GEMMV_STAGES - 1 < nt) load_stage(t + GEMMV_STAGES - 1);
+        cp_async_commit();
+        // A fragment: row m = k (lane >> 2), col = datapoint (lane & 3)  ->  As[n][k]
+        const double* At = As + ((t % GEMMV_STAGES) * GEMMV_NT + (lane & 3)) * GEMMV_S + wm * 32 + (lane >> 2);
+        const double* Bt = Bs + ((t % GEMMV_STAGES) * GEMMV_NT + (lane & 3)) * GEMMV_S + cb + (lane >> 2);
+#pragma unroll
+        for (int n4 = 0; n4 < GEMMV_NT / 4; ++n4) {
+            double a[4], b[8];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = At[n4 * 4 * GEMMV_S + i * 8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) b[j] = j < nfw ? Bt[n4 * 4 * GEMMV_S + j * 8] : 0.0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (j < nfw) {
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int k = k0 + wm * 32 + i * 8 + (lane >> 2);
+        if (k >= d.K) continue;
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (j < nfw) {
+                const int c = cb + j * 8 + 2 * (lane & 3);
+                *reinterpret_cast<double2*>(p.G + (long long)k * p.RP + c) = make_double2(acc[i][j][0], acc[i][j][1]);
+            }
+    }
+}
+
+// gP[n][c] = g[n][r0 + c] (zero beyond R)
+template <typename T>
+__global__ void __launch_bounds__(256) fk_pad_g_kernel(const T* __restrict__ g, double* __restrict__ gP, int N, int R, int r0, int RP) {
+    const long long total = (long long)N * RP;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const int n = (int)(t / RP), c = (int)(t - (long long)n * RP);
+        gP[t] = r0 + c < R ? (double)g[(long long)n * R + r0 + c] : 0.0;
+    }
+}
+
+// VJP stage 2 for the replica-innermost G: one CTA per (alpha, i), one thread per replica of the pass.
+//   df[r][alpha][i] = sum_{c: a_c = alpha} sum_j G[k(i,j,c)][r] f[r][b_c][j] + sum_{c: b_c = alpha} sum_j G[k(j,i,c)][r] f[r][a_c][j]
+// Every load is coalesced along r; 4 interleaved chains per thread, combined in a fixed order.
+struct GatherRParams {
+    TableDesc desc;
+    ChannelList chan;
+    const double* fT;   // [slots][RP]
+    const double* G;    // [K][RP]
+    void* df;           // [R][nfl][nx]
+    int R, r0, RP;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(128) fk_vjp_gather_r_kernel(const __grid_constant__ GatherRParams p) {
+    __shared__ short listA[MAX_C], listB[MAX_C];
+    __shared__ int cnt[2];
+    const TableDesc& d = p.desc;
+    const int nx = d.nx, C = d.C;
+    const int slot = blockIdx.x;
+    const int alpha = slot / nx, i = slot - alpha * nx;
+    const bool had = d.kind == KIND_HADRONIC;
+    if (threadIdx.x == 0) {
+        int na = 0, nb = 0;
+        for (int c = 0; c < C; ++c) {
+            if (p.chan.a[c] == alpha) listA[na++] = (short)c;
+            if (had && p.chan.b[c] == alpha) listB[nb++] = (short)c;
+        }
+        cnt[0] = na;
+        cnt[1] = nb;
+    }
+    __syncthreads();
+    const int na = cnt[0], nb = cnt[1];
+    const int c0 = blockIdx.y * blockDim.x + threadIdx.x;  // replica column of this pass
+    if (c0 >= p.RP || p.r0 + c0 >= p.R) return;
+    const double* __restrict__ G = p.G + c0;
+    const double* __restrict__ fT = p.fT + c0;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    if (had) {
+        for (int q = 0; q < na; ++q) {
+            const int c = listA[q];
+            const long long fo = (long long)p.chan.b[c] * nx;
+            for (int j = 0; j < nx; ++j) {
+                const int k = encode_k(d, i, j, c);
+                acc[j & 3] = fma(G[(long long)k * p.RP], fT[(fo + j) * p.RP], acc[j & 3]);
+            }
+        }
+        for (int q = 0; q < nb; ++q) {
+            const int c = listB[q];
+            const long long fo = (long long)p.chan.a[c] * nx;
+            for (int j = 0; j < nx; ++j) {
+                const int k = encode_k(d, j, i, c);
+                acc[j & 3] = fma(G[(long long)k * p.RP], fT[(fo + j) * p.RP], acc[j & 3]);
+            }
+        }
+    } else {
+        for (int q = 0; q < na; ++q) acc[q & 3] += G[(long long)encode_k(d, i, 0, listA[q]) * p.RP];
+    }
+    const double s = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+    reinterpret_cast<T*>(p.df)[d.f_off * p.R + ((long long)(p.r0 + c0) * d.nfl + alpha) * nx + i] = (T)s;
+}
+
 }  // namespace fk
