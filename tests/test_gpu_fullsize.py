@@ -1,0 +1,148 @@
+"""GPU-vs-oracle parity at BASELINE.json's full sizes, in the launch configuration bench.py times
+(resident PACK tables, R_hint given at create, grouped launch for config 4), through the C-ABI.
+
+Config 2 (1.0 GB) is compared element by element: the oracle finishes it in about a second.
+Config 3 (R=128) and config 4 at R=100 are compared on sampled replicas: column r of sigma and
+slice r of df depend on replica r only (Eq. (1), holds per replica), so the oracle
+computes exactly those replicas one by one.  Config 4 at R=1 is compared element by element, table
+by table (reading R15: the explicit distributions, 14.8 GB).
+Also here: the same-sign closed-form stress test that a long serial fp64 chain fails.
+"""
+import numpy as np
+import pytest
+
+from oracle import fk_oracle as O
+from paper_1909_10547_b200 import synth
+from tests._parity import TOL32, TOL64, rel_err, to_dev
+
+pytestmark = pytest.mark.gpu
+
+SAMPLED = [0, 1, 63, 64, 127]
+
+
+@pytest.fixture(scope="module")
+def K():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    from paper_1909_10547_b200 import fkconv
+    return fkconv
+
+
+@pytest.fixture(scope="module")
+def cfg2(K):
+    import torch
+    case = synth.config2(R=1)
+    fk_d = to_dev(case.fk)
+    t64 = K.FkTable(K.FK_KIND_HADRONIC, fk_d, case.pairs, case.nfl, K.FK_F64, K.FK_STORE_PACK, R_hint=128)
+    t32 = K.FkTable(K.FK_KIND_HADRONIC, fk_d, case.pairs, case.nfl, K.FK_F32, K.FK_STORE_PACK, R_hint=128)
+    del fk_d
+    torch.cuda.empty_cache()
+    yield case, t64, t32
+    t64.destroy(); t32.destroy()
+
+
+def test_config2_full_elementwise(K, cfg2):
+    case, t64, _ = cfg2
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    f_d, g_d = to_dev(case.f), to_dev(case.g)
+    e_s = rel_err(t64.conv(f_d).cpu().numpy(), ref, scale)
+    e_d = rel_err(t64.vjp(f_d, g_d).cpu().numpy(), dref, D)
+    print(f"config 2: forward {e_s:.2e} vjp {e_d:.2e}")
+    assert e_s <= TOL64 and e_d <= TOL64
+    # host-buffer calls (what bench.py's e2e leg times)
+    sig = np.empty((case.N, 1)); df = np.empty_like(case.f)
+    t64.conv_host(case.f, sig); t64.vjp_host(case.f, case.g, df)
+    assert rel_err(sig, ref, scale) <= TOL64 and rel_err(df, dref, D) <= TOL64
+
+
+def test_config3_sampled_replicas_fp64_and_fp32(K, cfg2):
+    import torch
+    case, t64, t32 = cfg2
+    R = 128
+    f = synth.pdf_grid(synth.pdf_params(synth.rng_for(2, synth.T_PDF, 0), R), 50)
+    g = np.ascontiguousarray(np.broadcast_to(case.g, (case.N, R)))
+    fs = np.ascontiguousarray(f[SAMPLED]); gs = np.ascontiguousarray(g[:, SAMPLED])
+    ref, scale = O.hadronic(case.fk, case.pairs, fs)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, fs, gs)
+    f_d, g_d = to_dev(f), to_dev(g)
+    sig = t64.conv(f_d).cpu().numpy()
+    df = t64.vjp(f_d, g_d).cpu().numpy()
+    e_s = rel_err(sig[:, SAMPLED], ref, scale); e_d = rel_err(df[SAMPLED], dref, D)
+    print(f"config 3 fp64: forward {e_s:.2e} vjp {e_d:.2e}")
+    assert e_s <= TOL64 and e_d <= TOL64
+    # every column is finite and non-trivial (the unsampled ones too)
+    assert np.all(np.isfinite(sig)) and np.all(np.abs(sig).max(axis=0) > 0)
+    f32 = torch.float32
+    sig32 = t32.conv(to_dev(f, f32)).cpu().numpy()
+    df32 = t32.vjp(to_dev(f, f32), to_dev(g, f32)).cpu().numpy()
+    e_s32 = rel_err(sig32[:, SAMPLED], ref, scale); e_d32 = rel_err(df32[SAMPLED], dref, D)
+    print(f"config 3 fp32: forward {e_s32:.2e} vjp {e_d32:.2e}")
+    assert sig32.dtype == np.float32 and e_s32 <= TOL32 and e_d32 <= TOL32
+
+
+@pytest.mark.parametrize("c", [0.3, 0.7, 1.1])
+def test_closed_form_same_sign_gpu(K, c):
+    """f = c, FK = 1 at config-2 shape: sigma = c^2 nx^2 C for every datapoint (BASELINE north_star).
+    All terms have one sign, so rounding errors do not cancel: a long serial fp64 chain fails 1e-13
+    here.  All rows are identical, so the oracle computes 2 of them."""
+    import torch
+    N, nx, C, nfl = 512, 50, 100, 14
+    pairs = synth.draw_pairs(synth.rng_for(2, synth.T_PAIRS, 0), C)
+    fk_d = torch.ones((N, nx, nx, C), dtype=torch.float64, device="cuda")
+    for R in (1, 3, 128):
+        f = np.full((R, nfl, nx), c)
+        ref, scale = O.hadronic(np.ones((2, nx, nx, C)), pairs, f)
+        exact = c * c * nx * nx * C
+        assert abs(ref[0, 0] - exact) <= 4e-16 * exact
+        tb = K.FkTable(K.FK_KIND_HADRONIC, fk_d, pairs, nfl, K.FK_F64, K.FK_STORE_BORROW, R_hint=R)
+        sig = tb.conv(to_dev(f)).cpu().numpy()
+        err = float(np.max(np.abs(sig - ref[0, 0]) / scale[0, 0]))
+        g = np.ones((N, R))
+        dref, D = O.hadronic_vjp(np.ones((2, nx, nx, C)), pairs, f, np.ones((2, R)))
+        df = tb.vjp(to_dev(f), to_dev(g)).cpu().numpy()
+        derr = rel_err(df, dref * (N / 2), D * (N / 2))
+        print(f"same-sign c={c} R={R}: forward {err:.2e} vjp {derr:.2e}")
+        assert err <= TOL64 and derr <= TOL64, (c, R, err, derr)
+        tb.destroy()
+
+
+def test_config4_full_grouped(K):
+    """All 60 tables (sum N = 12 437, 14.8 GB) in one grouped launch: R=1 element by element,
+    R=100 on sampled replicas."""
+    import torch
+    shapes = synth.config4_shapes()
+    R = 100
+    sampled = [0, 57, 99]
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    tabs, fs, gs, refs = [], [], [], []
+    for t in range(shapes.T):
+        c = synth.config4_table(t, shapes, R, params)
+        fk_d = to_dev(c.fk)
+        tabs.append(K.FkTable(K.FK_KIND_HADRONIC, fk_d, c.pairs, c.nfl, K.FK_F64, K.FK_STORE_PACK, R_hint=1))
+        del fk_d
+        fsub = np.ascontiguousarray(c.f[sampled]); gsub = np.ascontiguousarray(c.g[:, sampled])
+        refs.append((O.hadronic(c.fk, c.pairs, fsub), O.hadronic_vjp(c.fk, c.pairs, fsub, gsub), c.N, c.nfl, c.nx))
+        fs.append(c.f); gs.append(c.g)
+    torch.cuda.empty_cache()
+    grp = K.FkGroup(tabs, R_hint=R)
+    for Rr in (1, R):
+        sel = [0] if Rr == 1 else list(range(R))
+        cols = [0] if Rr == 1 else sampled
+        fo, so = grp.offsets(Rr)
+        f_cat = torch.cat([to_dev(np.ascontiguousarray(f[sel])).reshape(-1) for f in fs])
+        g_cat = torch.cat([to_dev(np.ascontiguousarray(g[:, sel])).reshape(-1) for g in gs])
+        sig = grp.conv(f_cat, Rr).cpu().numpy()
+        df = grp.vjp(f_cat, g_cat, Rr).cpu().numpy()
+        worst_s = worst_d = 0.0
+        for t, ((ref, scale), (dref, D), N, nfl, nx) in enumerate(refs):
+            s_t = sig[so[t]:so[t + 1]].reshape(N, Rr)[:, cols]
+            d_t = df[fo[t]:fo[t + 1]].reshape(Rr, nfl, nx)[cols]
+            k = len(cols)
+            worst_s = max(worst_s, rel_err(s_t, ref[:, :k], scale[:, :k]))
+            worst_d = max(worst_d, rel_err(d_t, dref[:k], D[:k]))
+        print(f"config 4 R={Rr}: forward {worst_s:.2e} vjp {worst_d:.2e} launches {grp.last_launches()}")
+        assert worst_s <= TOL64 and worst_d <= TOL64, (Rr, worst_s, worst_d)
+    grp.destroy()
+    for t in tabs:
+        t.destroy()
