@@ -29,6 +29,7 @@ constexpr int GEMM_SA = GEMM_KT + 4;       // shared row stride of the FK tile (
 constexpr int GEMM_BN = 128;               // replicas per pass
 constexpr int GEMM_SB = GEMM_BN + 4;       // shared row stride of the L tile
 constexpr int GEMM_STAGES = 3;
+constexpr int GEMM_FLUSH = 16;             // K-tiles between flushes of the register tile (chain <= 512 FMAs)
 constexpr int GEMM_SMEM_BYTES = (GEMM_STAGES * GEMM_BM * GEMM_SA + 2 * GEMM_KT * GEMM_SB) * 8;
 constexpr uint32_t KDEC_NONE = 0xffffu;    // DIS: no second factor
 
@@ -152,6 +153,25 @@ fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
 #pragma unroll
         for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
+    // ---- level-1 partial tile gpart[ks][n][c] (+)= acc, acc = 0 ----------------------------------------
+    double* out = p.gpart + (long long)ks * d.N * p.RP;
+    auto flush = [&](bool first) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int n = m0 + wm * 32 + i * 8 + (lane >> 2);
+            double2* q = reinterpret_cast<double2*>(out + (long long)n * p.RP + cb + 2 * (lane & 3));
+            double2 o[8];  // all loads of a row first: one L2 round trip per row, not per fragment
+#pragma unroll
+            for (int j = 0; j < 8; ++j) o[j] = (!first && j < nfw && n < d.N) ? q[j * 4] : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (j < nfw && n < d.N) {
+                    q[j * 4] = make_double2(acc[i][j][0] + o[j].x, acc[i][j][1] + o[j].y);
+                    acc[i][j][0] = acc[i][j][1] = 0.0;
+                }
+        }
+    };
+
 #pragma unroll
     for (int s = 0; s < GEMM_STAGES - 1; ++s) {
         if (s < nk) load_fk(s);
@@ -185,21 +205,14 @@ fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
                 }
         }
         if (t + 1 < nk) store_L(t + 1);
+        // bounded chains: every GEMM_FLUSH K-tiles (512 FMAs per accumulator) the register tile is added
+        // into this CTA's partial tile in gpart (thread-private addresses, L2-resident) and cleared, so a
+        // same-sign sum cannot build up a long serial rounding bias
+        if ((t + 1) % GEMM_FLUSH == 0 && t + 1 < nk) {
+            flush(t + 1 == GEMM_FLUSH);
+        }
     }
-
-    // ---- level-1 partial tile -> gpart[ks][n][c] -------------------------------------------------
-    double* out = p.gpart + (long long)ks * d.N * p.RP;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int n = m0 + wm * 32 + i * 8 + (lane >> 2);
-        if (n >= d.N) continue;
-#pragma unroll
-        for (int j = 0; j < 8; ++j)
-            if (j < nfw) {
-                const int c = cb + j * 8 + 2 * (lane & 3);
-                *reinterpret_cast<double2*>(out + (long long)n * p.RP + c) = make_double2(acc[i][j][0], acc[i][j][1]);
-            }
-    }
+    flush(nk <= GEMM_FLUSH);
 }
 
 // level 2: sigma[n][r0 + c] = sum over K ranges, fixed order
