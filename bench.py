@@ -253,33 +253,41 @@ def run_extras(K, torch, level, table2, case2, peak):
 
 
 def run_config4(K, torch, peak):
-    """BASELINE config 4 (reading R15: the explicit distributions; ~14-15 GB): grouped forward + VJP."""
+    """BASELINE config 4 (reading R15: the explicit distributions; ~14.8 GB): grouped forward + VJP at
+    R=1 (HBM-bound) and R=100 (FP64-bound)."""
     out = {}
     shapes = synth.config4_shapes()
     stream = torch.cuda.current_stream()
-    for R in (1,):
-        params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
-        tabs, fs, gs = [], [], []
-        for t in range(shapes.T):
-            c = synth.config4_table(t, shapes, R, params)
-            fk_d = torch.from_numpy(c.fk).cuda()
-            tabs.append(K.FkTable(K.FK_KIND_HADRONIC, fk_d, c.pairs, c.nfl, R_hint=1))
-            del fk_d
-            fs.append(torch.from_numpy(c.f).reshape(-1)); gs.append(torch.from_numpy(c.g).reshape(-1))
-        grp = K.FkGroup(tabs, R_hint=R)
-        f_cat = torch.cat(fs).cuda(); g_cat = torch.cat(gs).cuda()
+    Rmax = 100
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), Rmax)
+    tabs, fs, gs = [], [], []
+    for t in range(shapes.T):
+        c = synth.config4_table(t, shapes, Rmax, params)
+        fk_d = torch.from_numpy(c.fk).cuda()
+        tabs.append(K.FkTable(K.FK_KIND_HADRONIC, fk_d, c.pairs, c.nfl, R_hint=1))
+        del fk_d
+        fs.append(c.f); gs.append(c.g)
+    torch.cuda.empty_cache()
+    grp = K.FkGroup(tabs, R_hint=Rmax)
+    nbytes = shapes.fk_elements() * 8
+    for R in (1, Rmax):
+        f_cat = torch.cat([torch.from_numpy(np.ascontiguousarray(f[:R])).reshape(-1) for f in fs]).cuda()
+        g_cat = torch.cat([torch.from_numpy(np.ascontiguousarray(g[:, :R])).reshape(-1) for g in gs]).cuda()
         _, so = grp.offsets(R)
         sig = torch.empty(int(so[-1]), dtype=torch.float64, device="cuda"); df = torch.empty_like(f_cat)
-        nbytes = shapes.fk_elements() * 8
-        ms = _bench_call(lambda: grp.conv(f_cat, R, sig), stream, steps=10, warmup=3)
+        flops = 2.0 * shapes.fk_elements() * R
+        nst = 10 if R == 1 else 3
+        ms = _bench_call(lambda: grp.conv(f_cat, R, sig), stream, steps=nst, warmup=3)
         out[f"cfg4_grouped_forward_R{R}"] = {"ms": ms, "GBps": nbytes / ms / 1e6, "frac_of_peak": nbytes / ms / 1e6 / peak,
+                                             "TFLOPs": flops / ms / 1e9, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS,
                                              "sumN": int(shapes.N.sum()), "GB": nbytes / 1e9, "launches": grp.last_launches()}
-        ms = _bench_call(lambda: grp.vjp(f_cat, g_cat, R, df), stream, steps=10, warmup=3)
+        ms = _bench_call(lambda: grp.vjp(f_cat, g_cat, R, df), stream, steps=nst, warmup=3)
         out[f"cfg4_grouped_vjp_R{R}"] = {"ms": ms, "GBps": nbytes / ms / 1e6, "frac_of_peak": nbytes / ms / 1e6 / peak,
+                                         "TFLOPs": flops / ms / 1e9, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS,
                                          "launches": grp.last_launches()}
-        grp.destroy()
-        for t in tabs:
-            t.destroy()
+    grp.destroy()
+    for t in tabs:
+        t.destroy()
     return out
 
 

@@ -257,8 +257,8 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
         kdec = kd;
     }
     static const bool attr_ok = [] {
-        return cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess &&
-               cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess;
+        return cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess &&
+               cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess;
     }();
     if (!attr_ok) return fail(FK_ERR_CUDA, "gemm: cannot reserve %d bytes of shared memory", fk::GEMM_SMEM_BYTES);
     const int mtiles = (d.N + fk::GEMM_BM - 1) / fk::GEMM_BM;
@@ -278,8 +278,8 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
         fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
         size_t slot = 0;
         const bool timed = r0 == 0 && g_prof.begin(s, slot);
-        if (d.vec_ok) fk::fk_gemm_fwd_kernel<2><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
-        else fk::fk_gemm_fwd_kernel<1><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        if (d.vec_ok) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        else fk::fk_gemm_fwd_kernel<1, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         if (timed) g_prof.end(s, slot);
         const long long outs = (long long)d.N * p.RP;
         fk::fk_gemm_reduce_kernel<double><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
@@ -306,8 +306,8 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
     double* gP = fT + (size_t)slots * RPmax;
     double* G = gP + (size_t)d.N * RPmax;
     static const bool attr_ok = [] {
-        return cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess &&
-               cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess;
+        return cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess &&
+               cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess;
     }();
     if (!attr_ok) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
     int nl = 0;
@@ -325,8 +325,8 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
         p.nfrag = RP / 8;
         p.nfw = (p.nfrag + 1) / 2;
         const int grid = (d.K + fk::GEMMV_BK - 1) / fk::GEMMV_BK;
-        if (d.vec_ok) fk::fk_gemm_vjp_kernel<2><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
-        else fk::fk_gemm_vjp_kernel<1><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        if (d.vec_ok) fk::fk_gemm_vjp_kernel<2, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        else fk::fk_gemm_vjp_kernel<1, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         fk::GatherRParams q;
         memset(&q, 0, sizeof q);
         q.desc = d;
@@ -337,7 +337,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
         q.R = R;
         q.r0 = r0;
         q.RP = RP;
-        fk::fk_vjp_gather_r_kernel<double><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
+        fk::fk_vjp_gather_r_kernel<double, false><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm vjp launch failed: %s", cudaGetErrorString(e));
         nl += 4;
@@ -667,6 +667,7 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
             if (e == cudaSuccess) e = cudaDeviceSynchronize();
         }
         if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: k codes: %s", cudaGetErrorString(e)); }
+        t->desc.kdec = t->kdec;
     }
 
     rc = ensure_scratch(t, table_scratch_need(t, std::max(1, R_hint)));

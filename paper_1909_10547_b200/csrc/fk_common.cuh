@@ -40,6 +40,11 @@ struct TableDesc {
     int nchunks;             // forward: number of k-blocks (= level-1 partials per row)
     int fsplit;              // forward: number of datapoint ranges per k-block
     int nsplit;              // VJP stage 1: number of datapoint ranges per k-block
+    // R >> 1 contraction (fk_gemm.cuh), grouped launches only
+    const uint32_t* kdec;    // device [K]: k -> (slot a, slot b) codes
+    long long gp_off;        // row offset of this table's split-K partial tiles (sum over earlier tables of ksplit * N)
+    long long k_off;         // offset of this table's column sums inside G_cat (sum of K over earlier tables)
+    int gksplit, gkper;      // K ranges of the forward contraction and their length
 };
 
 // Work list entry of the column kernels (forward and VJP stage 1): one CTA = one (k-block, datapoint range).

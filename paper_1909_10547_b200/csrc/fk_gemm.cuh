@@ -42,6 +42,9 @@ struct GemmFwdParams {
     int nfrag;             // 8-replica fragments in use (<= 16)
     int nfw;               // fragments per warp column (2 warp columns; <= 8)
     int ksplit, kper;      // K ranges and their length (multiple of GEMM_KT)
+    // grouped launch: one CTA per item (table, datapoint tile, K range); per-table kdec / offsets in descs
+    const TableDesc* descs;
+    const ColSeg* items;   // {table, kblock = datapoint tile, split = K range}
 };
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32_t src_bytes) {
@@ -80,7 +83,7 @@ __global__ void __launch_bounds__(256) fk_transpose_f_kernel(const T* __restrict
     }
 }
 
-template <int VEC>
+template <int VEC, bool GROUPED>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
     extern __shared__ __align__(16) unsigned char fk_smem[];
@@ -88,13 +91,31 @@ fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
     double* Ls = As + GEMM_STAGES * GEMM_BM * GEMM_SA;                 // [2][KT][SB]
     const uint32_t As_s = (uint32_t)__cvta_generic_to_shared(As);
 
-    const TableDesc& d = p.desc;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int mtiles = (d.N + GEMM_BM - 1) / GEMM_BM;
-    const int mt = blockIdx.x % mtiles, ks = blockIdx.x / mtiles;
+    const TableDesc* dp = &p.desc;
+    const uint32_t* __restrict__ kdec = p.kdec;
+    const double* __restrict__ fT = p.fT;
+    double* gpart = p.gpart;
+    int mt, ks, kper;
+    if constexpr (GROUPED) {
+        const ColSeg it = p.items[blockIdx.x];
+        dp = &p.descs[it.table];
+        kdec = dp->kdec;
+        fT += dp->f_off * p.RP;
+        gpart += dp->gp_off * p.RP;
+        mt = it.kblock;
+        ks = it.split;
+        kper = dp->gkper;
+    } else {
+        const int mtiles = (p.desc.N + GEMM_BM - 1) / GEMM_BM;
+        mt = blockIdx.x % mtiles;
+        ks = blockIdx.x / mtiles;
+        kper = p.kper;
+    }
+    const TableDesc& d = *dp;
     const int m0 = mt * GEMM_BM;
-    const int kbeg = ks * p.kper;
-    const int kend = min(d.K, kbeg + p.kper);
+    const int kbeg = ks * kper;
+    const int kend = min(d.K, kbeg + kper);
     const int nk = kend > kbeg ? (kend - kbeg + GEMM_KT - 1) / GEMM_KT : 0;
     const bool had = d.kind == KIND_HADRONIC;
 
@@ -127,9 +148,9 @@ fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
             la[j] = make_double2(0.0, 0.0);
             lb[j] = make_double2(1.0, 1.0);
             if (ccol && k < kend) {
-                const uint32_t code = __ldg(p.kdec + k);
-                la[j] = __ldg(reinterpret_cast<const double2*>(p.fT + (long long)(code & 0xffffu) * p.RP) + c2);
-                if (had) lb[j] = __ldg(reinterpret_cast<const double2*>(p.fT + (long long)(code >> 16) * p.RP) + c2);
+                const uint32_t code = __ldg(kdec + k);
+                la[j] = __ldg(reinterpret_cast<const double2*>(fT + (long long)(code & 0xffffu) * p.RP) + c2);
+                if (had) lb[j] = __ldg(reinterpret_cast<const double2*>(fT + (long long)(code >> 16) * p.RP) + c2);
             }
         }
     };
@@ -154,7 +175,7 @@ fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
         for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     // ---- level-1 partial tile gpart[ks][n][c] (+)= acc, acc = 0 ----------------------------------------
-    double* out = p.gpart + (long long)ks * d.N * p.RP;
+    double* out = gpart + (long long)ks * d.N * p.RP;
     auto flush = [&](bool first) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -229,6 +250,53 @@ __global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const double* __res
     }
 }
 
+// last table t with prefix[t] <= x  (prefix has T + 1 entries)
+__device__ __forceinline__ int table_of(const int* __restrict__ prefix, int T, long long x) {
+    int lo = 0, hi = T;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (prefix[mid] <= x) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// grouped: fT_cat[global slot][c] = f_cat[f_off_t * R + (r0 + c) * slots_t + slot]
+template <typename T>
+__global__ void __launch_bounds__(256) fk_transpose_f_grouped_kernel(const T* __restrict__ f_cat, double* __restrict__ fT,
+                                                                      const int* __restrict__ ai_prefix, int ntab,
+                                                                      long long slots_total, int R, int r0, int RP) {
+    const long long total = slots_total * RP;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long gs = t / RP;
+        const int c = (int)(t - gs * RP), r = r0 + c;
+        const int tb = table_of(ai_prefix, ntab, gs);
+        const long long base = ai_prefix[tb], slots = ai_prefix[tb + 1] - base;
+        fT[t] = r < R ? (double)f_cat[base * R + (long long)r * slots + (gs - base)] : 0.0;
+    }
+}
+
+// grouped level 2: sigma_cat[global row][r0 + c] = sum over the K ranges of the row's table, fixed order
+template <typename T>
+__global__ void __launch_bounds__(256) fk_gemm_reduce_grouped_kernel(const double* __restrict__ gpart, T* __restrict__ sigma,
+                                                                      const TableDesc* __restrict__ descs,
+                                                                      const int* __restrict__ row_prefix, int ntab,
+                                                                      long long rows_total, int R, int r0, int RP) {
+    const long long total = rows_total * RP;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long grow = t / RP;
+        const int c = (int)(t - grow * RP);
+        if (r0 + c >= R) continue;
+        const int tb = table_of(row_prefix, ntab, grow);
+        const TableDesc& d = descs[tb];
+        const long long n = grow - row_prefix[tb];
+        const double* src = gpart + (d.gp_off + n) * RP + c;
+        const long long stride = (long long)d.N * RP;
+        double s = 0.0;
+        for (int ks = 0; ks < d.gksplit; ++ks) s += src[ks * stride];
+        sigma[grow * R + r0 + c] = (T)s;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // VJP stage 1 for R >> 1 (minimal-flop order): G[k][c] = sum_n FK[n][k] * g[n][r0 + c].
 // Same machinery with the FK tile used transposed: CTA = 128 consecutive k (1 KB of every row), the
@@ -239,6 +307,8 @@ struct GemmVjpParams {
     const double* gP;   // [N][RP]: g of this pass, replica innermost, zero padded
     double* G;          // [K][RP] column sums, replica innermost
     int RP, nfrag, nfw;
+    const TableDesc* descs;  // grouped launch: one CTA per item {table, kblock = 128-k tile}
+    const ColSeg* items;
 };
 
 constexpr int GEMMV_BK = 128;                // k per CTA tile (the M dimension of the MMA)
@@ -247,7 +317,7 @@ constexpr int GEMMV_S = GEMMV_BK + 4;        // shared row stride of both tiles
 constexpr int GEMMV_STAGES = 3;
 constexpr int GEMMV_SMEM_BYTES = GEMMV_STAGES * 2 * GEMMV_NT * GEMMV_S * 8;
 
-template <int VEC>
+template <int VEC, bool GROUPED>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 fk_gemm_vjp_kernel(const __grid_constant__ GemmVjpParams p) {
     extern __shared__ __align__(16) unsigned char fk_smem[];
@@ -255,9 +325,20 @@ fk_gemm_vjp_kernel(const __grid_constant__ GemmVjpParams p) {
     double* Bs = As + GEMMV_STAGES * GEMMV_NT * GEMMV_S;         // [STAGES][NT][S]  g tile, replica innermost
     const uint32_t As_s = (uint32_t)__cvta_generic_to_shared(As), Bs_s = (uint32_t)__cvta_generic_to_shared(Bs);
 
-    const TableDesc& d = p.desc;
+    const TableDesc* dp = &p.desc;
+    const double* __restrict__ gP = p.gP;
+    double* __restrict__ G = p.G;
+    int kt = blockIdx.x;
+    if constexpr (GROUPED) {
+        const ColSeg it = p.items[blockIdx.x];
+        dp = &p.descs[it.table];
+        gP += dp->out_off * p.RP;
+        G += dp->k_off * p.RP;
+        kt = it.kblock;
+    }
+    const TableDesc& d = *dp;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int k0 = blockIdx.x * GEMMV_BK;
+    const int k0 = kt * GEMMV_BK;
     const int nt = (d.N + GEMMV_NT - 1) / GEMMV_NT;
 
     auto load_stage = [&](int t) {
@@ -283,7 +364,7 @@ fk_gemm_vjp_kernel(const __grid_constant__ GemmVjpParams p) {
                 const int row = q / CH, cc = q - row * CH;
                 const int n = n0 + row;
                 const bool ok = n < d.N;
-                const double* src = p.gP + (long long)(ok ? n : 0) * p.RP + cc * 2;
+                const double* src = gP + (long long)(ok ? n : 0) * p.RP + cc * 2;
                 cp_async16(Bs_s + (uint32_t)(((slot * GEMMV_NT + row) * GEMMV_S + cc * 2) * 8), src, ok ? 16u : 0u);
             }
         }
@@ -334,7 +415,7 @@ fk_gemm_vjp_kernel(const __grid_constant__ GemmVjpParams p) {
         for (int j = 0; j < 8; ++j)
             if (j < nfw) {
                 const int c = cb + j * 8 + 2 * (lane & 3);
-                *reinterpret_cast<double2*>(p.G + (long long)k * p.RP + c) = make_double2(acc[i][j][0], acc[i][j][1]);
+                *reinterpret_cast<double2*>(G + (long long)k * p.RP + c) = make_double2(acc[i][j][0], acc[i][j][1]);
             }
     }
 }
@@ -359,22 +440,40 @@ struct GatherRParams {
     const double* G;    // [K][RP]
     void* df;           // [R][nfl][nx]
     int R, r0, RP;
+    const TableDesc* descs;  // grouped launch: blockIdx.x = global (alpha, i) slot
+    const int* ai_prefix;
+    int T;
 };
 
-template <typename T>
+template <typename T, bool GROUPED>
 __global__ void __launch_bounds__(128) fk_vjp_gather_r_kernel(const __grid_constant__ GatherRParams p) {
     __shared__ short listA[MAX_C], listB[MAX_C];
+    __shared__ uint8_t other[2][MAX_C];  // flavour of the opposite leg of every listed channel
     __shared__ int cnt[2];
-    const TableDesc& d = p.desc;
+    const TableDesc* dp = &p.desc;
+    const uint8_t* __restrict__ ca = p.chan.a;
+    const uint8_t* __restrict__ cb = p.chan.b;
+    const double* __restrict__ G = p.G;
+    const double* __restrict__ fT = p.fT;
+    int slot = blockIdx.x;
+    if constexpr (GROUPED) {
+        const int tb = table_of(p.ai_prefix, p.T, slot);
+        dp = &p.descs[tb];
+        slot -= p.ai_prefix[tb];
+        ca = dp->chan_a;
+        cb = dp->chan_b;
+        G += dp->k_off * p.RP;
+        fT += dp->f_off * p.RP;
+    }
+    const TableDesc& d = *dp;
     const int nx = d.nx, C = d.C;
-    const int slot = blockIdx.x;
     const int alpha = slot / nx, i = slot - alpha * nx;
     const bool had = d.kind == KIND_HADRONIC;
     if (threadIdx.x == 0) {
         int na = 0, nb = 0;
         for (int c = 0; c < C; ++c) {
-            if (p.chan.a[c] == alpha) listA[na++] = (short)c;
-            if (had && p.chan.b[c] == alpha) listB[nb++] = (short)c;
+            if (ca[c] == alpha) { other[0][na] = cb[c]; listA[na++] = (short)c; }
+            if (had && cb[c] == alpha) { other[1][nb] = ca[c]; listB[nb++] = (short)c; }
         }
         cnt[0] = na;
         cnt[1] = nb;
@@ -383,13 +482,13 @@ __global__ void __launch_bounds__(128) fk_vjp_gather_r_kernel(const __grid_const
     const int na = cnt[0], nb = cnt[1];
     const int c0 = blockIdx.y * blockDim.x + threadIdx.x;  // replica column of this pass
     if (c0 >= p.RP || p.r0 + c0 >= p.R) return;
-    const double* __restrict__ G = p.G + c0;
-    const double* __restrict__ fT = p.fT + c0;
+    G += c0;
+    fT += c0;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
     if (had) {
         for (int q = 0; q < na; ++q) {
             const int c = listA[q];
-            const long long fo = (long long)p.chan.b[c] * nx;
+            const long long fo = (long long)other[0][q] * nx;
             for (int j = 0; j < nx; ++j) {
                 const int k = encode_k(d, i, j, c);
                 acc[j & 3] = fma(G[(long long)k * p.RP], fT[(fo + j) * p.RP], acc[j & 3]);
@@ -397,7 +496,7 @@ __global__ void __launch_bounds__(128) fk_vjp_gather_r_kernel(const __grid_const
         }
         for (int q = 0; q < nb; ++q) {
             const int c = listB[q];
-            const long long fo = (long long)p.chan.a[c] * nx;
+            const long long fo = (long long)other[1][q] * nx;
             for (int j = 0; j < nx; ++j) {
                 const int k = encode_k(d, j, i, c);
                 acc[j & 3] = fma(G[(long long)k * p.RP], fT[(fo + j) * p.RP], acc[j & 3]);

@@ -18,6 +18,13 @@ struct fk_group {
     int nfsegs = 0;
     fk::ColSeg* d_csegs = nullptr;  // VJP stage-1 CTAs
     int ncsegs = 0;
+    // R >> 1 contraction (fk_gemm.cuh): items {table, datapoint tile, K range} / {table, 128-k tile}
+    bool gemm_ok = false;
+    fk::ColSeg* d_gitems = nullptr;
+    int ngitems = 0;
+    fk::ColSeg* d_vitems = nullptr;
+    int nvitems = 0;
+    long long gp_rows = 0, K_total = 0;
     double* scratch = nullptr;
     size_t scratch_elems = 0;
     int last_launches = 0;
@@ -35,10 +42,111 @@ int group_scratch(fk_group* g, size_t elems) {
     return FK_OK;
 }
 
+bool group_gemm_wanted(const fk_group* g, int R) {
+    return g->gemm_ok && g->dtype == FK_F64 && R >= env_int("FKCONV_GEMM_MIN_R", 5);
+}
+
+size_t group_scratch_need(const fk_group* g, int R) {
+    if (group_gemm_wanted(g, R)) {
+        const size_t RP = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+        const size_t fwd = (size_t)g->gp_rows, vjp = (size_t)g->rows_total + (size_t)g->K_total;
+        return ((size_t)g->ai_total + std::max(fwd, vjp)) * RP;
+    }
+    return std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * R;
+}
+
+int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, cudaStream_t s) {
+    const int RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    double* fT = g->scratch;
+    double* gpart = fT + (size_t)g->ai_total * RPmax;
+    static const bool attr_ok = [] {
+        return cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess &&
+               cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess;
+    }();
+    if (!attr_ok) return fail(FK_ERR_CUDA, "grouped gemm: cannot reserve %d bytes of shared memory", fk::GEMM_SMEM_BYTES);
+    int nl = 0;
+    for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
+        fk::GemmFwdParams p;
+        memset(&p, 0, sizeof p);
+        p.fT = fT;
+        p.gpart = gpart;
+        p.RP = (std::min(fk::GEMM_BN, R - r0) + 7) / 8 * 8;
+        p.nfrag = p.RP / 8;
+        p.nfw = (p.nfrag + 1) / 2;
+        p.descs = g->d_descs;
+        p.items = g->d_gitems;
+        const long long tf = g->ai_total * p.RP;
+        fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
+            f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, p.RP);
+        if (g->all_vec) fk::fk_gemm_fwd_kernel<2, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        else fk::fk_gemm_fwd_kernel<1, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        const long long outs = g->rows_total * p.RP;
+        fk::fk_gemm_reduce_grouped_kernel<double><<<(int)std::min<long long>(8192, (outs + 255) / 256), 256, 0, s>>>(
+            gpart, sigma_cat, g->d_descs, g->d_row_prefix, g->T, g->rows_total, R, r0, p.RP);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gemm forward launch failed: %s", cudaGetErrorString(e));
+        nl += 3;
+    }
+    g->last_launches = nl;
+    return FK_OK;
+}
+
+int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double* df_cat, int R, cudaStream_t s) {
+    const int RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    double* fT = g->scratch;
+    double* gP = fT + (size_t)g->ai_total * RPmax;
+    double* G = gP + (size_t)g->rows_total * RPmax;
+    static const bool attr_ok = [] {
+        return cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess &&
+               cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess;
+    }();
+    if (!attr_ok) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
+    int nl = 0;
+    for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
+        const int RP = (std::min(fk::GEMM_BN, R - r0) + 7) / 8 * 8;
+        const long long tf = g->ai_total * RP, tg = g->rows_total * RP;
+        fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
+            f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, RP);
+        // g_cat is [global row][R]: the single-table kernel pads all tables at once
+        fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(4096, (tg + 255) / 256), 256, 0, s>>>(g_cat, gP, (int)g->rows_total, R, r0, RP);
+        fk::GemmVjpParams p;
+        memset(&p, 0, sizeof p);
+        p.gP = gP;
+        p.G = G;
+        p.RP = RP;
+        p.nfrag = RP / 8;
+        p.nfw = (p.nfrag + 1) / 2;
+        p.descs = g->d_descs;
+        p.items = g->d_vitems;
+        if (g->all_vec) fk::fk_gemm_vjp_kernel<2, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        else fk::fk_gemm_vjp_kernel<1, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        fk::GatherRParams q;
+        memset(&q, 0, sizeof q);
+        q.fT = fT;
+        q.G = G;
+        q.df = df_cat;
+        q.R = R;
+        q.r0 = r0;
+        q.RP = RP;
+        q.descs = g->d_descs;
+        q.ai_prefix = g->d_ai_prefix;
+        q.T = g->T;
+        fk::fk_vjp_gather_r_kernel<double, true><<<dim3((unsigned)g->ai_total, (RP + 127) / 128), 128, 0, s>>>(q);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gemm vjp launch failed: %s", cudaGetErrorString(e));
+        nl += 4;
+    }
+    g->last_launches = nl;
+    return FK_OK;
+}
+
 template <typename T>
 int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStream_t s) {
-    int rc = group_scratch(g, std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * R);
+    int rc = group_scratch(g, group_scratch_need(g, R));
     if (rc) return rc;
+    if constexpr (std::is_same<T, double>::value) {
+        if (group_gemm_wanted(g, R)) return group_conv_gemm(g, (const double*)f_cat, (double*)sigma_cat, R, s);
+    }
     int nl = 0;
     fk::FwdParams p;
     memset(&p, 0, sizeof p);
@@ -79,8 +187,12 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
 
 template <typename T>
 int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat, int R, cudaStream_t s) {
-    int rc = group_scratch(g, std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * R);
+    int rc = group_scratch(g, group_scratch_need(g, R));
     if (rc) return rc;
+    if constexpr (std::is_same<T, double>::value) {
+        if (group_gemm_wanted(g, R))
+            return group_vjp_gemm(g, (const double*)f_cat, (const double*)g_cat, (double*)df_cat, R, s);
+    }
     int nl = 0;
     fk::ColsumParams p;
     memset(&p, 0, sizeof p);
@@ -135,10 +247,33 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
         if (tb->dtype != g->dtype) { delete g; return fail(FK_ERR_INVALID_ARG, "fk_group_create: mixed dtypes"); }
         g->all_vec = g->all_vec && tb->desc.vec_ok;
     }
-    std::vector<fk::ColSeg> fsegs, csegs;
+    // R >> 1 contraction: every item (128-datapoint tile x K range) costs about the same DMMA time
+    g->gemm_ok = g->dtype == FK_F64;
+    long long tile_k = 0;
+    for (int t = 0; t < T; ++t) {
+        g->gemm_ok = g->gemm_ok && tables[t]->kdec != nullptr;
+        tile_k += (long long)((tables[t]->desc.N + fk::GEMM_BM - 1) / fk::GEMM_BM) * tables[t]->desc.K;
+    }
+    const long long want_items = (long long)std::max(1, sm_count()) * std::max(1, env_int("FKCONV_GROUP_GEMM_WAVES", 4));
+    long long kper_target = (tile_k + want_items - 1) / want_items;
+    kper_target = std::max<long long>(fk::GEMM_KT * 8, (kper_target + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT);
+    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems;
     for (int t = 0; t < T; ++t) {
         fk_table* tb = tables[t];
         fk::TableDesc d = tb->desc;
+        {
+            const int ksplit0 = (int)std::max<long long>(1, (d.K + kper_target - 1) / kper_target);
+            d.gkper = ((d.K + ksplit0 - 1) / ksplit0 + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT;
+            d.gksplit = (d.K + d.gkper - 1) / d.gkper;
+            d.gp_off = g->gp_rows;
+            d.k_off = g->K_total;
+            g->gp_rows += (long long)d.gksplit * d.N;
+            g->K_total += d.K;
+            const int mtiles = (d.N + fk::GEMM_BM - 1) / fk::GEMM_BM;
+            for (int ks = 0; ks < d.gksplit; ++ks)
+                for (int mt = 0; mt < mtiles; ++mt) gitems.push_back(fk::ColSeg{t, mt, ks, 0});
+            for (int kt = 0; kt < (d.K + fk::GEMMV_BK - 1) / fk::GEMMV_BK; ++kt) vitems.push_back(fk::ColSeg{t, kt, 0, 0});
+        }
         if (!g->all_vec && d.vec_ok) {  // one kernel instantiation per launch: the whole group takes the 64-bit path
             d.vec_ok = 0;
             Plan pl;
@@ -169,6 +304,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     }
     g->nfsegs = (int)fsegs.size();
     g->ncsegs = (int)csegs.size();
+    g->ngitems = (int)gitems.size();
+    g->nvitems = (int)vitems.size();
     auto bail = [&](int code) { fk_group_destroy(g); return code; };
     cudaError_t e = cudaMalloc((void**)&g->d_descs, T * sizeof(fk::TableDesc));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_row_prefix, (T + 1) * sizeof(int));
@@ -176,12 +313,16 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_csegs, csegs.size() * sizeof(fk::ColSeg));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_fsegs, fsegs.size() * sizeof(fk::ColSeg));
     if (e == cudaSuccess) e = cudaMemcpy(g->d_fsegs, fsegs.data(), fsegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_gitems, gitems.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_vitems, vitems.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_gitems, gitems.data(), gitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_vitems, vitems.data(), vitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_descs, g->descs.data(), T * sizeof(fk::TableDesc), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_row_prefix, row_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_ai_prefix, ai_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_csegs, csegs.data(), csegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_group_create: %s", cudaGetErrorString(e)); }
-    int rc = group_scratch(g, std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * std::max(1, R_hint));
+    int rc = group_scratch(g, std::max(group_scratch_need(g, 1), group_scratch_need(g, std::max(1, R_hint))));
     if (rc) return bail(rc);
     *out = g;
     return FK_OK;
@@ -194,6 +335,8 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_ai_prefix) cudaFree(g->d_ai_prefix);
     if (g->d_csegs) cudaFree(g->d_csegs);
     if (g->d_fsegs) cudaFree(g->d_fsegs);
+    if (g->d_gitems) cudaFree(g->d_gitems);
+    if (g->d_vitems) cudaFree(g->d_vitems);
     if (g->scratch) cudaFree(g->scratch);
     delete g;
     return FK_OK;

@@ -197,7 +197,7 @@ def test_host_buffer_calls(K):
 
 
 # ------------------------------------------------------------------ grouped ragged launch
-@pytest.mark.parametrize("R", [1, 3])
+@pytest.mark.parametrize("R", [1, 3, 6, 130])
 @pytest.mark.parametrize("store", ["pack", "borrow"])
 def test_grouped_small_ragged(K, R, store):
     import torch
@@ -225,10 +225,11 @@ def test_grouped_small_ragged(K, R, store):
     assert grp.last_launches() >= 2
 
 
-def test_grouped_mixed_dis_and_hadronic(K):
-    """A 'global' group: DIS and hadronic tables in one launch."""
+@pytest.mark.parametrize("R", [2, 9])
+def test_grouped_mixed_dis_and_hadronic(K, R):
+    """A 'global' group: DIS and hadronic tables in one launch; R=9 takes the
+    grouped R >> 1 contraction."""
     import torch
-    R = 2
     h = synth.hadronic_case(6, 30, 12, 17, R, sub=7)
     d = synth.config1(R=R, N=200)
     th = K.FkTable(K.FK_KIND_HADRONIC, to_dev(h.fk), h.pairs, h.nfl)
