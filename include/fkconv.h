@@ -53,7 +53,8 @@ enum { FK_KIND_DIS = 0, FK_KIND_HADRONIC = 1 };
 enum { FK_F64 = 0, FK_F32 = 1 };
 /* table storage: BORROW keeps the caller's logical-layout buffer (no copy; it must outlive the
  * table); PACK copies into the library's device layout: channel-major, x innermost
- * ([N][C][nx][nx] resp. [N][nA][nx]), each datapoint row padded to a multiple of 16 bytes. */
+ * ([N][C][nx*nx rounded up to 4, zero padded] resp. [N][nA][nx]), each datapoint row padded to a
+ * multiple of 16 bytes, so every channel block and every row starts on a 32- resp. 16-byte boundary. */
 enum { FK_STORE_BORROW = 0, FK_STORE_PACK = 1 };
 
 typedef struct fk_table fk_table; /* opaque: one FK table resident in HBM + its scratch */

@@ -145,7 +145,7 @@ int check_dims(const char* who, int kind, int N, int nx, int nfl, int C, int R) 
         return fail(FK_ERR_INVALID_ARG, "%s: non-positive size (N=%d nx=%d nfl=%d C=%d R=%d)", who, N, nx, nfl, C, R);
     if (nfl > fk::MAX_NFL || C > fk::MAX_C)
         return fail(FK_ERR_UNSUPPORTED, "%s: nfl=%d > %d or C=%d > %d", who, nfl, fk::MAX_NFL, C, fk::MAX_C);
-    const long long K = kind == FK_KIND_HADRONIC ? (long long)C * nx * nx : (long long)C * nx;
+    const long long K = kind == FK_KIND_HADRONIC ? (long long)C * ((long long)nx * nx + 3) : (long long)C * nx;
     if (K >= (1LL << 31) - 4096) return fail(FK_ERR_UNSUPPORTED, "%s: K=%lld does not fit 31 bits", who, K);
     if ((long long)nfl * nx >= (1LL << 24)) return fail(FK_ERR_UNSUPPORTED, "%s: nfl*nx too large", who);
     if (kind == FK_KIND_DIS && C > nfl)
@@ -171,7 +171,8 @@ fk::TableDesc make_desc(int kind, int layout, const void* fkp, int N, int nx, in
     fk::TableDesc d;
     memset(&d, 0, sizeof d);
     d.fk = fkp;
-    d.K = kind == FK_KIND_HADRONIC ? C * nx * nx : C * nx;
+    d.cstride = (layout == fk::LAYOUT_PACKED && kind == FK_KIND_HADRONIC) ? (nx * nx + 3) / 4 * 4 : nx * nx;
+    d.K = kind == FK_KIND_HADRONIC ? C * d.cstride : C * nx;
     d.row_stride = row_stride > 0 ? row_stride : d.K;
     d.N = N; d.nx = nx; d.nfl = nfl; d.C = C;
     d.kind = kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS;
@@ -628,7 +629,8 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
     if (rc) { delete t; return rc; }
     t->dtype = dtype; t->store = store; t->kind = kind;
 
-    const int K = kind == FK_KIND_HADRONIC ? C * nx * nx : C * nx;
+    const int cstride = (nx * nx + 3) / 4 * 4;  // packed hadronic channel block (fk_common.cuh)
+    const int K = kind == FK_KIND_HADRONIC ? C * (store == FK_STORE_PACK ? cstride : nx * nx) : C * nx;
     auto bail = [&](int code) { fk_table_destroy(t); return code; };
     if (store == FK_STORE_PACK) {
         const int vecw = dtype == FK_F64 ? 2 : 4;
@@ -640,10 +642,10 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
         const int grid = (int)std::min<long long>((total + 255) / 256, 148LL * 64);
         if (dtype == FK_F64)
             fk::fk_pack_kernel<double><<<grid, 256>>>(fk_logical, (double*)t->owned_fk, N, nx, C,
-                                                     kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, row_stride);
+                                                     kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, cstride, row_stride);
         else
             fk::fk_pack_kernel<float><<<grid, 256>>>(fk_logical, (float*)t->owned_fk, N, nx, C,
-                                                    kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, row_stride);
+                                                    kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, cstride, row_stride);
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaDeviceSynchronize();
         if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: pack kernel: %s", cudaGetErrorString(e)); }

@@ -10,7 +10,7 @@ namespace fk {
 constexpr int KIND_DIS = 0;
 constexpr int KIND_HADRONIC = 1;
 constexpr int LAYOUT_LOGICAL = 0;  // hadronic k = (i*nx + j)*C + c ; DIS k = i*nA + c   (BASELINE.json order)
-constexpr int LAYOUT_PACKED = 1;   // hadronic k = (c*nx + i)*nx + j ; DIS k = c*nx + i   (x innermost)
+constexpr int LAYOUT_PACKED = 1;   // hadronic k = c*cstride + i*nx + j, cstride = nx*nx rounded up to 4 (zero padded) ; DIS k = c*nx + i
 
 constexpr int MAX_C = 1024;   // active flavour pairs / flavours per table
 constexpr int MAX_NFL = 256;  // flavour indices are stored as uint8
@@ -28,6 +28,7 @@ struct TableDesc {
     long long row_stride; // elements (>= K; PACK pads it to a 16-byte multiple)
     int K;                // contraction length per datapoint: C*nx*nx (hadronic) or nA*nx (DIS)
     int N, nx, nfl, C;
+    int cstride;          // PACKED hadronic: elements per channel block (nx*nx rounded up to a multiple of 4)
     int kind, layout;
     int vec_ok;           // rows are 16-byte aligned -> 128-bit loads
     // grouped launches only
@@ -53,7 +54,7 @@ struct ColSeg {
 };
 
 // Offsets (inside one replica's f[nfl][nx]) of the two PDF factors of contraction index k.
-// Hadronic: L[k] = f[ia] * f[ib];  DIS: L[k] = f[ia] (ib = -1).
+// Hadronic: L[k] = f[ia] * f[ib];  DIS: L[k] = f[ia] (ib = -1);  ia = -1: padding, L[k] = 0.
 __device__ __forceinline__ void decode_k(const TableDesc& d, const uint8_t* __restrict__ ca,
                                          const uint8_t* __restrict__ cb, int k, int& ia, int& ib) {
     const int nx = d.nx;
@@ -65,10 +66,14 @@ __device__ __forceinline__ void decode_k(const TableDesc& d, const uint8_t* __re
             i = p / nx;
             j = p - i * nx;
         } else {
-            const int q = k / nx;
-            j = k - q * nx;
-            c = q / nx;
-            i = q - c * nx;
+            c = k / d.cstride;
+            const int rem = k - c * d.cstride;
+            if (rem >= nx * nx) {  // zero padding at the end of a channel block: no luminosity
+                ia = ib = -1;
+                return;
+            }
+            i = rem / nx;
+            j = rem - i * nx;
         }
         ia = (int)ca[c] * nx + i;
         ib = (int)cb[c] * nx + j;
@@ -89,7 +94,7 @@ __device__ __forceinline__ void decode_k(const TableDesc& d, const uint8_t* __re
 // Contraction index of (i, j, c) resp. (i, c) in the table's k-order (inverse of decode_k).
 __device__ __forceinline__ int encode_k(const TableDesc& d, int i, int j, int c) {
     if (d.kind == KIND_HADRONIC)
-        return d.layout == LAYOUT_LOGICAL ? (i * d.nx + j) * d.C + c : (c * d.nx + i) * d.nx + j;
+        return d.layout == LAYOUT_LOGICAL ? (i * d.nx + j) * d.C + c : c * d.cstride + i * d.nx + j;
     return d.layout == LAYOUT_LOGICAL ? i * d.C + c : c * d.nx + i;
 }
 

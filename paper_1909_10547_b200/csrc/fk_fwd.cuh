@@ -94,8 +94,9 @@ fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
 #pragma unroll
         for (int e = 0; e < VEC; ++e) {
             int ia = 0, ib = -1;
-            const bool in = k + e < d.K;
+            bool in = k + e < d.K;
             if (in) decode_k(d, ca, cb, k + e, ia, ib);
+            in = in && ia >= 0;
 #pragma unroll
             for (int r = 0; r < RT; ++r) {
                 const int rr = p.r0 + r;

@@ -67,7 +67,8 @@ __global__ void __launch_bounds__(256) fk_kdec_kernel(TableDesc d, ChannelList c
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < d.K; k += gridDim.x * blockDim.x) {
         int ia, ib;
         decode_k(d, chan.a, chan.b, k, ia, ib);
-        kdec[k] = (uint32_t)ia | ((ib >= 0 ? (uint32_t)ib : KDEC_NONE) << 16);
+        // padding (ia < 0): FK is exactly 0 there, any finite luminosity will do -> slots (0, 0)
+        kdec[k] = ia < 0 ? 0u : ((uint32_t)ia | ((ib >= 0 ? (uint32_t)ib : KDEC_NONE) << 16));
     }
 }
 

@@ -8,11 +8,12 @@
 
 namespace fk {
 
-// out[n][kp] = (T) in[n][klog(kp)],  kp in packed order; pad columns [K, row_stride) = 0
+// out[n][kp] = (T) in[n][klog(kp)],  kp in packed order (hadronic: channel blocks of cstride elements,
+// the tail of each block zero); pad columns [K, row_stride) = 0
 template <typename T>
 __global__ void __launch_bounds__(256)
 fk_pack_kernel(const double* __restrict__ in, T* __restrict__ out, int N, int nx, int C, int kind,
-               int K, long long row_stride) {
+               int K, int cstride, long long row_stride) {
     const long long total = (long long)N * row_stride;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
          t += (long long)gridDim.x * blockDim.x) {
@@ -20,16 +21,21 @@ fk_pack_kernel(const double* __restrict__ in, T* __restrict__ out, int N, int nx
         const int kp = (int)(t - n * row_stride);
         T v = T(0);
         if (kp < K) {
-            int klog;
+            int klog = -1;
+            long long klen;  // logical row length
             if (kind == KIND_HADRONIC) {
-                const int q = kp / nx, j = kp - q * nx;
-                const int c = q / nx, i = q - c * nx;
-                klog = (i * nx + j) * C + c;
+                const int c = kp / cstride, rem = kp - c * cstride;
+                if (rem < nx * nx) {
+                    const int i = rem / nx, j = rem - i * nx;
+                    klog = (i * nx + j) * C + c;
+                }
+                klen = (long long)C * nx * nx;
             } else {
                 const int c = kp / nx, i = kp - c * nx;
                 klog = i * C + c;
+                klen = (long long)C * nx;
             }
-            v = (T)in[n * (long long)K + klog];  // fp64 -> fp32: cvt.rn
+            if (klog >= 0) v = (T)in[n * klen + klog];  // fp64 -> fp32: cvt.rn
         }
         out[t] = v;
     }
