@@ -20,6 +20,7 @@
 
 #include "fk_common.cuh"
 #include "fk_gemm.cuh"
+#include "fk_gemm_ws.cuh"
 #include "fk_pack.cuh"
 #include "fk_fwd.cuh"
 #include "fk_vjp.cuh"
@@ -244,6 +245,14 @@ size_t gemm_fwd_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
     return (size_t)d.nfl * d.nx * gp.RPmax + (size_t)gp.ksplit * d.N * gp.RPmax + (with_kdec ? ((size_t)d.K + 1) / 2 : 0);
 }
 
+constexpr size_t MAX_DYN_SMEM = 232448;  // 227 KB per CTA on sm_100a
+
+// the warp-specialised kernel (fk_gemm_ws.cuh) serves packed hadronic tables whose f[b_c] tiles fit next to the FK ring
+bool ws_ok(const fk::TableDesc& d, int RP) {
+    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok && env_int("FKCONV_WS", 1) &&
+           fk::ws_smem_bytes(d.nx, RP) <= MAX_DYN_SMEM;
+}
+
 int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint32_t* kdec, const double* f,
                   double* sigma, int R, double* scratch, cudaStream_t s, int* launches) {
     const GemmPlan gp = gemm_plan(d, R);
@@ -251,7 +260,13 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
     double* fT = scratch;
     double* gpart = fT + (size_t)slots * gp.RPmax;
     int nl = 0;
-    if (!kdec) {
+    const bool ws = ws_ok(d, gp.RPmax);
+    if (ws) {
+        static const bool ws_attr = cudaFuncSetAttribute(fk::fk_gemm_fwd_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                         (int)MAX_DYN_SMEM) == cudaSuccess;
+        if (!ws_attr) return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
+    }
+    if (!kdec && !ws) {
         uint32_t* kd = reinterpret_cast<uint32_t*>(gpart + (size_t)gp.ksplit * d.N * gp.RPmax);
         fk::fk_kdec_kernel<<<std::min(1024, (d.K + 255) / 256), 256, 0, s>>>(d, ch, kd);
         ++nl;
@@ -279,7 +294,20 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
         fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
         size_t slot = 0;
         const bool timed = r0 == 0 && g_prof.begin(s, slot);
-        if (d.vec_ok) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        if (ws) {
+            fk::WsFwdParams w;
+            memset(&w, 0, sizeof w);
+            w.desc = d;
+            w.chan = ch;
+            w.fT = fT;
+            w.gpart = gpart;
+            w.RP = p.RP;
+            w.nfrag = p.nfrag;
+            w.nfw = p.nfw;
+            w.ksplit = gp.ksplit;
+            w.kper = gp.kper;
+            fk::fk_gemm_fwd_ws_kernel<false><<<mtiles * gp.ksplit, fk::WS_THREADS, fk::ws_smem_bytes(d.nx, p.RP), s>>>(w);
+        } else if (d.vec_ok) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_fwd_kernel<1, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         if (timed) g_prof.end(s, slot);
         const long long outs = (long long)d.N * p.RP;

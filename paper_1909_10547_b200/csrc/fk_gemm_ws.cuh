@@ -1,0 +1,272 @@
+// fk_gemm_ws.cuh -- R >> 1 dense contraction for PACKED hadronic tables, warp-specialised (SURVEY 8(a) rows a1 + a4).
+//
+//   Sigma[n][r] = sum_k FK[n][k] * L[k][r],   L[(c,i,j)][r] = f[r][a_c][i] * f[r][b_c][j]       Eq. (1)
+//
+// What differs from the generic kernel in fk_gemm.cuh (which stays for logical-layout and DIS tables):
+//   * one PRODUCER warp moves data with bulk async copies (cp.async.bulk, UBLKCP) that complete on
+//     mbarriers; eight CONSUMER warps do nothing but shared-memory fragment loads and DMMA.  The consumers
+//     never compute a global address and never meet at a CTA-wide barrier, so the FP64 tensor pipe does not
+//     drain once per K-tile while every warp plays producer (ncu on the generic kernel: 2 warps per
+//     scheduler stall together at each stage hand-over).
+//   * the luminosity tile is never built.  In the packed order k = c*cstride + i*nx + j the factor
+//     f[b_c][j] of a whole channel is one contiguous [nx][RP] block of the replica-innermost copy fT: it is
+//     bulk-copied into shared memory once per channel (double buffered) and serves nx*nx values of k;
+//     the other factor f[a_c][i] changes every nx steps of k and lives in 8 registers per thread.  The B
+//     fragment of an MMA k-step is formed at load time: b = fB[j][r] * fA[i][r]  (8 DMUL per 32 DMMA).
+//     No k -> (slot, slot) codes, no gathers, no luminosity tile in shared memory or HBM.
+//   * FK tiles [128 n][32 k] arrive as one 256-byte bulk copy per datapoint row into rows padded to 36
+//     doubles (conflict-free A fragments); channel blocks are padded to 4 elements by the pack kernel, so an
+//     MMA k-step never straddles a channel and every copy is 32-byte aligned.
+// Split-K partials, the periodic flush that bounds the accumulation chains, and the fixed-order level-2
+// reduction are those of fk_gemm.cuh.  Results are bitwise repeatable.
+#pragma once
+
+#include "fk_common.cuh"
+#include "fk_gemm.cuh"
+
+namespace fk {
+
+constexpr int WS_CONSUMER_WARPS = 8;
+constexpr int WS_THREADS = (WS_CONSUMER_WARPS + 4) * 32;  // + the producer's warpgroup (1 working warp): register
+                                                          // reallocation (setmaxnreg) works on whole warpgroups
+constexpr int WS_STAGES = 3;
+constexpr int WS_STAGE_DOUBLES = GEMM_BM * GEMM_SA;        // FK tile [128][36]
+constexpr int WS_NBAR = 2 * WS_STAGES + 4;                 // full[S], empty[S], fb_full[2], fb_empty[2]
+
+__host__ __device__ inline size_t ws_smem_bytes(int nx, int RP) {
+    return (size_t)(WS_STAGES * WS_STAGE_DOUBLES + 2 * nx * (RP + 4)) * 8 + WS_NBAR * 8;
+}
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nW_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra D_%=;\nbra W_%=;\nD_%=:\n}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
+// Same fields as GemmFwdParams where they mean the same thing.
+struct WsFwdParams {
+    TableDesc desc;        // single-table launch
+    ChannelList chan;      // single-table launch
+    const double* fT;      // [nfl*nx][RP] replica-innermost f (grouped: + desc.f_off * RP)
+    double* gpart;         // [ksplit][N][RP] level-1 partials (grouped: + desc.gp_off * RP)
+    int RP, nfrag, nfw;
+    int ksplit, kper;      // single-table launch
+    const TableDesc* descs;  // grouped launch
+    const ColSeg* items;     // grouped launch {table, datapoint tile, K range}
+};
+
+template <bool GROUPED>
+__global__ void __launch_bounds__(WS_THREADS, 1)
+fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
+    extern __shared__ __align__(128) unsigned char fk_smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    const TableDesc* dp = &p.desc;
+    const uint8_t* __restrict__ cha = p.chan.a;
+    const uint8_t* __restrict__ chb = p.chan.b;
+    const double* __restrict__ fT = p.fT;
+    double* gpart = p.gpart;
+    int mt, ks, kper;
+    if constexpr (GROUPED) {
+        const ColSeg it = p.items[blockIdx.x];
+        dp = &p.descs[it.table];
+        cha = dp->chan_a;
+        chb = dp->chan_b;
+        fT += dp->f_off * p.RP;
+        gpart += dp->gp_off * p.RP;
+        mt = it.kblock;
+        ks = it.split;
+        kper = dp->gkper;
+    } else {
+        const int mtiles = (p.desc.N + GEMM_BM - 1) / GEMM_BM;
+        mt = blockIdx.x % mtiles;
+        ks = blockIdx.x / mtiles;
+        kper = p.kper;
+    }
+    const TableDesc& d = *dp;
+    const int nx = d.nx, RP = p.RP, SB = RP + 4, cstride = d.cstride;
+    const int m0 = mt * GEMM_BM;
+    const int kbeg = ks * kper, kend = min(d.K, kbeg + kper);
+    if (kbeg >= kend) return;
+    const int c0 = kbeg / cstride, c1 = (kend - 1) / cstride;
+
+    double* As = reinterpret_cast<double*>(fk_smem);       // [STAGES][128][36]
+    double* Bs = As + WS_STAGES * WS_STAGE_DOUBLES;         // [2][nx][SB]   f[b_c][j][r] of two channels
+    const uint32_t As_s = (uint32_t)__cvta_generic_to_shared(As);
+    const uint32_t Bs_s = (uint32_t)__cvta_generic_to_shared(Bs);
+    const uint32_t bar0 = Bs_s + (uint32_t)(2 * nx * SB * 8);
+    auto bar_full = [&](int s) { return bar0 + 8u * s; };
+    auto bar_empty = [&](int s) { return bar0 + 8u * (WS_STAGES + s); };
+    auto bar_fbfull = [&](int b) { return bar0 + 8u * (2 * WS_STAGES + b); };
+    auto bar_fbempty = [&](int b) { return bar0 + 8u * (2 * WS_STAGES + 2 + b); };
+    if (tid == 0) {
+        for (int s = 0; s < WS_STAGES; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_empty(s), WS_CONSUMER_WARPS);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_fbfull(b), 1);
+            mbar_init(bar_fbempty(b), WS_CONSUMER_WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp >= WS_CONSUMER_WARPS) {
+        // ================================ producer warp ================================
+        // 384 threads cap the kernel at 168 registers; the producer warpgroup hands its share to the consumers
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
+        if (warp != WS_CONSUMER_WARPS) return;
+        const double* __restrict__ fk = reinterpret_cast<const double*>(d.fk);
+        const int rows_valid = min(GEMM_BM, d.N - m0);
+        auto issue_fb = [&](int c, int ccn) {  // f[b_c][.][.] of channel c -> buffer ccn & 1
+            const int buf = ccn & 1;
+            mbar_wait(bar_fbempty(buf), ((ccn >> 1) & 1) ^ 1);
+            if (lane == 0) mbar_expect_tx(bar_fbfull(buf), (uint32_t)(nx * RP * 8));
+            __syncwarp();
+            const double* src = fT + (long long)chb[c] * nx * RP;
+            for (int row = lane; row < nx; row += 32)
+                bulk_g2s(Bs_s + (uint32_t)((buf * nx + row) * SB * 8), src + (long long)row * RP, (uint32_t)(RP * 8), bar_fbfull(buf));
+        };
+        int it = 0, cc = 0;
+        issue_fb(c0, 0);
+        for (int c = c0; c <= c1; ++c, ++cc) {
+            const int sb = max(kbeg, c * cstride), se = min(kend, (c + 1) * cstride);
+            bool next_issued = c == c1;
+            int tiles = 0;
+            for (int k0 = sb; k0 < se; k0 += GEMM_KT, ++it, ++tiles) {
+                // the buffer of channel c + 1 was released when the consumers left channel c - 1, which they
+                // had to do before tile WS_STAGES of this channel can be issued: this wait never blocks here
+                if (!next_issued && tiles == WS_STAGES) {
+                    issue_fb(c + 1, cc + 1);
+                    next_issued = true;
+                }
+                const int len = min(GEMM_KT, se - k0);
+                const int stage = it % WS_STAGES;
+                mbar_wait(bar_empty(stage), ((it / WS_STAGES) & 1) ^ 1);
+                if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(rows_valid * len * 8));
+                __syncwarp();
+#pragma unroll
+                for (int q = 0; q < GEMM_BM / 32; ++q) {
+                    const int row = lane + 32 * q;
+                    if (row < rows_valid)
+                        bulk_g2s(As_s + (uint32_t)(((stage * GEMM_BM + row) * GEMM_SA) * 8),
+                                 fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(len * 8), bar_full(stage));
+                }
+            }
+            if (!next_issued) issue_fb(c + 1, cc + 1);
+        }
+        return;
+    }
+
+    // ================================ consumer warps: warp tile 32 datapoints x (8 * nfw) replicas ================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
+    const int wm = warp & 3, wn = warp >> 2;
+    const int nfw = min(p.nfw, max(0, p.nfrag - wn * p.nfw));  // 8-replica fragments of this warp column
+    const int cbcol = wn * p.nfw * 8;
+    double acc[4][8][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    // level-1 partial tile gpart[ks][n][c] (+)= acc, acc = 0   (thread-private addresses, L2 resident)
+    double* out = gpart + (long long)ks * d.N * RP;
+    auto flush = [&](bool first) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int n = m0 + wm * 32 + i * 8 + (lane >> 2);
+            double2* q = reinterpret_cast<double2*>(out + (long long)n * RP + cbcol + 2 * (lane & 3));
+            double2 o[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) o[j] = (!first && j < nfw && n < d.N) ? q[j * 4] : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (j < nfw && n < d.N) {
+                    q[j * 4] = make_double2(acc[i][j][0] + o[j].x, acc[i][j][1] + o[j].y);
+                    acc[i][j][0] = acc[i][j][1] = 0.0;
+                }
+        }
+    };
+
+    int it = 0, cc = 0;
+    bool flushed = false;
+    for (int c = c0; c <= c1; ++c, ++cc) {
+        const int sb = max(kbeg, c * cstride), se = min(kend, (c + 1) * cstride);
+        const int buf = cc & 1;
+        mbar_wait(bar_fbfull(buf), (cc >> 1) & 1);
+        const double* Bt = Bs + (long long)buf * nx * SB + cbcol + (lane >> 2);
+        const double* __restrict__ fa_base = fT + (long long)cha[c] * nx * RP + cbcol + (lane >> 2);
+        // this lane's k of every MMA k-step is 4*step + (lane & 3): its own (i, j), walked incrementally
+        int i, j;
+        {
+            const int kl = sb - c * cstride + (lane & 3);
+            i = kl / nx;
+            j = kl - i * nx;
+        }
+        double fa[8];  // f[a_c][i][r] for the 8 replica columns of this lane's B fragments
+        auto load_fa = [&]() {
+            const double* src = fa_base + (long long)min(i, nx - 1) * RP;  // i == nx only on the zero padding
+#pragma unroll
+            for (int j8 = 0; j8 < 8; ++j8) fa[j8] = j8 < nfw ? __ldg(src + j8 * 8) : 0.0;
+        };
+        load_fa();
+        for (int k0 = sb; k0 < se; k0 += GEMM_KT, ++it) {
+            const int nsteps = min(GEMM_KT, se - k0) >> 2;
+            const int stage = it % WS_STAGES;
+            mbar_wait(bar_full(stage), (it / WS_STAGES) & 1);
+            const double* At = As + ((stage * GEMM_BM) + wm * 32 + (lane >> 2)) * GEMM_SA + (lane & 3);
+#pragma unroll
+            for (int s = 0; s < GEMM_KT / 4; ++s) {
+                if (s < nsteps) {
+                    double a[4], b[8];
+#pragma unroll
+                    for (int i4 = 0; i4 < 4; ++i4) a[i4] = At[i4 * 8 * GEMM_SA + s * 4];
+#pragma unroll
+                    for (int j8 = 0; j8 < 8; ++j8) b[j8] = j8 < nfw ? Bt[j * SB + j8 * 8] * fa[j8] : 0.0;
+#pragma unroll
+                    for (int j8 = 0; j8 < 8; ++j8)
+                        if (j8 < nfw) {
+#pragma unroll
+                            for (int i4 = 0; i4 < 4; ++i4) dmma884(acc[i4][j8][0], acc[i4][j8][1], a[i4], b[j8]);
+                        }
+                    j += 4;
+                    if (j >= nx) {
+                        do {
+                            j -= nx;
+                            ++i;
+                        } while (j >= nx);
+                        load_fa();
+                    }
+                    __syncwarp();
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty(stage));
+            if ((it + 1) % GEMM_FLUSH == 0) {
+                flush(!flushed);
+                flushed = true;
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_fbempty(buf));
+    }
+    flush(!flushed);
+}
+
+}  // namespace fk
