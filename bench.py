@@ -35,6 +35,7 @@ from paper_1909_10547_b200 import synth  # noqa: E402  (seeded inputs only; no m
 FP64_PEAK_TFLOPS = 37.2  # 148 SM x 64 FMA/clk x 2 x 1.965 GHz (probe: profiles/r01_fp64_peak.md)
 METRIC = "fk_convolution_achieved_hbm_bandwidth"
 UNIT = "GB/s"
+DOMINANT_KERNEL = "fk_fwd_column_kernel<double,2,1,8,0>"
 WORKLOAD = "config2: hadronic FK N=512 nx=50 nfl=14 C=100 R=1 fp64 (1.024 GB), forward + VJP per step"
 
 
@@ -379,7 +380,7 @@ def run_ours(args):
     fkb = case.fk.nbytes
     kernel_ms = kms.value if kcount.value > 0 else None
     roofline = {
-        "bound": "hbm", "kernel": "fk_stream_kernel<double,VEC=2,RT=1> (forward streaming contraction, rows a1+a2)",
+        "bound": "hbm", "kernel": DOMINANT_KERNEL + " (forward column kernel: luminosity + streaming contraction + level-1 reduction, rows a1+a2+a3)",
         "achieved": (fkb / kernel_ms / 1e6) if kernel_ms else None, "peak": peak, "unit": "GB/s",
         "frac": (fkb / kernel_ms / 1e6 / peak) if kernel_ms else None, "peak_source": peak_src,
         "kernel_ms": kernel_ms, "kernel_launches_timed": kcount.value, "bytes_per_launch": fkb,
@@ -415,14 +416,16 @@ def run_ours(args):
 
 
 def _ncu_traffic():
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary, if any."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(p):
-        try:
-            with open(p) as fh:
-                return json.load(fh).get("fk_stream_kernel_dram_bytes_per_launch")
-        except Exception:
-            return None
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    summary of the ncu --set full capture (profiles/r01_traffic.csv), or None."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    try:
+        with open(p) as fh:
+            for ln in fh:
+                if ln.startswith(DOMINANT_KERNEL + ","):
+                    return int(ln[len(DOMINANT_KERNEL) + 1:].split(",")[2])
+    except Exception:
+        pass
     return None
 
 
