@@ -235,7 +235,7 @@ GemmPlan gemm_plan(const fk::TableDesc& d, int R) {
     int ksplit = std::max(1, target / mtiles);
     gp.kper = ((d.K + ksplit - 1) / ksplit + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT;
     gp.ksplit = (d.K + gp.kper - 1) / gp.kper;
-    gp.RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    gp.RPmax = fk::gemm_rp(R);
     return gp;
 }
 
@@ -253,6 +253,26 @@ bool ws_ok(const fk::TableDesc& d, int RP) {
            fk::ws_smem_bytes(d.nx, RP) <= MAX_DYN_SMEM;
 }
 
+template <bool GROUPED>
+bool ws_set_attr() {
+    bool ok = true;
+#define FK_WS_ATTR(NFW) ok = ok && cudaFuncSetAttribute(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MAX_DYN_SMEM) == cudaSuccess
+    FK_WS_ATTR(1); FK_WS_ATTR(2); FK_WS_ATTR(3); FK_WS_ATTR(4); FK_WS_ATTR(5); FK_WS_ATTR(6); FK_WS_ATTR(7); FK_WS_ATTR(8);
+#undef FK_WS_ATTR
+    return ok;
+}
+
+// RP = 16 * NFW (fk::gemm_rp): one instantiation per fragment count of a warp column
+template <bool GROUPED>
+void ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) {
+    switch (w.RP / 16) {
+#define FK_WS_CASE(NFW) case NFW: fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, smem, s>>>(w); break
+        FK_WS_CASE(1); FK_WS_CASE(2); FK_WS_CASE(3); FK_WS_CASE(4); FK_WS_CASE(5); FK_WS_CASE(6); FK_WS_CASE(7);
+        default: FK_WS_CASE(8);
+#undef FK_WS_CASE
+    }
+}
+
 int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint32_t* kdec, const double* f,
                   double* sigma, int R, double* scratch, cudaStream_t s, int* launches) {
     const GemmPlan gp = gemm_plan(d, R);
@@ -262,8 +282,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
     int nl = 0;
     const bool ws = ws_ok(d, gp.RPmax);
     if (ws) {
-        static const bool ws_attr = cudaFuncSetAttribute(fk::fk_gemm_fwd_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                         (int)MAX_DYN_SMEM) == cudaSuccess;
+        static const bool ws_attr = ws_set_attr<false>();
         if (!ws_attr) return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
     }
     if (!kdec && !ws) {
@@ -285,7 +304,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
         p.kdec = kdec;
         p.fT = fT;
         p.gpart = gpart;
-        p.RP = (std::min(fk::GEMM_BN, R - r0) + 7) / 8 * 8;
+        p.RP = fk::gemm_rp(R - r0);
         p.nfrag = p.RP / 8;
         p.nfw = (p.nfrag + 1) / 2;
         p.ksplit = gp.ksplit;
@@ -302,11 +321,9 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
             w.fT = fT;
             w.gpart = gpart;
             w.RP = p.RP;
-            w.nfrag = p.nfrag;
-            w.nfw = p.nfw;
             w.ksplit = gp.ksplit;
             w.kper = gp.kper;
-            fk::fk_gemm_fwd_ws_kernel<false><<<mtiles * gp.ksplit, fk::WS_THREADS, fk::ws_smem_bytes(d.nx, p.RP), s>>>(w);
+            ws_launch<false>(w, mtiles * gp.ksplit, fk::ws_smem_bytes(d.nx, p.RP), s);
         } else if (d.vec_ok) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_fwd_kernel<1, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         if (timed) g_prof.end(s, slot);
@@ -323,13 +340,13 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
 
 // doubles: fT [slots][RPmax] + gP [N][RPmax] + G [K][RPmax]
 size_t gemm_vjp_scratch_elems(const fk::TableDesc& d, int R) {
-    const size_t RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    const size_t RPmax = fk::gemm_rp(R);
     return ((size_t)d.nfl * d.nx + (size_t)d.N + (size_t)d.K) * RPmax;
 }
 
 int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double* f, const double* g, double* df,
                  int R, double* scratch, cudaStream_t s, int* launches) {
-    const int RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    const int RPmax = fk::gemm_rp(R);
     const int slots = d.nfl * d.nx;
     double* fT = scratch;
     double* gP = fT + (size_t)slots * RPmax;
@@ -341,7 +358,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
     if (!attr_ok) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
     int nl = 0;
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
-        const int RP = (std::min(fk::GEMM_BN, R - r0) + 7) / 8 * 8;
+        const int RP = fk::gemm_rp(R - r0);
         const long long tf = (long long)slots * RP, tg = (long long)d.N * RP;
         fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tf + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, RP);
         fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(2048, (tg + 255) / 256), 256, 0, s>>>(g + d.out_off * R, gP, d.N, R, r0, RP);

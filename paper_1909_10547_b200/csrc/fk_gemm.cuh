@@ -33,6 +33,13 @@ constexpr int GEMM_FLUSH = 16;             // K-tiles between flushes of the reg
 constexpr int GEMM_SMEM_BYTES = (GEMM_STAGES * GEMM_BM * GEMM_SA + 2 * GEMM_KT * GEMM_SB) * 8;
 constexpr uint32_t KDEC_NONE = 0xffffu;    // DIS: no second factor
 
+// padded replica count of a pass over `r` replicas: a multiple of 16 (two warp columns of whole 8-replica
+// MMA fragments each, so that the fragment count per warp is a compile-time constant), at most GEMM_BN
+__host__ __device__ inline int gemm_rp(int r) {
+    const int rp = (r + 15) / 16 * 16;
+    return rp < GEMM_BN ? rp : GEMM_BN;
+}
+
 struct GemmFwdParams {
     TableDesc desc;
     const uint32_t* kdec;  // [K]: slot_a | slot_b << 16, slot = flavour * nx + x  (slot_b = KDEC_NONE for DIS)

@@ -64,13 +64,15 @@ struct WsFwdParams {
     ChannelList chan;      // single-table launch
     const double* fT;      // [nfl*nx][RP] replica-innermost f (grouped: + desc.f_off * RP)
     double* gpart;         // [ksplit][N][RP] level-1 partials (grouped: + desc.gp_off * RP)
-    int RP, nfrag, nfw;
+    int RP;                // padded replicas of this pass = 16 * NFW
     int ksplit, kper;      // single-table launch
     const TableDesc* descs;  // grouped launch
     const ColSeg* items;     // grouped launch {table, datapoint tile, K range}
 };
 
-template <bool GROUPED>
+// NFW = 8-replica fragments per warp column = RP / 16, a compile-time constant: the 4 x NFW DMMAs of a k-step
+// carry no predicates, so ptxas is free to batch the fragment loads and the DMULs ahead of them.
+template <int NFW, bool GROUPED>
 __global__ void __launch_bounds__(WS_THREADS, 1)
 fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
     extern __shared__ __align__(128) unsigned char fk_smem[];
@@ -177,13 +179,12 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
     // ================================ consumer warps: warp tile 32 datapoints x (8 * nfw) replicas ================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
     const int wm = warp & 3, wn = warp >> 2;
-    const int nfw = min(p.nfw, max(0, p.nfrag - wn * p.nfw));  // 8-replica fragments of this warp column
-    const int cbcol = wn * p.nfw * 8;
-    double acc[4][8][2];
+    const int cbcol = wn * NFW * 8;
+    double acc[4][NFW][2];
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        for (int j = 0; j < NFW; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     // level-1 partial tile gpart[ks][n][c] (+)= acc, acc = 0   (thread-private addresses, L2 resident)
     double* out = gpart + (long long)ks * d.N * RP;
@@ -192,15 +193,14 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
         for (int i = 0; i < 4; ++i) {
             const int n = m0 + wm * 32 + i * 8 + (lane >> 2);
             double2* q = reinterpret_cast<double2*>(out + (long long)n * RP + cbcol + 2 * (lane & 3));
-            double2 o[8];
+            double2 o[NFW];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) o[j] = (!first && j < nfw && n < d.N) ? q[j * 4] : make_double2(0.0, 0.0);
+            for (int j = 0; j < NFW; ++j) o[j] = (!first && n < d.N) ? q[j * 4] : make_double2(0.0, 0.0);
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-                if (j < nfw && n < d.N) {
-                    q[j * 4] = make_double2(acc[i][j][0] + o[j].x, acc[i][j][1] + o[j].y);
-                    acc[i][j][0] = acc[i][j][1] = 0.0;
-                }
+            for (int j = 0; j < NFW; ++j) {
+                if (n < d.N) q[j * 4] = make_double2(acc[i][j][0] + o[j].x, acc[i][j][1] + o[j].y);
+                acc[i][j][0] = acc[i][j][1] = 0.0;
+            }
         }
     };
 
@@ -219,13 +219,16 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
             i = kl / nx;
             j = kl - i * nx;
         }
-        double fa[8];  // f[a_c][i][r] for the 8 replica columns of this lane's B fragments
-        auto load_fa = [&]() {
-            const double* src = fa_base + (long long)min(i, nx - 1) * RP;  // i == nx only on the zero padding
+        // f[a_c][i][r] for the 8 replica columns of this lane's B fragments, and the same for row i + 1,
+        // fetched one x-row (nx values of k) ahead so that the row switch never waits for L2
+        double fa[NFW], fan[NFW];
+        auto load_row = [&](double (&dst)[NFW], int row) {
+            const double* src = fa_base + (long long)min(row, nx - 1) * RP;  // row >= nx only on the zero padding
 #pragma unroll
-            for (int j8 = 0; j8 < 8; ++j8) fa[j8] = j8 < nfw ? __ldg(src + j8 * 8) : 0.0;
+            for (int j8 = 0; j8 < NFW; ++j8) dst[j8] = __ldg(src + j8 * 8);
         };
-        load_fa();
+        load_row(fa, i);
+        load_row(fan, i + 1);
         for (int k0 = sb; k0 < se; k0 += GEMM_KT, ++it) {
             const int nsteps = min(GEMM_KT, se - k0) >> 2;
             const int stage = it % WS_STAGES;
@@ -234,31 +237,39 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
 #pragma unroll
             for (int s = 0; s < GEMM_KT / 4; ++s) {
                 if (s < nsteps) {
-                    double a[4], b[8];
+                    double a[4], b[NFW];
 #pragma unroll
                     for (int i4 = 0; i4 < 4; ++i4) a[i4] = At[i4 * 8 * GEMM_SA + s * 4];
 #pragma unroll
-                    for (int j8 = 0; j8 < 8; ++j8) b[j8] = j8 < nfw ? Bt[j * SB + j8 * 8] * fa[j8] : 0.0;
+                    for (int j8 = 0; j8 < NFW; ++j8) b[j8] = Bt[j * SB + j8 * 8] * fa[j8];
 #pragma unroll
-                    for (int j8 = 0; j8 < 8; ++j8)
-                        if (j8 < nfw) {
+                    for (int j8 = 0; j8 < NFW; ++j8)
 #pragma unroll
-                            for (int i4 = 0; i4 < 4; ++i4) dmma884(acc[i4][j8][0], acc[i4][j8][1], a[i4], b[j8]);
-                        }
+                        for (int i4 = 0; i4 < 4; ++i4) dmma884(acc[i4][j8][0], acc[i4][j8][1], a[i4], b[j8]);
                     j += 4;
                     if (j >= nx) {
-                        do {
-                            j -= nx;
-                            ++i;
-                        } while (j >= nx);
-                        load_fa();
+                        j -= nx;
+                        ++i;
+                        if (j < nx) {
+#pragma unroll
+                            for (int j8 = 0; j8 < NFW; ++j8) fa[j8] = fan[j8];
+                        } else {  // nx < 4: more than one row per MMA k-step
+                            do {
+                                j -= nx;
+                                ++i;
+                            } while (j >= nx);
+                            load_row(fa, i);
+                        }
+                        load_row(fan, i + 1);
                     }
                     __syncwarp();
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty(stage));
-            if ((it + 1) % GEMM_FLUSH == 0) {
+            // the two warp columns share the SM's four schedulers pairwise: they flush half a period apart, so one
+            // warp of a scheduler keeps the FP64 pipe busy while the other waits for its partials from L2
+            if ((it + 1 + wn * (GEMM_FLUSH / 2)) % GEMM_FLUSH == 0) {
                 flush(!flushed);
                 flushed = true;
             }

@@ -48,7 +48,7 @@ bool group_gemm_wanted(const fk_group* g, int R) {
 
 size_t group_scratch_need(const fk_group* g, int R) {
     if (group_gemm_wanted(g, R)) {
-        const size_t RP = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+        const size_t RP = fk::gemm_rp(R);
         const size_t fwd = (size_t)g->gp_rows, vjp = (size_t)g->rows_total + (size_t)g->K_total;
         return ((size_t)g->ai_total + std::max(fwd, vjp)) * RP;
     }
@@ -56,7 +56,7 @@ size_t group_scratch_need(const fk_group* g, int R) {
 }
 
 int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, cudaStream_t s) {
-    const int RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    const int RPmax = fk::gemm_rp(R);
     double* fT = g->scratch;
     double* gpart = fT + (size_t)g->ai_total * RPmax;
     static const bool attr_ok = [] {
@@ -70,7 +70,7 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
         memset(&p, 0, sizeof p);
         p.fT = fT;
         p.gpart = gpart;
-        p.RP = (std::min(fk::GEMM_BN, R - r0) + 7) / 8 * 8;
+        p.RP = fk::gemm_rp(R - r0);
         p.nfrag = p.RP / 8;
         p.nfw = (p.nfrag + 1) / 2;
         p.descs = g->d_descs;
@@ -92,7 +92,7 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
 }
 
 int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double* df_cat, int R, cudaStream_t s) {
-    const int RPmax = std::min(fk::GEMM_BN, (R + 7) / 8 * 8);
+    const int RPmax = fk::gemm_rp(R);
     double* fT = g->scratch;
     double* gP = fT + (size_t)g->ai_total * RPmax;
     double* G = gP + (size_t)g->rows_total * RPmax;
@@ -103,7 +103,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
     if (!attr_ok) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
     int nl = 0;
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
-        const int RP = (std::min(fk::GEMM_BN, R - r0) + 7) / 8 * 8;
+        const int RP = fk::gemm_rp(R - r0);
         const long long tf = g->ai_total * RP, tg = g->rows_total * RP;
         fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
             f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, RP);
