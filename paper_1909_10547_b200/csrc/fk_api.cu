@@ -21,6 +21,7 @@
 #include "fk_common.cuh"
 #include "fk_gemm.cuh"
 #include "fk_gemm_ws.cuh"
+#include "fk_vjp_fold.cuh"
 #include "fk_pack.cuh"
 #include "fk_fwd.cuh"
 #include "fk_vjp.cuh"
@@ -273,6 +274,29 @@ void ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) 
     }
 }
 
+// the persistent warp-specialised VJP contraction needs 16-byte aligned, 16-byte multiple row pieces
+bool wsv_ok(const fk::TableDesc& d) { return d.vec_ok && d.K % 2 == 0 && env_int("FKCONV_WS", 1); }
+
+template <bool GROUPED>
+bool wsv_set_attr() {
+    bool ok = true;
+#define FK_WSV_ATTR(NFW) ok = ok && cudaFuncSetAttribute(fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fk::WSV_SMEM_BYTES) == cudaSuccess
+    FK_WSV_ATTR(1); FK_WSV_ATTR(2); FK_WSV_ATTR(3); FK_WSV_ATTR(4); FK_WSV_ATTR(5); FK_WSV_ATTR(6); FK_WSV_ATTR(7); FK_WSV_ATTR(8);
+#undef FK_WSV_ATTR
+    return ok;
+}
+
+template <bool GROUPED>
+void wsv_launch(const fk::WsVjpParams& w, cudaStream_t s) {
+    const int grid = std::max(1, std::min(w.ntiles, sm_count() * std::max(1, env_int("FKCONV_WSV_CTAS_PER_SM", 1))));
+    switch (w.RP / 16) {
+#define FK_WSV_CASE(NFW) case NFW: fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break
+        FK_WSV_CASE(1); FK_WSV_CASE(2); FK_WSV_CASE(3); FK_WSV_CASE(4); FK_WSV_CASE(5); FK_WSV_CASE(6); FK_WSV_CASE(7);
+        default: FK_WSV_CASE(8);
+#undef FK_WSV_CASE
+    }
+}
+
 int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint32_t* kdec, const double* f,
                   double* sigma, int R, double* scratch, cudaStream_t s, int* launches) {
     const GemmPlan gp = gemm_plan(d, R);
@@ -338,10 +362,31 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
     return FK_OK;
 }
 
-// doubles: fT [slots][RPmax] + gP [N][RPmax] + G [K][RPmax]
+// the single-pass fold (fk_vjp_fold.cuh) serves packed hadronic tables with nx <= 64; others take the gather
+bool fold_ok(const fk::TableDesc& d) {
+    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.nx <= fk::FOLD_MAX_NX && env_int("FKCONV_FOLD", 1);
+}
+// x-row chunks per channel: the CTA count (channels x chunks) that fills whole waves best (1 CTA of 256 threads
+// per SM by registers), preferring fewer chunks (each chunk writes its own B partial)
+int fold_chunks(long long channels) {
+    const int forced = env_int("FKCONV_FOLD_CHUNKS", 0);
+    if (forced > 0) return std::min(8, forced);
+    const long long slots = std::max(1, sm_count());
+    int best = 1;
+    double best_eff = 0.0;
+    for (int n = 1; n <= 8; ++n) {
+        const long long ctas = channels * n, waves = (ctas + slots - 1) / slots;
+        const double eff = (double)ctas / (double)(waves * slots) - 0.01 * n;
+        if (eff > best_eff) { best_eff = eff; best = n; }
+    }
+    return best;
+}
+constexpr int FOLD_MAX_CHUNKS = 8;
+
+// doubles: fT [slots][RPmax] + gP [N][RPmax] + G [K][RPmax] + fold partials [C*nx][4 + chunks][RPmax]
 size_t gemm_vjp_scratch_elems(const fk::TableDesc& d, int R) {
     const size_t RPmax = fk::gemm_rp(R);
-    return ((size_t)d.nfl * d.nx + (size_t)d.N + (size_t)d.K) * RPmax;
+    return ((size_t)d.nfl * d.nx + (size_t)d.N + (size_t)d.K + (size_t)d.C * d.nx * (fk::FOLD_JQ + FOLD_MAX_CHUNKS)) * RPmax;
 }
 
 int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double* f, const double* g, double* df,
@@ -371,19 +416,50 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
         p.nfrag = RP / 8;
         p.nfw = (p.nfrag + 1) / 2;
         const int grid = (d.K + fk::GEMMV_BK - 1) / fk::GEMMV_BK;
-        if (d.vec_ok) fk::fk_gemm_vjp_kernel<2, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        if (wsv_ok(d)) {
+            static const bool wsv_attr = wsv_set_attr<false>();
+            if (!wsv_attr) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
+            fk::WsVjpParams w;
+            memset(&w, 0, sizeof w);
+            w.desc = d;
+            w.gP = gP;
+            w.G = G;
+            w.RP = RP;
+            w.ntiles = grid;
+            wsv_launch<false>(w, s);
+        } else if (d.vec_ok) fk::fk_gemm_vjp_kernel<2, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_vjp_kernel<1, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
-        fk::GatherRParams q;
-        memset(&q, 0, sizeof q);
-        q.desc = d;
-        q.chan = ch;
-        q.fT = fT;
-        q.G = G;
-        q.df = df;
-        q.R = R;
-        q.r0 = r0;
-        q.RP = RP;
-        fk::fk_vjp_gather_r_kernel<double, false><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
+        if (fold_ok(d)) {
+            fk::FoldParams q;
+            memset(&q, 0, sizeof q);
+            q.desc = d;
+            q.desc.cx_off = 0;
+            q.chan = ch;
+            q.fT = fT;
+            q.G = G;
+            q.PA = G + (size_t)d.K * RPmax;
+            q.PB = q.PA + (size_t)d.C * d.nx * fk::FOLD_JQ * RPmax;
+            q.df = df;
+            q.R = R;
+            q.r0 = r0;
+            q.RP = RP;
+            q.nchunk = fold_chunks(d.C);
+            fk::fk_vjp_fold_kernel<false><<<d.C * q.nchunk, fk::FOLD_THREADS, 0, s>>>(q);
+            fk::fk_vjp_fold_final_kernel<double, false><<<slots, fk::GEMM_BN, 0, s>>>(q);
+            ++nl;
+        } else {
+            fk::GatherRParams q;
+            memset(&q, 0, sizeof q);
+            q.desc = d;
+            q.chan = ch;
+            q.fT = fT;
+            q.G = G;
+            q.df = df;
+            q.R = R;
+            q.r0 = r0;
+            q.RP = RP;
+            fk::fk_vjp_gather_r_kernel<double, false><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
+        }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm vjp launch failed: %s", cudaGetErrorString(e));
         nl += 4;

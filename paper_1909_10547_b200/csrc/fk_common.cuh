@@ -46,6 +46,7 @@ struct TableDesc {
     long long gp_off;        // row offset of this table's split-K partial tiles (sum over earlier tables of ksplit * N)
     long long k_off;         // offset of this table's column sums inside G_cat (sum of K over earlier tables)
     int gksplit, gkper;      // K ranges of the forward contraction and their length
+    long long cx_off;        // sum of C * nx over earlier tables: first (channel, x) slot of the VJP fold partials
 };
 
 // Work list entry of the column kernels (forward and VJP stage 1): one CTA = one (k-block, datapoint range).

@@ -281,3 +281,155 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
 }
 
 }  // namespace fk
+
+namespace fk {
+
+// ---------------------------------------------------------------------------------------------------
+// VJP stage 1 for R >> 1, warp-specialised and persistent:  G[k][c] = sum_n FK[n][k] * g[n][r0 + c]
+// (the same contraction as fk_gemm_vjp_kernel in fk_gemm.cuh, which stays for tables
+// whose rows cannot be bulk-copied).  A CTA walks the 128-k tiles  first, first + grid, ...  of the launch;
+// its producer warp streams [32 n][128 k] FK pieces and [32 n][RP] upstream-gradient pieces through a ring of
+// mbarrier-completed bulk copies and runs ahead across tile boundaries, so the consumers' FP64 tensor pipe
+// only drains for the register -> HBM store of a finished G tile.  Shared memory is zeroed once: rows a
+// short last stage does not copy hold finite stale values and are masked on the g side.
+struct WsVjpParams {
+    TableDesc desc;     // single-table launch
+    const double* gP;   // [N][RP]: g of this pass, replica innermost, zero padded (grouped: + out_off * RP)
+    double* G;          // [K][RP] column sums (grouped: + k_off * RP)
+    int RP, ntiles;     // ntiles: 128-k tiles (single) or items (grouped) of the launch
+    const TableDesc* descs;  // grouped launch
+    const ColSeg* items;     // grouped launch {table, kblock = 128-k tile}
+};
+
+constexpr int WSV_STAGE_DOUBLES = 2 * GEMMV_NT * GEMMV_S;   // FK piece + g piece
+constexpr size_t WSV_SMEM_BYTES = (size_t)GEMMV_STAGES * WSV_STAGE_DOUBLES * 8 + 2 * GEMMV_STAGES * 8;
+
+template <int NFW, bool GROUPED>
+__global__ void __launch_bounds__(WS_THREADS, 1)
+fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
+    extern __shared__ __align__(128) unsigned char fk_smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    double* Sm = reinterpret_cast<double*>(fk_smem);  // [STAGES][2][NT][S]
+    const uint32_t Sm_s = (uint32_t)__cvta_generic_to_shared(Sm);
+    const uint32_t bar0 = Sm_s + (uint32_t)(GEMMV_STAGES * WSV_STAGE_DOUBLES * 8);
+    auto bar_full = [&](int s) { return bar0 + 8u * s; };
+    auto bar_empty = [&](int s) { return bar0 + 8u * (GEMMV_STAGES + s); };
+    for (int q = tid; q < GEMMV_STAGES * WSV_STAGE_DOUBLES; q += WS_THREADS) Sm[q] = 0.0;
+    if (tid == 0) {
+        for (int s = 0; s < GEMMV_STAGES; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_empty(s), WS_CONSUMER_WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the zeros are ordered before the bulk copies
+    __syncthreads();
+    const int RP = p.RP;
+
+    auto tile_of = [&](int t, const TableDesc*& d, const double*& gP, double*& G, int& kt) {
+        if constexpr (GROUPED) {
+            const ColSeg it = p.items[t];
+            d = &p.descs[it.table];
+            gP = p.gP + d->out_off * RP;
+            G = p.G + d->k_off * RP;
+            kt = it.kblock;
+        } else {
+            d = &p.desc;
+            gP = p.gP;
+            G = p.G;
+            kt = t;
+        }
+    };
+
+    if (warp >= WS_CONSUMER_WARPS) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
+        if (warp != WS_CONSUMER_WARPS) return;
+        int it = 0;
+        for (int t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
+            const TableDesc* d;
+            const double* gP;
+            double* G;
+            int kt;
+            tile_of(t, d, gP, G, kt);
+            const int k0 = kt * GEMMV_BK, klen = min(GEMMV_BK, d->K - k0);
+            const double* __restrict__ fk = reinterpret_cast<const double*>(d->fk) + k0;
+            for (int n0 = 0; n0 < d->N; n0 += GEMMV_NT, ++it) {
+                const int stage = it % GEMMV_STAGES, rows = min(GEMMV_NT, d->N - n0);
+                mbar_wait(bar_empty(stage), ((it / GEMMV_STAGES) & 1) ^ 1);
+                if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(rows * (klen + RP) * 8));
+                __syncwarp();
+                if (lane < rows) {
+                    const uint32_t dstA = Sm_s + (uint32_t)((stage * WSV_STAGE_DOUBLES + lane * GEMMV_S) * 8);
+                    bulk_g2s(dstA, fk + (long long)(n0 + lane) * d->row_stride, (uint32_t)(klen * 8), bar_full(stage));
+                    bulk_g2s(dstA + (uint32_t)(GEMMV_NT * GEMMV_S * 8), gP + (long long)(n0 + lane) * RP, (uint32_t)(RP * 8), bar_full(stage));
+                }
+            }
+        }
+        return;
+    }
+
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
+    const int wm = warp & 3, wn = warp >> 2;
+    const int cbcol = wn * NFW * 8;
+    int it = 0;
+    for (int t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
+        const TableDesc* d;
+        const double* gP;
+        double* G;
+        int kt;
+        tile_of(t, d, gP, G, kt);
+        double acc[4][NFW][2];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < NFW; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        for (int n0 = 0; n0 < d->N; n0 += GEMMV_NT, ++it) {
+            const int stage = it % GEMMV_STAGES, rows = min(GEMMV_NT, d->N - n0);
+            mbar_wait(bar_full(stage), (it / GEMMV_STAGES) & 1);
+            // A fragment: row m = k (lane >> 2), col = datapoint (lane & 3)  ->  As[n][k]
+            const double* At = Sm + stage * WSV_STAGE_DOUBLES + (lane & 3) * GEMMV_S + wm * 32 + (lane >> 2);
+            const double* Bt = Sm + stage * WSV_STAGE_DOUBLES + GEMMV_NT * GEMMV_S + (lane & 3) * GEMMV_S + cbcol + (lane >> 2);
+            if (rows == GEMMV_NT) {
+#pragma unroll
+                for (int n4 = 0; n4 < GEMMV_NT / 4; ++n4) {
+                    double a[4], b[NFW];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) a[i] = At[n4 * 4 * GEMMV_S + i * 8];
+#pragma unroll
+                    for (int j = 0; j < NFW; ++j) b[j] = Bt[n4 * 4 * GEMMV_S + j * 8];
+#pragma unroll
+                    for (int j = 0; j < NFW; ++j)
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                }
+            } else {
+                for (int n4 = 0; n4 * 4 < rows; ++n4) {
+                    const bool live = n4 * 4 + (lane & 3) < rows;
+                    double a[4], b[NFW];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) a[i] = At[n4 * 4 * GEMMV_S + i * 8];
+#pragma unroll
+                    for (int j = 0; j < NFW; ++j) b[j] = live ? Bt[n4 * 4 * GEMMV_S + j * 8] : 0.0;
+#pragma unroll
+                    for (int j = 0; j < NFW; ++j)
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty(stage));
+        }
+        const int k0 = kt * GEMMV_BK;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int k = k0 + wm * 32 + i * 8 + (lane >> 2);
+            if (k < d->K) {
+#pragma unroll
+                for (int j = 0; j < NFW; ++j)
+                    *reinterpret_cast<double2*>(G + (long long)k * RP + cbcol + j * 8 + 2 * (lane & 3)) = make_double2(acc[i][j][0], acc[i][j][1]);
+            }
+        }
+    }
+}
+
+}  // namespace fk

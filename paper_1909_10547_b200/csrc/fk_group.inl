@@ -24,7 +24,12 @@ struct fk_group {
     int ngitems = 0;
     fk::ColSeg* d_vitems = nullptr;
     int nvitems = 0;
-    long long gp_rows = 0, K_total = 0;
+    long long gp_rows = 0, K_total = 0, cx_total = 0;
+    bool wsv_all = true;            // every table can take the persistent warp-specialised VJP contraction
+    bool fold_all = true;           // every table can take the single-pass VJP fold (fk_vjp_fold.cuh)
+    int fold_nchunk = 1;
+    fk::ColSeg* d_foitems = nullptr;  // fold CTAs: {table, channel, x-row chunk}
+    int nfoitems = 0;
     double* scratch = nullptr;
     size_t scratch_elems = 0;
     int last_launches = 0;
@@ -49,7 +54,8 @@ bool group_gemm_wanted(const fk_group* g, int R) {
 size_t group_scratch_need(const fk_group* g, int R) {
     if (group_gemm_wanted(g, R)) {
         const size_t RP = fk::gemm_rp(R);
-        const size_t fwd = (size_t)g->gp_rows, vjp = (size_t)g->rows_total + (size_t)g->K_total;
+        const size_t fwd = (size_t)g->gp_rows,
+                     vjp = (size_t)g->rows_total + (size_t)g->K_total + (size_t)g->cx_total * (fk::FOLD_JQ + g->fold_nchunk);
         return ((size_t)g->ai_total + std::max(fwd, vjp)) * RP;
     }
     return std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * R;
@@ -118,20 +124,53 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
         p.nfw = (p.nfrag + 1) / 2;
         p.descs = g->d_descs;
         p.items = g->d_vitems;
-        if (g->all_vec) fk::fk_gemm_vjp_kernel<2, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        if (g->wsv_all) {
+            static const bool wsv_attr = wsv_set_attr<true>();
+            if (!wsv_attr) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
+            fk::WsVjpParams w;
+            memset(&w, 0, sizeof w);
+            w.gP = gP;
+            w.G = G;
+            w.RP = RP;
+            w.ntiles = g->nvitems;
+            w.descs = g->d_descs;
+            w.items = g->d_vitems;
+            wsv_launch<true>(w, s);
+        } else if (g->all_vec) fk::fk_gemm_vjp_kernel<2, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_vjp_kernel<1, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
-        fk::GatherRParams q;
-        memset(&q, 0, sizeof q);
-        q.fT = fT;
-        q.G = G;
-        q.df = df_cat;
-        q.R = R;
-        q.r0 = r0;
-        q.RP = RP;
-        q.descs = g->d_descs;
-        q.ai_prefix = g->d_ai_prefix;
-        q.T = g->T;
-        fk::fk_vjp_gather_r_kernel<double, true><<<dim3((unsigned)g->ai_total, (RP + 127) / 128), 128, 0, s>>>(q);
+        if (g->fold_all) {
+            fk::FoldParams q;
+            memset(&q, 0, sizeof q);
+            q.fT = fT;
+            q.G = G;
+            q.PA = G + (size_t)g->K_total * RPmax;
+            q.PB = q.PA + (size_t)g->cx_total * fk::FOLD_JQ * RPmax;
+            q.df = df_cat;
+            q.R = R;
+            q.r0 = r0;
+            q.RP = RP;
+            q.nchunk = g->fold_nchunk;
+            q.descs = g->d_descs;
+            q.items = g->d_foitems;
+            q.ai_prefix = g->d_ai_prefix;
+            q.T = g->T;
+            fk::fk_vjp_fold_kernel<true><<<g->nfoitems, fk::FOLD_THREADS, 0, s>>>(q);
+            fk::fk_vjp_fold_final_kernel<double, true><<<(unsigned)g->ai_total, fk::GEMM_BN, 0, s>>>(q);
+            ++nl;
+        } else {
+            fk::GatherRParams q;
+            memset(&q, 0, sizeof q);
+            q.fT = fT;
+            q.G = G;
+            q.df = df_cat;
+            q.R = R;
+            q.r0 = r0;
+            q.RP = RP;
+            q.descs = g->d_descs;
+            q.ai_prefix = g->d_ai_prefix;
+            q.T = g->T;
+            fk::fk_vjp_gather_r_kernel<double, true><<<dim3((unsigned)g->ai_total, (RP + 127) / 128), 128, 0, s>>>(q);
+        }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gemm vjp launch failed: %s", cudaGetErrorString(e));
         nl += 4;
@@ -257,7 +296,12 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     const long long want_items = (long long)std::max(1, sm_count()) * std::max(1, env_int("FKCONV_GROUP_GEMM_WAVES", 4));
     long long kper_target = (tile_k + want_items - 1) / want_items;
     kper_target = std::max<long long>(fk::GEMM_KT * 8, (kper_target + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT);
-    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems;
+    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems, foitems;
+    {
+        long long channels = 0;
+        for (int t = 0; t < T; ++t) channels += tables[t]->desc.C;
+        g->fold_nchunk = fold_chunks(channels);
+    }
     for (int t = 0; t < T; ++t) {
         fk_table* tb = tables[t];
         fk::TableDesc d = tb->desc;
@@ -273,6 +317,12 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             for (int ks = 0; ks < d.gksplit; ++ks)
                 for (int mt = 0; mt < mtiles; ++mt) gitems.push_back(fk::ColSeg{t, mt, ks, 0});
             for (int kt = 0; kt < (d.K + fk::GEMMV_BK - 1) / fk::GEMMV_BK; ++kt) vitems.push_back(fk::ColSeg{t, kt, 0, 0});
+            d.cx_off = g->cx_total;
+            g->cx_total += (long long)d.C * d.nx;
+            g->fold_all = g->fold_all && fold_ok(d);
+            g->wsv_all = g->wsv_all && wsv_ok(d);
+            for (int c = 0; c < d.C; ++c)
+                for (int ch = 0; ch < g->fold_nchunk; ++ch) foitems.push_back(fk::ColSeg{t, c, ch, 0});
         }
         if (!g->all_vec && d.vec_ok) {  // one kernel instantiation per launch: the whole group takes the 64-bit path
             d.vec_ok = 0;
@@ -306,6 +356,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     g->ncsegs = (int)csegs.size();
     g->ngitems = (int)gitems.size();
     g->nvitems = (int)vitems.size();
+    g->nfoitems = (int)foitems.size();
     auto bail = [&](int code) { fk_group_destroy(g); return code; };
     cudaError_t e = cudaMalloc((void**)&g->d_descs, T * sizeof(fk::TableDesc));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_row_prefix, (T + 1) * sizeof(int));
@@ -315,6 +366,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     if (e == cudaSuccess) e = cudaMemcpy(g->d_fsegs, fsegs.data(), fsegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_gitems, gitems.size() * sizeof(fk::ColSeg));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_vitems, vitems.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_foitems, foitems.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_foitems, foitems.data(), foitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_gitems, gitems.data(), gitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_vitems, vitems.data(), vitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_descs, g->descs.data(), T * sizeof(fk::TableDesc), cudaMemcpyHostToDevice);
@@ -337,6 +390,7 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_fsegs) cudaFree(g->d_fsegs);
     if (g->d_gitems) cudaFree(g->d_gitems);
     if (g->d_vitems) cudaFree(g->d_vitems);
+    if (g->d_foitems) cudaFree(g->d_foitems);
     if (g->scratch) cudaFree(g->scratch);
     delete g;
     return FK_OK;
