@@ -219,7 +219,7 @@ cudaError_t colsum_dispatch(bool vec_ok, int rt, const fk::ColsumParams& p, int 
 
 // ---- R >> 1: FP64 tensor-core contraction (fk_gemm.cuh) ---------------------------------------------
 struct GemmPlan {
-    int ksplit, kper, RPmax;
+    int ksplit, kper, RPmax, ksub_rem;
 };
 
 template <typename T>
@@ -236,6 +236,9 @@ GemmPlan gemm_plan(const fk::TableDesc& d, int R) {
     int ksplit = std::max(1, target / mtiles);
     gp.kper = ((d.K + ksplit - 1) / ksplit + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT;
     gp.ksplit = (d.K + gp.kper - 1) / gp.kper;
+    // a partial last datapoint tile is cut into k sub-splits (fk_gemm_ws.cuh): whole groups of K ranges
+    gp.ksub_rem = d.N % fk::GEMM_BM ? fk::ws_ksub_for_rows(d.N % fk::GEMM_BM) : 1;
+    gp.ksplit = (gp.ksplit + gp.ksub_rem - 1) / gp.ksub_rem * gp.ksub_rem;
     gp.RPmax = fk::gemm_rp(R);
     return gp;
 }
@@ -347,7 +350,9 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
             w.RP = p.RP;
             w.ksplit = gp.ksplit;
             w.kper = gp.kper;
-            ws_launch<false>(w, mtiles * gp.ksplit, fk::ws_smem_bytes(d.nx, p.RP), s);
+            w.ksub_rem = gp.ksub_rem;
+            const int nfull = d.N / fk::GEMM_BM;
+            ws_launch<false>(w, nfull * gp.ksplit + (d.N % fk::GEMM_BM ? gp.ksplit / gp.ksub_rem : 0), fk::ws_smem_bytes(d.nx, p.RP), s);
         } else if (d.vec_ok) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_fwd_kernel<1, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         if (timed) g_prof.end(s, slot);

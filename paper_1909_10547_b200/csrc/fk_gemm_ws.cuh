@@ -21,6 +21,8 @@
 // reduction are those of fk_gemm.cuh.  Results are bitwise repeatable.
 #pragma once
 
+#include <type_traits>
+
 #include "fk_common.cuh"
 #include "fk_gemm.cuh"
 
@@ -28,7 +30,9 @@ namespace fk {
 
 constexpr int WS_CONSUMER_WARPS = 8;
 constexpr int WS_THREADS = (WS_CONSUMER_WARPS + 4) * 32;  // + the producer's warpgroup (1 working warp): register
-                                                          // reallocation (setmaxnreg) works on whole warpgroups
+                                                          // reallocation (setmaxnreg) works on whole warpgroups.
+                                                          // (9 warps would not help: registers are per scheduler,
+                                                          // 3 warps on one of them still cap a thread at 170.)
 constexpr int WS_STAGES = 3;
 constexpr int WS_STAGE_DOUBLES = GEMM_BM * GEMM_SA;        // FK tile [128][36]
 constexpr int WS_NBAR = 2 * WS_STAGES + 4;                 // full[S], empty[S], fb_full[2], fb_empty[2]
@@ -65,10 +69,18 @@ struct WsFwdParams {
     const double* fT;      // [nfl*nx][RP] replica-innermost f (grouped: + desc.f_off * RP)
     double* gpart;         // [ksplit][N][RP] level-1 partials (grouped: + desc.gp_off * RP)
     int RP;                // padded replicas of this pass = 16 * NFW
-    int ksplit, kper;      // single-table launch
+    int ksplit, kper;      // single-table launch: K ranges (a multiple of ksub_rem) and their length
+    int ksub_rem;          // single-table launch: k sub-splits (1, 2, 4) of the last, partial datapoint tile
     const TableDesc* descs;  // grouped launch
-    const ColSeg* items;     // grouped launch {table, datapoint tile, K range}
+    const ColSeg* items;     // grouped launch {table, kblock = first datapoint, split = K range of the item, pad_ = k sub-splits}
 };
+
+// Ragged datapoint counts: a tile of TM = 128 / KSUB datapoints (KSUB = 1, 2, 4) keeps all 8 consumer warps on
+// real rows.  The 4 warp rows become (TM / 32) row blocks x KSUB k sub-splits: sub-split q takes the MMA
+// k-steps q, q + KSUB, ... of a stage that is KSUB times longer in k ([TM][32 * KSUB] doubles, the same bytes),
+// covers KSUB base K ranges per item and writes its own level-1 partial slice, so an item costs the same
+// DMMA time and the reduction sees the same number of slices whatever the tile height.
+__host__ __device__ inline int ws_ksub_for_rows(int rows) { return rows <= 32 ? 4 : rows <= 64 ? 2 : 1; }
 
 // NFW = 8-replica fragments per warp column = RP / 16, a compile-time constant: the 4 x NFW DMMAs of a k-step
 // carry no predicates, so ptxas is free to batch the fragment loads and the DMULs ahead of them.
@@ -83,7 +95,7 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
     const uint8_t* __restrict__ chb = p.chan.b;
     const double* __restrict__ fT = p.fT;
     double* gpart = p.gpart;
-    int mt, ks, kper;
+    int m0, ks, kper, KSUB;
     if constexpr (GROUPED) {
         const ColSeg it = p.items[blockIdx.x];
         dp = &p.descs[it.table];
@@ -91,21 +103,29 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
         chb = dp->chan_b;
         fT += dp->f_off * p.RP;
         gpart += dp->gp_off * p.RP;
-        mt = it.kblock;
+        m0 = it.kblock;
         ks = it.split;
+        KSUB = it.pad_;
         kper = dp->gkper;
     } else {
-        const int mtiles = (p.desc.N + GEMM_BM - 1) / GEMM_BM;
-        mt = blockIdx.x % mtiles;
-        ks = blockIdx.x / mtiles;
+        const int nfull = p.desc.N / GEMM_BM, nb_full = nfull * p.ksplit;
+        if ((int)blockIdx.x < nb_full) {
+            m0 = ((int)blockIdx.x % nfull) * GEMM_BM;
+            ks = (int)blockIdx.x / nfull;
+            KSUB = 1;
+        } else {
+            m0 = nfull * GEMM_BM;
+            ks = (int)blockIdx.x - nb_full;
+            KSUB = p.ksub_rem;
+        }
         kper = p.kper;
     }
     const TableDesc& d = *dp;
     const int nx = d.nx, RP = p.RP, SB = RP + 4, cstride = d.cstride;
-    const int m0 = mt * GEMM_BM;
-    const int kbeg = ks * kper, kend = min(d.K, kbeg + kper);
-    if (kbeg >= kend) return;
-    const int c0 = kbeg / cstride, c1 = (kend - 1) / cstride;
+    const int TM = GEMM_BM / KSUB, KTv = GEMM_KT * KSUB, SAv = KTv + 4;  // tile rows, k per stage, shared row stride
+    const int kbeg = min(d.K, ks * kper * KSUB), kend = min(d.K, kbeg + kper * KSUB);
+    // an empty K range (more slices than K-tiles) still writes its zero partials
+    const int c0 = kbeg / cstride, c1 = kbeg < kend ? (kend - 1) / cstride : c0 - 1;
 
     double* As = reinterpret_cast<double*>(fk_smem);       // [STAGES][128][36]
     double* Bs = As + WS_STAGES * WS_STAGE_DOUBLES;         // [2][nx][SB]   f[b_c][j][r] of two channels
@@ -131,11 +151,12 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
 
     if (warp >= WS_CONSUMER_WARPS) {
         // ================================ producer warp ================================
-        // 384 threads cap the kernel at 168 registers; the producer warpgroup hands its share to the consumers
+        // 384 threads cap the kernel at 168 registers; the producer warpgroup hands its share to the consumers:
+        // 256 x 232 + 128 x 40 = 384 x 168 exactly (asking for more than the CTA owns would block forever)
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
         if (warp != WS_CONSUMER_WARPS) return;
         const double* __restrict__ fk = reinterpret_cast<const double*>(d.fk);
-        const int rows_valid = min(GEMM_BM, d.N - m0);
+        const int rows_valid = min(TM, d.N - m0);
         auto issue_fb = [&](int c, int ccn) {  // f[b_c][.][.] of channel c -> buffer ccn & 1
             const int buf = ccn & 1;
             mbar_wait(bar_fbempty(buf), ((ccn >> 1) & 1) ^ 1);
@@ -146,19 +167,19 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
                 bulk_g2s(Bs_s + (uint32_t)((buf * nx + row) * SB * 8), src + (long long)row * RP, (uint32_t)(RP * 8), bar_fbfull(buf));
         };
         int it = 0, cc = 0;
-        issue_fb(c0, 0);
+        if (c0 <= c1) issue_fb(c0, 0);
         for (int c = c0; c <= c1; ++c, ++cc) {
             const int sb = max(kbeg, c * cstride), se = min(kend, (c + 1) * cstride);
             bool next_issued = c == c1;
             int tiles = 0;
-            for (int k0 = sb; k0 < se; k0 += GEMM_KT, ++it, ++tiles) {
+            for (int k0 = sb; k0 < se; k0 += KTv, ++it, ++tiles) {
                 // the buffer of channel c + 1 was released when the consumers left channel c - 1, which they
                 // had to do before tile WS_STAGES of this channel can be issued: this wait never blocks here
                 if (!next_issued && tiles == WS_STAGES) {
                     issue_fb(c + 1, cc + 1);
                     next_issued = true;
                 }
-                const int len = min(GEMM_KT, se - k0);
+                const int len = min(KTv, se - k0);
                 const int stage = it % WS_STAGES;
                 mbar_wait(bar_empty(stage), ((it / WS_STAGES) & 1) ^ 1);
                 if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(rows_valid * len * 8));
@@ -167,7 +188,7 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
                 for (int q = 0; q < GEMM_BM / 32; ++q) {
                     const int row = lane + 32 * q;
                     if (row < rows_valid)
-                        bulk_g2s(As_s + (uint32_t)(((stage * GEMM_BM + row) * GEMM_SA) * 8),
+                        bulk_g2s(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * SAv) * 8),
                                  fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(len * 8), bar_full(stage));
                 }
             }
@@ -178,106 +199,117 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
 
     // ================================ consumer warps: warp tile 32 datapoints x (8 * nfw) replicas ================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
-    const int wm = warp & 3, wn = warp >> 2;
-    const int cbcol = wn * NFW * 8;
-    double acc[4][NFW][2];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < NFW; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    auto consume = [&](auto ks_tag) {
+        const int wm = warp & 3, wn = warp >> 2;
+        constexpr int KS = decltype(ks_tag)::value;            // compile-time k sub-splits: immediate shared-memory offsets
+        constexpr int KTc = GEMM_KT * KS, SAc = KTc + 4;
+        const int rb = wm % (4 / KS), ksub = wm / (4 / KS);    // row block and k sub-split of this warp row
+        constexpr int kst = 4 * KS;                            // k between consecutive MMA k-steps of this warp
+        const int cbcol = wn * NFW * 8;
+        double acc[4][NFW][2];
+    #pragma unroll
+        for (int i = 0; i < 4; ++i)
+    #pragma unroll
+            for (int j = 0; j < NFW; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    // level-1 partial tile gpart[ks][n][c] (+)= acc, acc = 0   (thread-private addresses, L2 resident)
-    double* out = gpart + (long long)ks * d.N * RP;
-    auto flush = [&](bool first) {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int n = m0 + wm * 32 + i * 8 + (lane >> 2);
-            double2* q = reinterpret_cast<double2*>(out + (long long)n * RP + cbcol + 2 * (lane & 3));
-            double2 o[NFW];
-#pragma unroll
-            for (int j = 0; j < NFW; ++j) o[j] = (!first && n < d.N) ? q[j * 4] : make_double2(0.0, 0.0);
-#pragma unroll
-            for (int j = 0; j < NFW; ++j) {
-                if (n < d.N) q[j * 4] = make_double2(acc[i][j][0] + o[j].x, acc[i][j][1] + o[j].y);
-                acc[i][j][0] = acc[i][j][1] = 0.0;
+        // level-1 partial tile gpart[ks][n][c] (+)= acc, acc = 0   (thread-private addresses, L2 resident)
+        double* out = gpart + (long long)(ks * KS + ksub) * d.N * RP;
+        auto flush = [&](bool first) {
+    #pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int n = m0 + rb * 32 + i * 8 + (lane >> 2);
+                double2* q = reinterpret_cast<double2*>(out + (long long)n * RP + cbcol + 2 * (lane & 3));
+                double2 o[NFW];
+    #pragma unroll
+                for (int j = 0; j < NFW; ++j) o[j] = (!first && n < d.N) ? q[j * 4] : make_double2(0.0, 0.0);
+    #pragma unroll
+                for (int j = 0; j < NFW; ++j) {
+                    if (n < d.N) q[j * 4] = make_double2(acc[i][j][0] + o[j].x, acc[i][j][1] + o[j].y);
+                    acc[i][j][0] = acc[i][j][1] = 0.0;
+                }
             }
-        }
-    };
-
-    int it = 0, cc = 0;
-    bool flushed = false;
-    for (int c = c0; c <= c1; ++c, ++cc) {
-        const int sb = max(kbeg, c * cstride), se = min(kend, (c + 1) * cstride);
-        const int buf = cc & 1;
-        mbar_wait(bar_fbfull(buf), (cc >> 1) & 1);
-        const double* Bt = Bs + (long long)buf * nx * SB + cbcol + (lane >> 2);
-        const double* __restrict__ fa_base = fT + (long long)cha[c] * nx * RP + cbcol + (lane >> 2);
-        // this lane's k of every MMA k-step is 4*step + (lane & 3): its own (i, j), walked incrementally
-        int i, j;
-        {
-            const int kl = sb - c * cstride + (lane & 3);
-            i = kl / nx;
-            j = kl - i * nx;
-        }
-        // f[a_c][i][r] for the 8 replica columns of this lane's B fragments, and the same for row i + 1,
-        // fetched one x-row (nx values of k) ahead so that the row switch never waits for L2
-        double fa[NFW], fan[NFW];
-        auto load_row = [&](double (&dst)[NFW], int row) {
-            const double* src = fa_base + (long long)min(row, nx - 1) * RP;  // row >= nx only on the zero padding
-#pragma unroll
-            for (int j8 = 0; j8 < NFW; ++j8) dst[j8] = __ldg(src + j8 * 8);
         };
-        load_row(fa, i);
-        load_row(fan, i + 1);
-        for (int k0 = sb; k0 < se; k0 += GEMM_KT, ++it) {
-            const int nsteps = min(GEMM_KT, se - k0) >> 2;
-            const int stage = it % WS_STAGES;
-            mbar_wait(bar_full(stage), (it / WS_STAGES) & 1);
-            const double* At = As + ((stage * GEMM_BM) + wm * 32 + (lane >> 2)) * GEMM_SA + (lane & 3);
-#pragma unroll
-            for (int s = 0; s < GEMM_KT / 4; ++s) {
-                if (s < nsteps) {
-                    double a[4], b[NFW];
-#pragma unroll
-                    for (int i4 = 0; i4 < 4; ++i4) a[i4] = At[i4 * 8 * GEMM_SA + s * 4];
-#pragma unroll
-                    for (int j8 = 0; j8 < NFW; ++j8) b[j8] = Bt[j * SB + j8 * 8] * fa[j8];
-#pragma unroll
-                    for (int j8 = 0; j8 < NFW; ++j8)
-#pragma unroll
-                        for (int i4 = 0; i4 < 4; ++i4) dmma884(acc[i4][j8][0], acc[i4][j8][1], a[i4], b[j8]);
-                    j += 4;
-                    if (j >= nx) {
-                        j -= nx;
-                        ++i;
-                        if (j < nx) {
-#pragma unroll
-                            for (int j8 = 0; j8 < NFW; ++j8) fa[j8] = fan[j8];
-                        } else {  // nx < 4: more than one row per MMA k-step
-                            do {
-                                j -= nx;
-                                ++i;
-                            } while (j >= nx);
-                            load_row(fa, i);
+
+        int it = 0, cc = 0;
+        bool flushed = false;
+        for (int c = c0; c <= c1; ++c, ++cc) {
+            const int sb = max(kbeg, c * cstride), se = min(kend, (c + 1) * cstride);
+            const int buf = cc & 1;
+            mbar_wait(bar_fbfull(buf), (cc >> 1) & 1);
+            const double* Bt = Bs + (long long)buf * nx * SB + cbcol + (lane >> 2);
+            const double* __restrict__ fa_base = fT + (long long)cha[c] * nx * RP + cbcol + (lane >> 2);
+            // this lane's k of every MMA k-step is 4*step + (lane & 3): its own (i, j), walked incrementally
+            int i, j;
+            {
+                const int kl = sb - c * cstride + ksub * 4 + (lane & 3);
+                i = kl / nx;
+                j = kl - i * nx;
+            }
+            // f[a_c][i][r] for the 8 replica columns of this lane's B fragments, and the same for row i + 1,
+            // fetched one x-row (nx values of k) ahead so that the row switch never waits for L2
+            double fa[NFW], fan[NFW];
+            auto load_row = [&](double (&dst)[NFW], int row) {
+                const double* src = fa_base + (long long)min(row, nx - 1) * RP;  // row >= nx only on the zero padding
+    #pragma unroll
+                for (int j8 = 0; j8 < NFW; ++j8) dst[j8] = __ldg(src + j8 * 8);
+            };
+            load_row(fa, i);
+            load_row(fan, i + 1);
+            for (int k0 = sb; k0 < se; k0 += KTc, ++it) {
+                const int nsteps = max(0, ((min(KTc, se - k0) >> 2) - ksub + KS - 1) / KS);
+                const int stage = it % WS_STAGES;
+                mbar_wait(bar_full(stage), (it / WS_STAGES) & 1);
+                const double* At = As + stage * WS_STAGE_DOUBLES + (rb * 32 + (lane >> 2)) * SAc + ksub * 4 + (lane & 3);
+    #pragma unroll
+                for (int s = 0; s < GEMM_KT / 4; ++s) {
+                    if (s < nsteps) {
+                        double a[4], b[NFW];
+    #pragma unroll
+                        for (int i4 = 0; i4 < 4; ++i4) a[i4] = At[i4 * 8 * SAc + s * kst];
+    #pragma unroll
+                        for (int j8 = 0; j8 < NFW; ++j8) b[j8] = Bt[j * SB + j8 * 8] * fa[j8];
+    #pragma unroll
+                        for (int j8 = 0; j8 < NFW; ++j8)
+    #pragma unroll
+                            for (int i4 = 0; i4 < 4; ++i4) dmma884(acc[i4][j8][0], acc[i4][j8][1], a[i4], b[j8]);
+                        j += kst;
+                        if (j >= nx) {
+                            j -= nx;
+                            ++i;
+                            if (j < nx) {
+    #pragma unroll
+                                for (int j8 = 0; j8 < NFW; ++j8) fa[j8] = fan[j8];
+                            } else {  // nx < 4: more than one row per MMA k-step
+                                do {
+                                    j -= nx;
+                                    ++i;
+                                } while (j >= nx);
+                                load_row(fa, i);
+                            }
+                            load_row(fan, i + 1);
                         }
-                        load_row(fan, i + 1);
+                        __syncwarp();
                     }
-                    __syncwarp();
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_empty(stage));
+                // the two warp columns share the SM's four schedulers pairwise: they flush half a period apart, so one
+                // warp of a scheduler keeps the FP64 pipe busy while the other waits for its partials from L2
+                if ((it + 1 + wn * (GEMM_FLUSH / 2)) % GEMM_FLUSH == 0) {
+                    flush(!flushed);
+                    flushed = true;
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_empty(stage));
-            // the two warp columns share the SM's four schedulers pairwise: they flush half a period apart, so one
-            // warp of a scheduler keeps the FP64 pipe busy while the other waits for its partials from L2
-            if ((it + 1 + wn * (GEMM_FLUSH / 2)) % GEMM_FLUSH == 0) {
-                flush(!flushed);
-                flushed = true;
-            }
+            if (lane == 0) mbar_arrive(bar_fbempty(buf));
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_fbempty(buf));
+        flush(!flushed);
+    };
+    switch (KSUB) {
+        case 1: consume(std::integral_constant<int, 1>{}); break;
+        case 2: consume(std::integral_constant<int, 2>{}); break;
+        default: consume(std::integral_constant<int, 4>{}); break;
     }
-    flush(!flushed);
 }
 
 }  // namespace fk

@@ -25,6 +25,10 @@ struct fk_group {
     fk::ColSeg* d_vitems = nullptr;
     int nvitems = 0;
     long long gp_rows = 0, K_total = 0, cx_total = 0;
+    bool ws_all = true;             // every table can take the warp-specialised forward contraction (fk_gemm_ws.cuh)
+    int nx_max = 0;
+    fk::ColSeg* d_witems = nullptr; // its items: {table, first datapoint, K range of the item, k sub-splits}
+    int nwitems = 0;
     bool wsv_all = true;            // every table can take the persistent warp-specialised VJP contraction
     bool fold_all = true;           // every table can take the single-pass VJP fold (fk_vjp_fold.cuh)
     int fold_nchunk = 1;
@@ -84,7 +88,19 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
         const long long tf = g->ai_total * p.RP;
         fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
             f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, p.RP);
-        if (g->all_vec) fk::fk_gemm_fwd_kernel<2, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        const size_t ws_smem = fk::ws_smem_bytes(g->nx_max, p.RP);
+        if (g->ws_all && env_int("FKCONV_WS", 1) && ws_smem <= MAX_DYN_SMEM) {
+            static const bool ws_attr = ws_set_attr<true>();
+            if (!ws_attr) return fail(FK_ERR_CUDA, "grouped gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
+            fk::WsFwdParams w;
+            memset(&w, 0, sizeof w);
+            w.fT = fT;
+            w.gpart = gpart;
+            w.RP = p.RP;
+            w.descs = g->d_descs;
+            w.items = g->d_witems;
+            ws_launch<true>(w, g->nwitems, ws_smem, s);
+        } else if (g->all_vec) fk::fk_gemm_fwd_kernel<2, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_fwd_kernel<1, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         const long long outs = g->rows_total * p.RP;
         fk::fk_gemm_reduce_grouped_kernel<double><<<(int)std::min<long long>(8192, (outs + 255) / 256), 256, 0, s>>>(
@@ -296,7 +312,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     const long long want_items = (long long)std::max(1, sm_count()) * std::max(1, env_int("FKCONV_GROUP_GEMM_WAVES", 4));
     long long kper_target = (tile_k + want_items - 1) / want_items;
     kper_target = std::max<long long>(fk::GEMM_KT * 8, (kper_target + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT);
-    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems, foitems;
+    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems, foitems, witems;
     {
         long long channels = 0;
         for (int t = 0; t < T; ++t) channels += tables[t]->desc.C;
@@ -309,6 +325,16 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             const int ksplit0 = (int)std::max<long long>(1, (d.K + kper_target - 1) / kper_target);
             d.gkper = ((d.K + ksplit0 - 1) / ksplit0 + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT;
             d.gksplit = (d.K + d.gkper - 1) / d.gkper;
+            // a partial last datapoint tile is cut into k sub-splits that take whole groups of K ranges
+            const int nfull = d.N / fk::GEMM_BM, rem = d.N % fk::GEMM_BM;
+            const int ksub_rem = rem ? fk::ws_ksub_for_rows(rem) : 1;
+            d.gksplit = (d.gksplit + ksub_rem - 1) / ksub_rem * ksub_rem;
+            for (int ks = 0; ks < d.gksplit; ++ks)
+                for (int mt = 0; mt < nfull; ++mt) witems.push_back(fk::ColSeg{t, mt * fk::GEMM_BM, ks, 1});
+            if (rem)
+                for (int ks = 0; ks < d.gksplit / ksub_rem; ++ks) witems.push_back(fk::ColSeg{t, nfull * fk::GEMM_BM, ks, ksub_rem});
+            g->ws_all = g->ws_all && d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok;
+            g->nx_max = std::max(g->nx_max, d.nx);
             d.gp_off = g->gp_rows;
             d.k_off = g->K_total;
             g->gp_rows += (long long)d.gksplit * d.N;
@@ -357,6 +383,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     g->ngitems = (int)gitems.size();
     g->nvitems = (int)vitems.size();
     g->nfoitems = (int)foitems.size();
+    g->nwitems = (int)witems.size();
     auto bail = [&](int code) { fk_group_destroy(g); return code; };
     cudaError_t e = cudaMalloc((void**)&g->d_descs, T * sizeof(fk::TableDesc));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_row_prefix, (T + 1) * sizeof(int));
@@ -367,6 +394,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_gitems, gitems.size() * sizeof(fk::ColSeg));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_vitems, vitems.size() * sizeof(fk::ColSeg));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_foitems, foitems.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_witems, std::max<size_t>(1, witems.size()) * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_witems, witems.data(), witems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_foitems, foitems.data(), foitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_gitems, gitems.data(), gitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_vitems, vitems.data(), vitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
@@ -391,6 +420,7 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_gitems) cudaFree(g->d_gitems);
     if (g->d_vitems) cudaFree(g->d_vitems);
     if (g->d_foitems) cudaFree(g->d_foitems);
+    if (g->d_witems) cudaFree(g->d_witems);
     if (g->scratch) cudaFree(g->scratch);
     delete g;
     return FK_OK;
