@@ -449,7 +449,12 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             q.r0 = r0;
             q.RP = RP;
             q.nchunk = fold_chunks(d.C);
-            fk::fk_vjp_fold_kernel<false><<<d.C * q.nchunk, fk::FOLD_THREADS, 0, s>>>(q);
+            q.nslots = fk::fold_slots(d.nx, RP, MAX_DYN_SMEM);
+            static const bool fold_attr = cudaFuncSetAttribute(fk::fk_vjp_fold_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                               (int)MAX_DYN_SMEM) == cudaSuccess;
+            if (!fold_attr || q.nslots < 1) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve shared memory for the fold ring");
+            fk::fk_vjp_fold_kernel<false><<<d.C * q.nchunk, fk::FOLD_THREADS,
+                                            (size_t)q.nslots * d.nx * RP * 8 + 2 * fk::FOLD_MAX_SLOTS * 8, s>>>(q);
             fk::fk_vjp_fold_final_kernel<double, false><<<slots, fk::GEMM_BN, 0, s>>>(q);
             ++nl;
         } else {

@@ -170,7 +170,12 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             q.items = g->d_foitems;
             q.ai_prefix = g->d_ai_prefix;
             q.T = g->T;
-            fk::fk_vjp_fold_kernel<true><<<g->nfoitems, fk::FOLD_THREADS, 0, s>>>(q);
+            q.nslots = fk::fold_slots(g->nx_max, RP, MAX_DYN_SMEM);
+            static const bool fold_attr = cudaFuncSetAttribute(fk::fk_vjp_fold_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                               (int)MAX_DYN_SMEM) == cudaSuccess;
+            if (!fold_attr || q.nslots < 1) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve shared memory for the fold ring");
+            fk::fk_vjp_fold_kernel<true><<<g->nfoitems, fk::FOLD_THREADS,
+                                           (size_t)q.nslots * g->nx_max * RP * 8 + 2 * fk::FOLD_MAX_SLOTS * 8, s>>>(q);
             fk::fk_vjp_fold_final_kernel<double, true><<<(unsigned)g->ai_total, fk::GEMM_BN, 0, s>>>(q);
             ++nl;
         } else {

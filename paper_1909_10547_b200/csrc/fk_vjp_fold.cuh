@@ -7,15 +7,16 @@
 //   df[r][alpha][x] = sum_{c: a_c = alpha} A[c][x][r] + sum_{c: b_c = alpha} B[c][x][r]
 //
 // fk_vjp_fold_kernel: CTA = (channel c, chunk of x-rows i); 256 threads = 4 j-classes (j mod 4) x 64 replica
-// pairs.  A thread walks its rows i, loads its <= 16 values of j as independent 128-bit streaming loads (the
-// CTA reads every (c, i) row of G as one contiguous nx*RP*8-byte piece), keeps f[b_c][j] and the B sums of
-// its j in registers, and writes one A partial per (i, j-class) and one B partial per (chunk, j).  No shared
-// memory, no barrier, no atomics; every G element is read exactly once (the gather form reads it twice
-// with a stride).  fk_vjp_fold_final_kernel adds the partials of a PDF slot in a fixed order.
+// pairs.  Every (c, i) row of G is one contiguous nx*RP*8-byte piece: it arrives in a shared-memory ring by ONE
+// bulk async copy (cp.async.bulk, mbarrier completion), several rows ahead of the threads that use it.  A
+// thread keeps f[b_c][j] and the B sums of its <= 16 values of j in registers and writes one A partial per
+// (i, j-class) and one B partial per (chunk, j).  No atomics; every G element crosses HBM exactly once (the
+// gather form reads it twice with a stride).  fk_vjp_fold_final_kernel adds the partials of a PDF slot in a fixed order.
 #pragma once
 
 #include "fk_common.cuh"
 #include "fk_gemm.cuh"
+#include "fk_gemm_ws.cuh"
 
 namespace fk {
 
@@ -33,6 +34,7 @@ struct FoldParams {
     double* PB;            // [(cx_off + c*nx) * nchunk + chunk*nx + j][RP]
     void* df;              // final kernel: [R][nfl][nx] (grouped: + f_off * R)
     int R, r0, RP, nchunk;
+    int nslots;            // fold kernel: rows of G in the shared-memory ring (>= 2)
     const TableDesc* descs;  // grouped launch
     const ColSeg* items;     // grouped fold launch: {table, kblock = channel, split = chunk}
     const int* ai_prefix;    // grouped final launch: first (alpha, x) slot of each table
@@ -45,9 +47,18 @@ __device__ __forceinline__ double2 ld_stream2(const double* p) {
     return r;
 }
 
+// shared memory: a ring of FOLD_SLOTS (c, i) rows of G ([nx][RP] doubles each) + 2 mbarriers per slot
+constexpr int FOLD_MAX_SLOTS = 4;
+__host__ __device__ inline int fold_slots(int nx, int RP, size_t max_bytes) {
+    const size_t row = (size_t)nx * RP * 8;
+    int s = (int)((max_bytes - 2 * FOLD_MAX_SLOTS * 8) / row);
+    return s > FOLD_MAX_SLOTS ? FOLD_MAX_SLOTS : s;
+}
+
 template <bool GROUPED>
 __global__ void __launch_bounds__(FOLD_THREADS)
 fk_vjp_fold_kernel(const __grid_constant__ FoldParams p) {
+    extern __shared__ __align__(128) unsigned char fk_smem[];
     const TableDesc* dp = &p.desc;
     const uint8_t* __restrict__ ca = p.chan.a;
     const uint8_t* __restrict__ cb = p.chan.b;
@@ -68,46 +79,80 @@ fk_vjp_fold_kernel(const __grid_constant__ FoldParams p) {
         chunk = blockIdx.x - c * p.nchunk;
     }
     const TableDesc& d = *dp;
-    const int nx = d.nx, RP = p.RP;
-    const int col = 2 * (threadIdx.x & 63), jq = threadIdx.x >> 6;
-    if (col >= RP) return;
+    const int nx = d.nx, RP = p.RP, S = p.nslots;
+    const int col = 2 * (threadIdx.x & 63), jq = threadIdx.x >> 6, lane = threadIdx.x & 31;
     const int i0 = (int)((long long)nx * chunk / p.nchunk), i1 = (int)((long long)nx * (chunk + 1) / p.nchunk);
+    const uint32_t row_bytes = (uint32_t)(nx * RP * 8);
 
+    // ring of (c, i) rows: each row of G is ONE contiguous piece, fetched by one bulk copy that completes on the
+    // slot's mbarrier; up to S rows are in flight per SM whatever the consumers do
+    double* ring = reinterpret_cast<double*>(fk_smem);
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(ring);
+    const uint32_t bar0 = ring_s + (uint32_t)S * row_bytes;
+    auto bar_full = [&](int s) { return bar0 + 8u * s; };
+    auto bar_empty = [&](int s) { return bar0 + 8u * (FOLD_MAX_SLOTS + s); };
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < S; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_empty(s), FOLD_THREADS / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const double* __restrict__ Gc = G + (long long)c * d.cstride * RP;
+    auto issue = [&](int i) {  // thread 0 only: row i -> slot (i - i0) % S
+        const int q = i - i0, s = q % S;
+        mbar_wait(bar_empty(s), ((q / S) & 1) ^ 1);
+        mbar_expect_tx(bar_full(s), row_bytes);
+        bulk_g2s(ring_s + (uint32_t)s * row_bytes, Gc + (long long)i * nx * RP, row_bytes, bar_full(s));
+    };
+    if (threadIdx.x == 0)
+        for (int i = i0; i < min(i1, i0 + S - 1); ++i) issue(i);
+
+    const bool active = col < RP;
     double2 fb[FOLD_NXQ], sb[FOLD_NXQ];
     {
         const double* src = fT + ((long long)cb[c] * nx + jq) * RP + col;
 #pragma unroll
         for (int m = 0; m < FOLD_NXQ; ++m) {
-            fb[m] = jq + FOLD_JQ * m < nx ? *reinterpret_cast<const double2*>(src + (long long)FOLD_JQ * m * RP) : make_double2(0.0, 0.0);
+            fb[m] = (active && jq + FOLD_JQ * m < nx) ? *reinterpret_cast<const double2*>(src + (long long)FOLD_JQ * m * RP) : make_double2(0.0, 0.0);
             sb[m] = make_double2(0.0, 0.0);
         }
     }
     const double* __restrict__ fa_col = fT + (long long)ca[c] * nx * RP + col;
-    const double* __restrict__ Gc = G + ((long long)c * d.cstride + jq) * RP + col;
     const long long cx = d.cx_off + (long long)c * nx;
     double* __restrict__ PA = p.PA + (cx * FOLD_JQ + jq) * RP + col;
 
     for (int i = i0; i < i1; ++i) {
-        const double* row = Gc + (long long)i * nx * RP;
-        double2 v[FOLD_NXQ];
+        const int q = i - i0, s = q % S;
+        if (threadIdx.x == 0 && i + S - 1 < i1) issue(i + S - 1);  // its slot was left by every warp after row i - 1
+        __syncwarp();
+        mbar_wait(bar_full(s), (q / S) & 1);
+        if (active) {
+            const double* row = ring + (size_t)s * nx * RP + jq * RP + col;
+            const double2 fa = *reinterpret_cast<const double2*>(fa_col + (long long)i * RP);
+            double2 a = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int m = 0; m < FOLD_NXQ; ++m) {
+                if (jq + FOLD_JQ * m < nx) {
+                    const double2 v = *reinterpret_cast<const double2*>(row + FOLD_JQ * m * RP);
+                    a.x = fma(v.x, fb[m].x, a.x);
+                    a.y = fma(v.y, fb[m].y, a.y);
+                    sb[m].x = fma(v.x, fa.x, sb[m].x);
+                    sb[m].y = fma(v.y, fa.y, sb[m].y);
+                }
+            }
+            *reinterpret_cast<double2*>(PA + (long long)i * FOLD_JQ * RP) = a;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty(s));
+    }
+    if (active) {
+        double* __restrict__ PB = p.PB + ((cx * p.nchunk + (long long)chunk * nx) + jq) * RP + col;
 #pragma unroll
         for (int m = 0; m < FOLD_NXQ; ++m)
-            v[m] = jq + FOLD_JQ * m < nx ? ld_stream2(row + (long long)FOLD_JQ * m * RP) : make_double2(0.0, 0.0);
-        const double2 fa = *reinterpret_cast<const double2*>(fa_col + (long long)i * RP);
-        double2 s = make_double2(0.0, 0.0);
-#pragma unroll
-        for (int m = 0; m < FOLD_NXQ; ++m) {
-            s.x = fma(v[m].x, fb[m].x, s.x);
-            s.y = fma(v[m].y, fb[m].y, s.y);
-            sb[m].x = fma(v[m].x, fa.x, sb[m].x);
-            sb[m].y = fma(v[m].y, fa.y, sb[m].y);
-        }
-        *reinterpret_cast<double2*>(PA + (long long)i * FOLD_JQ * RP) = s;
+            if (jq + FOLD_JQ * m < nx) *reinterpret_cast<double2*>(PB + (long long)FOLD_JQ * m * RP) = sb[m];
     }
-    double* __restrict__ PB = p.PB + ((cx * p.nchunk + (long long)chunk * nx) + jq) * RP + col;
-#pragma unroll
-    for (int m = 0; m < FOLD_NXQ; ++m)
-        if (jq + FOLD_JQ * m < nx) *reinterpret_cast<double2*>(PB + (long long)FOLD_JQ * m * RP) = sb[m];
 }
 
 // one CTA per PDF slot (alpha, x), one thread per replica of the pass: channels in list order, partials in index
