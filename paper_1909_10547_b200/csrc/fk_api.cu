@@ -138,6 +138,16 @@ void make_plan(fk::TableDesc& d, int dtype, Plan& pl) {
 
 size_t part_elems_per_replica(const fk::TableDesc& d) { return d.nchunks > 1 ? (size_t)d.N * d.nchunks : 0; }
 size_t G_elems_per_replica(const fk::TableDesc& d) { return (size_t)d.nsplit * d.K; }
+// small-R VJP stage 2 in one pass over G (fk_vjp_foldk_kernel): hadronic tables whose nx x nx block fits shared memory
+bool foldk_ok(const fk::TableDesc& d) { return d.kind == fk::KIND_HADRONIC && d.nx <= 128 && env_int("FKCONV_FOLDK", 1); }
+size_t foldk_smem(int nx) { return (size_t)nx * (nx | 1) * 8; }
+constexpr int FOLDK_MAX_CHUNKS = 8;
+// x-row chunks per channel so that a table (or group) with few channels still covers the GPU about twice
+int foldk_chunks(long long channels) {
+    const long long want = 2LL * std::max(1, sm_count());
+    return (int)std::max<long long>(1, std::min<long long>(FOLDK_MAX_CHUNKS, (want + channels - 1) / std::max<long long>(1, channels)));
+}
+size_t foldk_elems_per_replica(const fk::TableDesc& d) { return foldk_ok(d) ? (1 + FOLDK_MAX_CHUNKS) * (size_t)d.C * d.nx : 0; }
 
 // ------------------------------------------------------------------------------------------------
 // validation
@@ -550,15 +560,38 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
             r0 += rt;
         }
     }
-    fk::GatherParams q;
-    memset(&q, 0, sizeof q);
-    q.desc = d;
-    q.chan = ch;
-    q.f = f;
-    q.G = G;
-    q.df = df;
-    q.R = R;
-    fk::fk_vjp_gather_kernel<T, false><<<dim3(d.nfl * d.nx, R), fk::GATHER_THREADS, 0, s>>>(q);
+    if (foldk_ok(d)) {
+        static const bool attr_ok = cudaFuncSetAttribute(fk::fk_vjp_foldk_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                         (int)foldk_smem(128)) == cudaSuccess;
+        if (!attr_ok) return fail(FK_ERR_CUDA, "vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
+        fk::FoldKParams q;
+        memset(&q, 0, sizeof q);
+        q.desc = d;
+        q.desc.cx_off = 0;
+        q.chan = ch;
+        q.f = f;
+        q.G = G;
+        q.cx_total = (long long)d.C * d.nx;
+        q.PA = G + G_elems_per_replica(d) * R;
+        q.PB = q.PA + q.cx_total * R;
+        q.nchunk = foldk_chunks(d.C);
+        q.df = df;
+        q.R = R;
+        const long long slots = (long long)d.nfl * d.nx;
+        fk::fk_vjp_foldk_kernel<T, false><<<dim3(d.C * q.nchunk, R), fk::FOLDK_THREADS, foldk_smem(d.nx), s>>>(q);
+        fk::fk_vjp_foldk_final_kernel<T, false><<<dim3((unsigned)((slots + 7) / 8), R), 256, 0, s>>>(q, slots);
+        ++nl;
+    } else {
+        fk::GatherParams q;
+        memset(&q, 0, sizeof q);
+        q.desc = d;
+        q.chan = ch;
+        q.f = f;
+        q.G = G;
+        q.df = df;
+        q.R = R;
+        fk::fk_vjp_gather_kernel<T, false><<<dim3(d.nfl * d.nx, R), fk::GATHER_THREADS, 0, s>>>(q);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gather kernel launch failed: %s", cudaGetErrorString(e));
     ++nl;
@@ -574,7 +607,7 @@ size_t conv_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
 template <typename T>
 size_t vjp_scratch_elems(const fk::TableDesc& d, int R) {
     if (gemm_wanted<T>(d, R)) return gemm_vjp_scratch_elems(d, R);
-    return G_elems_per_replica(d) * R;
+    return (G_elems_per_replica(d) + foldk_elems_per_replica(d)) * R;
 }
 
 // stateless front end shared by the fp64 / fp32 entry points

@@ -29,6 +29,9 @@ struct fk_group {
     int nx_max = 0;
     fk::ColSeg* d_witems = nullptr; // its items: {table, first datapoint, K range of the item, k sub-splits}
     int nwitems = 0;
+    bool foldk_all = true;          // every table can take the small-R single-pass fold (fk_vjp_foldk_kernel)
+    fk::ColSeg* d_kitems = nullptr; // its CTAs: {table, channel}
+    int nkitems = 0;
     bool wsv_all = true;            // every table can take the persistent warp-specialised VJP contraction
     bool fold_all = true;           // every table can take the single-pass VJP fold (fk_vjp_fold.cuh)
     int fold_nchunk = 1;
@@ -62,7 +65,7 @@ size_t group_scratch_need(const fk_group* g, int R) {
                      vjp = (size_t)g->rows_total + (size_t)g->K_total + (size_t)g->cx_total * (fk::FOLD_JQ + g->fold_nchunk);
         return ((size_t)g->ai_total + std::max(fwd, vjp)) * RP;
     }
-    return std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1) * R;
+    return std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1 + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R;
 }
 
 int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, cudaStream_t s) {
@@ -269,16 +272,39 @@ int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat,
         ++nl;
         r0 += rt;
     }
-    fk::GatherParams q;
-    memset(&q, 0, sizeof q);
-    q.descs = g->d_descs;
-    q.ai_prefix = g->d_ai_prefix;
-    q.T = g->T;
-    q.f = f_cat;
-    q.G = g->scratch;
-    q.df = df_cat;
-    q.R = R;
-    fk::fk_vjp_gather_kernel<T, true><<<dim3((unsigned)g->ai_total, R), fk::GATHER_THREADS, 0, s>>>(q);
+    if (g->foldk_all) {
+        static const bool attr_ok = cudaFuncSetAttribute(fk::fk_vjp_foldk_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                         (int)foldk_smem(128)) == cudaSuccess;
+        if (!attr_ok) return fail(FK_ERR_CUDA, "grouped vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
+        fk::FoldKParams q;
+        memset(&q, 0, sizeof q);
+        q.descs = g->d_descs;
+        q.items = g->d_kitems;
+        q.ai_prefix = g->d_ai_prefix;
+        q.T = g->T;
+        q.f = f_cat;
+        q.G = g->scratch;
+        q.cx_total = g->cx_total;
+        q.PA = g->scratch + (size_t)g->G_total1 * R;
+        q.PB = q.PA + (size_t)g->cx_total * R;
+        q.nchunk = foldk_chunks(g->nkitems);
+        q.df = df_cat;
+        q.R = R;
+        fk::fk_vjp_foldk_kernel<T, true><<<dim3((unsigned)(g->nkitems * q.nchunk), R), fk::FOLDK_THREADS, foldk_smem(g->nx_max), s>>>(q);
+        fk::fk_vjp_foldk_final_kernel<T, true><<<dim3((unsigned)((g->ai_total + 7) / 8), R), 256, 0, s>>>(q, g->ai_total);
+        ++nl;
+    } else {
+        fk::GatherParams q;
+        memset(&q, 0, sizeof q);
+        q.descs = g->d_descs;
+        q.ai_prefix = g->d_ai_prefix;
+        q.T = g->T;
+        q.f = f_cat;
+        q.G = g->scratch;
+        q.df = df_cat;
+        q.R = R;
+        fk::fk_vjp_gather_kernel<T, true><<<dim3((unsigned)g->ai_total, R), fk::GATHER_THREADS, 0, s>>>(q);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gather launch failed: %s", cudaGetErrorString(e));
     ++nl;
@@ -314,10 +340,12 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
         g->gemm_ok = g->gemm_ok && tables[t]->kdec != nullptr;
         tile_k += (long long)((tables[t]->desc.N + fk::GEMM_BM - 1) / fk::GEMM_BM) * tables[t]->desc.K;
     }
-    const long long want_items = (long long)std::max(1, sm_count()) * std::max(1, env_int("FKCONV_GROUP_GEMM_WAVES", 4));
+    const long long want_items = (long long)std::max(1, sm_count()) * std::max(1, env_int("FKCONV_GROUP_GEMM_WAVES", 16));
     long long kper_target = (tile_k + want_items - 1) / want_items;
     kper_target = std::max<long long>(fk::GEMM_KT * 8, (kper_target + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT);
-    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems, foitems, witems;
+    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems, foitems, witems, kitems;
+    long long group_kblocks = 0;
+    for (int t = 0; t < T; ++t) group_kblocks += tables[t]->desc.nchunks;
     {
         long long channels = 0;
         for (int t = 0; t < T; ++t) channels += tables[t]->desc.C;
@@ -352,6 +380,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             g->cx_total += (long long)d.C * d.nx;
             g->fold_all = g->fold_all && fold_ok(d);
             g->wsv_all = g->wsv_all && wsv_ok(d);
+            g->foldk_all = g->foldk_all && foldk_ok(d);
+            for (int c = 0; c < d.C; ++c) kitems.push_back(fk::ColSeg{t, c, 0, 0});
             for (int c = 0; c < d.C; ++c)
                 for (int ch = 0; ch < g->fold_nchunk; ++ch) foitems.push_back(fk::ColSeg{t, c, ch, 0});
         }
@@ -359,6 +389,15 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             d.vec_ok = 0;
             Plan pl;
             make_plan(d, g->dtype, pl);
+        }
+        {   // VJP stage 1: the GROUP has to fill the GPU, not every table on its own -- fewer datapoint ranges per
+            // k-block mean fewer column-sum slices G[nsplit][R][K] to write and to gather (a table planned alone asks
+            // for ~24 CTAs per SM and gets up to N/16 slices)
+            const long long want = (long long)env_int("FKCONV_COLSUM_CTAS_PER_SM", 24) * std::max(1, sm_count());
+            int ns = (int)std::min<long long>(std::max<long long>(1, (want + group_kblocks - 1) / std::max<long long>(1, group_kblocks)),
+                                              std::max(1, d.N / 16));
+            ns = std::max(ns, (d.N + fk::COLSUM_MAX_ROWS - 1) / fk::COLSUM_MAX_ROWS);
+            d.nsplit = std::max(1, std::min(ns, d.N));
         }
         d.f_off = g->f_total1;
         d.out_off = g->rows_total;
@@ -389,6 +428,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     g->nvitems = (int)vitems.size();
     g->nfoitems = (int)foitems.size();
     g->nwitems = (int)witems.size();
+    g->nkitems = (int)kitems.size();
     auto bail = [&](int code) { fk_group_destroy(g); return code; };
     cudaError_t e = cudaMalloc((void**)&g->d_descs, T * sizeof(fk::TableDesc));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_row_prefix, (T + 1) * sizeof(int));
@@ -399,6 +439,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_gitems, gitems.size() * sizeof(fk::ColSeg));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_vitems, vitems.size() * sizeof(fk::ColSeg));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_foitems, foitems.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_kitems, kitems.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_kitems, kitems.data(), kitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_witems, std::max<size_t>(1, witems.size()) * sizeof(fk::ColSeg));
     if (e == cudaSuccess) e = cudaMemcpy(g->d_witems, witems.data(), witems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_foitems, foitems.data(), foitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
@@ -425,6 +467,7 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_gitems) cudaFree(g->d_gitems);
     if (g->d_vitems) cudaFree(g->d_vitems);
     if (g->d_foitems) cudaFree(g->d_foitems);
+    if (g->d_kitems) cudaFree(g->d_kitems);
     if (g->d_witems) cudaFree(g->d_witems);
     if (g->scratch) cudaFree(g->scratch);
     delete g;

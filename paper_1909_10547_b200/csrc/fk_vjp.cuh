@@ -205,4 +205,122 @@ fk_vjp_gather_kernel(const __grid_constant__ GatherParams p) {
     }
 }
 
+// ---- stage 2 for hadronic tables, small R: one pass over the column sums, both legs at once -----------
+//   A[r][c][i] = sum_j G[r][k(i,j,c)] f[r][b_c][j]      B[r][c][j] = sum_i G[r][k(i,j,c)] f[r][a_c][i]
+//   df[r][alpha][x] = sum_{c: a_c = alpha} A[r][c][x] + sum_{c: b_c = alpha} B[r][c][x]
+// fk_vjp_foldk_kernel: CTA = (channel, replica).  The channel's nx x nx block of G (the datapoint splits added
+// in a fixed order) goes to shared memory with coalesced loads, rows padded to an odd stride; thread x < nx
+// then sums row x (A) and thread nx + x sums column x (B), each a sequential chain in index order.  The gather
+// kernel above reads G twice with a stride and rebuilds the channel lists in every CTA; it stays for DIS.
+struct FoldKParams {
+    TableDesc desc;           // single
+    ChannelList chan;         // single
+    const TableDesc* descs;   // grouped (device)
+    const ColSeg* items;      // grouped fold launch: {table, kblock = channel}
+    const int* ai_prefix;     // grouped final launch [T+1]
+    int T;
+    const void* f;
+    const double* G;
+    double* PA;               // [R][cx_total]: (cx_off + c*nx + x)
+    double* PB;               // [R][nchunk][cx_total]
+    long long cx_total;
+    int nchunk;               // x-row chunks per channel (B partials per chunk)
+    void* df;
+    int R;
+};
+
+constexpr int FOLDK_THREADS = 256;
+
+template <typename T, bool GROUPED>
+__global__ void __launch_bounds__(FOLDK_THREADS)
+fk_vjp_foldk_kernel(const __grid_constant__ FoldKParams p) {
+    extern __shared__ __align__(16) unsigned char fk_smem[];
+    double* Gs = reinterpret_cast<double*>(fk_smem);  // [nx][nx | 1]
+    const TableDesc* dp = &p.desc;
+    const uint8_t* __restrict__ ca = p.chan.a;
+    const uint8_t* __restrict__ cb = p.chan.b;
+    int c = blockIdx.x / p.nchunk;
+    const int chunk = blockIdx.x % p.nchunk;
+    if constexpr (GROUPED) {
+        const ColSeg it = p.items[c];
+        dp = &p.descs[it.table];
+        ca = dp->chan_a;
+        cb = dp->chan_b;
+        c = it.kblock;
+    }
+    const TableDesc& d = *dp;
+    const int nx = d.nx, R = p.R, r = blockIdx.y, ld = nx | 1;
+    const int i0 = (int)((long long)nx * chunk / p.nchunk), i1 = (int)((long long)nx * (chunk + 1) / p.nchunk);
+    const double* __restrict__ G = p.G + d.g_off * R + (long long)r * d.K;
+    const long long split_stride = (long long)R * d.K;
+    for (int t = threadIdx.x + i0 * nx; t < i1 * nx; t += FOLDK_THREADS) {
+        const int i = t / nx, j = t - i * nx;
+        const int k = encode_k(d, i, j, c);
+        double v = G[k];
+        int s = 1;
+        for (; s + 4 <= d.nsplit; s += 4) {  // four independent loads in flight, added in index order
+            const double v0 = G[s * split_stride + k], v1 = G[(s + 1) * split_stride + k];
+            const double v2 = G[(s + 2) * split_stride + k], v3 = G[(s + 3) * split_stride + k];
+            v = (((v + v0) + v1) + v2) + v3;
+        }
+        for (; s < d.nsplit; ++s) v += G[s * split_stride + k];
+        Gs[(i - i0) * ld + j] = v;
+    }
+    __syncthreads();
+    const T* __restrict__ f = reinterpret_cast<const T*>(p.f) + d.f_off * R + (long long)r * d.nfl * nx;
+    const long long o = (long long)r * p.cx_total + d.cx_off + (long long)c * nx;
+    const int ni = i1 - i0;
+    for (int t = threadIdx.x; t < ni + nx; t += FOLDK_THREADS) {
+        double acc = 0.0;
+        if (t < ni) {
+            const T* fb = f + (int)cb[c] * nx;
+            for (int j = 0; j < nx; ++j) acc = fma(Gs[t * ld + j], (double)fb[j], acc);
+            p.PA[o + i0 + t] = acc;
+        } else {
+            const int x = t - ni;
+            const T* fa = f + (int)ca[c] * nx + i0;
+            for (int i = 0; i < ni; ++i) acc = fma(Gs[i * ld + x], (double)fa[i], acc);
+            p.PB[o + ((long long)r * (p.nchunk - 1) + chunk) * p.cx_total + x] = acc;
+        }
+    }
+}
+
+// one warp per (PDF slot, replica): lane l adds the channels l, l + 32, ... of this flavour in index order, then a
+// fixed xor butterfly
+template <typename T, bool GROUPED>
+__global__ void __launch_bounds__(256)
+fk_vjp_foldk_final_kernel(const __grid_constant__ FoldKParams p, long long slots_total) {
+    const long long gs = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (gs >= slots_total) return;
+    const TableDesc* dp = &p.desc;
+    const uint8_t* __restrict__ ca = p.chan.a;
+    const uint8_t* __restrict__ cb = p.chan.b;
+    int slot = (int)gs;
+    if constexpr (GROUPED) {
+        int lo = 0, hi = p.T;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (p.ai_prefix[mid] <= gs) lo = mid; else hi = mid;
+        }
+        dp = &p.descs[lo];
+        slot = (int)(gs - p.ai_prefix[lo]);
+        ca = dp->chan_a;
+        cb = dp->chan_b;
+    }
+    const TableDesc& d = *dp;
+    const int nx = d.nx, R = p.R, r = blockIdx.y;
+    const int alpha = slot / nx, x = slot - alpha * nx;
+    const double* __restrict__ PA = p.PA + (long long)r * p.cx_total + d.cx_off + x;
+    const double* __restrict__ PB = p.PB + (long long)r * p.nchunk * p.cx_total + d.cx_off + x;
+    double s = 0.0;
+    for (int c = lane; c < d.C; c += 32) {
+        if (ca[c] == alpha) s += PA[c * nx];
+        if (cb[c] == alpha)
+            for (int ch = 0; ch < p.nchunk; ++ch) s += PB[ch * p.cx_total + c * nx];
+    }
+    s = warp_sum(s);
+    if (lane == 0) reinterpret_cast<T*>(p.df)[d.f_off * R + ((long long)r * d.nfl + alpha) * nx + x] = (T)s;
+}
+
 }  // namespace fk
