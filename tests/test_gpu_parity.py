@@ -83,6 +83,40 @@ def test_ragged_shapes_hadronic(K, shape, R):
             assert np.all(dn[:, a, :] == 0.0)
 
 
+# R >> 1 path: every fragment count of the warp-specialised DMMA kernels (replica passes are padded to 16),
+# datapoint tiles of 128 / 64 / 32 rows (k sub-splits 1 / 2 / 4), K ranges that end inside a channel block
+@pytest.mark.parametrize("R", [8, 17, 33, 49, 70, 81, 100, 113, 128, 150])
+@pytest.mark.parametrize("shape", [(70, 13, 14, 17), (200, 30, 14, 9), (20, 21, 6, 5)])
+def test_dense_path_replica_counts(K, shape, R):
+    N, nx, nfl, C = shape
+    case = synth.hadronic_case(6, N, nx, C, R, nfl=nfl, sub=N * 1000 + nx + R)
+    # a general upstream gradient g[n][r] (reading R8), not the broadcast weights of config 4
+    g = synth.rng_for(6, synth.T_G, 7 + R).standard_normal(size=(N, R))
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, g)
+    fk_d, idx, tb, tp = _tables(K, case, K.FK_KIND_HADRONIC)
+    f_d, g_d = to_dev(case.f), to_dev(g)
+    for name, t in (("borrow", tb), ("pack", tp)):
+        assert rel_err(t.conv(f_d).cpu().numpy(), ref, scale) <= TOL64, (name, shape, R)
+        assert rel_err(t.vjp(f_d, g_d).cpu().numpy(), dref, D) <= TOL64, (name, shape, R)
+    assert np.array_equal(tp.conv(f_d).cpu().numpy(), tp.conv(f_d).cpu().numpy())
+    assert np.array_equal(tp.vjp(f_d, g_d).cpu().numpy(), tp.vjp(f_d, g_d).cpu().numpy())
+
+
+# x-grids beyond what the single-pass VJP folds hold (nx > 64 at R >> 1, nx > 128 at small R): gather fallbacks
+@pytest.mark.parametrize("shape_R", [((12, 70, 3, 4), 6), ((12, 70, 3, 4), 1), ((6, 131, 2, 2), 1), ((6, 131, 2, 2), 5)])
+def test_large_x_grids(K, shape_R):
+    (N, nx, nfl, C), R = shape_R
+    case = synth.hadronic_case(7, N, nx, C, R, nfl=nfl, sub=nx)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    fk_d, idx, tb, tp = _tables(K, case, K.FK_KIND_HADRONIC)
+    f_d, g_d = to_dev(case.f), to_dev(case.g)
+    for name, t in (("borrow", tb), ("pack", tp)):
+        assert rel_err(t.conv(f_d).cpu().numpy(), ref, scale) <= TOL64, (name, shape_R)
+        assert rel_err(t.vjp(f_d, g_d).cpu().numpy(), dref, D) <= TOL64, (name, shape_R)
+
+
 # ------------------------------------------------------------------ config 1 (DIS)
 @pytest.mark.parametrize("R", [1, 100])
 def test_config1_dis(K, R):
