@@ -219,7 +219,11 @@ def run_extras(K, torch, level, table2, case2, peak):
     ms = _bench_call(lambda: table2.vjp(f2, g2, d2), stream)
     out["cfg2_vjp"] = {"ms": ms, "GBps": fkb / ms / 1e6, "frac_of_peak": fkb / ms / 1e6 / peak}
 
-    # config 0 (tiny hadronic) and config 1 (DIS): latency-bound, L2 flushed before each call
+    # forward + VJP from ONE read of FK (fk_table_conv_vjp: g known before the forward pass).
+    # GBps counts the FK bytes that really move (once); step_equiv_GBps the two-pass step it replaces.
+    ms = _bench_call(lambda: table2.conv_vjp(f2, g2, s2, d2), stream)
+    out["cfg2_conv_vjp_one_read"] = {"ms": ms, "GBps": fkb / ms / 1e6, "frac_of_peak": fkb / ms / 1e6 / peak,
+                                     "step_equiv_GBps": 2 * fkb / ms / 1e6}
     c0 = synth.config0()
     t0 = K.FkTable(K.FK_KIND_HADRONIC, torch.from_numpy(c0.fk).cuda(), c0.pairs, c0.nfl)
     f0 = torch.from_numpy(c0.f).cuda(); s0 = torch.empty((c0.N, 1), dtype=torch.float64, device="cuda")

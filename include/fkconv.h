@@ -117,6 +117,13 @@ int fk_table_info(const fk_table* t, int* N, int* nx, int* nfl, int* C, int64_t*
 /* f, sigma, g, df: dev, in the table's dtype (double for FK_F64, float for FK_F32). */
 int fk_table_conv(fk_table* t, const void* f, void* sigma, int R, void* stream);
 int fk_table_vjp(fk_table* t, const void* f, const void* g, void* df, int R, void* stream);
+/* Convolution (Eq. (1)) AND its VJP for an upstream gradient g[N][R] that is known
+ * before the forward pass (a loss linear in sigma, e.g. fixed weights w_n): FK is read ONCE for both -- the
+ * column kernel accumulates the column sums sum_n g[n][r] FK[n][k] from the registers that hold the row pieces.
+ * Results equal fk_table_conv + fk_table_vjp within the tolerance (same level-1 partials; the column sums are
+ * cut into the forward's datapoint ranges).  R >= 5 (dense path) and DIS tables run the two passes one after
+ * the other.  sigma[N][R], df[R][nfl][nx]: dev, overwritten; asynchronous on `stream`. */
+int fk_table_conv_vjp(fk_table* t, const void* f, const void* g, void* sigma, void* df, int R, void* stream);
 /* Same with HOST buffers: H2D of f (and g) and D2H of the result run inside the call, through
  * pinned staging, on `stream`; the call returns after the result has landed in host memory. */
 int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R, void* stream);

@@ -599,6 +599,88 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
     return FK_OK;
 }
 
+// forward + VJP from one read of FK (fk_fused_column_kernel), small R, hadronic tables.
+// scratch: part [N][R][nchunks] | G [fsplit][R][K] | fold partials
+template <typename T>
+bool fused_ok(const fk::TableDesc& d, int R) {
+    return !gemm_wanted<T>(d, R) && foldk_ok(d) && (d.N + d.fsplit - 1) / d.fsplit <= 64 && env_int("FKCONV_FUSED", 1);
+}
+size_t fused_scratch_elems(const fk::TableDesc& d, int R) {
+    return (part_elems_per_replica(d) + (size_t)d.fsplit * d.K + (1 + FOLDK_MAX_CHUNKS) * (size_t)d.C * d.nx) * R;
+}
+
+template <typename T>
+int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const Plan& pl, const T* f, const T* g,
+                       T* sigma, T* df, int R, double* scratch, cudaStream_t s, int* launches) {
+    constexpr int VW = fk::VecWidth<T>::value;
+    fk::TableDesc d = d0;
+    d.nsplit = d.fsplit;  // the column sums are cut into the forward's datapoint ranges
+    double* part = scratch;
+    double* G = part + part_elems_per_replica(d) * R;
+    int nl = 0;
+    fk::FusedParams p;
+    memset(&p, 0, sizeof p);
+    p.fwd.desc = d;
+    p.fwd.chan = ch;
+    p.fwd.f = f;
+    p.fwd.part = part;
+    p.fwd.sigma = sigma;
+    p.fwd.R = R;
+    p.g = g;
+    p.G = G;
+    const int grid = pl.nkb * pl.fsplit;
+    for (int r0 = 0; r0 < R;) {
+        const int rt = pick_rt(R - r0);
+        p.fwd.r0 = r0;
+#define FK_FUSED(V, RTv) fk::fk_fused_column_kernel<T, V, RTv, FWD_U><<<grid, fk::FWD_THREADS, 0, s>>>(p)
+        if (d.vec_ok) {
+            if (rt == 1) FK_FUSED(VW, 1); else if (rt == 2) FK_FUSED(VW, 2); else FK_FUSED(VW, 4);
+        } else {
+            if (rt == 1) FK_FUSED(1, 1); else if (rt == 2) FK_FUSED(1, 2); else FK_FUSED(1, 4);
+        }
+#undef FK_FUSED
+        ++nl;
+        r0 += rt;
+    }
+    if (pl.nkb > 1) {
+        fk::ReduceParams q;
+        memset(&q, 0, sizeof q);
+        q.desc = d;
+        q.part = part;
+        q.sigma = sigma;
+        q.rows = d.N;
+        q.R = R;
+        const long long outs = (long long)d.N * R;
+        const int rgrid = (int)std::min<long long>((outs + 7) / 8, (long long)sm_count() * 8);
+        fk::fk_reduce_chunks_kernel<T, false><<<std::max(1, rgrid), 256, 0, s>>>(q);
+        ++nl;
+    }
+    static const bool attr_ok = cudaFuncSetAttribute(fk::fk_vjp_foldk_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                     (int)foldk_smem(128)) == cudaSuccess;
+    if (!attr_ok) return fail(FK_ERR_CUDA, "conv_vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
+    fk::FoldKParams q;
+    memset(&q, 0, sizeof q);
+    q.desc = d;
+    q.desc.cx_off = 0;
+    q.chan = ch;
+    q.f = f;
+    q.G = G;
+    q.cx_total = (long long)d.C * d.nx;
+    q.PA = G + (size_t)d.fsplit * d.K * R;
+    q.PB = q.PA + q.cx_total * R;
+    q.nchunk = foldk_chunks(d.C);
+    q.df = df;
+    q.R = R;
+    const long long slots = (long long)d.nfl * d.nx;
+    fk::fk_vjp_foldk_kernel<T, false><<<dim3(d.C * q.nchunk, R), fk::FOLDK_THREADS, foldk_smem(d.nx), s>>>(q);
+    fk::fk_vjp_foldk_final_kernel<T, false><<<dim3((unsigned)((slots + 7) / 8), R), 256, 0, s>>>(q, slots);
+    nl += 2;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "fused forward + VJP launch failed: %s", cudaGetErrorString(e));
+    if (launches) *launches = nl;
+    return FK_OK;
+}
+
 template <typename T>
 size_t conv_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
     if (gemm_wanted<T>(d, R)) return gemm_fwd_scratch_elems(d, R, with_kdec);
@@ -705,6 +787,22 @@ int table_vjp_t(fk_table* t, const void* f, const void* g, void* df, int R, cuda
     if (rc) return rc;
     return run_vjp_single<T>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)df, R, t->scratch, s,
                              &t->last_launches);
+}
+
+template <typename T>
+int table_conv_vjp_t(fk_table* t, const void* f, const void* g, void* sigma, void* df, int R, cudaStream_t s) {
+    if (!fused_ok<T>(t->desc, R)) {
+        int rc = table_conv_t<T>(t, f, sigma, R, s);
+        if (rc) return rc;
+        const int nl = t->last_launches;
+        rc = table_vjp_t<T>(t, f, g, df, R, s);
+        t->last_launches += nl;
+        return rc;
+    }
+    int rc = ensure_scratch(t, std::max(table_scratch_need(t, R), fused_scratch_elems(t->desc, R)));
+    if (rc) return rc;
+    return run_conv_vjp_fused<T>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)sigma, (T*)df, R, t->scratch, s,
+                                 &t->last_launches);
 }
 
 }  // namespace
@@ -883,6 +981,14 @@ int fk_table_vjp(fk_table* t, const void* f, const void* g, void* df, int R, voi
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp: R=%d", R);
     return t->dtype == FK_F64 ? table_vjp_t<double>(t, f, g, df, R, (cudaStream_t)stream)
                               : table_vjp_t<float>(t, f, g, df, R, (cudaStream_t)stream);
+}
+
+int fk_table_conv_vjp(fk_table* t, const void* f, const void* g, void* sigma, void* df, int R, void* stream) {
+    g_err.clear();
+    if (!t || !f || !g || !sigma || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp: R=%d", R);
+    return t->dtype == FK_F64 ? table_conv_vjp_t<double>(t, f, g, sigma, df, R, (cudaStream_t)stream)
+                              : table_conv_vjp_t<float>(t, f, g, sigma, df, R, (cudaStream_t)stream);
 }
 
 int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R, void* stream) {

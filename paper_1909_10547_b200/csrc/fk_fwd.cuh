@@ -152,6 +152,129 @@ fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
     }
 }
 
+// ---- one read of FK for both passes: when the upstream gradient g[n][r] is known before the
+// forward pass (a loss linear in sigma, e.g. config 4's seeded weights), the column kernel also accumulates
+// VJP stage 1, G[split][r][k] = sum_{n in range} g[n][r] FK[n][k], from the registers that already hold the row
+// pieces.  Same decomposition, same level-1 partials, same fixed orders as the two separate kernels; stage 2 of
+// the VJP (fk_vjp_foldk_kernel) and level 2 of the forward (fk_reduce_chunks_kernel) follow unchanged.
+struct FusedParams {
+    FwdParams fwd;
+    const void* g;   // g[N][R]
+    double* G;       // [fsplit][R][K] column sums, one slice per datapoint range
+};
+
+template <typename T, int VEC, int RT, int U>
+__global__ void __launch_bounds__(FWD_THREADS)
+fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
+    using V = Vec<T, VEC>;
+    constexpr int LPR = 32 / U;
+    constexpr int MAX_ROWS = 64;  // datapoints per range (the plan uses <= 32)
+    __shared__ double red[2][FWD_WARPS][U][RT];
+    __shared__ T gs[(MAX_ROWS + U) * RT];
+    const FwdParams& p = q.fwd;
+    const TableDesc& d = p.desc;
+    const uint8_t* __restrict__ ca = p.chan.a;
+    const uint8_t* __restrict__ cb = p.chan.b;
+    const int kblock = blockIdx.x % d.nchunks, split = blockIdx.x / d.nchunks;
+    const int R = p.R;
+    const int rb = (int)((long long)d.N * split / d.fsplit);
+    const int re = (int)((long long)d.N * (split + 1) / d.fsplit);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    {   // g tile of this datapoint range, zero padded to a multiple of U rows
+        const T* __restrict__ g = reinterpret_cast<const T*>(q.g);
+        const int rows = re - rb, rows_pad = (rows + U - 1) / U * U;
+        for (int t = threadIdx.x; t < rows_pad * RT; t += FWD_THREADS) {
+            const int m = t / RT, r = t - m * RT, rr = p.r0 + r;
+            gs[t] = (m < rows && rr < R) ? __ldg(g + (long long)(rb + m) * R + rr) : T(0);
+        }
+    }
+    const int k = (kblock * FWD_THREADS + threadIdx.x) * VEC;
+    const bool kin = k < d.K;
+    T L[RT][VEC];
+    {
+        const int fstride = d.nfl * d.nx;
+        const T* __restrict__ f = reinterpret_cast<const T*>(p.f);
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) {
+            int ia = 0, ib = -1;
+            bool in = k + e < d.K;
+            if (in) decode_k(d, ca, cb, k + e, ia, ib);
+            in = in && ia >= 0;
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                const int rr = p.r0 + r;
+                T l = T(0);
+                if (in && rr < R) {
+                    l = __ldg(f + (long long)rr * fstride + ia);
+                    if (ib >= 0) l *= __ldg(f + (long long)rr * fstride + ib);
+                }
+                L[r][e] = l;
+            }
+        }
+    }
+    T cs[2][RT][VEC];  // two interleaved column-sum chains
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int r = 0; r < RT; ++r)
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) cs[a][r][e] = T(0);
+    const T* __restrict__ col = reinterpret_cast<const T*>(d.fk) + (kin ? k : 0);
+    __syncthreads();
+
+    int buf = 0;
+    for (int m = rb; m < re; m += U, buf ^= 1) {
+        V x[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) x[u] = ld_stream(col + (long long)min(m + u, re - 1) * d.row_stride, (V*)nullptr);
+        double pr[RT][U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const bool live = kin && (m + u < re);
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                T s = x[u].v[0] * L[r][0];
+#pragma unroll
+                for (int e = 1; e < VEC; ++e) s = fma(x[u].v[e], L[r][e], s);
+                pr[r][u] = live ? (double)s : 0.0;
+                const T gv = gs[(m - rb + u) * RT + r];  // 0 on the padded rows
+#pragma unroll
+                for (int e = 0; e < VEC; ++e) cs[u & 1][r][e] = fma(gv, x[u].v[e], cs[u & 1][r][e]);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const double s = fold_rows<U>(pr[r], lane);
+            if ((lane & (LPR - 1)) == 0) red[buf][warp][lane / LPR][r] = s;
+        }
+        __syncthreads();
+        if (threadIdx.x < U * RT) {
+            const int u = threadIdx.x / RT, r = threadIdx.x - u * RT;
+            double s = red[buf][0][u][r];
+#pragma unroll
+            for (int w = 1; w < FWD_WARPS; ++w) s += red[buf][w][u][r];
+            const int n = m + u, rr = p.r0 + r;
+            if (n < re && rr < R) {
+                if (d.nchunks == 1)
+                    reinterpret_cast<T*>(p.sigma)[(long long)n * R + rr] = (T)s;
+                else
+                    p.part[((long long)n * R + rr) * d.nchunks + kblock] = s;
+            }
+        }
+    }
+    if (kin) {
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const int rr = p.r0 + r;
+            if (rr >= R) continue;
+#pragma unroll
+            for (int e = 0; e < VEC; ++e)
+                if (k + e < d.K) q.G[((long long)split * R + rr) * d.K + k + e] = (double)cs[0][r][e] + (double)cs[1][r][e];
+        }
+    }
+}
+
 // ---- a3 level 2: sigma[n][r] = sum over k-blocks, fixed order (lane-strided chains + butterfly) ----
 struct ReduceParams {
     TableDesc desc;           // single

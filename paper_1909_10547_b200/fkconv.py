@@ -28,7 +28,7 @@ SYMBOLS = (
     "fk_last_error_string", "fk_version", "fk_compiled_arch", "fk_profile_enable", "fk_profile_read",
     "fk_conv_dis", "fk_conv_hadronic", "fk_conv_hadronic_vjp", "fk_conv_dis_vjp",
     "fk_conv_dis_f32", "fk_conv_hadronic_f32", "fk_conv_hadronic_vjp_f32",
-    "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp",
+    "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp", "fk_table_conv_vjp",
     "fk_table_conv_host", "fk_table_vjp_host", "fk_table_last_launches",
     "fk_group_create", "fk_group_destroy", "fk_group_offsets", "fk_conv_grouped",
     "fk_conv_grouped_vjp", "fk_group_last_launches",
@@ -56,6 +56,7 @@ lib.fk_table_destroy.argtypes = [_vp]
 lib.fk_table_info.argtypes = [_vp] + [ctypes.POINTER(_ci)] * 4 + [ctypes.POINTER(ctypes.c_int64)] * 3
 lib.fk_table_conv.argtypes = [_vp, _vp, _vp, _ci, _vp]
 lib.fk_table_vjp.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
+lib.fk_table_conv_vjp.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _vp]
 lib.fk_table_conv_host.argtypes = [_vp, _vp, _vp, _ci, _vp]
 lib.fk_table_vjp_host.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
 lib.fk_table_last_launches.argtypes = [_vp]
@@ -205,6 +206,17 @@ class FkTable:
         _check(lib.fk_table_vjp(self.handle, _dev(f, self.tdtype), _dev(g, self.tdtype), _dev(df, self.tdtype),
                                 R, _stream(stream)), "fk_table_vjp")
         return df
+
+    def conv_vjp(self, f, g, sigma=None, df=None, stream=None):
+        """sigma and df from ONE read of FK, for an upstream gradient g known before the forward pass."""
+        R = f.shape[0]
+        if sigma is None:
+            sigma = torch.empty((self.N, R), dtype=self.tdtype, device=self.device)
+        if df is None:
+            df = torch.empty_like(f)
+        _check(lib.fk_table_conv_vjp(self.handle, _dev(f, self.tdtype), _dev(g, self.tdtype), _dev(sigma, self.tdtype),
+                                     _dev(df, self.tdtype), R, _stream(stream)), "fk_table_conv_vjp")
+        return sigma, df
 
     def conv_host(self, f_host: np.ndarray, sigma_host: np.ndarray, stream=None):
         R = f_host.shape[0]

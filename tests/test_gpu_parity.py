@@ -117,6 +117,44 @@ def test_large_x_grids(K, shape_R):
         assert rel_err(t.vjp(f_d, g_d).cpu().numpy(), dref, D) <= TOL64, (name, shape_R)
 
 
+# forward + VJP from one read of FK (fk_table_conv_vjp)
+@pytest.mark.parametrize("shape", RAGGED + [(512, 20, 14, 60)])
+@pytest.mark.parametrize("R", [1, 2, 3, 4, 6])
+def test_conv_vjp_one_read(K, shape, R):
+    N, nx, nfl, C = shape
+    case = synth.hadronic_case(8, N, nx, C, R, nfl=nfl, sub=N * 1000 + nx)
+    g = synth.rng_for(8, synth.T_G, 11 + R).standard_normal(size=(N, R))
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, g)
+    fk_d, idx, tb, tp = _tables(K, case, K.FK_KIND_HADRONIC)
+    f_d, g_d = to_dev(case.f), to_dev(g)
+    for name, t in (("borrow", tb), ("pack", tp)):
+        sig, df = t.conv_vjp(f_d, g_d)
+        assert rel_err(sig.cpu().numpy(), ref, scale) <= TOL64, (name, shape, R)
+        assert rel_err(df.cpu().numpy(), dref, D) <= TOL64, (name, shape, R)
+        sig2, df2 = t.conv_vjp(f_d, g_d)
+        assert np.array_equal(sig.cpu().numpy(), sig2.cpu().numpy()) and np.array_equal(df.cpu().numpy(), df2.cpu().numpy())
+    # the forward half is the same arithmetic as fk_table_conv: bit for bit
+    assert np.array_equal(tp.conv_vjp(f_d, g_d)[0].cpu().numpy(), tp.conv(f_d).cpu().numpy())
+
+
+def test_conv_vjp_one_read_dis_and_fp32(K):
+    dis = synth.config1(R=2, N=300)
+    rd, sd = O.dis(dis.fk, dis.flav, dis.f)
+    g = synth.rng_for(8, synth.T_G, 3).standard_normal(size=(dis.N, 2))
+    dref, D = O.dis_vjp(dis.fk, dis.flav, dis.f, g)
+    t = K.FkTable(K.FK_KIND_DIS, to_dev(dis.fk), dis.flav, dis.nfl)
+    sig, df = t.conv_vjp(to_dev(dis.f), to_dev(g))
+    assert rel_err(sig.cpu().numpy(), rd, sd) <= TOL64 and rel_err(df.cpu().numpy(), dref, D) <= TOL64
+    import torch
+    case = synth.hadronic_case(8, 96, 24, 30, 2, sub=5)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    t32 = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl, K.FK_F32)
+    sig, df = t32.conv_vjp(to_dev(case.f, torch.float32), to_dev(case.g, torch.float32))
+    assert rel_err(sig.cpu().numpy(), ref, scale) <= TOL32 and rel_err(df.cpu().numpy(), dref, D) <= TOL32
+
+
 # ------------------------------------------------------------------ config 1 (DIS)
 @pytest.mark.parametrize("R", [1, 100])
 def test_config1_dis(K, R):
