@@ -159,7 +159,7 @@ int check_dims(const char* who, int kind, int N, int nx, int nfl, int C, int R) 
         return fail(FK_ERR_UNSUPPORTED, "%s: nfl=%d > %d or C=%d > %d", who, nfl, fk::MAX_NFL, C, fk::MAX_C);
     const long long K = kind == FK_KIND_HADRONIC ? (long long)C * ((long long)nx * nx + 3) : (long long)C * nx;
     if (K >= (1LL << 31) - 4096) return fail(FK_ERR_UNSUPPORTED, "%s: K=%lld does not fit 31 bits", who, K);
-    if ((long long)nfl * nx >= (1LL << 24)) return fail(FK_ERR_UNSUPPORTED, "%s: nfl*nx too large", who);
+    if ((long long)nfl * nx >= (1LL << 31) - 4096) return fail(FK_ERR_UNSUPPORTED, "%s: nfl*nx does not fit 31 bits", who);
     if (kind == FK_KIND_DIS && C > nfl)
         return fail(FK_ERR_INVALID_ARG, "%s: nA=%d > nfl=%d", who, C, nfl);
     return FK_OK;
@@ -236,7 +236,11 @@ template <typename T>
 bool gemm_wanted(const fk::TableDesc& d, int R) {
     if (dtype_of<T>() != FK_F64) return false;  // the fp32 variant stays on the FFMA column kernel (reading R18)
     if ((long long)d.nfl * d.nx >= (long long)fk::KDEC_NONE) return false;
-    return R >= env_int("FKCONV_GEMM_MIN_R", 5);
+    // packed hadronic tables take the warp-specialised kernel, which beats the <= 4-replica column passes from
+    // R = 5 on; the generic cp.async kernel (DIS, logical layout) streams FK at ~2 TB/s and only wins once the
+    // column kernel would need more than 3 passes
+    const bool ws = d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok;
+    return R >= env_int("FKCONV_GEMM_MIN_R", ws ? 5 : 13);
 }
 
 GemmPlan gemm_plan(const fk::TableDesc& d, int R) {

@@ -55,7 +55,7 @@ int group_scratch(fk_group* g, size_t elems) {
 }
 
 bool group_gemm_wanted(const fk_group* g, int R) {
-    return g->gemm_ok && g->dtype == FK_F64 && R >= env_int("FKCONV_GEMM_MIN_R", 5);
+    return g->gemm_ok && g->dtype == FK_F64 && R >= env_int("FKCONV_GEMM_MIN_R", g->ws_all ? 5 : 13);
 }
 
 size_t group_scratch_need(const fk_group* g, int R) {

@@ -170,6 +170,23 @@ def test_config1_dis(K, R):
         assert rel_err(d.cpu().numpy(), dref, D) <= TOL64, name
 
 
+@pytest.mark.parametrize("shape_R", [((8, 3571, 1), 1), ((8, 3571, 1), 7), ((100, 1021, 1), 3), ((33, 2048, 1), 40)])
+def test_flat_matrix_view_of_table3(K, shape_R):
+    """The paper's Table-3 operation: flat FK[N x K] . PDF[K x R] with a pre-built PDF matrix =
+    the DIS convolution with one pseudo-flavour and nx = K (f = PDF^T)."""
+    (N, Kc, nA), R = shape_R
+    rng = synth.rng_for(9, synth.T_FK, Kc + R)
+    fk = rng.standard_normal(size=(N, Kc, nA))
+    f = rng.standard_normal(size=(R, 1, Kc))
+    flav = np.zeros(1, dtype=np.int32)
+    ref, scale = O.dis(fk, flav, f)
+    t = K.FkTable(K.FK_KIND_DIS, to_dev(fk), flav, 1, K.FK_F64, K.FK_STORE_BORROW)
+    assert rel_err(t.conv(to_dev(f)).cpu().numpy(), ref, scale) <= TOL64
+    assert rel_err(K.fk_conv_dis(to_dev(fk), flav, to_dev(f)).cpu().numpy(), ref, scale) <= TOL64
+    flat = fk.reshape(N, Kc) @ f.reshape(R, Kc).T  # library GEMM of the same flat view
+    assert rel_err(t.conv(to_dev(f)).cpu().numpy(), flat, scale) <= 1e-12
+
+
 def test_dis_small_unsorted_flavours(K):
     rng = np.random.default_rng(3)
     N, nx, nfl = 19, 11, 6
