@@ -185,3 +185,32 @@ int fk_oracle_dis_vjp(const double *fk, const int32_t *flav, const double *f, co
     }
     return fail ? -1 : 0;
 }
+
+/* Figure of merit of the fit step that follows the convolution (reading R22: the paper
+ * only says "gradient descent optimization", and never prints the loss -- this is the standard quadratic
+ * form over the data covariance):
+ *     chi2[r] = sum_{n,m} d[n][r] Cinv[n][m] d[m][r],   d[n][r] = sigma[n][r] - data[n]
+ *     g[n][r] = d chi2[r] / d sigma[n][r] = 2 sum_m Cinv[n][m] d[m][r]        (Cinv symmetric)
+ * Literal double loops, long double accumulation; cscale[r] / gscale[n][r] = sum |terms| (tolerance denominators). */
+int fk_oracle_chi2(const double *sigma, const double *data, const double *cinv, double *chi2, double *cscale,
+                   double *g, double *gscale, int N, int R) {
+    if (!sigma || !data || !cinv || !chi2 || !g || N <= 0 || R <= 0) return -1;
+    for (int r = 0; r < R; ++r) {
+        acc_t tot = 0, totabs = 0;
+        for (int n = 0; n < N; ++n) {
+            const acc_t dn = (acc_t)sigma[(size_t)n * R + r] - (acc_t)data[n];
+            acc_t row = 0, rowabs = 0;
+            for (int m = 0; m < N; ++m) {
+                const acc_t dm = (acc_t)sigma[(size_t)m * R + r] - (acc_t)data[m];
+                const acc_t t = (acc_t)cinv[(size_t)n * N + m] * dm;
+                row += t;  rowabs += fabsl(t);
+                tot += dn * t;  totabs += fabsl(dn * t);
+            }
+            g[(size_t)n * R + r] = (double)(2 * row);
+            if (gscale) gscale[(size_t)n * R + r] = (double)(2 * rowabs);
+        }
+        chi2[r] = (double)tot;
+        if (cscale) cscale[r] = (double)totabs;
+    }
+    return 0;
+}

@@ -31,7 +31,7 @@ def _load():
     if _lib is None:
         _lib = ctypes.CDLL(build())
         for name in ("fk_oracle_hadronic2", "fk_oracle_hadronic", "fk_oracle_dis",
-                     "fk_oracle_hadronic_vjp", "fk_oracle_dis_vjp"):
+                     "fk_oracle_hadronic_vjp", "fk_oracle_dis_vjp", "fk_oracle_chi2"):
             getattr(_lib, name).restype = ctypes.c_int
         _lib.fk_oracle_num_threads.restype = ctypes.c_int
     return _lib
@@ -103,3 +103,15 @@ def dis_vjp(fk, flav, f, g):
     if rc != 0:
         raise ValueError("fk_oracle_dis_vjp: invalid argument")
     return df, D
+
+
+def chi2(sigma, data, cinv):
+    """chi2[R], cscale[R], g[N][R], gscale[N][R] for sigma[N][R], data[N], symmetric cinv[N][N] (reading R22)."""
+    sigma, data, cinv = _d(sigma), _d(data), _d(cinv)
+    N, R = sigma.shape
+    assert data.shape == (N,) and cinv.shape == (N, N)
+    c = np.empty(R); cs = np.empty(R); g = np.empty((N, R)); gs = np.empty((N, R))
+    rc = _load().fk_oracle_chi2(_p(sigma), _p(data), _p(cinv), _p(c), _p(cs), _p(g), _p(gs), N, R)
+    if rc != 0:
+        raise ValueError("fk_oracle_chi2: invalid argument")
+    return c, cs, g, gs

@@ -310,3 +310,64 @@ def test_invalid_arguments_rejected():
         O.hadronic_vjp(fk, bad, f, g)
     with pytest.raises(ValueError):
         O.dis(np.ones((2, 4, 2)), np.array([0, -1], dtype=np.int32), f)
+
+
+# ------------------------------------------------------------------ chi2 of the fit step (reading R22)
+def _spd(rng, N):
+    a = rng.standard_normal(size=(N, N))
+    return a @ a.T / N + np.eye(N)
+
+
+def test_chi2_identity_covariance_exact_integers():
+    """Cinv = 1: chi2 = sum d^2 and g = 2 d, exact for integer inputs."""
+    rng = np.random.default_rng(7)
+    N, R = 23, 3
+    sigma = rng.integers(-8, 9, size=(N, R)).astype(np.float64)
+    data = rng.integers(-8, 9, size=N).astype(np.float64)
+    c, cs, g, gs = O.chi2(sigma, data, np.eye(N))
+    d = sigma - data[:, None]
+    assert np.array_equal(c, (d * d).sum(axis=0)) and np.array_equal(g, 2 * d)
+    assert np.array_equal(cs, c) and np.array_equal(gs, 2 * np.abs(d))
+
+
+def test_chi2_brute_force_fractions():
+    rng = np.random.default_rng(8)
+    N, R = 3, 2
+    sigma = rng.integers(-5, 6, size=(N, R)) / 4.0
+    data = rng.integers(-5, 6, size=N) / 8.0
+    cinv = rng.integers(-4, 5, size=(N, N)) / 2.0
+    cinv = cinv + cinv.T
+    c, _, g, _ = O.chi2(sigma, data, cinv)
+    F = Fraction
+    for r in range(R):
+        d = [F(sigma[n, r]) - F(data[n]) for n in range(N)]
+        tot = sum(d[n] * F(cinv[n, m]) * d[m] for n in range(N) for m in range(N))
+        assert c[r] == float(tot)
+        for n in range(N):
+            assert g[n, r] == float(2 * sum(F(cinv[n, m]) * d[m] for m in range(N)))
+
+
+def test_chi2_matches_numpy_quadratic_form_and_euler_identity():
+    rng = np.random.default_rng(9)
+    N, R = 61, 4
+    sigma, data, cinv = rng.standard_normal(size=(N, R)), rng.standard_normal(size=N), _spd(rng, N)
+    c, cs, g, gs = O.chi2(sigma, data, cinv)
+    d = sigma - data[:, None]
+    ref = np.einsum("nr,nm,mr->r", d, cinv, d)
+    assert np.all(np.abs(c - ref) <= 1e-14 * cs)
+    assert np.all(np.abs(g - 2 * cinv @ d) <= 1e-14 * gs)
+    # chi2 is homogeneous of degree 2 in d: sum_n g_n d_n = 2 chi2
+    assert np.all(np.abs((g * d).sum(axis=0) - 2 * c) <= 1e-13 * cs)
+
+
+def test_chi2_gradient_is_the_central_difference():
+    """A quadratic form has no third derivative: the central difference is exact up to rounding for any h."""
+    rng = np.random.default_rng(10)
+    N = 17
+    sigma, data, cinv = rng.standard_normal(size=(N, 1)), rng.standard_normal(size=N), _spd(rng, N)
+    _, cs, g, _ = O.chi2(sigma, data, cinv)
+    h = 1e-3
+    for n in (0, 5, 16):
+        e = np.zeros((N, 1)); e[n] = h
+        cp = O.chi2(sigma + e, data, cinv)[0][0]; cm = O.chi2(sigma - e, data, cinv)[0][0]
+        assert abs((cp - cm) / (2 * h) - g[n, 0]) <= 1e-15 * cs[0] / h + 1e-12 * abs(g[n, 0])  # rounding of chi2 / h
