@@ -224,6 +224,16 @@ def run_extras(K, torch, level, table2, case2, peak):
     ms = _bench_call(lambda: table2.conv_vjp(f2, g2, s2, d2), stream)
     out["cfg2_conv_vjp_one_read"] = {"ms": ms, "GBps": fkb / ms / 1e6, "frac_of_peak": fkb / ms / 1e6 / peak,
                                      "step_equiv_GBps": 2 * fkb / ms / 1e6}
+    # one fit iteration (fk_table_fit_step): forward -> chi2 and its gradient -> VJP, all on the device
+    rng = np.random.default_rng(190910547 + 2001)
+    a_ = rng.standard_normal(size=(case2.N, case2.N))
+    cinv2 = torch.from_numpy(a_ @ a_.T / case2.N + np.eye(case2.N)).cuda()
+    data2 = torch.from_numpy(rng.standard_normal(size=case2.N)).cuda()
+    gg = torch.empty_like(s2); c2 = torch.empty(1, dtype=torch.float64, device="cuda")
+    ms = _bench_call(lambda: table2.fit_step(f2, data2, cinv2, s2, gg, c2, d2), stream)
+    out["cfg2_fit_step"] = {"ms": ms, "GBps": 2 * fkb / ms / 1e6, "frac_of_peak": 2 * fkb / ms / 1e6 / peak,
+                            "fit_iterations_per_s": 1e3 / ms}
+    # config 0 (tiny hadronic) and config 1 (DIS): latency-bound, L2 flushed before each call
     c0 = synth.config0()
     t0 = K.FkTable(K.FK_KIND_HADRONIC, torch.from_numpy(c0.fk).cuda(), c0.pairs, c0.nfl)
     f0 = torch.from_numpy(c0.f).cuda(); s0 = torch.empty((c0.N, 1), dtype=torch.float64, device="cuda")

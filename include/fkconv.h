@@ -124,6 +124,16 @@ int fk_table_vjp(fk_table* t, const void* f, const void* g, void* df, int R, voi
  * cut into the forward's datapoint ranges).  R >= 5 (dense path) and DIS tables run the two passes one after
  * the other.  sigma[N][R], df[R][nfl][nx]: dev, overwritten; asynchronous on `stream`. */
 int fk_table_conv_vjp(fk_table* t, const void* f, const void* g, void* sigma, void* df, int R, void* stream);
+/* The step that follows the convolution in a fit iteration (reading R22; the paper names the
+ * "gradient descent optimization", but never prints the loss): with d[n][r] = sigma[n][r] - data[n],
+ *     chi2[r] = sum_{n,m} d[n][r] cinv[n][m] d[m][r],      g[n][r] = 2 sum_m cinv[n][m] d[m][r]
+ * sigma[N][R], data[N], cinv[N][N] (symmetric, row-major): dev, read; chi2[R], g[N][R]: dev, overwritten.  fp64. */
+int fk_chi2(const double* sigma, const double* data, const double* cinv, double* chi2, double* g, int N, int R,
+            void* stream);
+/* One fit iteration on a resident table, all on `stream`: sigma = conv(f); (chi2, g) = fk_chi2(sigma); df = vjp(f, g).
+ * Equal, bit for bit, to the three calls made one after the other.  fp64 tables only. */
+int fk_table_fit_step(fk_table* t, const double* f, const double* data, const double* cinv, double* sigma, double* g,
+                      double* chi2, double* df, int R, void* stream);
 /* Same with HOST buffers: H2D of f (and g) and D2H of the result run inside the call, through
  * pinned staging, on `stream`; the call returns after the result has landed in host memory. */
 int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R, void* stream);

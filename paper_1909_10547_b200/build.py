@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfkconv.so")
 SOURCES = ["fk_api.cu"]
-DEPS = ["fk_api.cu", "fk_group.inl", "fk_common.cuh", "fk_fwd.cuh", "fk_vjp.cuh", "fk_gemm.cuh", "fk_gemm_ws.cuh", "fk_vjp_fold.cuh", "fk_pack.cuh"]
+DEPS = ["fk_api.cu", "fk_group.inl", "fk_common.cuh", "fk_fwd.cuh", "fk_vjp.cuh", "fk_gemm.cuh", "fk_gemm_ws.cuh", "fk_vjp_fold.cuh", "fk_chi2.cuh", "fk_pack.cuh"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -25,6 +25,7 @@
 #include "fk_pack.cuh"
 #include "fk_fwd.cuh"
 #include "fk_vjp.cuh"
+#include "fk_chi2.cuh"
 
 namespace {
 
@@ -993,6 +994,33 @@ int fk_table_conv_vjp(fk_table* t, const void* f, const void* g, void* sigma, vo
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp: R=%d", R);
     return t->dtype == FK_F64 ? table_conv_vjp_t<double>(t, f, g, sigma, df, R, (cudaStream_t)stream)
                               : table_conv_vjp_t<float>(t, f, g, sigma, df, R, (cudaStream_t)stream);
+}
+
+int fk_chi2(const double* sigma, const double* data, const double* cinv, double* chi2, double* g, int N, int R, void* stream) {
+    g_err.clear();
+    if (!sigma || !data || !cinv || !chi2 || !g) return fail(FK_ERR_INVALID_ARG, "fk_chi2: null pointer");
+    if (N <= 0 || R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_chi2: non-positive size (N=%d R=%d)", N, R);
+    cudaStream_t s = (cudaStream_t)stream;
+    fk::fk_chi2_grad_kernel<<<N, dim3(32, 8), 0, s>>>(sigma, data, cinv, g, N, R);
+    fk::fk_chi2_sum_kernel<<<(R + 7) / 8, 256, 0, s>>>(sigma, data, g, chi2, N, R);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "fk_chi2 launch failed: %s", cudaGetErrorString(e));
+    return FK_OK;
+}
+
+int fk_table_fit_step(fk_table* t, const double* f, const double* data, const double* cinv, double* sigma, double* g,
+                      double* chi2, double* df, int R, void* stream) {
+    g_err.clear();
+    if (!t || !f || !data || !cinv || !sigma || !g || !chi2 || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_fit_step: null pointer");
+    if (t->dtype != FK_F64) return fail(FK_ERR_UNSUPPORTED, "fk_table_fit_step: fp64 tables only");
+    int rc = fk_table_conv(t, f, sigma, R, stream);
+    if (rc) return rc;
+    const int nl = t->last_launches;
+    rc = fk_chi2(sigma, data, cinv, chi2, g, t->desc.N, R, stream);
+    if (rc) return rc;
+    rc = fk_table_vjp(t, f, g, df, R, stream);
+    t->last_launches += nl + 2;
+    return rc;
 }
 
 int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R, void* stream) {

@@ -28,7 +28,7 @@ SYMBOLS = (
     "fk_last_error_string", "fk_version", "fk_compiled_arch", "fk_profile_enable", "fk_profile_read",
     "fk_conv_dis", "fk_conv_hadronic", "fk_conv_hadronic_vjp", "fk_conv_dis_vjp",
     "fk_conv_dis_f32", "fk_conv_hadronic_f32", "fk_conv_hadronic_vjp_f32",
-    "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp", "fk_table_conv_vjp",
+    "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp", "fk_table_conv_vjp", "fk_chi2", "fk_table_fit_step",
     "fk_table_conv_host", "fk_table_vjp_host", "fk_table_last_launches",
     "fk_group_create", "fk_group_destroy", "fk_group_offsets", "fk_conv_grouped",
     "fk_conv_grouped_vjp", "fk_group_last_launches",
@@ -56,6 +56,8 @@ lib.fk_table_destroy.argtypes = [_vp]
 lib.fk_table_info.argtypes = [_vp] + [ctypes.POINTER(_ci)] * 4 + [ctypes.POINTER(ctypes.c_int64)] * 3
 lib.fk_table_conv.argtypes = [_vp, _vp, _vp, _ci, _vp]
 lib.fk_table_vjp.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
+lib.fk_chi2.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, _vp]
+lib.fk_table_fit_step.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _ci, _vp]
 lib.fk_table_conv_vjp.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _vp]
 lib.fk_table_conv_host.argtypes = [_vp, _vp, _vp, _ci, _vp]
 lib.fk_table_vjp_host.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
@@ -162,6 +164,18 @@ def fk_conv_dis_vjp(fk, flav, f, g, df=None, stream=None):
     return df
 
 
+def fk_chi2(sigma, data, cinv, chi2=None, g=None, stream=None):
+    """chi2[R], g[N][R] for sigma[N][R], data[N], symmetric cinv[N][N] (fp64, device)."""
+    N, R = sigma.shape
+    if chi2 is None:
+        chi2 = torch.empty(R, dtype=torch.float64, device=sigma.device)
+    if g is None:
+        g = torch.empty_like(sigma)
+    _check(lib.fk_chi2(_dev(sigma, torch.float64), _dev(data, torch.float64), _dev(cinv, torch.float64),
+                       _dev(chi2, torch.float64), _dev(g, torch.float64), N, R, _stream(stream)), "fk_chi2")
+    return chi2, g
+
+
 # ------------------------------------------------------------------ resident tables
 class FkTable:
     """fk_table handle.  `fk_logical` is the fp64 logical-layout table on the device; with
@@ -217,6 +231,18 @@ class FkTable:
         _check(lib.fk_table_conv_vjp(self.handle, _dev(f, self.tdtype), _dev(g, self.tdtype), _dev(sigma, self.tdtype),
                                      _dev(df, self.tdtype), R, _stream(stream)), "fk_table_conv_vjp")
         return sigma, df
+
+    def fit_step(self, f, data, cinv, sigma=None, g=None, chi2=None, df=None, stream=None):
+        """One fit iteration: sigma = conv(f), (chi2, g) = fk_chi2(sigma, data, cinv), df = vjp(f, g)."""
+        R = f.shape[0]
+        sigma = torch.empty((self.N, R), dtype=self.tdtype, device=self.device) if sigma is None else sigma
+        g = torch.empty_like(sigma) if g is None else g
+        chi2 = torch.empty(R, dtype=torch.float64, device=self.device) if chi2 is None else chi2
+        df = torch.empty_like(f) if df is None else df
+        _check(lib.fk_table_fit_step(self.handle, _dev(f, torch.float64), _dev(data, torch.float64), _dev(cinv, torch.float64),
+                                     _dev(sigma, torch.float64), _dev(g, torch.float64), _dev(chi2, torch.float64),
+                                     _dev(df, torch.float64), R, _stream(stream)), "fk_table_fit_step")
+        return sigma, chi2, g, df
 
     def conv_host(self, f_host: np.ndarray, sigma_host: np.ndarray, stream=None):
         R = f_host.shape[0]

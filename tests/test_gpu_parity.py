@@ -349,3 +349,46 @@ def test_error_paths_on_device(K):
         K.FkTable(K.FK_KIND_HADRONIC, fk_d, bad, case.nfl)
     with pytest.raises(K.FkError):
         K.FkTable(K.FK_KIND_HADRONIC, fk_d, case.pairs, case.nfl, K.FK_F32, K.FK_STORE_BORROW)
+
+
+# ------------------------------------------------------------------ chi2 and the fit step (reading R22)
+def _spd(rng, N):
+    a = rng.standard_normal(size=(N, N))
+    return a @ a.T / N + np.eye(N)
+
+
+@pytest.mark.parametrize("N_R", [(1, 1), (7, 3), (100, 1), (257, 9), (512, 128)])
+def test_chi2_against_oracle(K, N_R):
+    N, R = N_R
+    rng = synth.rng_for(10, synth.T_G, N + R)
+    sigma, data, cinv = rng.standard_normal(size=(N, R)), rng.standard_normal(size=N), _spd(rng, N)
+    c, cs, g, gs = O.chi2(sigma, data, cinv)
+    cd, gd = K.fk_chi2(to_dev(sigma), to_dev(data), to_dev(cinv))
+    assert rel_err(cd.cpu().numpy(), c, cs) <= TOL64
+    assert rel_err(gd.cpu().numpy(), g, gs) <= TOL64
+    # exact integers: bit for bit
+    si = rng.integers(-8, 9, size=(N, R)).astype(np.float64); di = rng.integers(-8, 9, size=N).astype(np.float64)
+    ci = rng.integers(-3, 4, size=(N, N)).astype(np.float64); ci = ci + ci.T
+    c, _, g, _ = O.chi2(si, di, ci)
+    cd, gd = K.fk_chi2(to_dev(si), to_dev(di), to_dev(ci))
+    assert np.array_equal(cd.cpu().numpy(), c) and np.array_equal(gd.cpu().numpy(), g)
+
+
+@pytest.mark.parametrize("R", [1, 3, 20])
+def test_fit_step_is_the_three_calls(K, R):
+    case = synth.hadronic_case(11, 70, 16, 25, R, sub=R)
+    rng = synth.rng_for(11, synth.T_G, 99)
+    data, cinv = rng.standard_normal(size=case.N) * 10, _spd(rng, case.N)
+    t = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl)
+    f_d, data_d, cinv_d = to_dev(case.f), to_dev(data), to_dev(cinv)
+    sig, chi2, g, df = t.fit_step(f_d, data_d, cinv_d)
+    s2 = t.conv(f_d); c2, g2 = K.fk_chi2(s2, data_d, cinv_d); d2 = t.vjp(f_d, g2)
+    for a, b in ((sig, s2), (chi2, c2), (g, g2), (df, d2)):
+        assert np.array_equal(a.cpu().numpy(), b.cpu().numpy())
+    # every stage against the oracle on the inputs that stage saw
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    assert rel_err(sig.cpu().numpy(), ref, scale) <= TOL64
+    c, cs, go, gs = O.chi2(sig.cpu().numpy(), data, cinv)
+    assert rel_err(chi2.cpu().numpy(), c, cs) <= TOL64 and rel_err(g.cpu().numpy(), go, gs) <= TOL64
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, g.cpu().numpy())
+    assert rel_err(df.cpu().numpy(), dref, D) <= TOL64
