@@ -392,3 +392,16 @@ def test_fit_step_is_the_three_calls(K, R):
     assert rel_err(chi2.cpu().numpy(), c, cs) <= TOL64 and rel_err(g.cpu().numpy(), go, gs) <= TOL64
     dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, g.cpu().numpy())
     assert rel_err(df.cpu().numpy(), dref, D) <= TOL64
+
+
+def test_sharded_table_single_rank(K):
+    """ShardedFkTable at world size 1 (the only size one GPU allows; world size 2 runs on CPU with gloo,
+    tests/test_sharded_cpu.py): the rank's slice is the whole table, no collective is issued."""
+    from paper_1909_10547_b200 import sharded
+    case = synth.hadronic_case(12, 37, 9, 11, 3, sub=4)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    t = sharded.ShardedFkTable(K.FK_KIND_HADRONIC, case.fk, case.pairs, case.nfl)
+    assert (t.n0, t.n1) == (0, case.N)
+    assert rel_err(t.conv_all(to_dev(case.f)).cpu().numpy(), ref, scale) <= TOL64
+    assert rel_err(t.vjp(to_dev(case.f), to_dev(case.g)).cpu().numpy(), dref, D) <= TOL64
