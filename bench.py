@@ -233,7 +233,15 @@ def run_extras(K, torch, level, table2, case2, peak):
     ms = _bench_call(lambda: table2.fit_step(f2, data2, cinv2, s2, gg, c2, d2), stream)
     out["cfg2_fit_step"] = {"ms": ms, "GBps": 2 * fkb / ms / 1e6, "frac_of_peak": 2 * fkb / ms / 1e6 / peak,
                             "fit_iterations_per_s": 1e3 / ms}
-    # config 0 (tiny hadronic) and config 1 (DIS): latency-bound, L2 flushed before each call
+    # config 2 with the table stored in fp32 and everything else fp64 (FK_F32S64): half the bytes
+    t32 = K.FkTable(K.FK_KIND_HADRONIC, torch.from_numpy(case2.fk).cuda(), case2.pairs, case2.nfl, K.FK_F32S64, K.FK_STORE_PACK)
+    torch.cuda.empty_cache()
+    ms = _bench_call(lambda: t32.conv(f2, s2), stream)
+    out["cfg2_forward_fp32_storage"] = {"ms": ms, "GBps": fkb / 2 / ms / 1e6, "frac_of_peak": fkb / 2 / ms / 1e6 / peak,
+                                        "predictions_per_s": case2.N / ms * 1e3, "tolerance": 1e-7}
+    ms = _bench_call(lambda: t32.vjp(f2, g2, d2), stream)
+    out["cfg2_vjp_fp32_storage"] = {"ms": ms, "GBps": fkb / 2 / ms / 1e6, "frac_of_peak": fkb / 2 / ms / 1e6 / peak}
+    t32.destroy()
     c0 = synth.config0()
     t0 = K.FkTable(K.FK_KIND_HADRONIC, torch.from_numpy(c0.fk).cuda(), c0.pairs, c0.nfl)
     f0 = torch.from_numpy(c0.f).cuda(); s0 = torch.empty((c0.N, 1), dtype=torch.float64, device="cuda")

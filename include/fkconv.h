@@ -50,7 +50,10 @@ typedef enum fk_status {
 } fk_status;
 
 enum { FK_KIND_DIS = 0, FK_KIND_HADRONIC = 1 };
-enum { FK_F64 = 0, FK_F32 = 1 };
+/* FK_F64: fp64 table, buffers and arithmetic.  FK_F32: table, buffers and arithmetic in fp32 (reading R18; 1e-5).
+ * FK_F32S64: the TABLE is demoted to fp32 with round-to-nearest (half the HBM bytes of the bandwidth-bound path),
+ * f, g, sigma, df and all arithmetic stay fp64 (error <= 2^-24 of sum|terms|: tolerance 1e-7). */
+enum { FK_F64 = 0, FK_F32 = 1, FK_F32S64 = 2 };
 /* table storage: BORROW keeps the caller's logical-layout buffer (no copy; it must outlive the
  * table); PACK copies into the library's device layout: channel-major, x innermost
  * ([N][C][nx*nx rounded up to 4, zero padded] resp. [N][nA][nx]), each datapoint row padded to a
@@ -114,7 +117,7 @@ int fk_table_destroy(fk_table* t);
 /* N, nx, nfl, C, K (= C*nx*nx or nA*nx), row stride in elements, device bytes held by the table. */
 int fk_table_info(const fk_table* t, int* N, int* nx, int* nfl, int* C, int64_t* K,
                   int64_t* row_stride, int64_t* device_bytes);
-/* f, sigma, g, df: dev, in the table's dtype (double for FK_F64, float for FK_F32). */
+/* f, sigma, g, df: dev; float for FK_F32 tables, double for FK_F64 and FK_F32S64. */
 int fk_table_conv(fk_table* t, const void* f, void* sigma, int R, void* stream);
 int fk_table_vjp(fk_table* t, const void* f, const void* g, void* df, int R, void* stream);
 /* Convolution (Eq. (1)) AND its VJP for an upstream gradient g[N][R] that is known

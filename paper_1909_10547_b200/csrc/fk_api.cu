@@ -95,7 +95,8 @@ struct Profiler {
 template <typename T> constexpr int dtype_of();
 template <> constexpr int dtype_of<double>() { return FK_F64; }
 template <> constexpr int dtype_of<float>() { return FK_F32; }
-size_t dtype_size(int dtype) { return dtype == FK_F64 ? 8 : 4; }
+size_t dtype_size(int dtype) { return dtype == FK_F64 ? 8 : 4; }     // storage element of the table
+size_t io_size(int dtype) { return dtype == FK_F32 ? 4 : 8; }        // element of f, sigma, g, df
 
 // ------------------------------------------------------------------------------------------------
 // plans
@@ -192,6 +193,7 @@ fk::TableDesc make_desc(int kind, int layout, const void* fkp, int N, int nx, in
     d.layout = layout;
     const int vecw = dtype == FK_F64 ? 2 : 4;
     d.vec_ok = ((uintptr_t)fkp % 16 == 0) && (d.row_stride % vecw == 0);
+    d.store32 = dtype != FK_F64;
     return d;
 }
 
@@ -201,10 +203,10 @@ fk::TableDesc make_desc(int kind, int layout, const void* fkp, int N, int nx, in
 // picks the replica tile for a pass starting at r0
 inline int pick_rt(int remaining) { return remaining >= 3 ? 4 : remaining; }
 
-template <typename T, bool GROUPED>
+template <typename T, bool GROUPED, typename TS = T>
 cudaError_t fwd_dispatch(bool vec_ok, int rt, const fk::FwdParams& p, int grid, cudaStream_t s) {
-    constexpr int VW = fk::VecWidth<T>::value;
-#define FK_FWD(V, RTv) fk::fk_fwd_column_kernel<T, V, RTv, FWD_U, GROUPED><<<grid, fk::FWD_THREADS, 0, s>>>(p)
+    constexpr int VW = fk::VecWidth<TS>::value;
+#define FK_FWD(V, RTv) fk::fk_fwd_column_kernel<T, V, RTv, FWD_U, GROUPED, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
     if (vec_ok) {
         if (rt == 1) FK_FWD(VW, 1); else if (rt == 2) FK_FWD(VW, 2); else FK_FWD(VW, 4);
     } else {
@@ -214,11 +216,11 @@ cudaError_t fwd_dispatch(bool vec_ok, int rt, const fk::FwdParams& p, int grid, 
     return cudaGetLastError();
 }
 
-template <typename T, bool GROUPED>
+template <typename T, bool GROUPED, typename TS = T>
 cudaError_t colsum_dispatch(bool vec_ok, int rt, const fk::ColsumParams& p, int grid, cudaStream_t s) {
-    constexpr int VW = fk::VecWidth<T>::value;
+    constexpr int VW = fk::VecWidth<TS>::value;
     constexpr int U = 8;
-#define FK_COLSUM(V, RTv) fk::fk_colsum_kernel<T, V, RTv, U, GROUPED><<<grid, fk::COLSUM_THREADS, 0, s>>>(p)
+#define FK_COLSUM(V, RTv) fk::fk_colsum_kernel<T, V, RTv, U, GROUPED, TS><<<grid, fk::COLSUM_THREADS, 0, s>>>(p)
     if (vec_ok) {
         if (rt == 1) FK_COLSUM(VW, 1); else if (rt == 2) FK_COLSUM(VW, 2); else FK_COLSUM(VW, 4);
     } else {
@@ -235,7 +237,7 @@ struct GemmPlan {
 
 template <typename T>
 bool gemm_wanted(const fk::TableDesc& d, int R) {
-    if (dtype_of<T>() != FK_F64) return false;  // the fp32 variant stays on the FFMA column kernel (reading R18)
+    if (dtype_of<T>() != FK_F64 || d.store32) return false;  // the fp32 variants stay on the column kernels (reading R18)
     if ((long long)d.nfl * d.nx >= (long long)fk::KDEC_NONE) return false;
     // packed hadronic tables take the warp-specialised kernel, which beats the <= 4-replica column passes from
     // R = 5 on; the generic cp.async kernel (DIS, logical layout) streams FK at ~2 TB/s and only wins once the
@@ -494,7 +496,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
 }
 
 // One table, any R.  `part` holds >= part_elems_per_replica * R doubles (may be null if nchunks == 1).
-template <typename T>
+template <typename T, typename TS = T>
 int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const uint32_t* kdec,
                     const T* f, T* sigma, int R, double* part, cudaStream_t s, int* launches) {
     int nl = 0;
@@ -515,7 +517,7 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
         p.r0 = r0;
         size_t slot = 0;
         const bool timed = r0 == 0 && g_prof.begin(s, slot);
-        cudaError_t e = fwd_dispatch<T, false>(d.vec_ok, rt, p, fgrid, s);
+        cudaError_t e = fwd_dispatch<T, false, TS>(d.vec_ok, rt, p, fgrid, s);
         if (timed) g_prof.end(s, slot);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "forward kernel launch failed: %s", cudaGetErrorString(e));
         ++nl;
@@ -541,7 +543,7 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
 }
 
 // `G` holds >= G_elems_per_replica * R doubles.
-template <typename T>
+template <typename T, typename TS = T>
 int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const T* f, const T* g, T* df,
                    int R, double* G, cudaStream_t s, int* launches) {
     int nl = 0;
@@ -559,7 +561,7 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
         for (int r0 = 0; r0 < R;) {
             const int rt = pick_rt(R - r0);
             p.r0 = r0;
-            cudaError_t e = colsum_dispatch<T, false>(d.vec_ok, rt, p, pl.nkb * pl.nsplit, s);
+            cudaError_t e = colsum_dispatch<T, false, TS>(d.vec_ok, rt, p, pl.nkb * pl.nsplit, s);
             if (e != cudaSuccess) return fail(FK_ERR_CUDA, "colsum kernel launch failed: %s", cudaGetErrorString(e));
             ++nl;
             r0 += rt;
@@ -614,10 +616,10 @@ size_t fused_scratch_elems(const fk::TableDesc& d, int R) {
     return (part_elems_per_replica(d) + (size_t)d.fsplit * d.K + (1 + FOLDK_MAX_CHUNKS) * (size_t)d.C * d.nx) * R;
 }
 
-template <typename T>
+template <typename T, typename TS = T>
 int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const Plan& pl, const T* f, const T* g,
                        T* sigma, T* df, int R, double* scratch, cudaStream_t s, int* launches) {
-    constexpr int VW = fk::VecWidth<T>::value;
+    constexpr int VW = fk::VecWidth<TS>::value;
     fk::TableDesc d = d0;
     d.nsplit = d.fsplit;  // the column sums are cut into the forward's datapoint ranges
     double* part = scratch;
@@ -637,7 +639,7 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.fwd.r0 = r0;
-#define FK_FUSED(V, RTv) fk::fk_fused_column_kernel<T, V, RTv, FWD_U><<<grid, fk::FWD_THREADS, 0, s>>>(p)
+#define FK_FUSED(V, RTv) fk::fk_fused_column_kernel<T, V, RTv, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
         if (d.vec_ok) {
             if (rt == 1) FK_FUSED(VW, 1); else if (rt == 2) FK_FUSED(VW, 2); else FK_FUSED(VW, 4);
         } else {
@@ -778,35 +780,35 @@ size_t table_scratch_need(const fk_table* t, int R) {
     return std::max(conv, vjp);
 }
 
-template <typename T>
+template <typename T, typename TS = T>
 int table_conv_t(fk_table* t, const void* f, void* sigma, int R, cudaStream_t s) {
     int rc = ensure_scratch(t, table_scratch_need(t, R));
     if (rc) return rc;
-    return run_conv_single<T>(t->desc, t->chan, t->plan, t->kdec, (const T*)f, (T*)sigma, R, t->scratch, s,
+    return run_conv_single<T, TS>(t->desc, t->chan, t->plan, t->kdec, (const T*)f, (T*)sigma, R, t->scratch, s,
                               &t->last_launches);
 }
 
-template <typename T>
+template <typename T, typename TS = T>
 int table_vjp_t(fk_table* t, const void* f, const void* g, void* df, int R, cudaStream_t s) {
     int rc = ensure_scratch(t, table_scratch_need(t, R));
     if (rc) return rc;
-    return run_vjp_single<T>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)df, R, t->scratch, s,
+    return run_vjp_single<T, TS>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)df, R, t->scratch, s,
                              &t->last_launches);
 }
 
-template <typename T>
+template <typename T, typename TS = T>
 int table_conv_vjp_t(fk_table* t, const void* f, const void* g, void* sigma, void* df, int R, cudaStream_t s) {
     if (!fused_ok<T>(t->desc, R)) {
-        int rc = table_conv_t<T>(t, f, sigma, R, s);
+        int rc = table_conv_t<T, TS>(t, f, sigma, R, s);
         if (rc) return rc;
         const int nl = t->last_launches;
-        rc = table_vjp_t<T>(t, f, g, df, R, s);
+        rc = table_vjp_t<T, TS>(t, f, g, df, R, s);
         t->last_launches += nl;
         return rc;
     }
     int rc = ensure_scratch(t, std::max(table_scratch_need(t, R), fused_scratch_elems(t->desc, R)));
     if (rc) return rc;
-    return run_conv_vjp_fused<T>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)sigma, (T*)df, R, t->scratch, s,
+    return run_conv_vjp_fused<T, TS>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)sigma, (T*)df, R, t->scratch, s,
                                  &t->last_launches);
 }
 
@@ -882,9 +884,9 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
     *out = nullptr;
     if (!fk_logical || !index_list) return fail(FK_ERR_INVALID_ARG, "fk_table_create: null pointer");
     if (kind != FK_KIND_DIS && kind != FK_KIND_HADRONIC) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad kind %d", kind);
-    if (dtype != FK_F64 && dtype != FK_F32) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad dtype %d", dtype);
+    if (dtype != FK_F64 && dtype != FK_F32 && dtype != FK_F32S64) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad dtype %d", dtype);
     if (store != FK_STORE_BORROW && store != FK_STORE_PACK) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad store %d", store);
-    if (dtype == FK_F32 && store == FK_STORE_BORROW)
+    if (dtype != FK_F64 && store == FK_STORE_BORROW)
         return fail(FK_ERR_INVALID_ARG, "fk_table_create: an fp32 table must be packed (the logical input is fp64)");
     int rc = check_dims("fk_table_create", kind, N, nx, nfl, C, std::max(1, R_hint));
     if (rc) return rc;
@@ -976,6 +978,7 @@ int fk_table_conv(fk_table* t, const void* f, void* sigma, int R, void* stream) 
     g_err.clear();
     if (!t || !f || !sigma) return fail(FK_ERR_INVALID_ARG, "fk_table_conv: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv: R=%d", R);
+    if (t->dtype == FK_F32S64) return table_conv_t<double, float>(t, f, sigma, R, (cudaStream_t)stream);
     return t->dtype == FK_F64 ? table_conv_t<double>(t, f, sigma, R, (cudaStream_t)stream)
                               : table_conv_t<float>(t, f, sigma, R, (cudaStream_t)stream);
 }
@@ -984,6 +987,7 @@ int fk_table_vjp(fk_table* t, const void* f, const void* g, void* df, int R, voi
     g_err.clear();
     if (!t || !f || !g || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp: R=%d", R);
+    if (t->dtype == FK_F32S64) return table_vjp_t<double, float>(t, f, g, df, R, (cudaStream_t)stream);
     return t->dtype == FK_F64 ? table_vjp_t<double>(t, f, g, df, R, (cudaStream_t)stream)
                               : table_vjp_t<float>(t, f, g, df, R, (cudaStream_t)stream);
 }
@@ -992,6 +996,7 @@ int fk_table_conv_vjp(fk_table* t, const void* f, const void* g, void* sigma, vo
     g_err.clear();
     if (!t || !f || !g || !sigma || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp: R=%d", R);
+    if (t->dtype == FK_F32S64) return table_conv_vjp_t<double, float>(t, f, g, sigma, df, R, (cudaStream_t)stream);
     return t->dtype == FK_F64 ? table_conv_vjp_t<double>(t, f, g, sigma, df, R, (cudaStream_t)stream)
                               : table_conv_vjp_t<float>(t, f, g, sigma, df, R, (cudaStream_t)stream);
 }
@@ -1012,7 +1017,7 @@ int fk_table_fit_step(fk_table* t, const double* f, const double* data, const do
                       double* chi2, double* df, int R, void* stream) {
     g_err.clear();
     if (!t || !f || !data || !cinv || !sigma || !g || !chi2 || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_fit_step: null pointer");
-    if (t->dtype != FK_F64) return fail(FK_ERR_UNSUPPORTED, "fk_table_fit_step: fp64 tables only");
+    if (t->dtype == FK_F32) return fail(FK_ERR_UNSUPPORTED, "fk_table_fit_step: tables with fp64 buffers only (FK_F64, FK_F32S64)");
     int rc = fk_table_conv(t, f, sigma, R, stream);
     if (rc) return rc;
     const int nl = t->last_launches;
@@ -1027,7 +1032,7 @@ int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R,
     g_err.clear();
     if (!t || !f_host || !sigma_host) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_host: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_host: R=%d", R);
-    const size_t es = dtype_size(t->dtype);
+    const size_t es = io_size(t->dtype);
     const size_t fb = (size_t)R * t->desc.nfl * t->desc.nx * es, sb = (size_t)t->desc.N * R * es;
     const size_t fb_al = (fb + 255) / 256 * 256;
     int rc = ensure_stage(t, 2 * fb_al + 2 * ((sb + 255) / 256 * 256));
@@ -1048,7 +1053,7 @@ int fk_table_vjp_host(fk_table* t, const void* f_host, const void* g_host, void*
     g_err.clear();
     if (!t || !f_host || !g_host || !df_host) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp_host: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp_host: R=%d", R);
-    const size_t es = dtype_size(t->dtype);
+    const size_t es = io_size(t->dtype);
     const size_t fb = (size_t)R * t->desc.nfl * t->desc.nx * es, gb = (size_t)t->desc.N * R * es;
     const size_t fb_al = (fb + 255) / 256 * 256, gb_al = (gb + 255) / 256 * 256;
     int rc = ensure_stage(t, 2 * fb_al + 2 * gb_al);

@@ -31,6 +31,7 @@ struct TableDesc {
     int cstride;          // PACKED hadronic: elements per channel block (nx*nx rounded up to a multiple of 4)
     int kind, layout;
     int vec_ok;           // rows are 16-byte aligned -> 128-bit loads
+    int store32;          // the table is stored in fp32 (FK_F32, FK_F32S64)
     // grouped launches only
     const uint8_t* chan_a;   // device copies of the channel list (a_c / b_c)
     const uint8_t* chan_b;

@@ -56,10 +56,11 @@ __device__ __forceinline__ double fold_rows(double (&p)[U], int lane) {
     return s;
 }
 
-template <typename T, int VEC, int RT, int U, bool GROUPED>
+// TS = storage type of the table (float for the fp32-storage variants), T = type of f, sigma and of the arithmetic
+template <typename T, int VEC, int RT, int U, bool GROUPED, typename TS = T>
 __global__ void __launch_bounds__(FWD_THREADS)
 fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
-    using V = Vec<T, VEC>;
+    using V = Vec<TS, VEC>;
     constexpr int LPR = 32 / U;  // lanes that end up holding the same row
     __shared__ double red[2][FWD_WARPS][U][RT];
 
@@ -109,7 +110,7 @@ fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
             }
         }
     }
-    const T* __restrict__ col = reinterpret_cast<const T*>(d.fk) + (kin ? k : 0);
+    const TS* __restrict__ col = reinterpret_cast<const TS*>(d.fk) + (kin ? k : 0);
 
     int buf = 0;
     for (int m = rb; m < re; m += U, buf ^= 1) {
@@ -123,9 +124,9 @@ fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
             const bool live = kin && (m + u < re);
 #pragma unroll
             for (int r = 0; r < RT; ++r) {
-                T s = x[u].v[0] * L[r][0];
+                T s = (T)x[u].v[0] * L[r][0];
 #pragma unroll
-                for (int e = 1; e < VEC; ++e) s = fma(x[u].v[e], L[r][e], s);
+                for (int e = 1; e < VEC; ++e) s = fma((T)x[u].v[e], L[r][e], s);
                 pr[r][u] = live ? (double)s : 0.0;
             }
         }
@@ -163,10 +164,10 @@ struct FusedParams {
     double* G;       // [fsplit][R][K] column sums, one slice per datapoint range
 };
 
-template <typename T, int VEC, int RT, int U>
+template <typename T, int VEC, int RT, int U, typename TS = T>
 __global__ void __launch_bounds__(FWD_THREADS)
 fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
-    using V = Vec<T, VEC>;
+    using V = Vec<TS, VEC>;
     constexpr int LPR = 32 / U;
     constexpr int MAX_ROWS = 64;  // datapoints per range (the plan uses <= 32)
     __shared__ double red[2][FWD_WARPS][U][RT];
@@ -220,7 +221,7 @@ fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
         for (int r = 0; r < RT; ++r)
 #pragma unroll
             for (int e = 0; e < VEC; ++e) cs[a][r][e] = T(0);
-    const T* __restrict__ col = reinterpret_cast<const T*>(d.fk) + (kin ? k : 0);
+    const TS* __restrict__ col = reinterpret_cast<const TS*>(d.fk) + (kin ? k : 0);
     __syncthreads();
 
     int buf = 0;
@@ -234,13 +235,13 @@ fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
             const bool live = kin && (m + u < re);
 #pragma unroll
             for (int r = 0; r < RT; ++r) {
-                T s = x[u].v[0] * L[r][0];
+                T s = (T)x[u].v[0] * L[r][0];
 #pragma unroll
-                for (int e = 1; e < VEC; ++e) s = fma(x[u].v[e], L[r][e], s);
+                for (int e = 1; e < VEC; ++e) s = fma((T)x[u].v[e], L[r][e], s);
                 pr[r][u] = live ? (double)s : 0.0;
                 const T gv = gs[(m - rb + u) * RT + r];  // 0 on the padded rows
 #pragma unroll
-                for (int e = 0; e < VEC; ++e) cs[u & 1][r][e] = fma(gv, x[u].v[e], cs[u & 1][r][e]);
+                for (int e = 0; e < VEC; ++e) cs[u & 1][r][e] = fma(gv, (T)x[u].v[e], cs[u & 1][r][e]);
             }
         }
 #pragma unroll

@@ -203,7 +203,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
     return FK_OK;
 }
 
-template <typename T>
+template <typename T, typename TS = T>
 int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStream_t s) {
     int rc = group_scratch(g, group_scratch_need(g, R));
     if (rc) return rc;
@@ -222,7 +222,7 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
-        cudaError_t e = fwd_dispatch<T, true>(g->all_vec, rt, p, g->nfsegs, s);
+        cudaError_t e = fwd_dispatch<T, true, TS>(g->all_vec, rt, p, g->nfsegs, s);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped forward launch failed: %s", cudaGetErrorString(e));
         ++nl;
         r0 += rt;
@@ -248,7 +248,7 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
     return FK_OK;
 }
 
-template <typename T>
+template <typename T, typename TS = T>
 int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat, int R, cudaStream_t s) {
     int rc = group_scratch(g, group_scratch_need(g, R));
     if (rc) return rc;
@@ -267,7 +267,7 @@ int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat,
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
-        cudaError_t e = colsum_dispatch<T, true>(g->all_vec, rt, p, g->ncsegs, s);
+        cudaError_t e = colsum_dispatch<T, true, TS>(g->all_vec, rt, p, g->ncsegs, s);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped colsum launch failed: %s", cudaGetErrorString(e));
         ++nl;
         r0 += rt;
@@ -489,6 +489,7 @@ int fk_conv_grouped(fk_group* g, const void* f_cat, void* sigma_cat, int R, void
     g_err.clear();
     if (!g || !f_cat || !sigma_cat) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped: R=%d", R);
+    if (g->dtype == FK_F32S64) return group_conv_t<double, float>(g, f_cat, sigma_cat, R, (cudaStream_t)stream);
     return g->dtype == FK_F64 ? group_conv_t<double>(g, f_cat, sigma_cat, R, (cudaStream_t)stream)
                               : group_conv_t<float>(g, f_cat, sigma_cat, R, (cudaStream_t)stream);
 }
@@ -497,6 +498,7 @@ int fk_conv_grouped_vjp(fk_group* g, const void* f_cat, const void* g_cat, void*
     g_err.clear();
     if (!g || !f_cat || !g_cat || !df_cat) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped_vjp: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped_vjp: R=%d", R);
+    if (g->dtype == FK_F32S64) return group_vjp_t<double, float>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream);
     return g->dtype == FK_F64 ? group_vjp_t<double>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream)
                               : group_vjp_t<float>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream);
 }

@@ -29,10 +29,10 @@ struct ColsumParams {
 constexpr int COLSUM_THREADS = 256;
 constexpr int COLSUM_MAX_ROWS = 512;  // datapoints per split (bounds the g tile in shared memory)
 
-template <typename T, int VEC, int RT, int UNROLL, bool GROUPED>
+template <typename T, int VEC, int RT, int UNROLL, bool GROUPED, typename TS = T>
 __global__ void __launch_bounds__(COLSUM_THREADS)
 fk_colsum_kernel(const __grid_constant__ ColsumParams p) {
-    using V = Vec<T, VEC>;
+    using V = Vec<TS, VEC>;
     constexpr int NACC = (RT == 1) ? 4 : 2;
     __shared__ T gs[(COLSUM_MAX_ROWS + UNROLL) * RT];
 
@@ -65,7 +65,7 @@ fk_colsum_kernel(const __grid_constant__ ColsumParams p) {
 
     const int k = (kblock * COLSUM_THREADS + threadIdx.x) * VEC;
     if (k >= d.K) return;
-    const T* __restrict__ col = reinterpret_cast<const T*>(d.fk) + k;
+    const TS* __restrict__ col = reinterpret_cast<const TS*>(d.fk) + k;
 
     T acc[NACC][RT][VEC];
 #pragma unroll
@@ -87,7 +87,7 @@ fk_colsum_kernel(const __grid_constant__ ColsumParams p) {
                 const T gv = gs[(m + u) * RT + r];  // broadcast; 0 on the padded rows
 #pragma unroll
                 for (int e = 0; e < VEC; ++e)
-                    acc[u % NACC][r][e] = fma(gv, x[u].v[e], acc[u % NACC][r][e]);
+                    acc[u % NACC][r][e] = fma(gv, (T)x[u].v[e], acc[u % NACC][r][e]);
             }
     }
 

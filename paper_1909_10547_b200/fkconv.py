@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libfkconv.so")
 
 FK_OK, FK_ERR_INVALID_ARG, FK_ERR_ALLOC, FK_ERR_CUDA, FK_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 FK_KIND_DIS, FK_KIND_HADRONIC = 0, 1
-FK_F64, FK_F32 = 0, 1
+FK_F64, FK_F32, FK_F32S64 = 0, 1, 2
 FK_STORE_BORROW, FK_STORE_PACK = 0, 1
 
 # every symbol include/fkconv.h declares
@@ -190,7 +190,7 @@ class FkTable:
             N, nx, C = fk_logical.shape
         self.N, self.nx, self.nfl, self.C = N, nx, nfl, C
         self.dtype = dtype
-        self.tdtype = torch.float64 if dtype == FK_F64 else torch.float32
+        self.tdtype = torch.float32 if dtype == FK_F32 else torch.float64  # FK_F32S64: fp32 table, fp64 buffers
         self.device = fk_logical.device
         self._keep = fk_logical if store == FK_STORE_BORROW else None
         h = _vp()

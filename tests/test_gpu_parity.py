@@ -405,3 +405,55 @@ def test_sharded_table_single_rank(K):
     assert (t.n0, t.n1) == (0, case.N)
     assert rel_err(t.conv_all(to_dev(case.f)).cpu().numpy(), ref, scale) <= TOL64
     assert rel_err(t.vjp(to_dev(case.f), to_dev(case.g)).cpu().numpy(), dref, D) <= TOL64
+
+
+# ------------------------------------------------------------------ fp32-stored table, fp64 everything else
+TOL32S = 1e-7  # each FK value carries one fp32 rounding (2^-24 = 6e-8 of its term); f, g and all sums are fp64
+
+
+@pytest.mark.parametrize("shape", [(37, 23, 14, 29), (130, 9, 5, 13), (3, 50, 14, 2), (512, 20, 14, 60)])
+@pytest.mark.parametrize("R", [1, 3, 6, 20])
+def test_fp32_storage_fp64_arithmetic(K, shape, R):
+    N, nx, nfl, C = shape
+    case = synth.hadronic_case(13, N, nx, C, R, nfl=nfl, sub=N + nx)
+    g = synth.rng_for(13, synth.T_G, R).standard_normal(size=(N, R))
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, g)
+    t = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl, K.FK_F32S64)
+    assert t.info()["device_bytes"] < 0.6 * case.fk.nbytes + (1 << 20)
+    f_d, g_d = to_dev(case.f), to_dev(g)
+    sig, df = t.conv(f_d), t.vjp(f_d, g_d)
+    assert sig.dtype == df.dtype and str(sig.dtype) == "torch.float64"
+    e1, e2 = rel_err(sig.cpu().numpy(), ref, scale), rel_err(df.cpu().numpy(), dref, D)
+    assert e1 <= TOL32S and e2 <= TOL32S, (e1, e2)
+    s2, d2 = t.conv_vjp(f_d, g_d)
+    assert rel_err(s2.cpu().numpy(), ref, scale) <= TOL32S and rel_err(d2.cpu().numpy(), dref, D) <= TOL32S
+    # against the oracle of the DEMOTED table the fp64 bar holds: the only difference is the storage rounding
+    fk32 = case.fk.astype(np.float32).astype(np.float64)
+    ref32, scale32 = O.hadronic(fk32, case.pairs, case.f)
+    dref32, D32 = O.hadronic_vjp(fk32, case.pairs, case.f, g)
+    assert rel_err(sig.cpu().numpy(), ref32, scale32) <= TOL64 and rel_err(df.cpu().numpy(), dref32, D32) <= TOL64
+
+
+def test_fp32_storage_grouped_and_dis(K):
+    import torch
+    shapes = synth.small_ragged_shapes(T=5)
+    R = 2
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    cases = [synth.config4_table(t, shapes, R, params) for t in range(shapes.T)]
+    tabs = [K.FkTable(K.FK_KIND_HADRONIC, to_dev(c.fk), c.pairs, c.nfl, K.FK_F32S64) for c in cases]
+    grp = K.FkGroup(tabs, R_hint=R)
+    fo, so = grp.offsets(R)
+    f_cat = torch.cat([to_dev(c.f).reshape(-1) for c in cases]); g_cat = torch.cat([to_dev(c.g).reshape(-1) for c in cases])
+    sig, df = grp.conv(f_cat, R).cpu().numpy(), grp.vjp(f_cat, g_cat, R).cpu().numpy()
+    for t, c in enumerate(cases):
+        ref, scale = O.hadronic(c.fk, c.pairs, c.f)
+        dref, D = O.hadronic_vjp(c.fk, c.pairs, c.f, c.g)
+        assert rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale) <= TOL32S
+        assert rel_err(df[fo[t]:fo[t + 1]].reshape(R, c.nfl, c.nx), dref, D) <= TOL32S
+    dis = synth.config1(R=3, N=200)
+    rd, sd = O.dis(dis.fk, dis.flav, dis.f)
+    dd, DD = O.dis_vjp(dis.fk, dis.flav, dis.f, dis.g)
+    td = K.FkTable(K.FK_KIND_DIS, to_dev(dis.fk), dis.flav, dis.nfl, K.FK_F32S64)
+    assert rel_err(td.conv(to_dev(dis.f)).cpu().numpy(), rd, sd) <= TOL32S
+    assert rel_err(td.vjp(to_dev(dis.f), to_dev(dis.g)).cpu().numpy(), dd, DD) <= TOL32S
