@@ -371,3 +371,18 @@ def test_chi2_gradient_is_the_central_difference():
         e = np.zeros((N, 1)); e[n] = h
         cp = O.chi2(sigma + e, data, cinv)[0][0]; cm = O.chi2(sigma - e, data, cinv)[0][0]
         assert abs((cp - cm) / (2 * h) - g[n, 0]) <= 1e-15 * cs[0] / h + 1e-12 * abs(g[n, 0])  # rounding of chi2 / h
+
+
+def test_oracle_matches_its_committed_golden_file():
+    """tests/golden/oracle_tiny.json is written by tests/golden/make_golden.py (oracle only): guards against silent
+    drift of the oracle or of the seeded generators."""
+    import importlib.util
+    import json
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    with open(os.path.join(here, "oracle_tiny.json")) as fh:
+        stored = json.load(fh)
+    assert mod.build() == stored
