@@ -359,13 +359,19 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             d.gkper = ((d.K + ksplit0 - 1) / ksplit0 + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT;
             d.gksplit = (d.K + d.gkper - 1) / d.gkper;
             // a partial last datapoint tile is cut into k sub-splits that take whole groups of K ranges
+            // (65..96 remaining datapoints take a 64-row and a 32-row tile instead of a 128-row one)
             const int nfull = d.N / fk::GEMM_BM, rem = d.N % fk::GEMM_BM;
-            const int ksub_rem = rem ? fk::ws_ksub_for_rows(rem) : 1;
+            const bool two = rem > 64 && rem <= 96;
+            const int ksub_rem = rem ? (two ? 4 : fk::ws_ksub_for_rows(rem)) : 1;
             d.gksplit = (d.gksplit + ksub_rem - 1) / ksub_rem * ksub_rem;
             for (int ks = 0; ks < d.gksplit; ++ks)
                 for (int mt = 0; mt < nfull; ++mt) witems.push_back(fk::ColSeg{t, mt * fk::GEMM_BM, ks, 1});
-            if (rem)
+            if (two) {
+                for (int ks = 0; ks < d.gksplit / 2; ++ks) witems.push_back(fk::ColSeg{t, nfull * fk::GEMM_BM, ks, 2});
+                for (int ks = 0; ks < d.gksplit / 4; ++ks) witems.push_back(fk::ColSeg{t, nfull * fk::GEMM_BM + 64, ks, 4});
+            } else if (rem) {
                 for (int ks = 0; ks < d.gksplit / ksub_rem; ++ks) witems.push_back(fk::ColSeg{t, nfull * fk::GEMM_BM, ks, ksub_rem});
+            }
             g->ws_all = g->ws_all && d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok;
             g->nx_max = std::max(g->nx_max, d.nx);
             d.gp_off = g->gp_rows;

@@ -457,3 +457,26 @@ def test_fp32_storage_grouped_and_dis(K):
     td = K.FkTable(K.FK_KIND_DIS, to_dev(dis.fk), dis.flav, dis.nfl, K.FK_F32S64)
     assert rel_err(td.conv(to_dev(dis.f)).cpu().numpy(), rd, sd) <= TOL32S
     assert rel_err(td.vjp(to_dev(dis.f), to_dev(dis.g)).cpu().numpy(), dd, DD) <= TOL32S
+
+
+@pytest.mark.parametrize("R", [20, 100])
+def test_grouped_dense_tile_heights(K, R):
+    """Grouped R >> 1 launch over tables whose last datapoint tile takes every height: 128 (97..128 rows left),
+    64 + 32 (65..96), 64 (33..64), 32 (<= 32), and none (N a multiple of 128)."""
+    import torch
+    shapes = synth.RaggedShapes(np.array([70, 96, 200, 129, 64, 97, 128, 257]), np.array([6, 9, 7, 5, 11, 8, 6, 5]),
+                                np.array([5, 3, 7, 9, 4, 6, 8, 10]))
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    cases = [synth.config4_table(t, shapes, R, params) for t in range(shapes.T)]
+    gs = [synth.rng_for(4, synth.T_G, 100 + t).standard_normal(size=(c.N, R)) for t, c in enumerate(cases)]
+    tabs = [K.FkTable(K.FK_KIND_HADRONIC, to_dev(c.fk), c.pairs, c.nfl) for c in cases]
+    grp = K.FkGroup(tabs, R_hint=R)
+    fo, so = grp.offsets(R)
+    f_cat = torch.cat([to_dev(c.f).reshape(-1) for c in cases]); g_cat = torch.cat([to_dev(g).reshape(-1) for g in gs])
+    sig, df = grp.conv(f_cat, R).cpu().numpy(), grp.vjp(f_cat, g_cat, R).cpu().numpy()
+    for t, c in enumerate(cases):
+        ref, scale = O.hadronic(c.fk, c.pairs, c.f)
+        dref, D = O.hadronic_vjp(c.fk, c.pairs, c.f, gs[t])
+        assert rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale) <= TOL64, t
+        assert rel_err(df[fo[t]:fo[t + 1]].reshape(R, c.nfl, c.nx), dref, D) <= TOL64, t
+    assert np.array_equal(grp.conv(f_cat, R).cpu().numpy(), sig)
