@@ -398,7 +398,7 @@ int fold_chunks(long long channels) {
     double best_eff = 0.0;
     for (int n = 1; n <= 8; ++n) {
         const long long ctas = channels * n, waves = (ctas + slots - 1) / slots;
-        const double eff = (double)ctas / (double)(waves * slots) - 0.01 * n;
+        const double eff = (double)ctas / (double)(waves * slots) - 0.03 * n;  // every CTA pays its own ring fill
         if (eff > best_eff) { best_eff = eff; best = n; }
     }
     return best;

@@ -123,14 +123,17 @@ fk_vjp_fold_kernel(const __grid_constant__ FoldParams p) {
     const long long cx = d.cx_off + (long long)c * nx;
     double* __restrict__ PA = p.PA + (cx * FOLD_JQ + jq) * RP + col;
 
+    // f[a_c][i] of the next row is fetched one row ahead: the L2 round trip is off the per-row critical path
+    double2 fa_next = active ? *reinterpret_cast<const double2*>(fa_col + (long long)i0 * RP) : make_double2(0.0, 0.0);
     for (int i = i0; i < i1; ++i) {
         const int q = i - i0, s = q % S;
         if (threadIdx.x == 0 && i + S - 1 < i1) issue(i + S - 1);  // its slot was left by every warp after row i - 1
         __syncwarp();
+        const double2 fa = fa_next;
+        if (active && i + 1 < i1) fa_next = *reinterpret_cast<const double2*>(fa_col + (long long)(i + 1) * RP);
         mbar_wait(bar_full(s), (q / S) & 1);
         if (active) {
             const double* row = ring + (size_t)s * nx * RP + jq * RP + col;
-            const double2 fa = *reinterpret_cast<const double2*>(fa_col + (long long)i * RP);
             double2 a = make_double2(0.0, 0.0);
 #pragma unroll
             for (int m = 0; m < FOLD_NXQ; ++m) {
