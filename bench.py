@@ -35,7 +35,7 @@ from paper_1909_10547_b200 import synth  # noqa: E402  (seeded inputs only; no m
 FP64_PEAK_TFLOPS = 37.2  # 148 SM x 64 FMA/clk x 2 x 1.965 GHz (probe: profiles/r01_fp64_peak.md)
 METRIC = "fk_convolution_achieved_hbm_bandwidth"
 UNIT = "GB/s"
-DOMINANT_KERNEL = "fk_fwd_column_kernel<double,2,1,8,0>"
+DOMINANT_KERNEL = "fk_fwd_column_kernel<double,2,1,8,0,double>"
 WORKLOAD = "config2: hadronic FK N=512 nx=50 nfl=14 C=100 R=1 fp64 (1.024 GB), forward + VJP per step"
 
 

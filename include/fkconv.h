@@ -29,7 +29,8 @@
  *  - logical layouts (BASELINE.json): hadronic FK[N][nx][nx][C] (i, j, channel; channel innermost),
  *    DIS FK[N][nx][nA], pairs[C][2] = (a_c, b_c) with i <-> a_c and j <-> b_c, flav[nA],
  *    f[R][nfl][nx], sigma[N][R], g[N][R], df[R][nfl][nx].
- *  - limits: 1 <= nfl <= 256, 1 <= C (or nA) <= 1024, N*K < 2^62, R >= 1.  Outside: FK_ERR_UNSUPPORTED.
+ *  - limits: 1 <= nfl <= 256, 1 <= C (or nA) <= 1024, K = C*nx*nx (DIS: nA*nx) < 2^31, nfl*nx < 2^31,
+ *    N*K < 2^62, R >= 1.  Outside: FK_ERR_UNSUPPORTED.
  *  - there is no CPU fallback: without a CUDA device every compute call returns FK_ERR_CUDA.
  */
 #ifndef FKCONV_H
