@@ -278,18 +278,18 @@ template <bool GROUPED>
 bool ws_set_attr() {
     bool ok = true;
 #define FK_WS_ATTR(NFW) ok = ok && cudaFuncSetAttribute(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MAX_DYN_SMEM) == cudaSuccess
-    FK_WS_ATTR(1); FK_WS_ATTR(2); FK_WS_ATTR(3); FK_WS_ATTR(4); FK_WS_ATTR(5); FK_WS_ATTR(6); FK_WS_ATTR(7); FK_WS_ATTR(8);
+    FK_WS_ATTR(2); FK_WS_ATTR(4); FK_WS_ATTR(6); FK_WS_ATTR(8); FK_WS_ATTR(10); FK_WS_ATTR(12); FK_WS_ATTR(14); FK_WS_ATTR(16);
 #undef FK_WS_ATTR
     return ok;
 }
 
-// RP = 16 * NFW (fk::gemm_rp): one instantiation per fragment count of a warp column
+// RP = 8 * NFRAG (fk::gemm_rp: a multiple of 16), NFRAG = 2, 4, ..., 16: one instantiation per fragment count
 template <bool GROUPED>
 void ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) {
-    switch (w.RP / 16) {
+    switch (w.RP / 8) {
 #define FK_WS_CASE(NFW) case NFW: fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, smem, s>>>(w); break
-        FK_WS_CASE(1); FK_WS_CASE(2); FK_WS_CASE(3); FK_WS_CASE(4); FK_WS_CASE(5); FK_WS_CASE(6); FK_WS_CASE(7);
-        default: FK_WS_CASE(8);
+        FK_WS_CASE(2); FK_WS_CASE(4); FK_WS_CASE(6); FK_WS_CASE(8); FK_WS_CASE(10); FK_WS_CASE(12); FK_WS_CASE(14);
+        default: FK_WS_CASE(16);
 #undef FK_WS_CASE
     }
 }
@@ -301,7 +301,8 @@ template <bool GROUPED>
 bool wsv_set_attr() {
     bool ok = true;
 #define FK_WSV_ATTR(NFW) ok = ok && cudaFuncSetAttribute(fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fk::WSV_SMEM_BYTES) == cudaSuccess
-    FK_WSV_ATTR(1); FK_WSV_ATTR(2); FK_WSV_ATTR(3); FK_WSV_ATTR(4); FK_WSV_ATTR(5); FK_WSV_ATTR(6); FK_WSV_ATTR(7); FK_WSV_ATTR(8);
+    FK_WSV_ATTR(2); FK_WSV_ATTR(3); FK_WSV_ATTR(4); FK_WSV_ATTR(5); FK_WSV_ATTR(6); FK_WSV_ATTR(7); FK_WSV_ATTR(8); FK_WSV_ATTR(9);
+    FK_WSV_ATTR(10); FK_WSV_ATTR(11); FK_WSV_ATTR(12); FK_WSV_ATTR(13); FK_WSV_ATTR(14); FK_WSV_ATTR(15); FK_WSV_ATTR(16);
 #undef FK_WSV_ATTR
     return ok;
 }
@@ -309,10 +310,11 @@ bool wsv_set_attr() {
 template <bool GROUPED>
 void wsv_launch(const fk::WsVjpParams& w, cudaStream_t s) {
     const int grid = std::max(1, std::min(w.ntiles, sm_count() * std::max(1, env_int("FKCONV_WSV_CTAS_PER_SM", 1))));
-    switch (w.RP / 16) {
+    switch (w.RP / 8) {
 #define FK_WSV_CASE(NFW) case NFW: fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break
-        FK_WSV_CASE(1); FK_WSV_CASE(2); FK_WSV_CASE(3); FK_WSV_CASE(4); FK_WSV_CASE(5); FK_WSV_CASE(6); FK_WSV_CASE(7);
-        default: FK_WSV_CASE(8);
+        FK_WSV_CASE(2); FK_WSV_CASE(3); FK_WSV_CASE(4); FK_WSV_CASE(5); FK_WSV_CASE(6); FK_WSV_CASE(7); FK_WSV_CASE(8); FK_WSV_CASE(9);
+        FK_WSV_CASE(10); FK_WSV_CASE(11); FK_WSV_CASE(12); FK_WSV_CASE(13); FK_WSV_CASE(14); FK_WSV_CASE(15);
+        default: FK_WSV_CASE(16);
 #undef FK_WSV_CASE
     }
 }
@@ -413,7 +415,7 @@ size_t gemm_vjp_scratch_elems(const fk::TableDesc& d, int R) {
 
 int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double* f, const double* g, double* df,
                  int R, double* scratch, cudaStream_t s, int* launches) {
-    const int RPmax = fk::gemm_rp(R);
+    const int RPmax = fk::gemm_rp8(R);
     const int slots = d.nfl * d.nx;
     double* fT = scratch;
     double* gP = fT + (size_t)slots * RPmax;
@@ -425,7 +427,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
     if (!attr_ok) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
     int nl = 0;
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
-        const int RP = fk::gemm_rp(R - r0);
+        const int RP = fk::gemm_rp8(R - r0);
         const long long tf = (long long)slots * RP, tg = (long long)d.N * RP;
         fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tf + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, RP);
         fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(2048, (tg + 255) / 256), 256, 0, s>>>(g + d.out_off * R, gP, d.N, R, r0, RP);

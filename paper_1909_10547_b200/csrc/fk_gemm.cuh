@@ -33,12 +33,20 @@ constexpr int GEMM_FLUSH = 16;             // K-tiles between flushes of the reg
 constexpr int GEMM_SMEM_BYTES = (GEMM_STAGES * GEMM_BM * GEMM_SA + 2 * GEMM_KT * GEMM_SB) * 8;
 constexpr uint32_t KDEC_NONE = 0xffffu;    // DIS: no second factor
 
-// padded replica count of a pass over `r` replicas: a multiple of 16 (two warp columns of whole 8-replica
-// MMA fragments each, so that the fragment count per warp is a compile-time constant), at most GEMM_BN
+// padded replica count of a pass over `r` replicas, at most GEMM_BN.  Forward kernels: a multiple of 16 (two warp
+// columns of the same whole number of 8-replica MMA fragments: one instruction stream for all consumer warps).
 __host__ __device__ inline int gemm_rp(int r) {
     const int rp = (r + 15) / 16 * 16;
     return rp < GEMM_BN ? rp : GEMM_BN;
 }
+// VJP contraction and fold: whole fragments, at least two; an odd count gives warp column 0 one fragment more than
+// column 1 (the columns share the schedulers pairwise, so the odd fragment costs half a slot, not a whole one)
+__host__ __device__ inline int gemm_rp8(int r) {
+    const int rp = (r + 7) / 8 * 8;
+    return rp < 16 ? 16 : rp < GEMM_BN ? rp : GEMM_BN;
+}
+// shared row stride of a [k][RP] tile whose rows are read by the 4 k-lanes of a B fragment: == 4 (mod 16) doubles
+__host__ __device__ inline int gemm_sb(int RP) { return RP + (RP % 16 ? 12 : 4); }
 
 struct GemmFwdParams {
     TableDesc desc;
@@ -94,7 +102,7 @@ __global__ void __launch_bounds__(256) fk_transpose_f_kernel(const T* __restrict
 template <int VEC, bool GROUPED>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
-    extern __shared__ __align__(16) unsigned char fk_smem[];
+    extern __shared__ __align__(128) unsigned char fk_smem[];
     double* As = reinterpret_cast<double*>(fk_smem);                  // [STAGES][BM][SA]
     double* Ls = As + GEMM_STAGES * GEMM_BM * GEMM_SA;                 // [2][KT][SB]
     const uint32_t As_s = (uint32_t)__cvta_generic_to_shared(As);
@@ -328,7 +336,7 @@ constexpr int GEMMV_SMEM_BYTES = GEMMV_STAGES * 2 * GEMMV_NT * GEMMV_S * 8;
 template <int VEC, bool GROUPED>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 fk_gemm_vjp_kernel(const __grid_constant__ GemmVjpParams p) {
-    extern __shared__ __align__(16) unsigned char fk_smem[];
+    extern __shared__ __align__(128) unsigned char fk_smem[];
     double* As = reinterpret_cast<double*>(fk_smem);            // [STAGES][NT][S]  FK tile, k innermost
     double* Bs = As + GEMMV_STAGES * GEMMV_NT * GEMMV_S;         // [STAGES][NT][S]  g tile, replica innermost
     const uint32_t As_s = (uint32_t)__cvta_generic_to_shared(As), Bs_s = (uint32_t)__cvta_generic_to_shared(Bs);

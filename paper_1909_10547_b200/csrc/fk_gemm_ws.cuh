@@ -38,7 +38,7 @@ constexpr int WS_STAGE_DOUBLES = GEMM_BM * GEMM_SA;        // FK tile [128][36]
 constexpr int WS_NBAR = 2 * WS_STAGES + 4;                 // full[S], empty[S], fb_full[2], fb_empty[2]
 
 __host__ __device__ inline size_t ws_smem_bytes(int nx, int RP) {
-    return (size_t)(WS_STAGES * WS_STAGE_DOUBLES + 2 * nx * (RP + 4)) * 8 + WS_NBAR * 8;
+    return (size_t)(WS_STAGES * WS_STAGE_DOUBLES + 2 * nx * gemm_sb(RP)) * 8 + WS_NBAR * 8;
 }
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -68,7 +68,7 @@ struct WsFwdParams {
     ChannelList chan;      // single-table launch
     const double* fT;      // [nfl*nx][RP] replica-innermost f (grouped: + desc.f_off * RP)
     double* gpart;         // [ksplit][N][RP] level-1 partials (grouped: + desc.gp_off * RP)
-    int RP;                // padded replicas of this pass = 16 * NFW
+    int RP;                // padded replicas of this pass = 8 * NFRAG
     int ksplit, kper;      // single-table launch: K ranges (a multiple of ksub_rem) and their length
     int ksub_rem;          // single-table launch: k sub-splits (1, 2, 4) of the last, partial datapoint tile
     const TableDesc* descs;  // grouped launch
@@ -82,9 +82,11 @@ struct WsFwdParams {
 // DMMA time and the reduction sees the same number of slices whatever the tile height.
 __host__ __device__ inline int ws_ksub_for_rows(int rows) { return rows <= 32 ? 4 : rows <= 64 ? 2 : 1; }
 
-// NFW = 8-replica fragments per warp column = RP / 16, a compile-time constant: the 4 x NFW DMMAs of a k-step
+// NFRAG = 8-replica fragments of the pass = RP / 8, even here: each of the two warp columns takes NFRAG / 2.  (An
+// uneven split, as in the VJP kernel below, was measured slower for this kernel: two instruction streams of this
+// size per SM.)  The fragment count of a warp is a compile-time constant: the 4 x NF DMMAs of a k-step
 // carry no predicates, so ptxas is free to batch the fragment loads and the DMULs ahead of them.
-template <int NFW, bool GROUPED>
+template <int NFRAG, bool GROUPED>
 __global__ void __launch_bounds__(WS_THREADS, 1)
 fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
     extern __shared__ __align__(128) unsigned char fk_smem[];
@@ -121,7 +123,8 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
         kper = p.kper;
     }
     const TableDesc& d = *dp;
-    const int nx = d.nx, RP = p.RP, SB = RP + 4, cstride = d.cstride;
+    const int nx = d.nx, RP = p.RP, SB = gemm_sb(RP), cstride = d.cstride;
+    constexpr int NFW0 = NFRAG / 2;
     const int TM = GEMM_BM / KSUB, KTv = GEMM_KT * KSUB, SAv = KTv + 4;  // tile rows, k per stage, shared row stride
     const int kbeg = min(d.K, ks * kper * KSUB), kend = min(d.K, kbeg + kper * KSUB);
     // an empty K range (more slices than K-tiles) still writes its zero partials
@@ -199,13 +202,14 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
 
     // ================================ consumer warps: warp tile 32 datapoints x (8 * nfw) replicas ================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
-    auto consume = [&](auto ks_tag) {
+    auto consume = [&](auto ks_tag, auto nf_tag) {
+        constexpr int NFW = decltype(nf_tag)::value;           // fragments of this warp's column
         const int wm = warp & 3, wn = warp >> 2;
         constexpr int KS = decltype(ks_tag)::value;            // compile-time k sub-splits: immediate shared-memory offsets
         constexpr int KTc = GEMM_KT * KS, SAc = KTc + 4;
         const int rb = wm % (4 / KS), ksub = wm / (4 / KS);    // row block and k sub-split of this warp row
         constexpr int kst = 4 * KS;                            // k between consecutive MMA k-steps of this warp
-        const int cbcol = wn * NFW * 8;
+        const int cbcol = wn * NFW0 * 8;
         double acc[4][NFW][2];
     #pragma unroll
         for (int i = 0; i < 4; ++i)
@@ -305,10 +309,11 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
         }
         flush(!flushed);
     };
+    static_assert(NFRAG % 2 == 0, "the forward kernel takes whole pairs of fragments (RP a multiple of 16)");
     switch (KSUB) {
-        case 1: consume(std::integral_constant<int, 1>{}); break;
-        case 2: consume(std::integral_constant<int, 2>{}); break;
-        default: consume(std::integral_constant<int, 4>{}); break;
+        case 1: consume(std::integral_constant<int, 1>{}, std::integral_constant<int, NFW0>{}); break;
+        case 2: consume(std::integral_constant<int, 2>{}, std::integral_constant<int, NFW0>{}); break;
+        default: consume(std::integral_constant<int, 4>{}, std::integral_constant<int, NFW0>{}); break;
     }
 }
 
@@ -336,7 +341,7 @@ struct WsVjpParams {
 constexpr int WSV_STAGE_DOUBLES = 2 * GEMMV_NT * GEMMV_S;   // FK piece + g piece
 constexpr size_t WSV_SMEM_BYTES = (size_t)GEMMV_STAGES * WSV_STAGE_DOUBLES * 8 + 2 * GEMMV_STAGES * 8;
 
-template <int NFW, bool GROUPED>
+template <int NFRAG, bool GROUPED>
 __global__ void __launch_bounds__(WS_THREADS, 1)
 fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
     extern __shared__ __align__(128) unsigned char fk_smem[];
@@ -401,8 +406,11 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
     }
 
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
+    constexpr int NFW0 = (NFRAG + 1) / 2, NFW1 = NFRAG / 2;
+    auto consume = [&](auto nf_tag) {
+    constexpr int NFW = decltype(nf_tag)::value;  // fragments of this warp's column
     const int wm = warp & 3, wn = warp >> 2;
-    const int cbcol = wn * NFW * 8;
+    const int cbcol = wn * NFW0 * 8;
     int it = 0;
     for (int t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
         const TableDesc* d;
@@ -462,6 +470,9 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
             }
         }
     }
+    };
+    if (warp < 4) consume(std::integral_constant<int, NFW0>{});
+    else consume(std::integral_constant<int, NFW1>{});
 }
 
 }  // namespace fk

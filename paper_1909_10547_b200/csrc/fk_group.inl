@@ -117,7 +117,7 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
 }
 
 int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double* df_cat, int R, cudaStream_t s) {
-    const int RPmax = fk::gemm_rp(R);
+    const int RPmax = fk::gemm_rp8(R);
     double* fT = g->scratch;
     double* gP = fT + (size_t)g->ai_total * RPmax;
     double* G = gP + (size_t)g->rows_total * RPmax;
@@ -128,7 +128,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
     if (!attr_ok) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
     int nl = 0;
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
-        const int RP = fk::gemm_rp(R - r0);
+        const int RP = fk::gemm_rp8(R - r0);
         const long long tf = g->ai_total * RP, tg = g->rows_total * RP;
         fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
             f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, RP);

@@ -234,7 +234,7 @@ constexpr int FOLDK_THREADS = 256;
 template <typename T, bool GROUPED>
 __global__ void __launch_bounds__(FOLDK_THREADS)
 fk_vjp_foldk_kernel(const __grid_constant__ FoldKParams p) {
-    extern __shared__ __align__(16) unsigned char fk_smem[];
+    extern __shared__ __align__(128) unsigned char fk_smem[];
     double* Gs = reinterpret_cast<double*>(fk_smem);  // [nx][nx | 1]
     const TableDesc* dp = &p.desc;
     const uint8_t* __restrict__ ca = p.chan.a;
