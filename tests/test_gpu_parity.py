@@ -46,6 +46,8 @@ def test_config0_forward_and_vjp(K, R):
     }
     for name, s in outs.items():
         assert rel_err(s.cpu().numpy(), ref, scale) <= TOL64, name
+    # same layout, same plan, same partials, same order: the stateless call and the borrowing table give the same bits
+    assert np.array_equal(outs["stateless"].cpu().numpy(), outs["borrow"].cpu().numpy())
     douts = {
         "stateless": K.fk_conv_hadronic_vjp(fk_d, idx, f_d, g_d),
         "borrow": tb.vjp(f_d, g_d),
