@@ -482,3 +482,24 @@ def test_grouped_dense_tile_heights(K, R):
         assert rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale) <= TOL64, t
         assert rel_err(df[fo[t]:fo[t + 1]].reshape(R, c.nfl, c.nx), dref, D) <= TOL64, t
     assert np.array_equal(grp.conv(f_cat, R).cpu().numpy(), sig)
+
+
+def test_grouped_fp32_variant(K):
+    """The fp32 variant (reading R18) through the grouped launch, against the fp64 oracle of the fp64 inputs."""
+    import torch
+    shapes = synth.small_ragged_shapes(T=5)
+    R = 3
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    cases = [synth.config4_table(t, shapes, R, params) for t in range(shapes.T)]
+    tabs = [K.FkTable(K.FK_KIND_HADRONIC, to_dev(c.fk), c.pairs, c.nfl, K.FK_F32) for c in cases]
+    grp = K.FkGroup(tabs, R_hint=R)
+    fo, so = grp.offsets(R)
+    f_cat = torch.cat([to_dev(c.f, torch.float32).reshape(-1) for c in cases])
+    g_cat = torch.cat([to_dev(c.g, torch.float32).reshape(-1) for c in cases])
+    sig, df = grp.conv(f_cat, R).cpu().numpy(), grp.vjp(f_cat, g_cat, R).cpu().numpy()
+    assert sig.dtype == np.float32
+    for t, c in enumerate(cases):
+        ref, scale = O.hadronic(c.fk, c.pairs, c.f)
+        dref, D = O.hadronic_vjp(c.fk, c.pairs, c.f, c.g)
+        assert rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale) <= TOL32, t
+        assert rel_err(df[fo[t]:fo[t + 1]].reshape(R, c.nfl, c.nx), dref, D) <= TOL32, t

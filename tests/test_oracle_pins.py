@@ -386,3 +386,37 @@ def test_oracle_matches_its_committed_golden_file():
     with open(os.path.join(here, "oracle_tiny.json")) as fh:
         stored = json.load(fh)
     assert mod.build() == stored
+
+
+# ------------------------------------------------------------------ property tests on random small shapes
+def test_random_shapes_algebraic_properties():
+    """Seeded sweep over small random shapes: linearity in FK, degree-2 homogeneity in f, invariance under a
+    permutation of the channel list together with FK's channel axis, replica independence, and the numpy einsum
+    of the flat view -- a wrong index, stride or bound in the oracle breaks one of them at some shape."""
+    rng = np.random.default_rng(20260001)
+    for _ in range(25):
+        N, nx, nfl = int(rng.integers(1, 6)), int(rng.integers(1, 8)), int(rng.integers(1, 6))
+        C = int(rng.integers(1, nfl * nfl + 1))
+        R = int(rng.integers(1, 4))
+        pairs = synth.draw_pairs(rng, C, nfl)
+        fk, fk2 = rng.standard_normal((N, nx, nx, C)), rng.standard_normal((N, nx, nx, C))
+        f = rng.standard_normal((R, nfl, nx))
+        s1, sc1 = O.hadronic(fk, pairs, f)
+        s2, sc2 = O.hadronic(fk2, pairs, f)
+        s12, _ = O.hadronic(fk + 2.0 * fk2, pairs, f)
+        tol = 4e-16 * (sc1 + 2 * sc2)
+        assert np.all(np.abs(s12 - (s1 + 2.0 * s2)) <= tol + 1e-300)
+        s3, _ = O.hadronic(fk, pairs, 3.0 * f)
+        assert np.all(np.abs(s3 - 9.0 * s1) <= 4e-15 * sc1 + 1e-300)
+        perm = rng.permutation(C)
+        sp, _ = O.hadronic(np.ascontiguousarray(fk[..., perm]), pairs[perm], f)
+        assert np.all(np.abs(sp - s1) <= 4e-16 * sc1 + 1e-300)
+        for r in range(R):
+            sr, _ = O.hadronic(fk, pairs, f[r:r + 1])
+            assert np.array_equal(sr[:, 0], s1[:, r])
+        L = np.einsum("rci,rcj->rcij", f[:, pairs[:, 0], :], f[:, pairs[:, 1], :])   # [R][C][i][j]
+        flat = np.einsum("nijc,rcij->nr", fk, L)
+        assert np.all(np.abs(flat - s1) <= 1e-14 * sc1 + 1e-300)
+        g = rng.standard_normal((N, R))
+        df, D = O.hadronic_vjp(fk, pairs, f, g)
+        assert np.all(np.abs((f * df).sum(axis=(1, 2)) - 2.0 * (g * s1).sum(axis=0)) <= 1e-13 * (np.abs(f) * D).sum(axis=(1, 2)) + 1e-300)
