@@ -514,12 +514,24 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
     p.sigma = sigma;
     p.R = R;
     const int fgrid = pl.nkb * pl.fsplit;
+    // few datapoints per range and very many k-blocks: CTAs that walk the k-blocks (fk_fwd_fewrows_kernel)
+    const bool fewrows = (d.N + pl.fsplit - 1) / pl.fsplit <= FWD_U && pl.nkb >= 64 * std::max(1, sm_count()) &&
+                         d.vec_ok && env_int("FKCONV_FEWROWS", 1);
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
         size_t slot = 0;
         const bool timed = r0 == 0 && g_prof.begin(s, slot);
-        cudaError_t e = fwd_dispatch<T, false, TS>(d.vec_ok, rt, p, fgrid, s);
+        cudaError_t e;
+        if (fewrows) {
+            constexpr int VW = fk::VecWidth<TS>::value;
+            const dim3 grid(std::max(1, sm_count()) * 16, pl.fsplit);
+            if (rt == 1) fk::fk_fwd_fewrows_kernel<T, VW, 1, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            else if (rt == 2) fk::fk_fwd_fewrows_kernel<T, VW, 2, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            else fk::fk_fwd_fewrows_kernel<T, VW, 4, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            e = cudaGetLastError();
+        } else
+            e = fwd_dispatch<T, false, TS>(d.vec_ok, rt, p, fgrid, s);
         if (timed) g_prof.end(s, slot);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "forward kernel launch failed: %s", cudaGetErrorString(e));
         ++nl;
@@ -529,6 +541,7 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
         fk::ReduceParams q;
         memset(&q, 0, sizeof q);
         q.desc = d;
+        if (fewrows) q.desc.nchunks = std::max(1, sm_count()) * 16;  // one partial per CTA of the few-rows kernel
         q.part = part;
         q.sigma = sigma;
         q.rows = d.N;

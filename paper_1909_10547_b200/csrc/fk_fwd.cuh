@@ -153,6 +153,86 @@ fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
     }
 }
 
+// ---- few datapoints, very long rows (the paper's N = 8 shapes of Table 3): with one batch of U rows
+// per (k-block, range) the column kernel above would launch ~K/512 CTAs that live for one round trip each, and
+// the CTA launch rate, not HBM, sets the pace (3.3 TB/s at K = 1e8).  Here a CTA walks k-blocks blockIdx.x,
+// blockIdx.x + gridDim.x, ... of its datapoint range and adds their CTA sums in walk order: same per-thread
+// arithmetic, one level-1 partial per CTA (a fixed grid: bitwise repeatable), same level 2.
+template <typename T, int VEC, int RT, int U, typename TS = T>
+__global__ void __launch_bounds__(FWD_THREADS)
+fk_fwd_fewrows_kernel(const __grid_constant__ FwdParams p) {
+    using V = Vec<TS, VEC>;
+    constexpr int LPR = 32 / U;
+    __shared__ double red[2][FWD_WARPS][U][RT];
+    const TableDesc& d = p.desc;
+    const uint8_t* __restrict__ ca = p.chan.a;
+    const uint8_t* __restrict__ cb = p.chan.b;
+    const int split = blockIdx.y, R = p.R;
+    const int rb = (int)((long long)d.N * split / d.fsplit);
+    const int re = (int)((long long)d.N * (split + 1) / d.fsplit);  // re - rb <= U
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int fstride = d.nfl * d.nx;
+    const T* __restrict__ f = reinterpret_cast<const T*>(p.f);
+    int buf = 0;
+    double tot = 0.0;  // threads < U * RT: this CTA's sum over its k-blocks, in walk order (one partial per CTA)
+    for (int kblock = blockIdx.x; kblock < d.nchunks; kblock += gridDim.x, buf ^= 1) {
+        const int k = (kblock * FWD_THREADS + threadIdx.x) * VEC;
+        const bool kin = k < d.K;
+        const TS* __restrict__ col = reinterpret_cast<const TS*>(d.fk) + (kin ? k : 0);
+        V x[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) x[u] = ld_stream(col + (long long)min(rb + u, re - 1) * d.row_stride, (V*)nullptr);
+        T L[RT][VEC];
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) {
+            int ia = 0, ib = -1;
+            bool in = k + e < d.K;
+            if (in) decode_k(d, ca, cb, k + e, ia, ib);
+            in = in && ia >= 0;
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                const int rr = p.r0 + r;
+                T l = T(0);
+                if (in && rr < R) {
+                    l = __ldg(f + (long long)rr * fstride + ia);
+                    if (ib >= 0) l *= __ldg(f + (long long)rr * fstride + ib);
+                }
+                L[r][e] = l;
+            }
+        }
+        double pr[RT][U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const bool live = kin && (rb + u < re);
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+                T s = (T)x[u].v[0] * L[r][0];
+#pragma unroll
+                for (int e = 1; e < VEC; ++e) s = fma((T)x[u].v[e], L[r][e], s);
+                pr[r][u] = live ? (double)s : 0.0;
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const double s = fold_rows<U>(pr[r], lane);
+            if ((lane & (LPR - 1)) == 0) red[buf][warp][lane / LPR][r] = s;
+        }
+        __syncthreads();
+        if (threadIdx.x < U * RT) {
+            const int u = threadIdx.x / RT, r = threadIdx.x - u * RT;
+            double s = red[buf][0][u][r];
+#pragma unroll
+            for (int w = 1; w < FWD_WARPS; ++w) s += red[buf][w][u][r];
+            tot += s;
+        }
+    }
+    if (threadIdx.x < U * RT) {
+        const int u = threadIdx.x / RT, r = threadIdx.x - u * RT;
+        const int n = rb + u, rr = p.r0 + r;
+        if (n < re && rr < R) p.part[((long long)n * R + rr) * gridDim.x + blockIdx.x] = tot;
+    }
+}
+
 // ---- one read of FK for both passes: when the upstream gradient g[n][r] is known before the
 // forward pass (a loss linear in sigma, e.g. config 4's seeded weights), the column kernel also accumulates
 // VJP stage 1, G[split][r][k] = sum_{n in range} g[n][r] FK[n][k], from the registers that already hold the row

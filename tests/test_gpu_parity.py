@@ -172,7 +172,8 @@ def test_config1_dis(K, R):
         assert rel_err(d.cpu().numpy(), dref, D) <= TOL64, name
 
 
-@pytest.mark.parametrize("shape_R", [((8, 3571, 1), 1), ((8, 3571, 1), 7), ((100, 1021, 1), 3), ((33, 2048, 1), 40)])
+@pytest.mark.parametrize("shape_R", [((8, 3571, 1), 1), ((8, 3571, 1), 7), ((100, 1021, 1), 3), ((33, 2048, 1), 40),
+                                     ((8, 5_000_000, 1), 1), ((5, 4_900_001, 1), 3)])  # the last two: fk_fwd_fewrows_kernel
 def test_flat_matrix_view_of_table3(K, shape_R):
     """The paper's Table-3 operation: flat FK[N x K] . PDF[K x R] with a pre-built PDF matrix =
     the DIS convolution with one pseudo-flavour and nx = K (f = PDF^T)."""
