@@ -391,9 +391,17 @@ __global__ void __launch_bounds__(256) fk_reduce_chunks_kernel(const __grid_cons
         const int nch = d->nchunks;
         if (nch == 1) continue;  // written directly by the column kernel
         const double* src = p.part + d->part_off * p.R + (n * p.R + r) * nch;
-        double s = 0.0;
-        for (int c = lane; c < nch; c += 32) s += src[c];
-        s = warp_sum(s);
+        // four lane-strided chains per lane (four loads in flight), combined pairwise, then the butterfly
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        int c = lane;
+        for (; c + 96 < nch; c += 128) {
+            a0 += src[c];
+            a1 += src[c + 32];
+            a2 += src[c + 64];
+            a3 += src[c + 96];
+        }
+        for (; c < nch; c += 32) a0 += src[c];
+        const double s = warp_sum((a0 + a1) + (a2 + a3));
         if (lane == 0) reinterpret_cast<T*>(p.sigma)[d->out_off * p.R + n * p.R + r] = (T)s;
     }
 }
