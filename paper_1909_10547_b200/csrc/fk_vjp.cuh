@@ -256,14 +256,14 @@ fk_vjp_foldk_kernel(const __grid_constant__ FoldKParams p) {
     for (int t = threadIdx.x + i0 * nx; t < i1 * nx; t += FOLDK_THREADS) {
         const int i = t / nx, j = t - i * nx;
         const int k = encode_k(d, i, j, c);
-        double v = G[k];
-        int s = 1;
-        for (; s + 4 <= d.nsplit; s += 4) {  // four independent loads in flight, added in index order
-            const double v0 = G[s * split_stride + k], v1 = G[(s + 1) * split_stride + k];
-            const double v2 = G[(s + 2) * split_stride + k], v3 = G[(s + 3) * split_stride + k];
-            v = (((v + v0) + v1) + v2) + v3;
+        double v = 0.0;
+        for (int s0 = 0; s0 < d.nsplit; s0 += 8) {  // eight independent loads in flight, added in index order
+            double w[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) w[q] = s0 + q < d.nsplit ? G[(long long)(s0 + q) * split_stride + k] : 0.0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) v += w[q];
         }
-        for (; s < d.nsplit; ++s) v += G[s * split_stride + k];
         Gs[(i - i0) * ld + j] = v;
     }
     __syncthreads();
