@@ -261,7 +261,13 @@ __global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const double* __res
         const int n = (int)(t / RP), c = (int)(t - (long long)n * RP);
         if (r0 + c >= R) continue;
         double s = 0.0;
-        for (int ks = 0; ks < ksplit; ++ks) s += gpart[(long long)ks * total + t];
+        for (int k0 = 0; k0 < ksplit; k0 += 8) {  // eight loads in flight, added in index order
+            double w[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) w[q] = k0 + q < ksplit ? gpart[(long long)(k0 + q) * total + t] : 0.0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) s += w[q];
+        }
         sigma[out_off + (long long)n * R + r0 + c] = (T)s;
     }
 }
@@ -308,7 +314,13 @@ __global__ void __launch_bounds__(256) fk_gemm_reduce_grouped_kernel(const doubl
         const double* src = gpart + (d.gp_off + n) * RP + c;
         const long long stride = (long long)d.N * RP;
         double s = 0.0;
-        for (int ks = 0; ks < d.gksplit; ++ks) s += src[ks * stride];
+        for (int k0 = 0; k0 < d.gksplit; k0 += 8) {  // eight loads in flight, added in index order
+            double w[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) w[q] = k0 + q < d.gksplit ? src[(k0 + q) * stride] : 0.0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) s += w[q];
+        }
         sigma[grow * R + r0 + c] = (T)s;
     }
 }
