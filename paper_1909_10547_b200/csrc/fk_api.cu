@@ -119,7 +119,7 @@ void make_plan(fk::TableDesc& d, int dtype, Plan& pl) {
 
     // forward: ~32 datapoints per CTA (finer for small tables so that the grid still covers the GPU a few
     // times over), never fewer than one batch of FWD_U rows
-    int rows = env_int("FKCONV_FWD_ROWS", 32);
+    int rows = env_int("FKCONV_FWD_ROWS", dtype == FK_F64 ? 32 : 64);  // fp32 storage: 4 luminosity values per thread to amortise
     const long long want_f = (long long)env_int("FKCONV_FWD_MIN_CTAS_PER_SM", 8) * sms;
     while (rows > FWD_U && (long long)pl.nkb * ((d.N + rows - 1) / rows) < want_f) rows /= 2;
     rows = std::max(rows, 1);
