@@ -636,6 +636,8 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
                        T* sigma, T* df, int R, double* scratch, cudaStream_t s, int* launches) {
     constexpr int VW = fk::VecWidth<TS>::value;
     fk::TableDesc d = d0;
+    // up to 64 datapoints per CTA (the forward alone takes ~32): half as many column-sum slices to write and to fold
+    d.fsplit = std::max(1, std::min(d0.fsplit, (d0.N + 63) / 64));
     d.nsplit = d.fsplit;  // the column sums are cut into the forward's datapoint ranges
     double* part = scratch;
     double* G = part + part_elems_per_replica(d) * R;
@@ -650,7 +652,7 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
     p.fwd.R = R;
     p.g = g;
     p.G = G;
-    const int grid = pl.nkb * pl.fsplit;
+    const int grid = pl.nkb * d.fsplit;
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.fwd.r0 = r0;
