@@ -24,13 +24,18 @@ def build():
     sigma, scale = O.hadronic(case.fk, case.pairs, case.f)
     df, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
     dis = synth.config1(R=1, N=4)
-    sd, _ = O.dis(dis.fk, dis.flav, dis.f)
+    sd, sds = O.dis(dis.fk, dis.flav, dis.f)
+    dd, ddD = O.dis_vjp(dis.fk, dis.flav, dis.f, dis.g)
     return {
         "about": "oracle outputs (hex floats) on seeded inputs: hadronic_case(14, N=3, nx=4, C=5, R=2, nfl=3, sub=1); config1(R=1, N=4)",
         "hadronic_sigma": [float(x).hex() for x in sigma.ravel()],
         "hadronic_scale": [float(x).hex() for x in scale.ravel()],
         "hadronic_df": [float(x).hex() for x in df.ravel()],
+        "hadronic_D": [float(x).hex() for x in D.ravel()],
         "dis_sigma": [float(x).hex() for x in sd.ravel()],
+        "dis_scale": [float(x).hex() for x in sds.ravel()],
+        "dis_df": [float(x).hex() for x in dd[:, dis.flav, :6].ravel()],      # active flavours, first 6 x-points
+        "dis_D": [float(x).hex() for x in ddD[:, dis.flav, :6].ravel()],
     }
 
 

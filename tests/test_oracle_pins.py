@@ -42,6 +42,7 @@ def test_brute_force_fraction_hadronic_and_vjp():
     F = lambda v: Fraction(float(v))
     for r in range(R):
         dref = [[Fraction(0)] * nx for _ in range(nfl)]
+        Dref = [[Fraction(0)] * nx for _ in range(nfl)]
         for n in range(N):
             acc = Fraction(0); S = Fraction(0)
             for c, (a, b) in enumerate(pairs):
@@ -49,13 +50,17 @@ def test_brute_force_fraction_hadronic_and_vjp():
                     for j in range(nx):
                         t = F(f[r, a, i]) * F(f[r, b, j]) * F(fk[n, i, j, c])
                         acc += t; S += abs(t)
-                        dref[a][i] += F(g[n, r]) * F(fk[n, i, j, c]) * F(f[r, b, j])
-                        dref[b][j] += F(g[n, r]) * F(fk[n, i, j, c]) * F(f[r, a, i])
+                        ta = F(g[n, r]) * F(fk[n, i, j, c]) * F(f[r, b, j])
+                        tb = F(g[n, r]) * F(fk[n, i, j, c]) * F(f[r, a, i])
+                        dref[a][i] += ta; Dref[a][i] += abs(ta)
+                        dref[b][j] += tb; Dref[b][j] += abs(tb)
             assert abs(Fraction(float(sigma[n, r])) - acc) <= 2 * U * S
             assert abs(Fraction(float(scale[n, r])) - S) <= 4 * U * S
         for a in range(nfl):
             for i in range(nx):
-                assert abs(Fraction(float(df[r, a, i])) - dref[a][i]) <= 2 * U * Fraction(float(D[r, a, i]))
+                assert abs(Fraction(float(df[r, a, i])) - dref[a][i]) <= 2 * U * Dref[a][i]
+                # the VJP tolerance denominator itself (reading R21): D = sum |g FK f| over every term of the slot
+                assert abs(Fraction(float(D[r, a, i])) - Dref[a][i]) <= 4 * U * Dref[a][i]
 
 
 def test_brute_force_fraction_dis():
@@ -71,11 +76,15 @@ def test_brute_force_fraction_dis():
     for r in range(R):
         for n in range(N):
             acc = sum(F(f[r, flav[c], i]) * F(fk[n, i, c]) for c in range(nA) for i in range(nx))
-            assert abs(F(sigma[n, r]) - acc) <= 2 * U * F(scale[n, r])
+            S = sum(abs(F(f[r, flav[c], i]) * F(fk[n, i, c])) for c in range(nA) for i in range(nx))
+            assert abs(F(sigma[n, r]) - acc) <= 2 * U * S
+            assert abs(F(scale[n, r]) - S) <= 4 * U * S          # the DIS tolerance denominator
         for a in range(nfl):
             for i in range(nx):
                 ref = sum(F(g[n, r]) * F(fk[n, i, c]) for n in range(N) for c in range(nA) if flav[c] == a)
-                assert abs(F(df[r, a, i]) - ref) <= 2 * U * F(D[r, a, i]) + (0 if ref else 0)
+                Dref = sum(abs(F(g[n, r]) * F(fk[n, i, c])) for n in range(N) for c in range(nA) if flav[c] == a)
+                assert abs(F(df[r, a, i]) - ref) <= 2 * U * Dref
+                assert abs(F(D[r, a, i]) - Dref) <= 4 * U * Dref   # the DIS-VJP tolerance denominator
                 if a not in flav:
                     assert df[r, a, i] == 0.0
 
@@ -180,6 +189,45 @@ def test_exact_integer_inputs_match_int64():
     assert np.array_equal(sigma, ref.astype(np.float64))
     refabs = np.einsum("rci,rcj,nijc->nr", np.abs(A), np.abs(B), np.abs(ki))
     assert np.array_equal(scale, refabs.astype(np.float64))
+
+
+def test_exact_integer_denominators_match_int64():
+    """The tolerance denominators every GPU gate divides by (reading R21) are exact sums of
+    integers here, so they must equal an int64 abs-einsum bit for bit: D of the hadronic VJP (scatter of
+    |g FK f| onto both legs), D of the DIS VJP and scale of the DIS forward.  A denominator inflated or deflated
+    by any factor fails this."""
+    case = synth.integer_hadronic_case(2, N=5, nx=8, C=12, R=3, nfl=6)
+    fi, ki, gi = np.abs(case.f.astype(np.int64)), np.abs(case.fk.astype(np.int64)), np.abs(case.g.astype(np.int64))
+    df, D = O.hadronic_vjp(case.fk, case.pairs, case.f, case.g)
+    Gabs = np.einsum("nr,nijc->rijc", gi, ki)                     # |g| |FK| summed over datapoints
+    Dref = np.zeros(case.f.shape, dtype=np.int64)
+    dref = np.zeros(case.f.shape, dtype=np.int64)
+    Gs = np.einsum("nr,nijc->rijc", case.g.astype(np.int64), case.fk.astype(np.int64))
+    fs = case.f.astype(np.int64)
+    for c, (a, b) in enumerate(case.pairs):
+        Dref[:, a, :] += np.einsum("rij,rj->ri", Gabs[..., c], fi[:, b, :])
+        Dref[:, b, :] += np.einsum("rij,ri->rj", Gabs[..., c], fi[:, a, :])
+        dref[:, a, :] += np.einsum("rij,rj->ri", Gs[..., c], fs[:, b, :])
+        dref[:, b, :] += np.einsum("rij,ri->rj", Gs[..., c], fs[:, a, :])
+    assert np.array_equal(D, Dref.astype(np.float64)) and np.array_equal(df, dref.astype(np.float64))
+    assert Dref.max() > 0 and np.any(Dref != np.abs(dref))        # cancellation: D is not |df|
+    # DIS: forward scale and VJP denominator
+    rng = synth.rng_for(7, synth.T_FK, 5)
+    N, nx, nfl, nA, R = 6, 9, 7, 4, 3
+    flav = np.array([5, 1, 6, 2], dtype=np.int32)
+    fkd = rng.integers(-8, 9, size=(N, nx, nA)).astype(np.float64)
+    f = rng.integers(-8, 9, size=(R, nfl, nx)).astype(np.float64)
+    g = rng.integers(-8, 9, size=(N, R)).astype(np.float64)
+    s, sc = O.dis(fkd, flav, f)
+    ka, fa, ga = np.abs(fkd.astype(np.int64)), np.abs(f.astype(np.int64)), np.abs(g.astype(np.int64))
+    assert np.array_equal(sc, np.einsum("nic,rci->nr", ka, fa[:, flav, :]).astype(np.float64))
+    assert np.array_equal(s, np.einsum("nic,rci->nr", fkd.astype(np.int64), f.astype(np.int64)[:, flav, :]).astype(np.float64))
+    dfd, Dd = O.dis_vjp(fkd, flav, f, g)
+    Dref = np.zeros((R, nfl, nx), dtype=np.int64); dref = np.zeros((R, nfl, nx), dtype=np.int64)
+    for c, a in enumerate(flav):
+        Dref[:, a, :] += np.einsum("nr,ni->ri", ga, ka[:, :, c])
+        dref[:, a, :] += np.einsum("nr,ni->ri", g.astype(np.int64), fkd.astype(np.int64)[:, :, c])
+    assert np.array_equal(Dd, Dref.astype(np.float64)) and np.array_equal(dfd, dref.astype(np.float64))
 
 
 # ---------------------------------------------------------------- algebraic structure
