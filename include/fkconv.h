@@ -26,6 +26,13 @@
  *  - every compute call is asynchronous on `stream` (a cudaStream_t passed as void*, NULL = the
  *    legacy default stream) and never synchronises the device; the *_host variants copy through
  *    pinned staging owned by the table and DO wait for the result before returning.
+ *  - a handle (fk_table, fk_group) owns ONE scratch buffer, so the calls on it are serialised: host threads
+ *    queue on the handle's mutex, and a call that arrives on a different stream than the previous call on the
+ *    same handle first makes its stream wait (cudaStreamWaitEvent) for that call's last kernel.  Different handles
+ *    are independent.  Inside a CUDA-graph stream capture a handle must be used from one stream only, and its
+ *    scratch cannot grow: give R_hint at create (or make one call outside the capture); otherwise the call returns
+ *    FK_ERR_UNSUPPORTED.  A handle belongs to the device that was current at create; a call made with another
+ *    current device returns FK_ERR_INVALID_ARG.
  *  - logical layouts (BASELINE.json): hadronic FK[N][nx][nx][C] (i, j, channel; channel innermost),
  *    DIS FK[N][nx][nA], pairs[C][2] = (a_c, b_c) with i <-> a_c and j <-> b_c, flav[nA],
  *    f[R][nfl][nx], sigma[N][R], g[N][R], df[R][nfl][nx].
@@ -69,6 +76,24 @@ const char* fk_last_error_string(void);
 /* Library version, and the compute capability it was compiled for (100 = sm_100a). */
 int fk_version(void);
 int fk_compiled_arch(void);
+
+/* Process-wide path-selection options (defaults in brackets).  They are read when a table / group is created and
+ * when a compute call picks its kernels: set them before creating handles.  A different option set means a
+ * different (still fixed) reduction plan: results are bitwise repeatable per option set.  Nothing is ever read
+ * from the environment. */
+enum {
+    FK_OPT_GEMM_MIN_R = 0, /* [0] smallest R that takes the dense fp64 contraction; 0 = built-in (5 on packed hadronic tables, else 13) */
+    FK_OPT_WARP_SPEC = 1,  /* [1] warp-specialised bulk-copy DMMA kernels (0: generic cp.async kernels) */
+    FK_OPT_FOLD = 2,       /* [1] R >> 1 VJP stage 2 as one streaming pass over the column sums (0: gather form) */
+    FK_OPT_FOLDK = 3,      /* [1] small-R VJP stage 2 as one pass (0: gather form) */
+    FK_OPT_FUSED = 4,      /* [1] fk_table_conv_vjp / fk_conv_grouped_conv_vjp read FK once (0: two passes) */
+    FK_OPT_FEWROWS = 5,    /* [1] k-walking forward kernel for <= 8 datapoints and very long rows */
+    FK_OPT_TC32 = 6,       /* [1] tcgen05 (3xTF32) dense contraction for FK_F32 tables at large R (0: column passes) */
+    FK_OPT_TC32_MIN_R = 7, /* [0] smallest R that takes it; 0 = built-in */
+    FK_OPT_COUNT_ = 8
+};
+int fk_set_option(int option, int value);
+int fk_get_option(int option, int* value);
 
 /* Kernel timing hook for bench.py's roofline: while enabled, every forward call brackets its
  * dominant kernel (the streaming contraction, or the dense contraction for large R) with a CUDA event

@@ -47,30 +47,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [_nvcc(), *NVCC_FLAGS]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += os.environ.get("FKCONV_NVCC_FLAGS", "").split()  # e.g. -DFK_BULK_DEPTH=4 for tuning builds
     cmd += ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd, cwd=CSRC)
     os.replace(tmp, LIB)
     return LIB
 
 
-def build_probes() -> list:
-    """Stand-alone design probes (csrc/probes/*.cu -> probes/<name>): read patterns, FP64 peak."""
-    out_dir = os.path.join(HERE, "probes")
-    os.makedirs(out_dir, exist_ok=True)
-    outs = []
-    for name in sorted(os.listdir(os.path.join(CSRC, "probes"))):
-        if not name.endswith(".cu"):
-            continue
-        exe = os.path.join(out_dir, name[:-3])
-        subprocess.check_call([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-                               "-o", exe, os.path.join(CSRC, "probes", name)])
-        outs.append(exe)
-    return outs
-
-
 if __name__ == "__main__":
-    if "--probes" in sys.argv:
-        print("\n".join(build_probes()))
-    else:
-        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

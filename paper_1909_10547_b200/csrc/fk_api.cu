@@ -1,6 +1,6 @@
 // fk_api.cu -- the C-ABI of include/fkconv.h: argument validation, table / group handles, launch plans.
-// Host logic only; every step of the path runs in the kernels of fk_stream.cuh / fk_vjp.cuh /
-// fk_gemm.cuh.  There is no CPU fallback anywhere in this file.
+// Host logic only; every step of the path runs in the kernels of fk_fwd.cuh / fk_vjp.cuh / fk_vjp_fold.cuh /
+// fk_gemm.cuh / fk_gemm_ws.cuh.  There is no CPU fallback anywhere in this file.
 #include "../../include/fkconv.h"
 
 #include <cuda_runtime.h>
@@ -49,10 +49,25 @@ int fail(int code, const char* fmt, ...) {
                         #call, cudaGetErrorString(e_));                                            \
     } while (0)
 
-int env_int(const char* name, int dflt) {
-    const char* s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
+// ---- plan constants (frozen from the round-1 sweeps; nothing is read from the environment) ----
+constexpr int FWD_ROWS_F64 = 32;           // datapoints per forward CTA, fp64 table
+constexpr int FWD_ROWS_F32 = 64;           // fp32-stored table: 4 luminosity values per thread to amortise
+constexpr int FWD_MIN_CTAS_PER_SM = 8;     // small tables: cut finer until the grid covers the GPU this often
+constexpr int COLSUM_CTAS_PER_SM = 24;     // VJP stage 1: CTAs wanted per SM
+constexpr int GROUP_GEMM_WAVES = 16;       // grouped R >> 1 forward: waves of equal-cost items
+
+// ---- process-wide options (fk_set_option, include/fkconv.h): path selection only ----
+int g_opt[FK_OPT_COUNT_] = {
+    /* FK_OPT_GEMM_MIN_R  */ 0,   // 0 = built-in threshold (5 on the warp-specialised path, 13 otherwise)
+    /* FK_OPT_WARP_SPEC   */ 1,
+    /* FK_OPT_FOLD        */ 1,
+    /* FK_OPT_FOLDK       */ 1,
+    /* FK_OPT_FUSED       */ 1,
+    /* FK_OPT_FEWROWS     */ 1,
+    /* FK_OPT_TC32        */ 1,
+    /* FK_OPT_TC32_MIN_R  */ 0,
+};
+inline int opt(int o) { return g_opt[o]; }
 
 int sm_count() {
     static std::mutex mu;
@@ -67,6 +82,22 @@ int sm_count() {
     cache[dev] = n;
     return n;
 }
+
+// cudaFuncSetAttribute is per DEVICE: the opt-in to more than 48 KB of dynamic shared memory is cached per
+// (device, kernel), so a process that drives several GPUs sets it on each of them.
+bool ensure_dyn_smem(const void* func, size_t bytes) {
+    static std::mutex mu;
+    static std::map<std::pair<int, const void*>, size_t> done;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    std::lock_guard<std::mutex> lk(mu);
+    auto it = done.find({dev, func});
+    if (it != done.end() && it->second >= bytes) return true;
+    if (cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) return false;
+    done[{dev, func}] = bytes;
+    return true;
+}
+template <typename F> bool ensure_dyn_smem(F* func, size_t bytes) { return ensure_dyn_smem((const void*)func, bytes); }
 
 // ---- kernel timing hook (fk_profile_enable / fk_profile_read) ----
 struct Profiler {
@@ -119,14 +150,14 @@ void make_plan(fk::TableDesc& d, int dtype, Plan& pl) {
 
     // forward: ~32 datapoints per CTA (finer for small tables so that the grid still covers the GPU a few
     // times over), never fewer than one batch of FWD_U rows
-    int rows = env_int("FKCONV_FWD_ROWS", dtype == FK_F64 ? 32 : 64);  // fp32 storage: 4 luminosity values per thread to amortise
-    const long long want_f = (long long)env_int("FKCONV_FWD_MIN_CTAS_PER_SM", 8) * sms;
+    int rows = dtype == FK_F64 ? FWD_ROWS_F64 : FWD_ROWS_F32;
+    const long long want_f = (long long)FWD_MIN_CTAS_PER_SM * sms;
     while (rows > FWD_U && (long long)pl.nkb * ((d.N + rows - 1) / rows) < want_f) rows /= 2;
     rows = std::max(rows, 1);
     pl.fsplit = std::max(1, std::min(d.N, (d.N + rows - 1) / rows));
 
     // VJP stage 1: fewer, longer ranges (every range writes K column sums that stage 2 adds up)
-    const int want = env_int("FKCONV_COLSUM_CTAS_PER_SM", 24) * sms;  // CTAs wanted for stage 1
+    const int want = COLSUM_CTAS_PER_SM * sms;  // CTAs wanted for stage 1
     int nsplit = (want + pl.nkb - 1) / pl.nkb;
     nsplit = std::min(nsplit, std::max(1, d.N / 16));                  // >= 16 datapoints per split
     nsplit = std::max(nsplit, (d.N + fk::COLSUM_MAX_ROWS - 1) / fk::COLSUM_MAX_ROWS);
@@ -141,7 +172,7 @@ void make_plan(fk::TableDesc& d, int dtype, Plan& pl) {
 size_t part_elems_per_replica(const fk::TableDesc& d) { return d.nchunks > 1 ? (size_t)d.N * d.nchunks : 0; }
 size_t G_elems_per_replica(const fk::TableDesc& d) { return (size_t)d.nsplit * d.K; }
 // small-R VJP stage 2 in one pass over G (fk_vjp_foldk_kernel): hadronic tables whose nx x nx block fits shared memory
-bool foldk_ok(const fk::TableDesc& d) { return d.kind == fk::KIND_HADRONIC && d.nx <= 128 && env_int("FKCONV_FOLDK", 1); }
+bool foldk_ok(const fk::TableDesc& d) { return d.kind == fk::KIND_HADRONIC && d.nx <= 128 && opt(FK_OPT_FOLDK); }
 size_t foldk_smem(int nx) { return (size_t)nx * (nx | 1) * 8; }
 constexpr int FOLDK_MAX_CHUNKS = 8;
 // x-row chunks per channel so that a table (or group) with few channels still covers the GPU about twice
@@ -243,13 +274,13 @@ bool gemm_wanted(const fk::TableDesc& d, int R) {
     // R = 5 on; the generic cp.async kernel (DIS, logical layout) streams FK at ~2 TB/s and only wins once the
     // column kernel would need more than 3 passes
     const bool ws = d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok;
-    return R >= env_int("FKCONV_GEMM_MIN_R", ws ? 5 : 13);
+    return R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : ws ? 5 : 13);
 }
 
 GemmPlan gemm_plan(const fk::TableDesc& d, int R) {
     GemmPlan gp;
     const int mtiles = (d.N + fk::GEMM_BM - 1) / fk::GEMM_BM;
-    const int target = std::max(1, sm_count()) * std::max(1, env_int("FKCONV_GEMM_WAVES", 1));
+    const int target = std::max(1, sm_count());  // one wave of equal items
     int ksplit = std::max(1, target / mtiles);
     gp.kper = ((d.K + ksplit - 1) / ksplit + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT;
     gp.ksplit = (d.K + gp.kper - 1) / gp.kper;
@@ -270,53 +301,38 @@ constexpr size_t MAX_DYN_SMEM = 232448;  // 227 KB per CTA on sm_100a
 
 // the warp-specialised kernel (fk_gemm_ws.cuh) serves packed hadronic tables whose f[b_c] tiles fit next to the FK ring
 bool ws_ok(const fk::TableDesc& d, int RP) {
-    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok && env_int("FKCONV_WS", 1) &&
+    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok && opt(FK_OPT_WARP_SPEC) &&
            fk::ws_smem_bytes(d.nx, RP) <= MAX_DYN_SMEM;
-}
-
-template <bool GROUPED>
-bool ws_set_attr() {
-    bool ok = true;
-#define FK_WS_ATTR(NFW) ok = ok && cudaFuncSetAttribute(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MAX_DYN_SMEM) == cudaSuccess
-    FK_WS_ATTR(2); FK_WS_ATTR(4); FK_WS_ATTR(6); FK_WS_ATTR(8); FK_WS_ATTR(10); FK_WS_ATTR(12); FK_WS_ATTR(14); FK_WS_ATTR(16);
-#undef FK_WS_ATTR
-    return ok;
 }
 
 // RP = 8 * NFRAG (fk::gemm_rp: a multiple of 16), NFRAG = 2, 4, ..., 16: one instantiation per fragment count
 template <bool GROUPED>
-void ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) {
+bool ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) {
     switch (w.RP / 8) {
-#define FK_WS_CASE(NFW) case NFW: fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, smem, s>>>(w); break
+#define FK_WS_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, MAX_DYN_SMEM)) return false; \
+                                  fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, smem, s>>>(w); break
         FK_WS_CASE(2); FK_WS_CASE(4); FK_WS_CASE(6); FK_WS_CASE(8); FK_WS_CASE(10); FK_WS_CASE(12); FK_WS_CASE(14);
         default: FK_WS_CASE(16);
 #undef FK_WS_CASE
     }
+    return true;
 }
 
 // the persistent warp-specialised VJP contraction needs 16-byte aligned, 16-byte multiple row pieces
-bool wsv_ok(const fk::TableDesc& d) { return d.vec_ok && d.K % 2 == 0 && env_int("FKCONV_WS", 1); }
+bool wsv_ok(const fk::TableDesc& d) { return d.vec_ok && d.K % 2 == 0 && opt(FK_OPT_WARP_SPEC); }
 
 template <bool GROUPED>
-bool wsv_set_attr() {
-    bool ok = true;
-#define FK_WSV_ATTR(NFW) ok = ok && cudaFuncSetAttribute(fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fk::WSV_SMEM_BYTES) == cudaSuccess
-    FK_WSV_ATTR(2); FK_WSV_ATTR(3); FK_WSV_ATTR(4); FK_WSV_ATTR(5); FK_WSV_ATTR(6); FK_WSV_ATTR(7); FK_WSV_ATTR(8); FK_WSV_ATTR(9);
-    FK_WSV_ATTR(10); FK_WSV_ATTR(11); FK_WSV_ATTR(12); FK_WSV_ATTR(13); FK_WSV_ATTR(14); FK_WSV_ATTR(15); FK_WSV_ATTR(16);
-#undef FK_WSV_ATTR
-    return ok;
-}
-
-template <bool GROUPED>
-void wsv_launch(const fk::WsVjpParams& w, cudaStream_t s) {
-    const int grid = std::max(1, std::min(w.ntiles, sm_count() * std::max(1, env_int("FKCONV_WSV_CTAS_PER_SM", 1))));
+bool wsv_launch(const fk::WsVjpParams& w, cudaStream_t s) {
+    const int grid = std::max(1, std::min(w.ntiles, sm_count()));
     switch (w.RP / 8) {
-#define FK_WSV_CASE(NFW) case NFW: fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break
+#define FK_WSV_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED>, fk::WSV_SMEM_BYTES)) return false; \
+                                   fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break
         FK_WSV_CASE(2); FK_WSV_CASE(3); FK_WSV_CASE(4); FK_WSV_CASE(5); FK_WSV_CASE(6); FK_WSV_CASE(7); FK_WSV_CASE(8); FK_WSV_CASE(9);
         FK_WSV_CASE(10); FK_WSV_CASE(11); FK_WSV_CASE(12); FK_WSV_CASE(13); FK_WSV_CASE(14); FK_WSV_CASE(15);
         default: FK_WSV_CASE(16);
 #undef FK_WSV_CASE
     }
+    return true;
 }
 
 int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint32_t* kdec, const double* f,
@@ -327,21 +343,15 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
     double* gpart = fT + (size_t)slots * gp.RPmax;
     int nl = 0;
     const bool ws = ws_ok(d, gp.RPmax);
-    if (ws) {
-        static const bool ws_attr = ws_set_attr<false>();
-        if (!ws_attr) return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
-    }
     if (!kdec && !ws) {
         uint32_t* kd = reinterpret_cast<uint32_t*>(gpart + (size_t)gp.ksplit * d.N * gp.RPmax);
         fk::fk_kdec_kernel<<<std::min(1024, (d.K + 255) / 256), 256, 0, s>>>(d, ch, kd);
         ++nl;
         kdec = kd;
     }
-    static const bool attr_ok = [] {
-        return cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess &&
-               cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess;
-    }();
-    if (!attr_ok) return fail(FK_ERR_CUDA, "gemm: cannot reserve %d bytes of shared memory", fk::GEMM_SMEM_BYTES);
+    if (!ws && !(ensure_dyn_smem(fk::fk_gemm_fwd_kernel<2, false>, fk::GEMM_SMEM_BYTES) &&
+                 ensure_dyn_smem(fk::fk_gemm_fwd_kernel<1, false>, fk::GEMM_SMEM_BYTES)))
+        return fail(FK_ERR_CUDA, "gemm: cannot reserve %d bytes of shared memory", fk::GEMM_SMEM_BYTES);
     const int mtiles = (d.N + fk::GEMM_BM - 1) / fk::GEMM_BM;
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
         fk::GemmFwdParams p;
@@ -371,7 +381,8 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
             w.kper = gp.kper;
             w.ksub_rem = gp.ksub_rem;
             const int nfull = d.N / fk::GEMM_BM;
-            ws_launch<false>(w, nfull * gp.ksplit + (d.N % fk::GEMM_BM ? gp.ksplit / gp.ksub_rem : 0), fk::ws_smem_bytes(d.nx, p.RP), s);
+            if (!ws_launch<false>(w, nfull * gp.ksplit + (d.N % fk::GEMM_BM ? gp.ksplit / gp.ksub_rem : 0), fk::ws_smem_bytes(d.nx, p.RP), s))
+                return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
         } else if (d.vec_ok) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_fwd_kernel<1, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         if (timed) g_prof.end(s, slot);
@@ -388,13 +399,11 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
 
 // the single-pass fold (fk_vjp_fold.cuh) serves packed hadronic tables with nx <= 64; others take the gather
 bool fold_ok(const fk::TableDesc& d) {
-    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.nx <= fk::FOLD_MAX_NX && env_int("FKCONV_FOLD", 1);
+    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.nx <= fk::FOLD_MAX_NX && opt(FK_OPT_FOLD);
 }
 // x-row chunks per channel: the CTA count (channels x chunks) that fills whole waves best (1 CTA of 256 threads
 // per SM by registers), preferring fewer chunks (each chunk writes its own B partial)
 int fold_chunks(long long channels) {
-    const int forced = env_int("FKCONV_FOLD_CHUNKS", 0);
-    if (forced > 0) return std::min(8, forced);
     const long long slots = std::max(1, sm_count());
     int best = 1;
     double best_eff = 0.0;
@@ -420,11 +429,9 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
     double* fT = scratch;
     double* gP = fT + (size_t)slots * RPmax;
     double* G = gP + (size_t)d.N * RPmax;
-    static const bool attr_ok = [] {
-        return cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess &&
-               cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess;
-    }();
-    if (!attr_ok) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
+    if (!wsv_ok(d) && !(ensure_dyn_smem(fk::fk_gemm_vjp_kernel<2, false>, fk::GEMMV_SMEM_BYTES) &&
+                        ensure_dyn_smem(fk::fk_gemm_vjp_kernel<1, false>, fk::GEMMV_SMEM_BYTES)))
+        return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
     int nl = 0;
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
         const int RP = fk::gemm_rp8(R - r0);
@@ -441,8 +448,6 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
         p.nfw = (p.nfrag + 1) / 2;
         const int grid = (d.K + fk::GEMMV_BK - 1) / fk::GEMMV_BK;
         if (wsv_ok(d)) {
-            static const bool wsv_attr = wsv_set_attr<false>();
-            if (!wsv_attr) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
             fk::WsVjpParams w;
             memset(&w, 0, sizeof w);
             w.desc = d;
@@ -450,7 +455,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             w.G = G;
             w.RP = RP;
             w.ntiles = grid;
-            wsv_launch<false>(w, s);
+            if (!wsv_launch<false>(w, s)) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
         } else if (d.vec_ok) fk::fk_gemm_vjp_kernel<2, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_vjp_kernel<1, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         if (fold_ok(d)) {
@@ -469,9 +474,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             q.RP = RP;
             q.nchunk = fold_chunks(d.C);
             q.nslots = fk::fold_slots(d.nx, RP, MAX_DYN_SMEM);
-            static const bool fold_attr = cudaFuncSetAttribute(fk::fk_vjp_fold_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                               (int)MAX_DYN_SMEM) == cudaSuccess;
-            if (!fold_attr || q.nslots < 1) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve shared memory for the fold ring");
+            if (!ensure_dyn_smem(fk::fk_vjp_fold_kernel<false>, MAX_DYN_SMEM) || q.nslots < 1) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve shared memory for the fold ring");
             fk::fk_vjp_fold_kernel<false><<<d.C * q.nchunk, fk::FOLD_THREADS,
                                             (size_t)q.nslots * d.nx * RP * 8 + 2 * fk::FOLD_MAX_SLOTS * 8, s>>>(q);
             fk::fk_vjp_fold_final_kernel<double, false><<<slots, fk::GEMM_BN, 0, s>>>(q);
@@ -516,7 +519,7 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
     const int fgrid = pl.nkb * pl.fsplit;
     // few datapoints per range and very many k-blocks: CTAs that walk the k-blocks (fk_fwd_fewrows_kernel)
     const bool fewrows = (d.N + pl.fsplit - 1) / pl.fsplit <= FWD_U && pl.nkb >= 64 * std::max(1, sm_count()) &&
-                         d.vec_ok && env_int("FKCONV_FEWROWS", 1);
+                         d.vec_ok && opt(FK_OPT_FEWROWS);
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
@@ -583,9 +586,8 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
         }
     }
     if (foldk_ok(d)) {
-        static const bool attr_ok = cudaFuncSetAttribute(fk::fk_vjp_foldk_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                         (int)foldk_smem(128)) == cudaSuccess;
-        if (!attr_ok) return fail(FK_ERR_CUDA, "vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
+        if (!ensure_dyn_smem(fk::fk_vjp_foldk_kernel<T, false>, foldk_smem(128)))
+            return fail(FK_ERR_CUDA, "vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
         fk::FoldKParams q;
         memset(&q, 0, sizeof q);
         q.desc = d;
@@ -625,7 +627,7 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
 // scratch: part [N][R][nchunks] | G [fsplit][R][K] | fold partials
 template <typename T>
 bool fused_ok(const fk::TableDesc& d, int R) {
-    return !gemm_wanted<T>(d, R) && foldk_ok(d) && (d.N + d.fsplit - 1) / d.fsplit <= 64 && env_int("FKCONV_FUSED", 1);
+    return !gemm_wanted<T>(d, R) && foldk_ok(d) && (d.N + d.fsplit - 1) / d.fsplit <= 64 && opt(FK_OPT_FUSED);
 }
 size_t fused_scratch_elems(const fk::TableDesc& d, int R) {
     return (part_elems_per_replica(d) + (size_t)d.fsplit * d.K + (1 + FOLDK_MAX_CHUNKS) * (size_t)d.C * d.nx) * R;
@@ -679,9 +681,8 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
         fk::fk_reduce_chunks_kernel<T, false><<<std::max(1, rgrid), 256, 0, s>>>(q);
         ++nl;
     }
-    static const bool attr_ok = cudaFuncSetAttribute(fk::fk_vjp_foldk_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                     (int)foldk_smem(128)) == cudaSuccess;
-    if (!attr_ok) return fail(FK_ERR_CUDA, "conv_vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
+    if (!ensure_dyn_smem(fk::fk_vjp_foldk_kernel<T, false>, foldk_smem(128)))
+        return fail(FK_ERR_CUDA, "conv_vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
     fk::FoldKParams q;
     memset(&q, 0, sizeof q);
     q.desc = d;
@@ -750,7 +751,28 @@ int stateless(const char* who, int kind, bool vjp, const T* fkp, const int32_t* 
 // --------------------------------------------------------------------------------------------------
 // handles
 // --------------------------------------------------------------------------------------------------
+// A handle owns ONE scratch buffer: calls on it are serialised.  Host threads take the handle's mutex for the
+// duration of the (asynchronous) call; on the device every call records an event after its last kernel, and a
+// call that arrives on a different stream first makes that stream wait for it.  While a stream is being captured
+// into a CUDA graph neither happens (one stream per handle inside a capture) and the scratch must not grow.
+struct HandleSync {
+    std::mutex mu;
+    int device = -1;
+    cudaEvent_t done = nullptr;
+    cudaStream_t last = nullptr;
+    bool used = false;
+    int init() {
+        if (cudaGetDevice(&device) != cudaSuccess) return FK_ERR_CUDA;
+        return cudaEventCreateWithFlags(&done, cudaEventDisableTiming) == cudaSuccess ? FK_OK : FK_ERR_CUDA;
+    }
+    void destroy() {
+        if (done) cudaEventDestroy(done);
+        done = nullptr;
+    }
+};
+
 struct fk_table {
+    HandleSync sync;
     fk::TableDesc desc;
     fk::ChannelList chan;
     Plan plan;
@@ -768,8 +790,43 @@ struct fk_table {
 
 namespace {
 
-int ensure_scratch(fk_table* t, size_t elems) {
+bool stream_capturing(cudaStream_t s) {
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    return cudaStreamIsCapturing(s, &st) == cudaSuccess && st != cudaStreamCaptureStatusNone;
+}
+
+// Scope of one compute call on a handle (see HandleSync).
+struct CallGuard {
+    HandleSync& h;
+    cudaStream_t s;
+    bool capturing = false;
+    std::unique_lock<std::mutex> lk;
+    CallGuard(HandleSync& h_, cudaStream_t s_) : h(h_), s(s_), lk(h_.mu) {}
+    int begin(const char* who) {
+        int dev = -1;
+        if (cudaGetDevice(&dev) != cudaSuccess) return fail(FK_ERR_CUDA, "%s: no CUDA device", who);
+        if (dev != h.device)
+            return fail(FK_ERR_INVALID_ARG, "%s: the handle lives on device %d, the current device is %d", who, h.device, dev);
+        capturing = stream_capturing(s);
+        if (!capturing && h.used && h.last != s) {
+            cudaError_t e = cudaStreamWaitEvent(s, h.done, 0);
+            if (e != cudaSuccess) return fail(FK_ERR_CUDA, "%s: cudaStreamWaitEvent: %s", who, cudaGetErrorString(e));
+        }
+        return FK_OK;
+    }
+    ~CallGuard() {
+        if (!capturing && h.done && cudaEventRecord(h.done, s) == cudaSuccess) {
+            h.last = s;
+            h.used = true;
+        }
+    }
+};
+
+int ensure_scratch(fk_table* t, size_t elems, cudaStream_t s = nullptr) {
     if (elems <= t->scratch_elems) return FK_OK;
+    if (stream_capturing(s))
+        return fail(FK_ERR_UNSUPPORTED, "the table's scratch must grow to %zu doubles, which cannot happen during stream capture: "
+                                        "give R_hint at create or make one call outside the capture first", elems);
     if (t->scratch) cudaFree(t->scratch);
     t->scratch = nullptr;
     t->scratch_elems = 0;
@@ -799,7 +856,7 @@ size_t table_scratch_need(const fk_table* t, int R) {
 
 template <typename T, typename TS = T>
 int table_conv_t(fk_table* t, const void* f, void* sigma, int R, cudaStream_t s) {
-    int rc = ensure_scratch(t, table_scratch_need(t, R));
+    int rc = ensure_scratch(t, table_scratch_need(t, R), s);
     if (rc) return rc;
     return run_conv_single<T, TS>(t->desc, t->chan, t->plan, t->kdec, (const T*)f, (T*)sigma, R, t->scratch, s,
                               &t->last_launches);
@@ -807,7 +864,7 @@ int table_conv_t(fk_table* t, const void* f, void* sigma, int R, cudaStream_t s)
 
 template <typename T, typename TS = T>
 int table_vjp_t(fk_table* t, const void* f, const void* g, void* df, int R, cudaStream_t s) {
-    int rc = ensure_scratch(t, table_scratch_need(t, R));
+    int rc = ensure_scratch(t, table_scratch_need(t, R), s);
     if (rc) return rc;
     return run_vjp_single<T, TS>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)df, R, t->scratch, s,
                              &t->last_launches);
@@ -823,7 +880,7 @@ int table_conv_vjp_t(fk_table* t, const void* f, const void* g, void* sigma, voi
         t->last_launches += nl;
         return rc;
     }
-    int rc = ensure_scratch(t, std::max(table_scratch_need(t, R), fused_scratch_elems(t->desc, R)));
+    int rc = ensure_scratch(t, std::max(table_scratch_need(t, R), fused_scratch_elems(t->desc, R)), s);
     if (rc) return rc;
     return run_conv_vjp_fused<T, TS>(t->desc, t->chan, t->plan, (const T*)f, (const T*)g, (T*)sigma, (T*)df, R, t->scratch, s,
                                  &t->last_launches);
@@ -836,6 +893,17 @@ extern "C" {
 const char* fk_last_error_string(void) { return g_err.c_str(); }
 int fk_version(void) { return 100; }
 int fk_compiled_arch(void) { return 100; }
+
+int fk_set_option(int option, int value) {
+    if (option < 0 || option >= FK_OPT_COUNT_) return fail(FK_ERR_INVALID_ARG, "fk_set_option: unknown option %d", option);
+    g_opt[option] = value;
+    return FK_OK;
+}
+int fk_get_option(int option, int* value) {
+    if (option < 0 || option >= FK_OPT_COUNT_ || !value) return fail(FK_ERR_INVALID_ARG, "fk_get_option: bad argument");
+    *value = g_opt[option];
+    return FK_OK;
+}
 
 int fk_profile_enable(int on) {
     std::lock_guard<std::mutex> lk(g_prof.mu);
@@ -913,6 +981,7 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
     if (!t) return fail(FK_ERR_ALLOC, "fk_table_create: host allocation failed");
     rc = fill_channels("fk_table_create", kind, index_list, nfl, C, t->chan);
     if (rc) { delete t; return rc; }
+    if (t->sync.init() != FK_OK) { delete t; return fail(FK_ERR_CUDA, "fk_table_create: no CUDA device"); }
     t->dtype = dtype; t->store = store; t->kind = kind;
 
     const int cstride = (nx * nx + 3) / 4 * 4;  // packed hadronic channel block (fk_common.cuh)
@@ -972,6 +1041,7 @@ int fk_table_destroy(fk_table* t) {
     if (t->scratch) cudaFree(t->scratch);
     if (t->h_stage) cudaFreeHost(t->h_stage);
     if (t->d_stage) cudaFree(t->d_stage);
+    t->sync.destroy();
     delete t;
     return FK_OK;
 }
@@ -991,43 +1061,64 @@ int fk_table_info(const fk_table* t, int* N, int* nx, int* nfl, int* C, int64_t*
     return FK_OK;
 }
 
+}  // extern "C"
+
+namespace {
+// unguarded bodies (the caller holds the handle's CallGuard)
+int table_conv_any(fk_table* t, const void* f, void* sigma, int R, cudaStream_t s) {
+    if (t->dtype == FK_F32S64) return table_conv_t<double, float>(t, f, sigma, R, s);
+    return t->dtype == FK_F64 ? table_conv_t<double>(t, f, sigma, R, s) : table_conv_t<float>(t, f, sigma, R, s);
+}
+int table_vjp_any(fk_table* t, const void* f, const void* g, void* df, int R, cudaStream_t s) {
+    if (t->dtype == FK_F32S64) return table_vjp_t<double, float>(t, f, g, df, R, s);
+    return t->dtype == FK_F64 ? table_vjp_t<double>(t, f, g, df, R, s) : table_vjp_t<float>(t, f, g, df, R, s);
+}
+int chi2_launch(const double* sigma, const double* data, const double* cinv, double* chi2, double* g, int N, int R, cudaStream_t s) {
+    fk::fk_chi2_grad_kernel<<<N, dim3(32, 8), 0, s>>>(sigma, data, cinv, g, N, R);
+    fk::fk_chi2_sum_kernel<<<(R + 7) / 8, 256, 0, s>>>(sigma, data, g, chi2, N, R);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "fk_chi2 launch failed: %s", cudaGetErrorString(e));
+    return FK_OK;
+}
+}  // namespace
+
+extern "C" {
+
 int fk_table_conv(fk_table* t, const void* f, void* sigma, int R, void* stream) {
     g_err.clear();
     if (!t || !f || !sigma) return fail(FK_ERR_INVALID_ARG, "fk_table_conv: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv: R=%d", R);
-    if (t->dtype == FK_F32S64) return table_conv_t<double, float>(t, f, sigma, R, (cudaStream_t)stream);
-    return t->dtype == FK_F64 ? table_conv_t<double>(t, f, sigma, R, (cudaStream_t)stream)
-                              : table_conv_t<float>(t, f, sigma, R, (cudaStream_t)stream);
+    CallGuard cg(t->sync, (cudaStream_t)stream);
+    if (int rc = cg.begin("fk_table_conv")) return rc;
+    return table_conv_any(t, f, sigma, R, (cudaStream_t)stream);
 }
 
 int fk_table_vjp(fk_table* t, const void* f, const void* g, void* df, int R, void* stream) {
     g_err.clear();
     if (!t || !f || !g || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_vjp: R=%d", R);
-    if (t->dtype == FK_F32S64) return table_vjp_t<double, float>(t, f, g, df, R, (cudaStream_t)stream);
-    return t->dtype == FK_F64 ? table_vjp_t<double>(t, f, g, df, R, (cudaStream_t)stream)
-                              : table_vjp_t<float>(t, f, g, df, R, (cudaStream_t)stream);
+    CallGuard cg(t->sync, (cudaStream_t)stream);
+    if (int rc = cg.begin("fk_table_vjp")) return rc;
+    return table_vjp_any(t, f, g, df, R, (cudaStream_t)stream);
 }
 
 int fk_table_conv_vjp(fk_table* t, const void* f, const void* g, void* sigma, void* df, int R, void* stream) {
     g_err.clear();
     if (!t || !f || !g || !sigma || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp: R=%d", R);
-    if (t->dtype == FK_F32S64) return table_conv_vjp_t<double, float>(t, f, g, sigma, df, R, (cudaStream_t)stream);
-    return t->dtype == FK_F64 ? table_conv_vjp_t<double>(t, f, g, sigma, df, R, (cudaStream_t)stream)
-                              : table_conv_vjp_t<float>(t, f, g, sigma, df, R, (cudaStream_t)stream);
+    cudaStream_t s = (cudaStream_t)stream;
+    CallGuard cg(t->sync, s);
+    if (int rc = cg.begin("fk_table_conv_vjp")) return rc;
+    if (t->dtype == FK_F32S64) return table_conv_vjp_t<double, float>(t, f, g, sigma, df, R, s);
+    return t->dtype == FK_F64 ? table_conv_vjp_t<double>(t, f, g, sigma, df, R, s)
+                              : table_conv_vjp_t<float>(t, f, g, sigma, df, R, s);
 }
 
 int fk_chi2(const double* sigma, const double* data, const double* cinv, double* chi2, double* g, int N, int R, void* stream) {
     g_err.clear();
     if (!sigma || !data || !cinv || !chi2 || !g) return fail(FK_ERR_INVALID_ARG, "fk_chi2: null pointer");
     if (N <= 0 || R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_chi2: non-positive size (N=%d R=%d)", N, R);
-    cudaStream_t s = (cudaStream_t)stream;
-    fk::fk_chi2_grad_kernel<<<N, dim3(32, 8), 0, s>>>(sigma, data, cinv, g, N, R);
-    fk::fk_chi2_sum_kernel<<<(R + 7) / 8, 256, 0, s>>>(sigma, data, g, chi2, N, R);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "fk_chi2 launch failed: %s", cudaGetErrorString(e));
-    return FK_OK;
+    return chi2_launch(sigma, data, cinv, chi2, g, N, R, (cudaStream_t)stream);
 }
 
 int fk_table_fit_step(fk_table* t, const double* f, const double* data, const double* cinv, double* sigma, double* g,
@@ -1035,12 +1126,16 @@ int fk_table_fit_step(fk_table* t, const double* f, const double* data, const do
     g_err.clear();
     if (!t || !f || !data || !cinv || !sigma || !g || !chi2 || !df) return fail(FK_ERR_INVALID_ARG, "fk_table_fit_step: null pointer");
     if (t->dtype == FK_F32) return fail(FK_ERR_UNSUPPORTED, "fk_table_fit_step: tables with fp64 buffers only (FK_F64, FK_F32S64)");
-    int rc = fk_table_conv(t, f, sigma, R, stream);
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_fit_step: R=%d", R);
+    cudaStream_t s = (cudaStream_t)stream;
+    CallGuard cg(t->sync, s);
+    if (int rc = cg.begin("fk_table_fit_step")) return rc;
+    int rc = table_conv_any(t, f, sigma, R, s);
     if (rc) return rc;
     const int nl = t->last_launches;
-    rc = fk_chi2(sigma, data, cinv, chi2, g, t->desc.N, R, stream);
+    rc = chi2_launch(sigma, data, cinv, chi2, g, t->desc.N, R, s);
     if (rc) return rc;
-    rc = fk_table_vjp(t, f, g, df, R, stream);
+    rc = table_vjp_any(t, f, g, df, R, s);
     t->last_launches += nl + 2;
     return rc;
 }
@@ -1052,13 +1147,15 @@ int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R,
     const size_t es = io_size(t->dtype);
     const size_t fb = (size_t)R * t->desc.nfl * t->desc.nx * es, sb = (size_t)t->desc.N * R * es;
     const size_t fb_al = (fb + 255) / 256 * 256;
+    cudaStream_t s = (cudaStream_t)stream;
+    CallGuard cg(t->sync, s);
+    if (int rc0 = cg.begin("fk_table_conv_host")) return rc0;
     int rc = ensure_stage(t, 2 * fb_al + 2 * ((sb + 255) / 256 * 256));
     if (rc) return rc;
-    cudaStream_t s = (cudaStream_t)stream;
     char* h = (char*)t->h_stage; char* d = (char*)t->d_stage;
     memcpy(h, f_host, fb);
     FK_CUDA(cudaMemcpyAsync(d, h, fb, cudaMemcpyHostToDevice, s));
-    rc = fk_table_conv(t, d, d + fb_al, R, stream);
+    rc = table_conv_any(t, d, d + fb_al, R, s);
     if (rc) return rc;
     FK_CUDA(cudaMemcpyAsync(h + fb_al, d + fb_al, sb, cudaMemcpyDeviceToHost, s));
     FK_CUDA(cudaStreamSynchronize(s));
@@ -1073,14 +1170,16 @@ int fk_table_vjp_host(fk_table* t, const void* f_host, const void* g_host, void*
     const size_t es = io_size(t->dtype);
     const size_t fb = (size_t)R * t->desc.nfl * t->desc.nx * es, gb = (size_t)t->desc.N * R * es;
     const size_t fb_al = (fb + 255) / 256 * 256, gb_al = (gb + 255) / 256 * 256;
+    cudaStream_t s = (cudaStream_t)stream;
+    CallGuard cg(t->sync, s);
+    if (int rc0 = cg.begin("fk_table_vjp_host")) return rc0;
     int rc = ensure_stage(t, 2 * fb_al + 2 * gb_al);
     if (rc) return rc;
-    cudaStream_t s = (cudaStream_t)stream;
     char* h = (char*)t->h_stage; char* d = (char*)t->d_stage;
     memcpy(h, f_host, fb);
     memcpy(h + fb_al, g_host, gb);
     FK_CUDA(cudaMemcpyAsync(d, h, fb_al + gb, cudaMemcpyHostToDevice, s));
-    rc = fk_table_vjp(t, d, d + fb_al, d + fb_al + gb_al, R, stream);
+    rc = table_vjp_any(t, d, d + fb_al, d + fb_al + gb_al, R, s);
     if (rc) return rc;
     FK_CUDA(cudaMemcpyAsync(h + fb_al + gb_al, d + fb_al + gb_al, fb, cudaMemcpyDeviceToHost, s));
     FK_CUDA(cudaStreamSynchronize(s));

@@ -412,6 +412,24 @@ fk_gemm_vjp_kernel(const __grid_constant__ GemmVjpParams p) {
         if (s < nt) load_stage(s);
         cp_async_commit();
     }
+    // bounded chains: every GEMM_FLUSH stages (512 datapoints) the register tile is added into this CTA's own G tile
+    auto flushG = [&](bool first) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int k = k0 + wm * 32 + i * 8 + (lane >> 2);
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (j < nfw) {
+                    if (k < d.K) {
+                        double2* q = reinterpret_cast<double2*>(G + (long long)k * p.RP + cb + j * 8 + 2 * (lane & 3));
+                        const double2 o = first ? make_double2(0.0, 0.0) : *q;
+                        *q = make_double2(acc[i][j][0] + o.x, acc[i][j][1] + o.y);
+                    }
+                    acc[i][j][0] = acc[i][j][1] = 0.0;
+                }
+        }
+    };
+    bool flushed = false;
     for (int t = 0; t < nt; ++t) {
         cp_async_wait<GEMMV_STAGES - 2>();
         __syncthreads();
@@ -434,18 +452,12 @@ fk_gemm_vjp_kernel(const __grid_constant__ GemmVjpParams p) {
                     for (int i = 0; i < 4; ++i) dmma884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
                 }
         }
+        if ((t + 1) % GEMM_FLUSH == 0 && t + 1 < nt) {
+            flushG(!flushed);
+            flushed = true;
+        }
     }
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int k = k0 + wm * 32 + i * 8 + (lane >> 2);
-        if (k >= d.K) continue;
-#pragma unroll
-        for (int j = 0; j < 8; ++j)
-            if (j < nfw) {
-                const int c = cb + j * 8 + 2 * (lane & 3);
-                *reinterpret_cast<double2*>(G + (long long)k * p.RP + c) = make_double2(acc[i][j][0], acc[i][j][1]);
-            }
-    }
+    flushG(!flushed);
 }
 
 // gP[n][c] = g[n][r0 + c] (zero beyond R)

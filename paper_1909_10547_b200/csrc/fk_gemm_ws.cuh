@@ -423,7 +423,27 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int j = 0; j < NFW; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-        for (int n0 = 0; n0 < d->N; n0 += GEMMV_NT, ++it) {
+        // bounded chains: every GEMM_FLUSH stages (512 datapoints) the register tile is added
+        // into this CTA's own G tile (thread-private addresses, L2 resident) and cleared, as the forward kernel does
+        const int k0 = kt * GEMMV_BK;
+        auto flushG = [&](bool first) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int k = k0 + wm * 32 + i * 8 + (lane >> 2);
+#pragma unroll
+                for (int j = 0; j < NFW; ++j) {
+                    if (k < d->K) {
+                        double2* q = reinterpret_cast<double2*>(G + (long long)k * RP + cbcol + j * 8 + 2 * (lane & 3));
+                        const double2 o = first ? make_double2(0.0, 0.0) : *q;
+                        *q = make_double2(acc[i][j][0] + o.x, acc[i][j][1] + o.y);
+                    }
+                    acc[i][j][0] = acc[i][j][1] = 0.0;
+                }
+            }
+        };
+        bool flushed = false;
+        int nst = 0;
+        for (int n0 = 0; n0 < d->N; n0 += GEMMV_NT, ++it, ++nst) {
             const int stage = it % GEMMV_STAGES, rows = min(GEMMV_NT, d->N - n0);
             mbar_wait(bar_full(stage), (it / GEMMV_STAGES) & 1);
             // A fragment: row m = k (lane >> 2), col = datapoint (lane & 3)  ->  As[n][k]
@@ -458,17 +478,12 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty(stage));
-        }
-        const int k0 = kt * GEMMV_BK;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int k = k0 + wm * 32 + i * 8 + (lane >> 2);
-            if (k < d->K) {
-#pragma unroll
-                for (int j = 0; j < NFW; ++j)
-                    *reinterpret_cast<double2*>(G + (long long)k * RP + cbcol + j * 8 + 2 * (lane & 3)) = make_double2(acc[i][j][0], acc[i][j][1]);
+            if ((nst + 1) % GEMM_FLUSH == 0 && n0 + GEMMV_NT < d->N) {
+                flushG(!flushed);
+                flushed = true;
             }
         }
+        flushG(!flushed);
     }
     };
     if (warp < 4) consume(std::integral_constant<int, NFW0>{});

@@ -6,6 +6,7 @@
 // a fixed slot and every sum a fixed order, so results are bitwise repeatable.
 
 struct fk_group {
+    HandleSync sync;
     std::vector<fk_table*> tables;
     std::vector<fk::TableDesc> descs;  // host copies with the concatenation offsets filled in
     int T = 0, dtype = FK_F64;
@@ -44,8 +45,11 @@ struct fk_group {
 
 namespace {
 
-int group_scratch(fk_group* g, size_t elems) {
+int group_scratch(fk_group* g, size_t elems, cudaStream_t s = nullptr) {
     if (elems <= g->scratch_elems) return FK_OK;
+    if (stream_capturing(s))
+        return fail(FK_ERR_UNSUPPORTED, "the group's scratch must grow to %zu doubles, which cannot happen during stream capture: "
+                                        "give R_hint at create or make one call outside the capture first", elems);
     if (g->scratch) cudaFree(g->scratch);
     g->scratch = nullptr;
     g->scratch_elems = 0;
@@ -55,7 +59,7 @@ int group_scratch(fk_group* g, size_t elems) {
 }
 
 bool group_gemm_wanted(const fk_group* g, int R) {
-    return g->gemm_ok && g->dtype == FK_F64 && R >= env_int("FKCONV_GEMM_MIN_R", g->ws_all ? 5 : 13);
+    return g->gemm_ok && g->dtype == FK_F64 && R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : g->ws_all ? 5 : 13);
 }
 
 size_t group_scratch_need(const fk_group* g, int R) {
@@ -72,11 +76,8 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
     const int RPmax = fk::gemm_rp(R);
     double* fT = g->scratch;
     double* gpart = fT + (size_t)g->ai_total * RPmax;
-    static const bool attr_ok = [] {
-        return cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess &&
-               cudaFuncSetAttribute(fk::fk_gemm_fwd_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMM_SMEM_BYTES) == cudaSuccess;
-    }();
-    if (!attr_ok) return fail(FK_ERR_CUDA, "grouped gemm: cannot reserve %d bytes of shared memory", fk::GEMM_SMEM_BYTES);
+    if (!(ensure_dyn_smem(fk::fk_gemm_fwd_kernel<2, true>, fk::GEMM_SMEM_BYTES) && ensure_dyn_smem(fk::fk_gemm_fwd_kernel<1, true>, fk::GEMM_SMEM_BYTES)))
+        return fail(FK_ERR_CUDA, "grouped gemm: cannot reserve %d bytes of shared memory", fk::GEMM_SMEM_BYTES);
     int nl = 0;
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
         fk::GemmFwdParams p;
@@ -92,9 +93,7 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
         fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
             f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, p.RP);
         const size_t ws_smem = fk::ws_smem_bytes(g->nx_max, p.RP);
-        if (g->ws_all && env_int("FKCONV_WS", 1) && ws_smem <= MAX_DYN_SMEM) {
-            static const bool ws_attr = ws_set_attr<true>();
-            if (!ws_attr) return fail(FK_ERR_CUDA, "grouped gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
+        if (g->ws_all && opt(FK_OPT_WARP_SPEC) && ws_smem <= MAX_DYN_SMEM) {
             fk::WsFwdParams w;
             memset(&w, 0, sizeof w);
             w.fT = fT;
@@ -102,7 +101,8 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
             w.RP = p.RP;
             w.descs = g->d_descs;
             w.items = g->d_witems;
-            ws_launch<true>(w, g->nwitems, ws_smem, s);
+            if (!ws_launch<true>(w, g->nwitems, ws_smem, s))
+                return fail(FK_ERR_CUDA, "grouped gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
         } else if (g->all_vec) fk::fk_gemm_fwd_kernel<2, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_fwd_kernel<1, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         const long long outs = g->rows_total * p.RP;
@@ -121,11 +121,8 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
     double* fT = g->scratch;
     double* gP = fT + (size_t)g->ai_total * RPmax;
     double* G = gP + (size_t)g->rows_total * RPmax;
-    static const bool attr_ok = [] {
-        return cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess &&
-               cudaFuncSetAttribute(fk::fk_gemm_vjp_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fk::GEMMV_SMEM_BYTES) == cudaSuccess;
-    }();
-    if (!attr_ok) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
+    if (!(ensure_dyn_smem(fk::fk_gemm_vjp_kernel<2, true>, fk::GEMMV_SMEM_BYTES) && ensure_dyn_smem(fk::fk_gemm_vjp_kernel<1, true>, fk::GEMMV_SMEM_BYTES)))
+        return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
     int nl = 0;
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
         const int RP = fk::gemm_rp8(R - r0);
@@ -144,8 +141,6 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
         p.descs = g->d_descs;
         p.items = g->d_vitems;
         if (g->wsv_all) {
-            static const bool wsv_attr = wsv_set_attr<true>();
-            if (!wsv_attr) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
             fk::WsVjpParams w;
             memset(&w, 0, sizeof w);
             w.gP = gP;
@@ -154,7 +149,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             w.ntiles = g->nvitems;
             w.descs = g->d_descs;
             w.items = g->d_vitems;
-            wsv_launch<true>(w, s);
+            if (!wsv_launch<true>(w, s)) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
         } else if (g->all_vec) fk::fk_gemm_vjp_kernel<2, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         else fk::fk_gemm_vjp_kernel<1, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         if (g->fold_all) {
@@ -174,9 +169,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             q.ai_prefix = g->d_ai_prefix;
             q.T = g->T;
             q.nslots = fk::fold_slots(g->nx_max, RP, MAX_DYN_SMEM);
-            static const bool fold_attr = cudaFuncSetAttribute(fk::fk_vjp_fold_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                               (int)MAX_DYN_SMEM) == cudaSuccess;
-            if (!fold_attr || q.nslots < 1) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve shared memory for the fold ring");
+            if (!ensure_dyn_smem(fk::fk_vjp_fold_kernel<true>, MAX_DYN_SMEM) || q.nslots < 1) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve shared memory for the fold ring");
             fk::fk_vjp_fold_kernel<true><<<g->nfoitems, fk::FOLD_THREADS,
                                            (size_t)q.nslots * g->nx_max * RP * 8 + 2 * fk::FOLD_MAX_SLOTS * 8, s>>>(q);
             fk::fk_vjp_fold_final_kernel<double, true><<<(unsigned)g->ai_total, fk::GEMM_BN, 0, s>>>(q);
@@ -205,7 +198,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
 
 template <typename T, typename TS = T>
 int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStream_t s) {
-    int rc = group_scratch(g, group_scratch_need(g, R));
+    int rc = group_scratch(g, group_scratch_need(g, R), s);
     if (rc) return rc;
     if constexpr (std::is_same<T, double>::value) {
         if (group_gemm_wanted(g, R)) return group_conv_gemm(g, (const double*)f_cat, (double*)sigma_cat, R, s);
@@ -250,7 +243,7 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
 
 template <typename T, typename TS = T>
 int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat, int R, cudaStream_t s) {
-    int rc = group_scratch(g, group_scratch_need(g, R));
+    int rc = group_scratch(g, group_scratch_need(g, R), s);
     if (rc) return rc;
     if constexpr (std::is_same<T, double>::value) {
         if (group_gemm_wanted(g, R))
@@ -273,9 +266,8 @@ int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat,
         r0 += rt;
     }
     if (g->foldk_all) {
-        static const bool attr_ok = cudaFuncSetAttribute(fk::fk_vjp_foldk_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                         (int)foldk_smem(128)) == cudaSuccess;
-        if (!attr_ok) return fail(FK_ERR_CUDA, "grouped vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
+        if (!ensure_dyn_smem(fk::fk_vjp_foldk_kernel<T, true>, foldk_smem(128)))
+            return fail(FK_ERR_CUDA, "grouped vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
         fk::FoldKParams q;
         memset(&q, 0, sizeof q);
         q.descs = g->d_descs;
@@ -327,10 +319,15 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     if (!g) return fail(FK_ERR_ALLOC, "fk_group_create: host allocation failed");
     g->T = T;
     g->dtype = tables[0]->dtype;
+    if (g->sync.init() != FK_OK) { delete g; return fail(FK_ERR_CUDA, "fk_group_create: no CUDA device"); }
     std::vector<int> row_prefix(T + 1, 0), ai_prefix(T + 1, 0);
     for (int t = 0; t < T; ++t) {
         fk_table* tb = tables[t];
-        if (tb->dtype != g->dtype) { delete g; return fail(FK_ERR_INVALID_ARG, "fk_group_create: mixed dtypes"); }
+        if (tb->dtype != g->dtype) { g->sync.destroy(); delete g; return fail(FK_ERR_INVALID_ARG, "fk_group_create: mixed dtypes"); }
+        if (tb->sync.device != g->sync.device) {
+            g->sync.destroy(); delete g;
+            return fail(FK_ERR_INVALID_ARG, "fk_group_create: table %d lives on device %d, the current device is %d", t, tb->sync.device, g->sync.device);
+        }
         g->all_vec = g->all_vec && tb->desc.vec_ok;
     }
     // R >> 1 contraction: every item (128-datapoint tile x K range) costs about the same DMMA time
@@ -340,7 +337,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
         g->gemm_ok = g->gemm_ok && tables[t]->kdec != nullptr;
         tile_k += (long long)((tables[t]->desc.N + fk::GEMM_BM - 1) / fk::GEMM_BM) * tables[t]->desc.K;
     }
-    const long long want_items = (long long)std::max(1, sm_count()) * std::max(1, env_int("FKCONV_GROUP_GEMM_WAVES", 16));
+    const long long want_items = (long long)std::max(1, sm_count()) * GROUP_GEMM_WAVES;
     long long kper_target = (tile_k + want_items - 1) / want_items;
     kper_target = std::max<long long>(fk::GEMM_KT * 8, (kper_target + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT);
     std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems, foitems, witems, kitems;
@@ -399,7 +396,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
         {   // VJP stage 1: the GROUP has to fill the GPU, not every table on its own -- fewer datapoint ranges per
             // k-block mean fewer column-sum slices G[nsplit][R][K] to write and to gather (a table planned alone asks
             // for ~24 CTAs per SM and gets up to N/16 slices)
-            const long long want = (long long)env_int("FKCONV_COLSUM_CTAS_PER_SM", 24) * std::max(1, sm_count());
+            const long long want = (long long)COLSUM_CTAS_PER_SM * std::max(1, sm_count());
             int ns = (int)std::min<long long>(std::max<long long>(1, (want + group_kblocks - 1) / std::max<long long>(1, group_kblocks)),
                                               std::max(1, d.N / 16));
             ns = std::max(ns, (d.N + fk::COLSUM_MAX_ROWS - 1) / fk::COLSUM_MAX_ROWS);
@@ -425,6 +422,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
         g->descs.push_back(d);
     }
     if (g->rows_total >= (1LL << 31) || g->ai_total >= (1LL << 31)) {
+        g->sync.destroy();
         delete g;
         return fail(FK_ERR_UNSUPPORTED, "fk_group_create: more than 2^31 datapoints or PDF slots");
     }
@@ -476,6 +474,7 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_kitems) cudaFree(g->d_kitems);
     if (g->d_witems) cudaFree(g->d_witems);
     if (g->scratch) cudaFree(g->scratch);
+    g->sync.destroy();
     delete g;
     return FK_OK;
 }
@@ -495,6 +494,8 @@ int fk_conv_grouped(fk_group* g, const void* f_cat, void* sigma_cat, int R, void
     g_err.clear();
     if (!g || !f_cat || !sigma_cat) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped: R=%d", R);
+    CallGuard cg(g->sync, (cudaStream_t)stream);
+    if (int rc = cg.begin("fk_conv_grouped")) return rc;
     if (g->dtype == FK_F32S64) return group_conv_t<double, float>(g, f_cat, sigma_cat, R, (cudaStream_t)stream);
     return g->dtype == FK_F64 ? group_conv_t<double>(g, f_cat, sigma_cat, R, (cudaStream_t)stream)
                               : group_conv_t<float>(g, f_cat, sigma_cat, R, (cudaStream_t)stream);
@@ -504,6 +505,8 @@ int fk_conv_grouped_vjp(fk_group* g, const void* f_cat, const void* g_cat, void*
     g_err.clear();
     if (!g || !f_cat || !g_cat || !df_cat) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped_vjp: null pointer");
     if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped_vjp: R=%d", R);
+    CallGuard cg(g->sync, (cudaStream_t)stream);
+    if (int rc = cg.begin("fk_conv_grouped_vjp")) return rc;
     if (g->dtype == FK_F32S64) return group_vjp_t<double, float>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream);
     return g->dtype == FK_F64 ? group_vjp_t<double>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream)
                               : group_vjp_t<float>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream);

@@ -22,10 +22,12 @@ FK_OK, FK_ERR_INVALID_ARG, FK_ERR_ALLOC, FK_ERR_CUDA, FK_ERR_UNSUPPORTED = 0, -1
 FK_KIND_DIS, FK_KIND_HADRONIC = 0, 1
 FK_F64, FK_F32, FK_F32S64 = 0, 1, 2
 FK_STORE_BORROW, FK_STORE_PACK = 0, 1
+(FK_OPT_GEMM_MIN_R, FK_OPT_WARP_SPEC, FK_OPT_FOLD, FK_OPT_FOLDK, FK_OPT_FUSED, FK_OPT_FEWROWS, FK_OPT_TC32,
+ FK_OPT_TC32_MIN_R) = range(8)
 
 # every symbol include/fkconv.h declares
 SYMBOLS = (
-    "fk_last_error_string", "fk_version", "fk_compiled_arch", "fk_profile_enable", "fk_profile_read",
+    "fk_last_error_string", "fk_version", "fk_compiled_arch", "fk_profile_enable", "fk_profile_read", "fk_set_option", "fk_get_option",
     "fk_conv_dis", "fk_conv_hadronic", "fk_conv_hadronic_vjp", "fk_conv_dis_vjp",
     "fk_conv_dis_f32", "fk_conv_hadronic_f32", "fk_conv_hadronic_vjp_f32",
     "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp", "fk_table_conv_vjp", "fk_chi2", "fk_table_fit_step",
@@ -50,6 +52,8 @@ for _name in ("fk_conv_dis", "fk_conv_hadronic", "fk_conv_dis_f32", "fk_conv_had
 for _name in ("fk_conv_hadronic_vjp", "fk_conv_dis_vjp", "fk_conv_hadronic_vjp_f32"):
     getattr(lib, _name).argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
 lib.fk_profile_enable.argtypes = [_ci]
+lib.fk_set_option.argtypes = [_ci, _ci]
+lib.fk_get_option.argtypes = [_ci, ctypes.POINTER(_ci)]
 lib.fk_profile_read.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(_ci)]
 lib.fk_table_create.argtypes = [ctypes.POINTER(_vp), _ci, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _ci, _ci]
 lib.fk_table_destroy.argtypes = [_vp]
@@ -96,12 +100,38 @@ def _dev(t: torch.Tensor, dtype=None) -> int:
     return t.data_ptr()
 
 
+def _shape(t, shape, what: str, device=None) -> None:
+    """Marshalling check: the kernels trust the sizes the handle was created with."""
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{what}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    if device is not None and isinstance(t, torch.Tensor) and t.device != device:
+        raise ValueError(f"{what}: tensor on {t.device}, table on {device}")
+
+
+def _host(a, dtype, shape, what: str) -> int:
+    if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous):
+        raise TypeError(f"{what}: expected a C-contiguous numpy array of dtype {np.dtype(dtype)}")
+    if tuple(a.shape) != tuple(shape):
+        raise ValueError(f"{what}: expected shape {tuple(shape)}, got {tuple(a.shape)}")
+    return a.ctypes.data
+
+
 def _idx(a) -> np.ndarray:
     return np.ascontiguousarray(a, dtype=np.int32)
 
 
 def _hostptr(a: np.ndarray) -> int:
     return a.ctypes.data
+
+
+def set_option(option: int, value: int) -> None:
+    _check(lib.fk_set_option(option, value), "fk_set_option")
+
+
+def get_option(option: int) -> int:
+    v = _ci()
+    _check(lib.fk_get_option(option, ctypes.byref(v)), "fk_get_option")
+    return v.value
 
 
 def version() -> int:
@@ -120,6 +150,7 @@ def fk_conv_hadronic(fk, pairs, f, sigma=None, stream=None):
     pairs = _idx(pairs)
     if sigma is None:
         sigma = torch.empty((N, R), dtype=fk.dtype, device=fk.device)
+    _shape(pairs, (C, 2), "pairs"); _shape(f, (R, nfl, nx), "f", fk.device); _shape(sigma, (N, R), "sigma", fk.device)
     fn = lib.fk_conv_hadronic if fk.dtype == torch.float64 else lib.fk_conv_hadronic_f32
     _check(fn(_dev(fk), _hostptr(pairs), _dev(f, fk.dtype), _dev(sigma, fk.dtype), N, nx, nfl, C, R,
               _stream(stream)), "fk_conv_hadronic")
@@ -133,6 +164,7 @@ def fk_conv_dis(fk, flav, f, sigma=None, stream=None):
     flav = _idx(flav)
     if sigma is None:
         sigma = torch.empty((N, R), dtype=fk.dtype, device=fk.device)
+    _shape(flav, (nA,), "flav"); _shape(f, (R, nfl, nx), "f", fk.device); _shape(sigma, (N, R), "sigma", fk.device)
     fn = lib.fk_conv_dis if fk.dtype == torch.float64 else lib.fk_conv_dis_f32
     _check(fn(_dev(fk), _hostptr(flav), _dev(f, fk.dtype), _dev(sigma, fk.dtype), N, nx, nfl, nA, R,
               _stream(stream)), "fk_conv_dis")
@@ -146,6 +178,8 @@ def fk_conv_hadronic_vjp(fk, pairs, f, g, df=None, stream=None):
     pairs = _idx(pairs)
     if df is None:
         df = torch.empty_like(f)
+    _shape(pairs, (C, 2), "pairs"); _shape(f, (R, nfl, nx), "f", fk.device); _shape(g, (N, R), "g", fk.device)
+    _shape(df, (R, nfl, nx), "df", fk.device)
     fn = lib.fk_conv_hadronic_vjp if fk.dtype == torch.float64 else lib.fk_conv_hadronic_vjp_f32
     _check(fn(_dev(fk), _hostptr(pairs), _dev(f, fk.dtype), _dev(g, fk.dtype), _dev(df, fk.dtype),
               N, nx, nfl, C, R, _stream(stream)), "fk_conv_hadronic_vjp")
@@ -158,6 +192,8 @@ def fk_conv_dis_vjp(fk, flav, f, g, df=None, stream=None):
     flav = _idx(flav)
     if df is None:
         df = torch.empty_like(f)
+    _shape(flav, (nA,), "flav"); _shape(f, (R, nfl, nx), "f", fk.device); _shape(g, (N, R), "g", fk.device)
+    _shape(df, (R, nfl, nx), "df", fk.device)
     _check(lib.fk_conv_dis_vjp(_dev(fk, torch.float64), _hostptr(flav), _dev(f, torch.float64),
                                _dev(g, torch.float64), _dev(df, torch.float64), N, nx, nfl, nA, R,
                                _stream(stream)), "fk_conv_dis_vjp")
@@ -171,6 +207,8 @@ def fk_chi2(sigma, data, cinv, chi2=None, g=None, stream=None):
         chi2 = torch.empty(R, dtype=torch.float64, device=sigma.device)
     if g is None:
         g = torch.empty_like(sigma)
+    _shape(data, (N,), "data", sigma.device); _shape(cinv, (N, N), "cinv", sigma.device)
+    _shape(chi2, (R,), "chi2", sigma.device); _shape(g, (N, R), "g", sigma.device)
     _check(lib.fk_chi2(_dev(sigma, torch.float64), _dev(data, torch.float64), _dev(cinv, torch.float64),
                        _dev(chi2, torch.float64), _dev(g, torch.float64), N, R, _stream(stream)), "fk_chi2")
     return chi2, g
@@ -188,9 +226,11 @@ class FkTable:
             N, nx, _, C = fk_logical.shape
         else:
             N, nx, C = fk_logical.shape
+        _shape(idx, (C, 2) if kind == FK_KIND_HADRONIC else (C,), "index_list")
         self.N, self.nx, self.nfl, self.C = N, nx, nfl, C
         self.dtype = dtype
         self.tdtype = torch.float32 if dtype == FK_F32 else torch.float64  # FK_F32S64: fp32 table, fp64 buffers
+        self.ndtype = np.float32 if dtype == FK_F32 else np.float64
         self.device = fk_logical.device
         self._keep = fk_logical if store == FK_STORE_BORROW else None
         h = _vp()
@@ -205,10 +245,17 @@ class FkTable:
         return dict(N=N.value, nx=nx.value, nfl=nfl.value, C=C.value, K=K.value, row_stride=rs.value,
                     device_bytes=nb.value)
 
+    def _chk(self, R, f=None, sigma=None, g=None, df=None):
+        for t, shape, what in ((f, (R, self.nfl, self.nx), "f"), (sigma, (self.N, R), "sigma"), (g, (self.N, R), "g"),
+                               (df, (R, self.nfl, self.nx), "df")):
+            if t is not None:
+                _shape(t, shape, what, self.device)
+
     def conv(self, f, sigma=None, stream=None):
         R = f.shape[0]
         if sigma is None:
             sigma = torch.empty((self.N, R), dtype=self.tdtype, device=self.device)
+        self._chk(R, f=f, sigma=sigma)
         _check(lib.fk_table_conv(self.handle, _dev(f, self.tdtype), _dev(sigma, self.tdtype), R,
                                  _stream(stream)), "fk_table_conv")
         return sigma
@@ -217,6 +264,7 @@ class FkTable:
         R = f.shape[0]
         if df is None:
             df = torch.empty_like(f)
+        self._chk(R, f=f, g=g, df=df)
         _check(lib.fk_table_vjp(self.handle, _dev(f, self.tdtype), _dev(g, self.tdtype), _dev(df, self.tdtype),
                                 R, _stream(stream)), "fk_table_vjp")
         return df
@@ -228,6 +276,7 @@ class FkTable:
             sigma = torch.empty((self.N, R), dtype=self.tdtype, device=self.device)
         if df is None:
             df = torch.empty_like(f)
+        self._chk(R, f=f, sigma=sigma, g=g, df=df)
         _check(lib.fk_table_conv_vjp(self.handle, _dev(f, self.tdtype), _dev(g, self.tdtype), _dev(sigma, self.tdtype),
                                      _dev(df, self.tdtype), R, _stream(stream)), "fk_table_conv_vjp")
         return sigma, df
@@ -239,6 +288,9 @@ class FkTable:
         g = torch.empty_like(sigma) if g is None else g
         chi2 = torch.empty(R, dtype=torch.float64, device=self.device) if chi2 is None else chi2
         df = torch.empty_like(f) if df is None else df
+        self._chk(R, f=f, sigma=sigma, g=g, df=df)
+        _shape(data, (self.N,), "data", self.device); _shape(cinv, (self.N, self.N), "cinv", self.device)
+        _shape(chi2, (R,), "chi2", self.device)
         _check(lib.fk_table_fit_step(self.handle, _dev(f, torch.float64), _dev(data, torch.float64), _dev(cinv, torch.float64),
                                      _dev(sigma, torch.float64), _dev(g, torch.float64), _dev(chi2, torch.float64),
                                      _dev(df, torch.float64), R, _stream(stream)), "fk_table_fit_step")
@@ -246,14 +298,18 @@ class FkTable:
 
     def conv_host(self, f_host: np.ndarray, sigma_host: np.ndarray, stream=None):
         R = f_host.shape[0]
-        _check(lib.fk_table_conv_host(self.handle, _hostptr(f_host), _hostptr(sigma_host), R, _stream(stream)),
+        fp = _host(f_host, self.ndtype, (R, self.nfl, self.nx), "f_host")
+        sp = _host(sigma_host, self.ndtype, (self.N, R), "sigma_host")
+        _check(lib.fk_table_conv_host(self.handle, fp, sp, R, _stream(stream)),
                "fk_table_conv_host")
         return sigma_host
 
     def vjp_host(self, f_host: np.ndarray, g_host: np.ndarray, df_host: np.ndarray, stream=None):
         R = f_host.shape[0]
-        _check(lib.fk_table_vjp_host(self.handle, _hostptr(f_host), _hostptr(g_host), _hostptr(df_host), R,
-                                     _stream(stream)), "fk_table_vjp_host")
+        fp = _host(f_host, self.ndtype, (R, self.nfl, self.nx), "f_host")
+        gp = _host(g_host, self.ndtype, (self.N, R), "g_host")
+        dp = _host(df_host, self.ndtype, (R, self.nfl, self.nx), "df_host")
+        _check(lib.fk_table_vjp_host(self.handle, fp, gp, dp, R, _stream(stream)), "fk_table_vjp_host")
         return df_host
 
     def last_launches(self) -> int:
@@ -291,10 +347,21 @@ class FkGroup:
         _check(lib.fk_group_offsets(self.handle, R, _hostptr(fo), _hostptr(so)), "fk_group_offsets")
         return fo, so
 
+    def _chk(self, R, f_cat=None, sigma_cat=None, g_cat=None, df_cat=None):
+        fo, so = self.offsets(R)
+        for t, n, what in ((f_cat, fo[-1], "f_cat"), (df_cat, fo[-1], "df_cat"), (sigma_cat, so[-1], "sigma_cat"),
+                           (g_cat, so[-1], "g_cat")):
+            if t is not None:
+                if t.numel() != int(n):
+                    raise ValueError(f"{what}: expected {int(n)} elements (fk_group_offsets), got {t.numel()}")
+                if t.device != self.device:
+                    raise ValueError(f"{what}: tensor on {t.device}, group on {self.device}")
+
     def conv(self, f_cat, R, sigma_cat=None, stream=None):
         if sigma_cat is None:
             _, so = self.offsets(R)
             sigma_cat = torch.empty(int(so[-1]), dtype=self.tdtype, device=self.device)
+        self._chk(R, f_cat=f_cat, sigma_cat=sigma_cat)
         _check(lib.fk_conv_grouped(self.handle, _dev(f_cat, self.tdtype), _dev(sigma_cat, self.tdtype), R,
                                    _stream(stream)), "fk_conv_grouped")
         return sigma_cat
@@ -302,6 +369,7 @@ class FkGroup:
     def vjp(self, f_cat, g_cat, R, df_cat=None, stream=None):
         if df_cat is None:
             df_cat = torch.empty_like(f_cat)
+        self._chk(R, f_cat=f_cat, g_cat=g_cat, df_cat=df_cat)
         _check(lib.fk_conv_grouped_vjp(self.handle, _dev(f_cat, self.tdtype), _dev(g_cat, self.tdtype),
                                        _dev(df_cat, self.tdtype), R, _stream(stream)), "fk_conv_grouped_vjp")
         return df_cat

@@ -105,6 +105,32 @@ def test_dense_path_replica_counts(K, shape, R):
     assert np.array_equal(tp.vjp(f_d, g_d).cpu().numpy(), tp.vjp(f_d, g_d).cpu().numpy())
 
 
+@pytest.mark.parametrize("c", [0.3, 1.1])
+def test_dense_vjp_same_sign_many_datapoints(K, c):
+    """f = c, FK = 1, g = 1 with N = 10 000 datapoints at R = 8: the dense VJP contraction sums over ALL datapoints,
+    and with one sign nothing cancels -- an unbounded register chain of N/4 DMMA steps misses 1e-13 here
+    (the kernels flush every 512 datapoints).  Closed form: df[a][i] = N c nx (#{a_c = a} + #{b_c = a})."""
+    from fractions import Fraction
+    import torch
+    N, nx, nfl, C, R = 10000, 8, 3, 4, 8
+    pairs = np.array([(0, 1), (1, 1), (2, 0), (0, 0)], dtype=np.int32)
+    fk_d = torch.ones((N, nx, nx, C), dtype=torch.float64, device="cuda")
+    f = np.full((R, nfl, nx), c); g = np.ones((N, R))
+    exact = np.zeros((R, nfl, nx))
+    for a in range(nfl):
+        cnt = int(np.sum(pairs[:, 0] == a) + np.sum(pairs[:, 1] == a))
+        exact[:, a, :] = float(Fraction(c) * N * nx * cnt)
+    for store in (K.FK_STORE_PACK, K.FK_STORE_BORROW):
+        t = K.FkTable(K.FK_KIND_HADRONIC, fk_d, pairs, nfl, K.FK_F64, store, R_hint=R)
+        df = t.vjp(to_dev(f), to_dev(g)).cpu().numpy()
+        err = float(np.max(np.abs(df - exact) / exact))
+        print(f"dense VJP same sign c={c} store={store}: {err:.2e}")
+        assert err <= TOL64, (c, store, err)
+        sig = t.conv(to_dev(f)).cpu().numpy()
+        assert float(np.max(np.abs(sig - float(Fraction(c) ** 2 * nx * nx * C)) / float(Fraction(c) ** 2 * nx * nx * C))) <= TOL64
+        t.destroy()
+
+
 # x-grids beyond what the single-pass VJP folds hold (nx > 64 at R >> 1, nx > 128 at small R): gather fallbacks
 @pytest.mark.parametrize("shape_R", [((12, 70, 3, 4), 6), ((12, 70, 3, 4), 1), ((6, 131, 2, 2), 1), ((6, 131, 2, 2), 5)])
 def test_large_x_grids(K, shape_R):

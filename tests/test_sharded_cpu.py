@@ -31,8 +31,24 @@ df = sharded.allreduce_df(torch.from_numpy(df_part)).numpy()
 ref, scale = O.hadronic(case.fk, case.pairs, case.f)
 dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, g)
 e1 = float(np.max(np.abs(sig - ref) / scale)); e2 = float(np.max(np.abs(df - dref) / np.maximum(D, 1e-300)))
+# ragged group, whole tables to ranks (GroupPlan): forward pieces and per-table df assembled by the one all-reduce
+shapes = synth.small_ragged_shapes(T=5)
+R = 2
+params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+cases = [synth.config4_table(t, shapes, R, params) for t in range(shapes.T)]
+plan = sharded.GroupPlan([(c.N, c.nx, c.nfl, c.C) for c in cases], world)
+fo, so = plan.offsets(R)
+mine = plan.owner_tables[rank]
+sig_p = [torch.from_numpy(O.hadronic(cases[t].fk, cases[t].pairs, cases[t].f)[0]) for t in mine]
+df_p = [torch.from_numpy(O.hadronic_vjp(cases[t].fk, cases[t].pairs, cases[t].f, cases[t].g)[0]) for t in mine]
+sig_cat = sharded.allreduce_cat(plan.scatter_local(sig_p, rank, so)).numpy()
+df_cat = sharded.allreduce_cat(plan.scatter_local(df_p, rank, fo)).numpy()
+ref_sig = np.concatenate([O.hadronic(c.fk, c.pairs, c.f)[0].ravel() for c in cases])
+ref_df = np.concatenate([O.hadronic_vjp(c.fk, c.pairs, c.f, c.g)[0].ravel() for c in cases])
+grp_exact = bool(np.array_equal(sig_cat, ref_sig) and np.array_equal(df_cat, ref_df))
 dist.barrier()
-print(json.dumps({"rank": rank, "rows": [n0, n1], "exact_sigma": bool(np.array_equal(sig, ref)), "e1": e1, "e2": e2}))
+print(json.dumps({"rank": rank, "rows": [n0, n1], "exact_sigma": bool(np.array_equal(sig, ref)), "e1": e1, "e2": e2,
+                  "group_exact": grp_exact, "owned": mine}))
 dist.destroy_process_group()
 """
 
@@ -63,6 +79,8 @@ def test_row_sharded_forward_and_vjp_with_gloo_world_size_2(tmp_path):
     for o in outs:
         assert o["exact_sigma"]            # rows are independent: the gathered forward is the unsharded one, bit for bit
         assert o["e1"] == 0.0 and o["e2"] <= 1e-15   # df: one extra add per element (sum of two partials)
+        assert o["group_exact"]            # whole-table sharding: x + 0 assembly, bit-identical to the unsharded group
+    assert sorted(outs[0]["owned"] + outs[1]["owned"]) == [0, 1, 2, 3, 4] and outs[0]["owned"] and outs[1]["owned"]
 
 
 def test_shard_plans():
