@@ -48,6 +48,15 @@ def _measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
 
 
+def _tf32_peak():
+    """Dense TF32 tensor peak in TFLOP/s: the measured bf16 cuBLAS burst figure x the guide's nominal TF32 / bf16 ratio (1/2)."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return 0.5 * float(json.load(fh)["bf16_tflops"])
+    return 0.5 * 1590.0
+
+
 # ------------------------------------------------------------------------------------------ clocks
 class ClockSampler:
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
@@ -270,6 +279,25 @@ def run_extras(K, torch, level, table2, case2, peak):
     d3 = torch.empty_like(f3)
     ms = _bench_call(lambda: table2.vjp(f3, g3, d3), stream, steps=5, warmup=2)
     out["cfg3_vjp_R128"] = {"ms": ms, "TFLOPs": flops / ms / 1e9, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS}
+    # config 3, fp32 variant (BASELINE cfg3: "fp64 and fp32 variant"): tcgen05 3xTF32 contraction (fk_tc32.cu) against the
+    # column-kernel passes it replaces.  HBM roofline: the 0.512 GB fp32 table once; tensor roofline: 3 TF32 products.
+    t32v = K.FkTable(K.FK_KIND_HADRONIC, torch.from_numpy(case2.fk).cuda(), case2.pairs, case2.nfl, K.FK_F32, K.FK_STORE_PACK, R_hint=R)
+    torch.cuda.empty_cache()
+    f3s = f3.to(torch.float32); s3s = torch.empty((case2.N, R), dtype=torch.float32, device="cuda")
+    ms = _bench_call(lambda: t32v.conv(f3s, s3s), stream, steps=10, warmup=3)
+    tf32_peak = _tf32_peak()
+    out["cfg3_forward_R128_fp32"] = {
+        "ms": ms, "launches": t32v.last_launches(), "GBps": fkb / 2 / ms / 1e6, "frac_of_peak": fkb / 2 / ms / 1e6 / peak,
+        "TFLOPs_useful": flops / ms / 1e9, "TFLOPs_tensor_3xTF32": 3 * flops / ms / 1e9,
+        "frac_of_tf32_peak": 3 * flops / ms / 1e9 / tf32_peak, "tf32_peak_TFLOPs": tf32_peak,
+        "replica_evals_per_s": R / ms * 1e3, "tolerance": 1e-5}
+    K.set_option(K.FK_OPT_TC32, 0)
+    try:
+        ms = _bench_call(lambda: t32v.conv(f3s, s3s), stream, steps=3, warmup=1)
+        out["cfg3_forward_R128_fp32_column_passes"] = {"ms": ms, "launches": t32v.last_launches()}
+    finally:
+        K.set_option(K.FK_OPT_TC32, 1)
+    t32v.destroy()
     if level == "all":
         out.update(run_config4(K, torch, peak))
     return out

@@ -26,6 +26,7 @@
 #include "fk_fwd.cuh"
 #include "fk_vjp.cuh"
 #include "fk_chi2.cuh"
+#include "fk_tc32.h"
 
 namespace {
 
@@ -500,6 +501,72 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
     return FK_OK;
 }
 
+// ---- fp32 variant at R >> 1: tcgen05 3xTF32 contraction (fk_tc32.cu) ------------------------------------------------
+constexpr int TC32_DEFAULT_MIN_R = 9;   // from 3 column passes of <= 4 replicas on
+struct Tc32Plan {
+    int ksplit, kper, RPmax, fk_stages;
+    size_t smem;
+};
+bool tc32_wanted(const fk::TableDesc& d, int R) {
+    if (!opt(FK_OPT_TC32) || !d.tmap || d.kind != fk::KIND_HADRONIC || d.layout != fk::LAYOUT_PACKED || d.nx < 8) return false;
+    if (R < (opt(FK_OPT_TC32_MIN_R) > 0 ? opt(FK_OPT_TC32_MIN_R) : TC32_DEFAULT_MIN_R)) return false;
+    return fk::tc32_smem_bytes(d.nx, fk::tc_rp(R), nullptr) > 0;
+}
+Tc32Plan tc32_plan(const fk::TableDesc& d, int R) {
+    Tc32Plan tp;
+    tp.RPmax = fk::tc_rp(R);
+    tp.smem = fk::tc32_smem_bytes(d.nx, tp.RPmax, &tp.fk_stages);
+    const int mtiles = fk::tc32_mtiles(d.N);
+    const int ksplit = std::max(1, std::max(1, sm_count()) / mtiles);   // one wave of equal items, one CTA per SM
+    tp.kper = ((d.K + ksplit - 1) / ksplit + fk::TC_KT - 1) / fk::TC_KT * fk::TC_KT;
+    tp.ksplit = (d.K + tp.kper - 1) / tp.kper;
+    return tp;
+}
+// scratch in doubles: fT32 [slots][RPmax] floats + level-1 partials [ksplit][N][RPmax] floats
+size_t tc32_scratch_elems(const fk::TableDesc& d, int R) {
+    const Tc32Plan tp = tc32_plan(d, R);
+    return ((size_t)d.nfl * d.nx * tp.RPmax + (size_t)tp.ksplit * d.N * tp.RPmax + 1) / 2 + 64;
+}
+
+int run_conv_tc32(const fk::TableDesc& d, const fk::ChannelList& ch, const float* f, float* sigma, int R, double* scratch,
+                  cudaStream_t s, int* launches) {
+    const Tc32Plan tp = tc32_plan(d, R);
+    const int slots = d.nfl * d.nx;
+    float* fT = reinterpret_cast<float*>(scratch);
+    float* gpart = fT + ((size_t)slots * tp.RPmax + 31) / 32 * 32;   // 128-byte aligned
+    int nl = 0;
+    for (int r0 = 0; r0 < R; r0 += fk::TC_MAX_RP) {
+        fk::Tc32Params p;
+        memset(&p, 0, sizeof p);
+        p.desc = d;
+        p.chan = ch;
+        p.tmap = d.tmap;
+        p.fT = fT;
+        p.gpart = gpart;
+        p.RP = fk::tc_rp(R - r0);
+        p.ksplit = tp.ksplit;
+        p.kper = tp.kper;
+        int st = 0;
+        const size_t smem = fk::tc32_smem_bytes(d.nx, p.RP, &st);
+        p.fk_stages = st;
+        const long long tot = (long long)slots * p.RP;
+        fk::fk_transpose_f_kernel<float, float><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
+        size_t slot = 0;
+        const bool timed = r0 == 0 && g_prof.begin(s, slot);
+        cudaError_t e = fk::tc32_fwd_launch(p, fk::tc32_mtiles(d.N) * tp.ksplit, false, smem, s);
+        if (timed) g_prof.end(s, slot);
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward launch failed: %s", cudaGetErrorString(e));
+        const long long outs = (long long)d.N * p.RP;
+        fk::fk_gemm_reduce_kernel<float, float><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
+            gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, tp.ksplit);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward reduce launch failed: %s", cudaGetErrorString(e));
+        nl += 3;
+    }
+    if (launches) *launches = nl;
+    return FK_OK;
+}
+
 // One table, any R.  `part` holds >= part_elems_per_replica * R doubles (may be null if nchunks == 1).
 template <typename T, typename TS = T>
 int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const uint32_t* kdec,
@@ -507,6 +574,9 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
     int nl = 0;
     if constexpr (std::is_same<T, double>::value) {
         if (gemm_wanted<T>(d, R)) return run_conv_gemm(d, ch, kdec, f, sigma, R, part, s, launches);
+    }
+    if constexpr (std::is_same<T, float>::value && std::is_same<TS, float>::value) {
+        if (tc32_wanted(d, R)) return run_conv_tc32(d, ch, f, sigma, R, part, s, launches);
     }
     fk::FwdParams p;
     memset(&p, 0, sizeof p);
@@ -709,6 +779,8 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
 template <typename T>
 size_t conv_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
     if (gemm_wanted<T>(d, R)) return gemm_fwd_scratch_elems(d, R, with_kdec);
+    if (std::is_same<T, float>::value && d.tmap && d.kind == fk::KIND_HADRONIC)   // either fp32 path may be selected later
+        return std::max(part_elems_per_replica(d) * R, fk::tc32_smem_bytes(d.nx, fk::tc_rp(R), nullptr) ? tc32_scratch_elems(d, R) : 0);
     return part_elems_per_replica(d) * R;
 }
 template <typename T>
@@ -780,6 +852,7 @@ struct fk_table {
     void* owned_fk = nullptr;
     uint8_t* dev_chan = nullptr;  // [2][C] for grouped launches
     uint32_t* kdec = nullptr;     // [K] k -> (slot a, slot b) codes for the R >> 1 contraction
+    void* d_tmap = nullptr;       // device copy of the CUtensorMap of a packed fp32 hadronic table (fk_tc32.cu)
     double* scratch = nullptr;    // forward partials / VJP column sums (one buffer, used by one call at a time)
     size_t scratch_elems = 0;
     void* h_stage = nullptr;      // pinned host staging for the *_host calls
@@ -1027,6 +1100,16 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
         t->desc.kdec = t->kdec;
     }
 
+    if (dtype == FK_F32 && store == FK_STORE_PACK && kind == FK_KIND_HADRONIC && t->desc.vec_ok) {
+        // tensor map for the tcgen05 path; a driver without the entry point simply leaves the table on the column kernels
+        alignas(64) unsigned char tm[fk::TC_TMAP_BYTES];
+        if (fk::tc32_encode_tensor_map(tm, t->owned_fk, t->desc.row_stride, t->desc.K, N)) {
+            e = cudaMalloc(&t->d_tmap, fk::TC_TMAP_BYTES);
+            if (e == cudaSuccess) e = cudaMemcpy(t->d_tmap, tm, fk::TC_TMAP_BYTES, cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: tensor map upload: %s", cudaGetErrorString(e)); }
+            t->desc.tmap = t->d_tmap;
+        }
+    }
     rc = ensure_scratch(t, table_scratch_need(t, std::max(1, R_hint)));
     if (rc) return bail(rc);
     *out = t;
@@ -1038,6 +1121,7 @@ int fk_table_destroy(fk_table* t) {
     if (t->owned_fk) cudaFree(t->owned_fk);
     if (t->dev_chan) cudaFree(t->dev_chan);
     if (t->kdec) cudaFree(t->kdec);
+    if (t->d_tmap) cudaFree(t->d_tmap);
     if (t->scratch) cudaFree(t->scratch);
     if (t->h_stage) cudaFreeHost(t->h_stage);
     if (t->d_stage) cudaFree(t->d_stage);

@@ -48,6 +48,10 @@ struct TableDesc {
     long long k_off;         // offset of this table's column sums inside G_cat (sum of K over earlier tables)
     int gksplit, gkper;      // K ranges of the forward contraction and their length
     long long cx_off;        // sum of C * nx over earlier tables: first (channel, x) slot of the VJP fold partials
+    // tcgen05 contraction of fp32 tables (fk_tc32.cu)
+    const void* tmap;        // device copy of the table's CUtensorMap (null: the table cannot take that path)
+    int tc_ksplit, tc_kper;  // grouped launches: K ranges of the tcgen05 contraction and their length (multiple of 32)
+    long long tc_gp_off;     // grouped launches: row offset of this table's tcgen05 split-K partials
 };
 
 // Work list entry of the column kernels (forward and VJP stage 1): one CTA = one (k-block, datapoint range).

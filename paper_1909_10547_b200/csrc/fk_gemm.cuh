@@ -88,14 +88,14 @@ __global__ void __launch_bounds__(256) fk_kdec_kernel(TableDesc d, ChannelList c
 }
 
 // fT[slot][r - r0] = f[r][slot] for r in [r0, r0 + RP), zero beyond R
-template <typename T>
-__global__ void __launch_bounds__(256) fk_transpose_f_kernel(const T* __restrict__ f, double* __restrict__ fT, int slots,
+template <typename T, typename O = double>
+__global__ void __launch_bounds__(256) fk_transpose_f_kernel(const T* __restrict__ f, O* __restrict__ fT, int slots,
                                                               int R, int r0, int RP) {
     const long long total = (long long)slots * RP;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
         const int s = (int)(t / RP), c = (int)(t - (long long)s * RP);
         const int r = r0 + c;
-        fT[t] = r < R ? (double)f[(long long)r * slots + s] : 0.0;
+        fT[t] = r < R ? (O)f[(long long)r * slots + s] : O(0);
     }
 }
 
@@ -253,8 +253,8 @@ fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
 }
 
 // level 2: sigma[n][r0 + c] = sum over K ranges, fixed order
-template <typename T>
-__global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const double* __restrict__ gpart, T* __restrict__ sigma,
+template <typename T, typename P = double>
+__global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const P* __restrict__ gpart, T* __restrict__ sigma,
                                                               long long out_off, int N, int R, int r0, int RP, int ksplit) {
     const long long total = (long long)N * RP;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const double* __res
         for (int k0 = 0; k0 < ksplit; k0 += 8) {  // eight loads in flight, added in index order
             double w[8];
 #pragma unroll
-            for (int q = 0; q < 8; ++q) w[q] = k0 + q < ksplit ? gpart[(long long)(k0 + q) * total + t] : 0.0;
+            for (int q = 0; q < 8; ++q) w[q] = k0 + q < ksplit ? (double)gpart[(long long)(k0 + q) * total + t] : 0.0;
 #pragma unroll
             for (int q = 0; q < 8; ++q) s += w[q];
         }

@@ -300,6 +300,65 @@ def test_fp32_variant(K, R):
     assert rel_err(d2.cpu().numpy(), dref, D) <= TOL32
 
 
+# fp32 variant at R >> 1: the tcgen05 (3xTF32) contraction.  Every padded replica count (multiples of 16), partial
+# datapoint tiles (N % 128 != 0), K ranges that end inside a channel, x-grids from 8 to 50, a pass boundary at
+# R > 128.  Gate: 1e-5 of sum|terms| against the fp64 oracle of the fp64 inputs (reading R18); printed next to the
+# error of the fp32 column kernels on the same inputs.
+@pytest.mark.parametrize("R", [9, 16, 33, 48, 70, 81, 100, 113, 128, 150])
+@pytest.mark.parametrize("shape", [(70, 13, 14, 17), (200, 30, 14, 9), (300, 8, 6, 5), (129, 50, 14, 3)])
+def test_tc32_dense_path_fp32_variant(K, shape, R):
+    import torch
+    N, nx, nfl, C = shape
+    case = synth.hadronic_case(8, N, nx, C, R, nfl=nfl, sub=N * 1000 + nx + R)
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f)
+    f32 = torch.float32
+    tp = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl, K.FK_F32, K.FK_STORE_PACK, R_hint=R)
+    f_d = to_dev(case.f, f32)
+    s = tp.conv(f_d)
+    nl = tp.last_launches()
+    e_tc = rel_err(s.cpu().numpy(), ref, scale)
+    K.set_option(K.FK_OPT_TC32, 0)
+    try:
+        s_col = tp.conv(f_d)
+        nl_col = tp.last_launches()
+    finally:
+        K.set_option(K.FK_OPT_TC32, 1)
+    e_col = rel_err(s_col.cpu().numpy(), ref, scale)
+    print(f"tc32 {shape} R={R}: tcgen05 {e_tc:.2e} ({nl} launches)  column kernels {e_col:.2e} ({nl_col} launches)")
+    assert nl == 3 * ((R + 127) // 128) and nl_col >= nl         # the tensor-core path really ran (transpose, contraction, reduce per pass)
+    assert s.dtype == f32 and e_tc <= TOL32 and e_col <= TOL32
+    assert torch.equal(s, tp.conv(f_d))                           # bitwise repeatable
+    tp.destroy()
+
+
+def test_tc32_same_sign_and_exact_small_integers(K):
+    """Two pins of the 3xTF32 split itself.  (1) Integers in [-2, 2] are exact in TF32 and every partial sum is exact
+    in fp32 (|sum| <= 2^24): the result must equal the oracle bit for bit.  (2) f = c, FK = 1 (closed form
+    c^2 nx^2 C): all terms have one sign, so the truncation of the split and of the tensor core's
+    accumulation cannot cancel -- the bounded TMEM chains keep it inside 1e-5."""
+    from fractions import Fraction
+    import torch
+    f32 = torch.float32
+    case = synth.integer_hadronic_case(9, N=150, nx=20, C=7, R=40, lim=2)
+    ref, _ = O.hadronic(case.fk, case.pairs, case.f)
+    tp = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl, K.FK_F32, K.FK_STORE_PACK, R_hint=40)
+    s = tp.conv(to_dev(case.f, f32)).cpu().numpy()
+    assert tp.last_launches() == 3 and np.array_equal(s.astype(np.float64), ref)
+    tp.destroy()
+    N, nx, C, nfl, R = 256, 50, 100, 14, 64
+    pairs = synth.draw_pairs(synth.rng_for(2, synth.T_PAIRS, 0), C)
+    fk_d = torch.ones((N, nx, nx, C), dtype=torch.float64, device="cuda")
+    tp = K.FkTable(K.FK_KIND_HADRONIC, fk_d, pairs, nfl, K.FK_F32, K.FK_STORE_PACK, R_hint=R)
+    for c in (0.3, 1.1):
+        c32 = float(np.float32(c))                       # the fp32 variant demotes f (reading R18)
+        exact = float(Fraction(c32) ** 2 * nx * nx * C)
+        s = tp.conv(torch.full((R, nfl, nx), c32, dtype=f32, device="cuda")).cpu().numpy().astype(np.float64)
+        err = float(np.max(np.abs(s - exact) / exact))
+        print(f"tc32 same sign c={c}: {err:.2e}")
+        assert tp.last_launches() == 3 and err <= TOL32
+    tp.destroy()
+
+
 # ------------------------------------------------------------------ host-buffer calls
 def test_host_buffer_calls(K):
     case = synth.hadronic_case(6, 48, 20, 30, 2, sub=5)
