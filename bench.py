@@ -12,8 +12,12 @@ host-buffer C-ABI calls (H2D of f and g, D2H of sigma and df inside the timed re
 itself stays resident, as in a fit: PAPER.md:29, :47).  Prints exactly one JSON line on stdout.
 
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
-workload.  N > 1: "replicas only" - every rank runs the same step on its own copy of the
-table, no data-path collective; value = N * bytes / max-over-ranks time.
+workload.  N > 1: one process per GPU; when WORLD_SIZE is not set, bench.py re-executes itself under
+torch.distributed.run with N ranks (and fails loudly when the node has fewer than N GPUs).  Default mode
+"replicas": every rank runs the same step on its own copy of the table, no data-path
+collective, value = N * bytes / max-over-ranks time, "scaling": "weak".  `--shard rows`: BASELINE config 4 with
+whole tables owned by ranks (sharded.ShardedFkGroup), forward + VJP + the ONE all-reduce that assembles df per
+step, total work fixed: "scaling": "strong".
 """
 from __future__ import annotations
 
@@ -35,7 +39,15 @@ from paper_1909_10547_b200 import synth  # noqa: E402  (seeded inputs only; no m
 FP64_PEAK_TFLOPS = 37.2  # 148 SM x 64 FMA/clk x 2 x 1.965 GHz (probe: profiles/r01_fp64_peak.md)
 METRIC = "fk_convolution_achieved_hbm_bandwidth"
 UNIT = "GB/s"
-DOMINANT_KERNEL = "fk_fwd_column_kernel<double,2,1,8,0,double>"
+# kernels of the config-2 step as the library's timing hook names them -> (what they are, S 8(a) rows, bound)
+STEP_KERNELS = {
+    "fk_fwd_column": ("forward column kernel: luminosity + streaming contraction + level-1 reduction", "a1+a2+a3", "hbm"),
+    "fk_reduce_chunks": ("level-2 reduction of the forward partials", "a3", "latency"),
+    "fk_colsum": ("VJP stage 1: column sums G = g^T FK", "a6", "hbm"),
+    "fk_vjp_foldk": ("VJP stage 2: one pass over G for both legs", "a6", "latency"),
+    "fk_vjp_foldk_final": ("VJP stage 2: fixed-order sum over channels", "a6", "latency"),
+}
+TRAFFIC_CSV = os.path.join("profiles", "r02_traffic.csv")
 WORKLOAD = "config2: hadronic FK N=512 nx=50 nfl=14 C=100 R=1 fp64 (1.024 GB), forward + VJP per step"
 
 
@@ -171,7 +183,7 @@ def run_reference(args):
     gbs = step_bytes(case) / sec / 1e9
     sample = f"first {rows} of 512 datapoints of config 2, forward + VJP, {steps} timed steps"
     line = {
-        "impl": "reference", "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": 1,   # rank 0's host cores, whatever --gpus says
         "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": sec * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOAD, "sample": sample},
@@ -429,9 +441,7 @@ def run_ours(args):
     if world > 1:
         torch.distributed.barrier()
 
-    # timed region: K steps, CUDA events on the launching stream; the dominant kernel (forward
-    # stream kernel) is timed inside the same region by the library's own event pairs
-    K.lib.fk_profile_enable(1)
+    # timed region: K steps, CUDA events on the launching stream, nothing between the launches of a step
     with ClockSampler(local) as clk:
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
@@ -442,10 +452,19 @@ def run_ours(args):
         e1.synchronize()
         torch.cuda.synchronize()
     ms_local = e0.elapsed_time(e1) / args.steps
-    import ctypes
-    kms, kcount = ctypes.c_double(0.0), ctypes.c_int(0)
-    K.lib.fk_profile_read(ctypes.byref(kms), ctypes.byref(kcount))
-    K.lib.fk_profile_enable(0)
+    # the same K steps once more with the library's per-launch event pairs (fk_profile_enable): every kernel of the
+    # step timed on the launching stream.  Separate from the region above because an event record between two
+    # launches serialises them (no programmatic dependent launch overlap), which would tax the headline number.
+    K.profile_enable(True)
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2.record(stream)
+    for _ in range(args.steps):
+        step()
+    e3.record(stream)
+    e3.synchronize()
+    ms_profiled = e2.elapsed_time(e3) / args.steps
+    kernel_times = K.profile_report()
+    K.profile_enable(False)
     if world > 1:
         torch.distributed.barrier()
     ms = aggregate_max(ms_local, world)
@@ -476,13 +495,27 @@ def run_ours(args):
         return 0
 
     fkb = case.fk.nbytes
-    kernel_ms = kms.value if kcount.value > 0 else None
+    traffic = _ncu_traffic()
+    kernels = []
+    for name, (n, tot_ms) in kernel_times.items():
+        what, rows, bound = STEP_KERNELS.get(name, (name, "?", "?"))
+        k_ms = tot_ms / n
+        kb = fkb if bound == "hbm" else None   # algorithmic bytes per launch: the FK table once
+        kernels.append({"name": name, "what": what, "rows": rows, "bound": bound, "launches": n, "ms": k_ms,
+                        "share_of_profiled_step": tot_ms / args.steps / ms_profiled, "bytes": kb,
+                        "achieved": (kb / k_ms / 1e6) if kb else None, "frac": (kb / k_ms / 1e6 / peak) if kb else None,
+                        "traffic": traffic.get(name)})
+    kernels.sort(key=lambda k: -k["ms"])
+    dom = kernels[0] if kernels else None
     roofline = {
-        "bound": "hbm", "kernel": DOMINANT_KERNEL + " (forward column kernel: luminosity + streaming contraction + level-1 reduction, rows a1+a2+a3)",
-        "achieved": (fkb / kernel_ms / 1e6) if kernel_ms else None, "peak": peak, "unit": "GB/s",
-        "frac": (fkb / kernel_ms / 1e6 / peak) if kernel_ms else None, "peak_source": peak_src,
-        "kernel_ms": kernel_ms, "kernel_launches_timed": kcount.value, "bytes_per_launch": fkb,
-        "traffic": _ncu_traffic(),
+        "bound": "hbm", "kernel": (dom["name"] + " (" + dom["what"] + ", rows " + dom["rows"] + ")") if dom else None,
+        "achieved": dom["achieved"] if dom else None, "peak": peak, "unit": "GB/s",
+        "frac": dom["frac"] if dom else None, "peak_source": peak_src,
+        "kernel_ms": dom["ms"] if dom else None, "kernel_launches_timed": dom["launches"] if dom else 0,
+        "bytes_per_launch": fkb, "traffic": dom["traffic"] if dom else None,
+        "traffic_source": "committed ncu --set full capture, " + TRAFFIC_CSV + " (dram read + write bytes per launch; not measured in this run)",
+        "timed_in": "second pass of the same K steps with per-launch CUDA event pairs on the launching stream",
+        "ms_per_step_profiled": ms_profiled, "kernels": kernels,
     }
     cpu_baseline = None
     if not args.no_cpu_baseline:
@@ -514,30 +547,130 @@ def run_ours(args):
 
 
 def _ncu_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    summary of the ncu --set full capture (profiles/r01_traffic.csv), or None."""
-    p = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    """{kernel name: dram__bytes_read.sum + dram__bytes_write.sum per launch} from the committed summary of the
+    ncu --set full capture (profiles/r02_traffic.csv: name,dram_read_bytes,dram_write_bytes,ncu kernel name), {} if absent."""
+    out = {}
     try:
-        with open(p) as fh:
+        with open(os.path.join(ROOT, TRAFFIC_CSV)) as fh:
             for ln in fh:
-                if ln.startswith(DOMINANT_KERNEL + ","):
-                    return int(ln[len(DOMINANT_KERNEL) + 1:].split(",")[2])
+                c = ln.strip().split(",")
+                if len(c) >= 3 and c[0] in STEP_KERNELS:
+                    out[c[0]] = int(float(c[1])) + int(float(c[2]))
     except Exception:
         pass
-    return None
+    return out
 
 
-def main():
+def _spawn(args, argv):
+    """--gpus N > 1 without a torchrun environment: re-execute under torch.distributed.run with N ranks on 127.0.0.1."""
+    import socket
+    import subprocess
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if args.impl != "reference" and have < args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but this node has {have} CUDA device(s): refusing to report an "
+                         f"N-GPU number from fewer GPUs")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + argv
+    return subprocess.call(cmd)
+
+
+def run_sharded(args):
+    """--shard rows: BASELINE config 4 (R = 1) with whole tables owned by ranks ('whole tables of a ragged
+    group, balanced by bytes').  Step = grouped forward (no exchange) + grouped VJP + the one all-reduce that assembles
+    df_cat on every rank.  Total work is fixed as N grows: "scaling": "strong"."""
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the FK convolution has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_1909_10547_b200 import fkconv as K
+    from paper_1909_10547_b200 import sharded
+    shapes = synth.config4_shapes()
+    R = 1
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    plan = sharded.GroupPlan([(int(shapes.N[t]), int(shapes.nx[t]), 14, int(shapes.C[t])) for t in range(shapes.T)], world)
+    mine = set(plan.owner_tables[rank])
+    cases, fs, gs = [], [], []
+    for t in range(shapes.T):
+        # tables of other ranks: shapes only (never generated or uploaded); f and g are needed in the global layout
+        c = synth.config4_table(t, shapes, R, params, with_fk=t in mine)
+        cases.append((K.FK_KIND_HADRONIC, c.fk, c.pairs, c.nfl))
+        fs.append(c.f); gs.append(c.g)
+    grp = sharded.ShardedFkGroup(cases, R_hint=R)
+    f_cat = torch.cat([torch.from_numpy(np.ascontiguousarray(f[:R])).reshape(-1) for f in fs]).cuda()
+    g_cat = torch.cat([torch.from_numpy(np.ascontiguousarray(g[:, :R])).reshape(-1) for g in gs]).cuda()
+    stream = torch.cuda.current_stream()
+    peak, peak_src = _measured_peaks()
+    nbytes = 2 * shapes.fk_elements() * 8   # whole job: every table read once per pass, two passes
+
+    def step():
+        grp.conv(f_cat, R)
+        grp.vjp(f_cat, g_cat, R)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    with ClockSampler(local) as clk:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            step()
+        e1.record(stream)
+        e1.synchronize()
+        torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = aggregate_max(e0.elapsed_time(e1) / args.steps, world)
+    launches = grp.local.last_launches()
+    if rank == 0:
+        value = nbytes / ms / 1e6
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config4: 60 ragged hadronic tables (14.83 GB) R=1, grouped forward + grouped VJP + all-reduce of df per step",
+                       "shard": "rows (whole tables to ranks by FK bytes, LPT greedy)", "tables_on_rank0": len(mine),
+                       "l2": "per-rank tables are larger than the 126 MB L2; no flush needed", "multi_gpu": "datapoint-sharded, one all-reduce"},
+            "frac_of_hbm_peak": value / world / peak, "roofline": None, "cpu_baseline": None, "e2e": None,
+            "gpu_launches_last_call_rank0": launches, "clocks": clk.summary()}))
+    grp.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    argv = list(sys.argv[1:] if argv is None else argv)
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--extras", default="fast", choices=["none", "fast", "all", "table3"])
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "rows"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
+    args = ap.parse_args(argv)
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
     if args.impl == "reference":
-        return run_reference(args)
+        return run_reference(args)   # rank 0's host cores only; never spawns
+    world = int(os.environ.get("WORLD_SIZE", "0") or 0)
+    if args.gpus > 1 and world == 0:
+        return _spawn(args, argv)
+    if world and world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    if args.shard == "rows":
+        return run_sharded(args)
     return run_ours(args)
 
 

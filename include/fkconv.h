@@ -90,17 +90,24 @@ enum {
     FK_OPT_FEWROWS = 5,    /* [1] k-walking forward kernel for <= 8 datapoints and very long rows */
     FK_OPT_TC32 = 6,       /* [1] tcgen05 (3xTF32) dense contraction for FK_F32 tables at large R (0: column passes) */
     FK_OPT_TC32_MIN_R = 7, /* [0] smallest R that takes it; 0 = built-in */
-    FK_OPT_COUNT_ = 8
+    FK_OPT_PDL = 8,        /* [1] later kernels of a call use programmatic dependent launch (0: plain stream order) */
+    FK_OPT_COUNT_ = 9
 };
 int fk_set_option(int option, int value);
 int fk_get_option(int option, int* value);
 
-/* Kernel timing hook for bench.py's roofline: while enabled, every forward call brackets its
- * dominant kernel (the streaming contraction, or the dense contraction for large R) with a CUDA event
- * pair on the caller's stream.  fk_profile_read waits for those events, returns the mean kernel
- * duration in milliseconds and the number of launches timed since the last read, and clears them. */
+/* Kernel timing hook for bench.py's roofline: while enabled, every kernel launch of every
+ * compute call is bracketed by a CUDA event pair on the caller's stream, keyed by a short kernel name.
+ * The pairs serialise neighbouring launches (programmatic dependent launch cannot overlap across an event
+ * record), so a profiled step is slightly slower than an unprofiled one: leave it off outside measurements.
+ * fk_profile_report waits for the recorded events, writes one line per kernel name
+ *     "<name>\t<launches>\t<total milliseconds>\n"
+ * into `buf` (host memory, `capacity` bytes including the terminating 0; FK_ERR_INVALID_ARG if too small)
+ * and clears the records.  fk_profile_read does the same but returns only the record with the largest
+ * total time: its mean duration in milliseconds and its launch count. */
 int fk_profile_enable(int on);
 int fk_profile_read(double* mean_kernel_ms, int* launches);
+int fk_profile_report(char* buf, int capacity);
 
 /* ------------------------------------------------------------------ stateless entry points (fp64)
  * Eq. (1) P:43 / DIS / VJP on the caller's logical-layout device buffers.  Level-1 partials live in

@@ -67,6 +67,7 @@ int g_opt[FK_OPT_COUNT_] = {
     /* FK_OPT_FEWROWS     */ 1,
     /* FK_OPT_TC32        */ 1,
     /* FK_OPT_TC32_MIN_R  */ 0,
+    /* FK_OPT_PDL         */ 1,
 };
 inline int opt(int o) { return g_opt[o]; }
 
@@ -100,29 +101,63 @@ bool ensure_dyn_smem(const void* func, size_t bytes) {
 }
 template <typename F> bool ensure_dyn_smem(F* func, size_t bytes) { return ensure_dyn_smem((const void*)func, bytes); }
 
-// ---- kernel timing hook (fk_profile_enable / fk_profile_read) ----
+// ---- kernel timing hook (fk_profile_enable / fk_profile_read / fk_profile_report) ----
+// While enabled, every kernel launch of a compute call is bracketed by an event pair on the caller's stream, keyed by a
+// short kernel name (FK_TIMED below).  Off by default: the pairs serialise neighbouring launches.
 struct Profiler {
     std::mutex mu;
     bool on = false;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> pairs;
+    struct Rec { cudaEvent_t a, b; const char* name; };
+    std::vector<Rec> recs;
     size_t used = 0;
-    bool begin(cudaStream_t s, size_t& slot) {
+    bool begin(cudaStream_t s, size_t& slot, const char* name) {
         std::lock_guard<std::mutex> lk(mu);
         if (!on) return false;
-        if (used == pairs.size()) {
-            cudaEvent_t a, b;
-            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return false;
-            pairs.emplace_back(a, b);
+        if (used == recs.size()) {
+            Rec r{nullptr, nullptr, name};
+            if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return false;
+            recs.push_back(r);
         }
         slot = used++;
-        cudaEventRecord(pairs[slot].first, s);
+        recs[slot].name = name;
+        cudaEventRecord(recs[slot].a, s);
         return true;
     }
     void end(cudaStream_t s, size_t slot) {
         std::lock_guard<std::mutex> lk(mu);
-        cudaEventRecord(pairs[slot].second, s);
+        cudaEventRecord(recs[slot].b, s);
     }
 } g_prof;
+struct ProfScope {
+    cudaStream_t s;
+    size_t slot = 0;
+    bool on;
+    ProfScope(cudaStream_t s_, const char* name) : s(s_) { on = g_prof.begin(s, slot, name); }
+    ~ProfScope() { if (on) g_prof.end(s, slot); }
+    ProfScope(const ProfScope&) = delete;
+};
+// FK_TIMED("name", stream) statement;   -- the statement's launches are one timed record (no dangling-else hazard)
+#define FK_TIMED(NAME, S) switch (ProfScope fk_ps_{S, NAME}; 0) default:
+
+// Launch of a LATER kernel of a compute call with programmatic stream serialisation (fk_common.cuh, pdl_wait): its CTAs
+// may be scheduled while the preceding kernel of the same call drains; the kernel itself waits (griddepcontrol.wait)
+// before it touches memory.  The first kernel of every call is a normal launch, so the caller's own preceding work
+// (which produced f, g) is complete and visible as usual.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args&&... args) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = opt(FK_OPT_PDL) ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(std::forward<Args>(args))...);
+}
 
 template <typename T> constexpr int dtype_of();
 template <> constexpr int dtype_of<double>() { return FK_F64; }
@@ -238,7 +273,7 @@ inline int pick_rt(int remaining) { return remaining >= 3 ? 4 : remaining; }
 template <typename T, bool GROUPED, typename TS = T>
 cudaError_t fwd_dispatch(bool vec_ok, int rt, const fk::FwdParams& p, int grid, cudaStream_t s) {
     constexpr int VW = fk::VecWidth<TS>::value;
-#define FK_FWD(V, RTv) fk::fk_fwd_column_kernel<T, V, RTv, FWD_U, GROUPED, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
+#define FK_FWD(V, RTv) FK_TIMED("fk_fwd_column", s) fk::fk_fwd_column_kernel<T, V, RTv, FWD_U, GROUPED, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
     if (vec_ok) {
         if (rt == 1) FK_FWD(VW, 1); else if (rt == 2) FK_FWD(VW, 2); else FK_FWD(VW, 4);
     } else {
@@ -252,7 +287,7 @@ template <typename T, bool GROUPED, typename TS = T>
 cudaError_t colsum_dispatch(bool vec_ok, int rt, const fk::ColsumParams& p, int grid, cudaStream_t s) {
     constexpr int VW = fk::VecWidth<TS>::value;
     constexpr int U = 8;
-#define FK_COLSUM(V, RTv) fk::fk_colsum_kernel<T, V, RTv, U, GROUPED, TS><<<grid, fk::COLSUM_THREADS, 0, s>>>(p)
+#define FK_COLSUM(V, RTv) FK_TIMED("fk_colsum", s) fk::fk_colsum_kernel<T, V, RTv, U, GROUPED, TS><<<grid, fk::COLSUM_THREADS, 0, s>>>(p)
     if (vec_ok) {
         if (rt == 1) FK_COLSUM(VW, 1); else if (rt == 2) FK_COLSUM(VW, 2); else FK_COLSUM(VW, 4);
     } else {
@@ -311,7 +346,7 @@ template <bool GROUPED>
 bool ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) {
     switch (w.RP / 8) {
 #define FK_WS_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, MAX_DYN_SMEM)) return false; \
-                                  fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, smem, s>>>(w); break
+                                  FK_TIMED("fk_gemm_fwd_ws", s) fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, smem, s>>>(w); break
         FK_WS_CASE(2); FK_WS_CASE(4); FK_WS_CASE(6); FK_WS_CASE(8); FK_WS_CASE(10); FK_WS_CASE(12); FK_WS_CASE(14);
         default: FK_WS_CASE(16);
 #undef FK_WS_CASE
@@ -327,7 +362,7 @@ bool wsv_launch(const fk::WsVjpParams& w, cudaStream_t s) {
     const int grid = std::max(1, std::min(w.ntiles, sm_count()));
     switch (w.RP / 8) {
 #define FK_WSV_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED>, fk::WSV_SMEM_BYTES)) return false; \
-                                   fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break
+                                   FK_TIMED("fk_gemm_vjp_ws", s) fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break
         FK_WSV_CASE(2); FK_WSV_CASE(3); FK_WSV_CASE(4); FK_WSV_CASE(5); FK_WSV_CASE(6); FK_WSV_CASE(7); FK_WSV_CASE(8); FK_WSV_CASE(9);
         FK_WSV_CASE(10); FK_WSV_CASE(11); FK_WSV_CASE(12); FK_WSV_CASE(13); FK_WSV_CASE(14); FK_WSV_CASE(15);
         default: FK_WSV_CASE(16);
@@ -346,7 +381,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
     const bool ws = ws_ok(d, gp.RPmax);
     if (!kdec && !ws) {
         uint32_t* kd = reinterpret_cast<uint32_t*>(gpart + (size_t)gp.ksplit * d.N * gp.RPmax);
-        fk::fk_kdec_kernel<<<std::min(1024, (d.K + 255) / 256), 256, 0, s>>>(d, ch, kd);
+        FK_TIMED("fk_kdec", s) fk::fk_kdec_kernel<<<std::min(1024, (d.K + 255) / 256), 256, 0, s>>>(d, ch, kd);
         ++nl;
         kdec = kd;
     }
@@ -367,9 +402,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
         p.ksplit = gp.ksplit;
         p.kper = gp.kper;
         const long long tot = (long long)slots * p.RP;
-        fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
-        size_t slot = 0;
-        const bool timed = r0 == 0 && g_prof.begin(s, slot);
+        FK_TIMED("fk_transpose_f", s) fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
         if (ws) {
             fk::WsFwdParams w;
             memset(&w, 0, sizeof w);
@@ -384,11 +417,10 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
             const int nfull = d.N / fk::GEMM_BM;
             if (!ws_launch<false>(w, nfull * gp.ksplit + (d.N % fk::GEMM_BM ? gp.ksplit / gp.ksub_rem : 0), fk::ws_smem_bytes(d.nx, p.RP), s))
                 return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
-        } else if (d.vec_ok) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
-        else fk::fk_gemm_fwd_kernel<1, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
-        if (timed) g_prof.end(s, slot);
+        } else if (d.vec_ok) FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        else FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<1, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         const long long outs = (long long)d.N * p.RP;
-        fk::fk_gemm_reduce_kernel<double><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
+        FK_TIMED("fk_gemm_reduce", s) fk::fk_gemm_reduce_kernel<double><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
             gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, gp.ksplit);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm forward launch failed: %s", cudaGetErrorString(e));
@@ -437,8 +469,8 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
         const int RP = fk::gemm_rp8(R - r0);
         const long long tf = (long long)slots * RP, tg = (long long)d.N * RP;
-        fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tf + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, RP);
-        fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(2048, (tg + 255) / 256), 256, 0, s>>>(g + d.out_off * R, gP, d.N, R, r0, RP);
+        FK_TIMED("fk_transpose_f", s) fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tf + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, RP);
+        FK_TIMED("fk_pad_g", s) fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(2048, (tg + 255) / 256), 256, 0, s>>>(g + d.out_off * R, gP, d.N, R, r0, RP);
         fk::GemmVjpParams p;
         memset(&p, 0, sizeof p);
         p.desc = d;
@@ -457,8 +489,8 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             w.RP = RP;
             w.ntiles = grid;
             if (!wsv_launch<false>(w, s)) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
-        } else if (d.vec_ok) fk::fk_gemm_vjp_kernel<2, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
-        else fk::fk_gemm_vjp_kernel<1, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        } else if (d.vec_ok) FK_TIMED("fk_gemm_vjp", s) fk::fk_gemm_vjp_kernel<2, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        else FK_TIMED("fk_gemm_vjp", s) fk::fk_gemm_vjp_kernel<1, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         if (fold_ok(d)) {
             fk::FoldParams q;
             memset(&q, 0, sizeof q);
@@ -476,9 +508,9 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             q.nchunk = fold_chunks(d.C);
             q.nslots = fk::fold_slots(d.nx, RP, MAX_DYN_SMEM);
             if (!ensure_dyn_smem(fk::fk_vjp_fold_kernel<false>, MAX_DYN_SMEM) || q.nslots < 1) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve shared memory for the fold ring");
-            fk::fk_vjp_fold_kernel<false><<<d.C * q.nchunk, fk::FOLD_THREADS,
+            FK_TIMED("fk_vjp_fold", s) fk::fk_vjp_fold_kernel<false><<<d.C * q.nchunk, fk::FOLD_THREADS,
                                             (size_t)q.nslots * d.nx * RP * 8 + 2 * fk::FOLD_MAX_SLOTS * 8, s>>>(q);
-            fk::fk_vjp_fold_final_kernel<double, false><<<slots, fk::GEMM_BN, 0, s>>>(q);
+            FK_TIMED("fk_vjp_fold_final", s) fk::fk_vjp_fold_final_kernel<double, false><<<slots, fk::GEMM_BN, 0, s>>>(q);
             ++nl;
         } else {
             fk::GatherRParams q;
@@ -491,7 +523,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             q.R = R;
             q.r0 = r0;
             q.RP = RP;
-            fk::fk_vjp_gather_r_kernel<double, false><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
+            FK_TIMED("fk_vjp_gather_r", s) fk::fk_vjp_gather_r_kernel<double, false><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
         }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm vjp launch failed: %s", cudaGetErrorString(e));
@@ -550,14 +582,12 @@ int run_conv_tc32(const fk::TableDesc& d, const fk::ChannelList& ch, const float
         const size_t smem = fk::tc32_smem_bytes(d.nx, p.RP, &st);
         p.fk_stages = st;
         const long long tot = (long long)slots * p.RP;
-        fk::fk_transpose_f_kernel<float, float><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
-        size_t slot = 0;
-        const bool timed = r0 == 0 && g_prof.begin(s, slot);
-        cudaError_t e = fk::tc32_fwd_launch(p, fk::tc32_mtiles(d.N) * tp.ksplit, false, smem, s);
-        if (timed) g_prof.end(s, slot);
+        FK_TIMED("fk_transpose_f", s) fk::fk_transpose_f_kernel<float, float><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
+        cudaError_t e = cudaSuccess;
+        FK_TIMED("fk_tc32_fwd", s) e = fk::tc32_fwd_launch(p, fk::tc32_mtiles(d.N) * tp.ksplit, false, smem, s);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward launch failed: %s", cudaGetErrorString(e));
         const long long outs = (long long)d.N * p.RP;
-        fk::fk_gemm_reduce_kernel<float, float><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
+        FK_TIMED("fk_gemm_reduce", s) fk::fk_gemm_reduce_kernel<float, float><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
             gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, tp.ksplit);
         e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward reduce launch failed: %s", cudaGetErrorString(e));
@@ -593,19 +623,16 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
-        size_t slot = 0;
-        const bool timed = r0 == 0 && g_prof.begin(s, slot);
         cudaError_t e;
         if (fewrows) {
             constexpr int VW = fk::VecWidth<TS>::value;
             const dim3 grid(std::max(1, sm_count()) * 16, pl.fsplit);
-            if (rt == 1) fk::fk_fwd_fewrows_kernel<T, VW, 1, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
-            else if (rt == 2) fk::fk_fwd_fewrows_kernel<T, VW, 2, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
-            else fk::fk_fwd_fewrows_kernel<T, VW, 4, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            if (rt == 1) FK_TIMED("fk_fwd_fewrows", s) fk::fk_fwd_fewrows_kernel<T, VW, 1, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            else if (rt == 2) FK_TIMED("fk_fwd_fewrows", s) fk::fk_fwd_fewrows_kernel<T, VW, 2, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            else FK_TIMED("fk_fwd_fewrows", s) fk::fk_fwd_fewrows_kernel<T, VW, 4, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
             e = cudaGetLastError();
         } else
             e = fwd_dispatch<T, false, TS>(d.vec_ok, rt, p, fgrid, s);
-        if (timed) g_prof.end(s, slot);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "forward kernel launch failed: %s", cudaGetErrorString(e));
         ++nl;
         r0 += rt;
@@ -621,7 +648,7 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
         q.R = R;
         const long long outs = (long long)d.N * R;
         const int grid = (int)std::min<long long>((outs + 7) / 8, (long long)sm_count() * 8);
-        fk::fk_reduce_chunks_kernel<T, false><<<std::max(1, grid), 256, 0, s>>>(q);
+        FK_TIMED("fk_reduce_chunks", s) launch_pdl(fk::fk_reduce_chunks_kernel<T, false>, std::max(1, grid), 256, 0, s, q);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "reduce kernel launch failed: %s", cudaGetErrorString(e));
         ++nl;
@@ -672,8 +699,8 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
         q.df = df;
         q.R = R;
         const long long slots = (long long)d.nfl * d.nx;
-        fk::fk_vjp_foldk_kernel<T, false><<<dim3(d.C * q.nchunk, R), fk::FOLDK_THREADS, foldk_smem(d.nx), s>>>(q);
-        fk::fk_vjp_foldk_final_kernel<T, false><<<dim3((unsigned)((slots + 7) / 8), R), 256, 0, s>>>(q, slots);
+        FK_TIMED("fk_vjp_foldk", s) launch_pdl(fk::fk_vjp_foldk_kernel<T, false>, dim3(d.C * q.nchunk, R), fk::FOLDK_THREADS, foldk_smem(d.nx), s, q);
+        FK_TIMED("fk_vjp_foldk_final", s) launch_pdl(fk::fk_vjp_foldk_final_kernel<T, false>, dim3((unsigned)((slots + 7) / 8), R), 256, 0, s, q, slots);
         ++nl;
     } else {
         fk::GatherParams q;
@@ -684,7 +711,7 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
         q.G = G;
         q.df = df;
         q.R = R;
-        fk::fk_vjp_gather_kernel<T, false><<<dim3(d.nfl * d.nx, R), fk::GATHER_THREADS, 0, s>>>(q);
+        FK_TIMED("fk_vjp_gather", s) fk::fk_vjp_gather_kernel<T, false><<<dim3(d.nfl * d.nx, R), fk::GATHER_THREADS, 0, s>>>(q);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gather kernel launch failed: %s", cudaGetErrorString(e));
@@ -728,7 +755,7 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.fwd.r0 = r0;
-#define FK_FUSED(V, RTv) fk::fk_fused_column_kernel<T, V, RTv, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
+#define FK_FUSED(V, RTv) FK_TIMED("fk_fused_column", s) fk::fk_fused_column_kernel<T, V, RTv, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
         if (d.vec_ok) {
             if (rt == 1) FK_FUSED(VW, 1); else if (rt == 2) FK_FUSED(VW, 2); else FK_FUSED(VW, 4);
         } else {
@@ -748,7 +775,7 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
         q.R = R;
         const long long outs = (long long)d.N * R;
         const int rgrid = (int)std::min<long long>((outs + 7) / 8, (long long)sm_count() * 8);
-        fk::fk_reduce_chunks_kernel<T, false><<<std::max(1, rgrid), 256, 0, s>>>(q);
+        FK_TIMED("fk_reduce_chunks", s) launch_pdl(fk::fk_reduce_chunks_kernel<T, false>, std::max(1, rgrid), 256, 0, s, q);
         ++nl;
     }
     if (!ensure_dyn_smem(fk::fk_vjp_foldk_kernel<T, false>, foldk_smem(128)))
@@ -767,8 +794,8 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
     q.df = df;
     q.R = R;
     const long long slots = (long long)d.nfl * d.nx;
-    fk::fk_vjp_foldk_kernel<T, false><<<dim3(d.C * q.nchunk, R), fk::FOLDK_THREADS, foldk_smem(d.nx), s>>>(q);
-    fk::fk_vjp_foldk_final_kernel<T, false><<<dim3((unsigned)((slots + 7) / 8), R), 256, 0, s>>>(q, slots);
+    FK_TIMED("fk_vjp_foldk", s) launch_pdl(fk::fk_vjp_foldk_kernel<T, false>, dim3(d.C * q.nchunk, R), fk::FOLDK_THREADS, foldk_smem(d.nx), s, q);
+    FK_TIMED("fk_vjp_foldk_final", s) launch_pdl(fk::fk_vjp_foldk_final_kernel<T, false>, dim3((unsigned)((slots + 7) / 8), R), 256, 0, s, q, slots);
     nl += 2;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(FK_ERR_CUDA, "fused forward + VJP launch failed: %s", cudaGetErrorString(e));
@@ -983,21 +1010,44 @@ int fk_profile_enable(int on) {
     g_prof.on = on != 0;
     return FK_OK;
 }
-int fk_profile_read(double* mean_kernel_ms, int* launches) {
-    std::lock_guard<std::mutex> lk(g_prof.mu);
-    double tot = 0.0;
-    int n = 0;
+// finished records of the current batch, summed per kernel name; clears the batch
+static void prof_collect(std::vector<std::pair<const char*, std::pair<int, double>>>& out) {
     for (size_t i = 0; i < g_prof.used; ++i) {
         float ms = 0.f;
-        if (cudaEventSynchronize(g_prof.pairs[i].second) == cudaSuccess &&
-            cudaEventElapsedTime(&ms, g_prof.pairs[i].first, g_prof.pairs[i].second) == cudaSuccess) {
-            tot += ms;
-            ++n;
-        }
+        if (cudaEventSynchronize(g_prof.recs[i].b) != cudaSuccess ||
+            cudaEventElapsedTime(&ms, g_prof.recs[i].a, g_prof.recs[i].b) != cudaSuccess)
+            continue;
+        bool found = false;
+        for (auto& o : out)
+            if (!strcmp(o.first, g_prof.recs[i].name)) { o.second.first++; o.second.second += ms; found = true; break; }
+        if (!found) out.push_back({g_prof.recs[i].name, {1, (double)ms}});
     }
     g_prof.used = 0;
-    if (mean_kernel_ms) *mean_kernel_ms = n ? tot / n : 0.0;
-    if (launches) *launches = n;
+}
+int fk_profile_read(double* mean_kernel_ms, int* launches) {
+    std::lock_guard<std::mutex> lk(g_prof.mu);
+    std::vector<std::pair<const char*, std::pair<int, double>>> v;
+    prof_collect(v);
+    // the record with the largest total time (the dominant kernel of what ran)
+    const std::pair<const char*, std::pair<int, double>>* best = nullptr;
+    for (auto& o : v)
+        if (!best || o.second.second > best->second.second) best = &o;
+    if (mean_kernel_ms) *mean_kernel_ms = best ? best->second.second / best->second.first : 0.0;
+    if (launches) *launches = best ? best->second.first : 0;
+    return FK_OK;
+}
+int fk_profile_report(char* buf, int capacity) {
+    if (!buf || capacity <= 0) return fail(FK_ERR_INVALID_ARG, "fk_profile_report: no buffer");
+    std::lock_guard<std::mutex> lk(g_prof.mu);
+    std::vector<std::pair<const char*, std::pair<int, double>>> v;
+    prof_collect(v);
+    int pos = 0;
+    buf[0] = 0;
+    for (auto& o : v) {
+        const int n = snprintf(buf + pos, (size_t)(capacity - pos), "%s\t%d\t%.9g\n", o.first, o.second.first, o.second.second);
+        if (n < 0 || n >= capacity - pos) return fail(FK_ERR_INVALID_ARG, "fk_profile_report: buffer of %d bytes is too small", capacity);
+        pos += n;
+    }
     return FK_OK;
 }
 
@@ -1158,8 +1208,8 @@ int table_vjp_any(fk_table* t, const void* f, const void* g, void* df, int R, cu
     return t->dtype == FK_F64 ? table_vjp_t<double>(t, f, g, df, R, s) : table_vjp_t<float>(t, f, g, df, R, s);
 }
 int chi2_launch(const double* sigma, const double* data, const double* cinv, double* chi2, double* g, int N, int R, cudaStream_t s) {
-    fk::fk_chi2_grad_kernel<<<N, dim3(32, 8), 0, s>>>(sigma, data, cinv, g, N, R);
-    fk::fk_chi2_sum_kernel<<<(R + 7) / 8, 256, 0, s>>>(sigma, data, g, chi2, N, R);
+    FK_TIMED("fk_chi2_grad", s) fk::fk_chi2_grad_kernel<<<N, dim3(32, 8), 0, s>>>(sigma, data, cinv, g, N, R);
+    FK_TIMED("fk_chi2_sum", s) fk::fk_chi2_sum_kernel<<<(R + 7) / 8, 256, 0, s>>>(sigma, data, g, chi2, N, R);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(FK_ERR_CUDA, "fk_chi2 launch failed: %s", cudaGetErrorString(e));
     return FK_OK;

@@ -12,6 +12,14 @@ constexpr int KIND_HADRONIC = 1;
 constexpr int LAYOUT_LOGICAL = 0;  // hadronic k = (i*nx + j)*C + c ; DIS k = i*nA + c   (BASELINE.json order)
 constexpr int LAYOUT_PACKED = 1;   // hadronic k = c*cstride + i*nx + j, cstride = nx*nx rounded up to 4 (zero padded) ; DIS k = c*nx + i
 
+// Programmatic dependent launch (PDL): the later kernels of a compute call are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization (fk_api.cu, launch_pdl).  A kernel calls pdl_trigger() first thing, so
+// that its successor's CTAs are scheduled (and run their prologue) as soon as every CTA of this grid has STARTED, and
+// pdl_wait() before its first access to global memory that a predecessor in the stream may write or still read: the wait
+// returns once the whole predecessor grid has completed and its memory is visible.  Both are no-ops in a normal launch.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 constexpr int MAX_C = 1024;   // active flavour pairs / flavours per table
 constexpr int MAX_NFL = 256;  // flavour indices are stored as uint8
 

@@ -60,6 +60,7 @@ __device__ __forceinline__ double fold_rows(double (&p)[U], int lane) {
 template <typename T, int VEC, int RT, int U, bool GROUPED, typename TS = T>
 __global__ void __launch_bounds__(FWD_THREADS)
 fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
+    pdl_trigger();   // first kernel of a call (normal launch): lets the level-2 reduction be scheduled under this grid's last wave
     using V = Vec<TS, VEC>;
     constexpr int LPR = 32 / U;  // lanes that end up holding the same row
     __shared__ double red[2][FWD_WARPS][U][RT];
@@ -161,6 +162,7 @@ fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
 template <typename T, int VEC, int RT, int U, typename TS = T>
 __global__ void __launch_bounds__(FWD_THREADS)
 fk_fwd_fewrows_kernel(const __grid_constant__ FwdParams p) {
+    pdl_trigger();
     using V = Vec<TS, VEC>;
     constexpr int LPR = 32 / U;
     __shared__ double red[2][FWD_WARPS][U][RT];
@@ -247,6 +249,7 @@ struct FusedParams {
 template <typename T, int VEC, int RT, int U, typename TS = T>
 __global__ void __launch_bounds__(FWD_THREADS)
 fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
+    pdl_trigger();
     using V = Vec<TS, VEC>;
     constexpr int LPR = 32 / U;
     constexpr int MAX_ROWS = 64;  // datapoints per range (the plan uses <= 32)
@@ -370,6 +373,8 @@ struct ReduceParams {
 
 template <typename T, bool GROUPED>
 __global__ void __launch_bounds__(256) fk_reduce_chunks_kernel(const __grid_constant__ ReduceParams p) {
+    pdl_trigger();
+    pdl_wait();   // the level-1 partials of the whole forward grid
     const int lane = threadIdx.x & 31;
     const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;

@@ -90,7 +90,7 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
         p.descs = g->d_descs;
         p.items = g->d_gitems;
         const long long tf = g->ai_total * p.RP;
-        fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
+        FK_TIMED("fk_transpose_f_grouped", s) fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
             f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, p.RP);
         const size_t ws_smem = fk::ws_smem_bytes(g->nx_max, p.RP);
         if (g->ws_all && opt(FK_OPT_WARP_SPEC) && ws_smem <= MAX_DYN_SMEM) {
@@ -103,10 +103,10 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
             w.items = g->d_witems;
             if (!ws_launch<true>(w, g->nwitems, ws_smem, s))
                 return fail(FK_ERR_CUDA, "grouped gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
-        } else if (g->all_vec) fk::fk_gemm_fwd_kernel<2, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
-        else fk::fk_gemm_fwd_kernel<1, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        } else if (g->all_vec) FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<2, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        else FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<1, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         const long long outs = g->rows_total * p.RP;
-        fk::fk_gemm_reduce_grouped_kernel<double><<<(int)std::min<long long>(8192, (outs + 255) / 256), 256, 0, s>>>(
+        FK_TIMED("fk_gemm_reduce_grouped", s) fk::fk_gemm_reduce_grouped_kernel<double><<<(int)std::min<long long>(8192, (outs + 255) / 256), 256, 0, s>>>(
             gpart, sigma_cat, g->d_descs, g->d_row_prefix, g->T, g->rows_total, R, r0, p.RP);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gemm forward launch failed: %s", cudaGetErrorString(e));
@@ -127,10 +127,10 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
         const int RP = fk::gemm_rp8(R - r0);
         const long long tf = g->ai_total * RP, tg = g->rows_total * RP;
-        fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
+        FK_TIMED("fk_transpose_f_grouped", s) fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
             f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, RP);
         // g_cat is [global row][R]: the single-table kernel pads all tables at once
-        fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(4096, (tg + 255) / 256), 256, 0, s>>>(g_cat, gP, (int)g->rows_total, R, r0, RP);
+        FK_TIMED("fk_pad_g", s) fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(4096, (tg + 255) / 256), 256, 0, s>>>(g_cat, gP, (int)g->rows_total, R, r0, RP);
         fk::GemmVjpParams p;
         memset(&p, 0, sizeof p);
         p.gP = gP;
@@ -150,8 +150,8 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             w.descs = g->d_descs;
             w.items = g->d_vitems;
             if (!wsv_launch<true>(w, s)) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
-        } else if (g->all_vec) fk::fk_gemm_vjp_kernel<2, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
-        else fk::fk_gemm_vjp_kernel<1, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        } else if (g->all_vec) FK_TIMED("fk_gemm_vjp", s) fk::fk_gemm_vjp_kernel<2, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
+        else FK_TIMED("fk_gemm_vjp", s) fk::fk_gemm_vjp_kernel<1, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         if (g->fold_all) {
             fk::FoldParams q;
             memset(&q, 0, sizeof q);
@@ -170,9 +170,9 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             q.T = g->T;
             q.nslots = fk::fold_slots(g->nx_max, RP, MAX_DYN_SMEM);
             if (!ensure_dyn_smem(fk::fk_vjp_fold_kernel<true>, MAX_DYN_SMEM) || q.nslots < 1) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve shared memory for the fold ring");
-            fk::fk_vjp_fold_kernel<true><<<g->nfoitems, fk::FOLD_THREADS,
+            FK_TIMED("fk_vjp_fold", s) fk::fk_vjp_fold_kernel<true><<<g->nfoitems, fk::FOLD_THREADS,
                                            (size_t)q.nslots * g->nx_max * RP * 8 + 2 * fk::FOLD_MAX_SLOTS * 8, s>>>(q);
-            fk::fk_vjp_fold_final_kernel<double, true><<<(unsigned)g->ai_total, fk::GEMM_BN, 0, s>>>(q);
+            FK_TIMED("fk_vjp_fold_final", s) fk::fk_vjp_fold_final_kernel<double, true><<<(unsigned)g->ai_total, fk::GEMM_BN, 0, s>>>(q);
             ++nl;
         } else {
             fk::GatherRParams q;
@@ -186,7 +186,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             q.descs = g->d_descs;
             q.ai_prefix = g->d_ai_prefix;
             q.T = g->T;
-            fk::fk_vjp_gather_r_kernel<double, true><<<dim3((unsigned)g->ai_total, (RP + 127) / 128), 128, 0, s>>>(q);
+            FK_TIMED("fk_vjp_gather_r", s) fk::fk_vjp_gather_r_kernel<double, true><<<dim3((unsigned)g->ai_total, (RP + 127) / 128), 128, 0, s>>>(q);
         }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gemm vjp launch failed: %s", cudaGetErrorString(e));
@@ -232,7 +232,7 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
         q.R = R;
         const long long outs = g->rows_total * R;
         const int grid = (int)std::min<long long>((outs + 7) / 8, (long long)sm_count() * 8);
-        fk::fk_reduce_chunks_kernel<T, true><<<std::max(1, grid), 256, 0, s>>>(q);
+        FK_TIMED("fk_reduce_chunks", s) launch_pdl(fk::fk_reduce_chunks_kernel<T, true>, std::max(1, grid), 256, 0, s, q);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped reduce launch failed: %s", cudaGetErrorString(e));
         ++nl;
@@ -282,8 +282,8 @@ int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat,
         q.nchunk = foldk_chunks(g->nkitems);
         q.df = df_cat;
         q.R = R;
-        fk::fk_vjp_foldk_kernel<T, true><<<dim3((unsigned)(g->nkitems * q.nchunk), R), fk::FOLDK_THREADS, foldk_smem(g->nx_max), s>>>(q);
-        fk::fk_vjp_foldk_final_kernel<T, true><<<dim3((unsigned)((g->ai_total + 7) / 8), R), 256, 0, s>>>(q, g->ai_total);
+        FK_TIMED("fk_vjp_foldk", s) launch_pdl(fk::fk_vjp_foldk_kernel<T, true>, dim3((unsigned)(g->nkitems * q.nchunk), R), fk::FOLDK_THREADS, foldk_smem(g->nx_max), s, q);
+        FK_TIMED("fk_vjp_foldk_final", s) launch_pdl(fk::fk_vjp_foldk_final_kernel<T, true>, dim3((unsigned)((g->ai_total + 7) / 8), R), 256, 0, s, q, g->ai_total);
         ++nl;
     } else {
         fk::GatherParams q;
@@ -295,7 +295,7 @@ int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat,
         q.G = g->scratch;
         q.df = df_cat;
         q.R = R;
-        fk::fk_vjp_gather_kernel<T, true><<<dim3((unsigned)g->ai_total, R), fk::GATHER_THREADS, 0, s>>>(q);
+        FK_TIMED("fk_vjp_gather", s) fk::fk_vjp_gather_kernel<T, true><<<dim3((unsigned)g->ai_total, R), fk::GATHER_THREADS, 0, s>>>(q);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gather launch failed: %s", cudaGetErrorString(e));

@@ -32,6 +32,8 @@ constexpr int COLSUM_MAX_ROWS = 512;  // datapoints per split (bounds the g tile
 template <typename T, int VEC, int RT, int UNROLL, bool GROUPED, typename TS = T>
 __global__ void __launch_bounds__(COLSUM_THREADS)
 fk_colsum_kernel(const __grid_constant__ ColsumParams p) {
+    pdl_trigger();
+    pdl_wait();
     using V = Vec<TS, VEC>;
     constexpr int NACC = (RT == 1) ? 4 : 2;
     __shared__ T gs[(COLSUM_MAX_ROWS + UNROLL) * RT];
@@ -234,6 +236,8 @@ constexpr int FOLDK_THREADS = 256;
 template <typename T, bool GROUPED>
 __global__ void __launch_bounds__(FOLDK_THREADS)
 fk_vjp_foldk_kernel(const __grid_constant__ FoldKParams p) {
+    pdl_trigger();
+    pdl_wait();   // the column sums G of the whole stage-1 grid
     extern __shared__ __align__(128) unsigned char fk_smem[];
     double* Gs = reinterpret_cast<double*>(fk_smem);  // [nx][nx | 1]
     const TableDesc* dp = &p.desc;
@@ -290,6 +294,7 @@ fk_vjp_foldk_kernel(const __grid_constant__ FoldKParams p) {
 template <typename T, bool GROUPED>
 __global__ void __launch_bounds__(256)
 fk_vjp_foldk_final_kernel(const __grid_constant__ FoldKParams p, long long slots_total) {
+    pdl_wait();   // PA / PB of the whole fold grid
     const long long gs = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (gs >= slots_total) return;

@@ -23,11 +23,11 @@ FK_KIND_DIS, FK_KIND_HADRONIC = 0, 1
 FK_F64, FK_F32, FK_F32S64 = 0, 1, 2
 FK_STORE_BORROW, FK_STORE_PACK = 0, 1
 (FK_OPT_GEMM_MIN_R, FK_OPT_WARP_SPEC, FK_OPT_FOLD, FK_OPT_FOLDK, FK_OPT_FUSED, FK_OPT_FEWROWS, FK_OPT_TC32,
- FK_OPT_TC32_MIN_R) = range(8)
+ FK_OPT_TC32_MIN_R, FK_OPT_PDL) = range(9)
 
 # every symbol include/fkconv.h declares
 SYMBOLS = (
-    "fk_last_error_string", "fk_version", "fk_compiled_arch", "fk_profile_enable", "fk_profile_read", "fk_set_option", "fk_get_option",
+    "fk_last_error_string", "fk_version", "fk_compiled_arch", "fk_profile_enable", "fk_profile_read", "fk_profile_report", "fk_set_option", "fk_get_option",
     "fk_conv_dis", "fk_conv_hadronic", "fk_conv_hadronic_vjp", "fk_conv_dis_vjp",
     "fk_conv_dis_f32", "fk_conv_hadronic_f32", "fk_conv_hadronic_vjp_f32",
     "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp", "fk_table_conv_vjp", "fk_chi2", "fk_table_fit_step",
@@ -55,6 +55,7 @@ lib.fk_profile_enable.argtypes = [_ci]
 lib.fk_set_option.argtypes = [_ci, _ci]
 lib.fk_get_option.argtypes = [_ci, ctypes.POINTER(_ci)]
 lib.fk_profile_read.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(_ci)]
+lib.fk_profile_report.argtypes = [ctypes.c_char_p, _ci]
 lib.fk_table_create.argtypes = [ctypes.POINTER(_vp), _ci, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _ci, _ci]
 lib.fk_table_destroy.argtypes = [_vp]
 lib.fk_table_info.argtypes = [_vp] + [ctypes.POINTER(_ci)] * 4 + [ctypes.POINTER(ctypes.c_int64)] * 3
@@ -132,6 +133,21 @@ def get_option(option: int) -> int:
     v = _ci()
     _check(lib.fk_get_option(option, ctypes.byref(v)), "fk_get_option")
     return v.value
+
+
+def profile_enable(on: bool) -> None:
+    _check(lib.fk_profile_enable(1 if on else 0), "fk_profile_enable")
+
+
+def profile_report() -> dict:
+    """{kernel name: (launches, total milliseconds)} of the launches recorded since the last report."""
+    buf = ctypes.create_string_buffer(1 << 16)
+    _check(lib.fk_profile_report(buf, len(buf)), "fk_profile_report")
+    out = {}
+    for ln in buf.value.decode().splitlines():
+        name, n, ms = ln.split("\t")
+        out[name] = (int(n), float(ms))
+    return out
 
 
 def version() -> int:

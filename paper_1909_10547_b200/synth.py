@@ -172,12 +172,13 @@ def config4_shapes(T: int = 60, scale_to_sumN: int | None = None) -> RaggedShape
     return RaggedShapes(N.astype(np.int64), nx.astype(np.int64), C.astype(np.int64))
 
 
-def config4_table(t: int, shapes: RaggedShapes, R: int, params=None) -> HadronicCase:
+def config4_table(t: int, shapes: RaggedShapes, R: int, params=None, with_fk: bool = True) -> HadronicCase:
     """Table t of the ragged batch.  One PDF (A,p,q) per replica, sampled on each table's own
-    x-grid (reading R14)."""
+    x-grid (reading R14).  with_fk=False: the table is a zero-memory placeholder of the right shape (a rank of a
+    sharded run needs f, g and the shapes of the tables it does not own, not their entries)."""
     N, nx, C = int(shapes.N[t]), int(shapes.nx[t]), int(shapes.C[t])
     pairs = draw_pairs(rng_for(4, T_PAIRS, t + 1), C)
-    fk = normal_table(rng_for(4, T_FK, t + 1), (N, nx, nx, C))
+    fk = normal_table(rng_for(4, T_FK, t + 1), (N, nx, nx, C)) if with_fk else np.broadcast_to(np.zeros((), dtype=np.float64), (N, nx, nx, C))
     if params is None:
         params = pdf_params(rng_for(4, T_PDF), R)
     f = pdf_grid(params, nx)

@@ -69,3 +69,31 @@ def test_step_bytes_counts_two_table_reads():
     case = synth.hadronic_case(6, 4, 5, 3, 1, sub=9)
     b = bench.step_bytes(case)
     assert b == 2 * case.fk.nbytes + 3 * case.f.nbytes + 2 * case.N * 8
+
+
+def test_gpus_n_fails_loudly_without_n_devices():
+    """`python bench.py --gpus 2` must never print an N=1 line: without a torchrun environment it spawns the ranks
+    itself, and on a node with fewer than 2 GPUs (this CPU box: 0) it refuses."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0"],
+                       env=env, capture_output=True, text=True, timeout=180)
+    assert p.returncode != 0
+    assert p.stdout.strip() == ""
+    assert "--gpus 2" in p.stderr and "refusing" in p.stderr
+
+
+def test_world_size_must_match_gpus_flag():
+    env = dict(os.environ, RANK="0", LOCAL_RANK="0", WORLD_SIZE="4")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0"],
+                       env=env, capture_output=True, text=True, timeout=180)
+    assert p.returncode != 0 and "WORLD_SIZE=4" in p.stderr
+
+
+def test_reference_arm_reports_one_gpu():
+    """The reference arm runs on rank 0's host cores: its line says n_gpus 1 whatever --gpus is."""
+    env = dict(os.environ, RANK="0", WORLD_SIZE="2", OMP_NUM_THREADS="4")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0, p.stderr
+    line = json.loads(p.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["n_gpus"] == 1 and line["value"] > 0
