@@ -226,7 +226,7 @@ int check_dims(const char* who, int kind, int N, int nx, int nfl, int C, int R) 
         return fail(FK_ERR_INVALID_ARG, "%s: non-positive size (N=%d nx=%d nfl=%d C=%d R=%d)", who, N, nx, nfl, C, R);
     if (nfl > fk::MAX_NFL || C > fk::MAX_C)
         return fail(FK_ERR_UNSUPPORTED, "%s: nfl=%d > %d or C=%d > %d", who, nfl, fk::MAX_NFL, C, fk::MAX_C);
-    const long long K = kind == FK_KIND_HADRONIC ? (long long)C * ((long long)nx * nx + 3) : (long long)C * nx;
+    const long long K = kind == FK_KIND_HADRONIC ? (long long)C * ((long long)nx * (nx + 3) + 3) : (long long)C * nx;   // padded x-rows (packed_jp)
     if (K >= (1LL << 31) - 4096) return fail(FK_ERR_UNSUPPORTED, "%s: K=%lld does not fit 31 bits", who, K);
     if ((long long)nfl * nx >= (1LL << 31) - 4096) return fail(FK_ERR_UNSUPPORTED, "%s: nfl*nx does not fit 31 bits", who);
     if (kind == FK_KIND_DIS && C > nfl)
@@ -247,12 +247,17 @@ int fill_channels(const char* who, int kind, const int32_t* idx, int nfl, int C,
     return FK_OK;
 }
 
+// x-row pitch of a packed hadronic table: fp32 tables (FK_F32) pad nx to a multiple of 4, so that every (c, i) row starts
+// on a 16-byte boundary -- what a TMA box needs (fk_tc32.cu); all others are dense (jp = nx)
+int packed_jp(int kind, int nx, int dtype) { return (kind == FK_KIND_HADRONIC && dtype == FK_F32) ? (nx + 3) / 4 * 4 : nx; }
+
 fk::TableDesc make_desc(int kind, int layout, const void* fkp, int N, int nx, int nfl, int C, long long row_stride,
                         int dtype) {
     fk::TableDesc d;
     memset(&d, 0, sizeof d);
     d.fk = fkp;
-    d.cstride = (layout == fk::LAYOUT_PACKED && kind == FK_KIND_HADRONIC) ? (nx * nx + 3) / 4 * 4 : nx * nx;
+    d.jp = layout == fk::LAYOUT_PACKED ? packed_jp(kind, nx, dtype) : nx;
+    d.cstride = (layout == fk::LAYOUT_PACKED && kind == FK_KIND_HADRONIC) ? (nx * d.jp + 3) / 4 * 4 : nx * nx;
     d.K = kind == FK_KIND_HADRONIC ? C * d.cstride : C * nx;
     d.row_stride = row_stride > 0 ? row_stride : d.K;
     d.N = N; d.nx = nx; d.nfl = nfl; d.C = C;
@@ -337,7 +342,7 @@ constexpr size_t MAX_DYN_SMEM = 232448;  // 227 KB per CTA on sm_100a
 
 // the warp-specialised kernel (fk_gemm_ws.cuh) serves packed hadronic tables whose f[b_c] tiles fit next to the FK ring
 bool ws_ok(const fk::TableDesc& d, int RP) {
-    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok && opt(FK_OPT_WARP_SPEC) &&
+    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok && d.jp == d.nx && opt(FK_OPT_WARP_SPEC) &&
            fk::ws_smem_bytes(d.nx, RP) <= MAX_DYN_SMEM;
 }
 
@@ -432,7 +437,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
 
 // the single-pass fold (fk_vjp_fold.cuh) serves packed hadronic tables with nx <= 64; others take the gather
 bool fold_ok(const fk::TableDesc& d) {
-    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.nx <= fk::FOLD_MAX_NX && opt(FK_OPT_FOLD);
+    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.jp == d.nx && d.nx <= fk::FOLD_MAX_NX && opt(FK_OPT_FOLD);
 }
 // x-row chunks per channel: the CTA count (channels x chunks) that fills whole waves best (1 CTA of 256 threads
 // per SM by registers), preferring fewer chunks (each chunk writes its own B partial)
@@ -534,24 +539,22 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
 }
 
 // ---- fp32 variant at R >> 1: tcgen05 3xTF32 contraction (fk_tc32.cu) ------------------------------------------------
-constexpr int TC32_DEFAULT_MIN_R = 9;   // from 3 column passes of <= 4 replicas on
+constexpr int TC32_DEFAULT_MIN_R = 5;   // from 2 column passes of <= 4 replicas on
 struct Tc32Plan {
-    int ksplit, kper, RPmax, fk_stages;
-    size_t smem;
+    int ksplit, tper, RPmax;
 };
 bool tc32_wanted(const fk::TableDesc& d, int R) {
-    if (!opt(FK_OPT_TC32) || !d.tmap || d.kind != fk::KIND_HADRONIC || d.layout != fk::LAYOUT_PACKED || d.nx < 8) return false;
-    if (R < (opt(FK_OPT_TC32_MIN_R) > 0 ? opt(FK_OPT_TC32_MIN_R) : TC32_DEFAULT_MIN_R)) return false;
-    return fk::tc32_smem_bytes(d.nx, fk::tc_rp(R), nullptr) > 0;
+    if (!opt(FK_OPT_TC32) || !d.tmap || d.kind != fk::KIND_HADRONIC || d.layout != fk::LAYOUT_PACKED || d.nx > fk::TC_MAX_NX || d.jp % 4) return false;
+    return R >= (opt(FK_OPT_TC32_MIN_R) > 0 ? opt(FK_OPT_TC32_MIN_R) : TC32_DEFAULT_MIN_R);
 }
 Tc32Plan tc32_plan(const fk::TableDesc& d, int R) {
     Tc32Plan tp;
     tp.RPmax = fk::tc_rp(R);
-    tp.smem = fk::tc32_smem_bytes(d.nx, tp.RPmax, &tp.fk_stages);
-    const int mtiles = fk::tc32_mtiles(d.N);
-    const int ksplit = std::max(1, std::max(1, sm_count()) / mtiles);   // one wave of equal items, one CTA per SM
-    tp.kper = ((d.K + ksplit - 1) / ksplit + fk::TC_KT - 1) / fk::TC_KT * fk::TC_KT;
-    tp.ksplit = (d.K + tp.kper - 1) / tp.kper;
+    const int ntiles = fk::tc32_ntiles(d.N), T = d.C * d.nx;   // datapoint tiles, (c, i) rows
+    int ksplit = std::max(1, std::min(T, std::max(1, sm_count()) / ntiles));   // one wave of equal items, one CTA per SM
+    ksplit = std::max(ksplit, (T + fk::TC_MAX_TILES - 1) / fk::TC_MAX_TILES);   // bounded fp32 chains in the epilogue
+    tp.tper = (T + ksplit - 1) / ksplit;
+    tp.ksplit = (T + tp.tper - 1) / tp.tper;
     return tp;
 }
 // scratch in doubles: fT32 [slots][RPmax] floats + level-1 partials [ksplit][N][RPmax] floats
@@ -577,14 +580,11 @@ int run_conv_tc32(const fk::TableDesc& d, const fk::ChannelList& ch, const float
         p.gpart = gpart;
         p.RP = fk::tc_rp(R - r0);
         p.ksplit = tp.ksplit;
-        p.kper = tp.kper;
-        int st = 0;
-        const size_t smem = fk::tc32_smem_bytes(d.nx, p.RP, &st);
-        p.fk_stages = st;
+        p.tper = tp.tper;
         const long long tot = (long long)slots * p.RP;
         FK_TIMED("fk_transpose_f", s) fk::fk_transpose_f_kernel<float, float><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
         cudaError_t e = cudaSuccess;
-        FK_TIMED("fk_tc32_fwd", s) e = fk::tc32_fwd_launch(p, fk::tc32_mtiles(d.N) * tp.ksplit, false, smem, s);
+        FK_TIMED("fk_tc32_fwd", s) e = fk::tc32_fwd_launch(p, fk::tc32_ntiles(d.N) * tp.ksplit, false, s);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward launch failed: %s", cudaGetErrorString(e));
         const long long outs = (long long)d.N * p.RP;
         FK_TIMED("fk_gemm_reduce", s) fk::fk_gemm_reduce_kernel<float, float><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
@@ -807,7 +807,7 @@ template <typename T>
 size_t conv_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
     if (gemm_wanted<T>(d, R)) return gemm_fwd_scratch_elems(d, R, with_kdec);
     if (std::is_same<T, float>::value && d.tmap && d.kind == fk::KIND_HADRONIC)   // either fp32 path may be selected later
-        return std::max(part_elems_per_replica(d) * R, fk::tc32_smem_bytes(d.nx, fk::tc_rp(R), nullptr) ? tc32_scratch_elems(d, R) : 0);
+        return std::max(part_elems_per_replica(d) * R, d.nx <= fk::TC_MAX_NX ? tc32_scratch_elems(d, R) : 0);
     return part_elems_per_replica(d) * R;
 }
 template <typename T>
@@ -1107,7 +1107,8 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
     if (t->sync.init() != FK_OK) { delete t; return fail(FK_ERR_CUDA, "fk_table_create: no CUDA device"); }
     t->dtype = dtype; t->store = store; t->kind = kind;
 
-    const int cstride = (nx * nx + 3) / 4 * 4;  // packed hadronic channel block (fk_common.cuh)
+    const int jp = packed_jp(kind, nx, dtype);
+    const int cstride = (nx * jp + 3) / 4 * 4;  // packed hadronic channel block (fk_common.cuh)
     const int K = kind == FK_KIND_HADRONIC ? C * (store == FK_STORE_PACK ? cstride : nx * nx) : C * nx;
     auto bail = [&](int code) { fk_table_destroy(t); return code; };
     if (store == FK_STORE_PACK) {
@@ -1120,10 +1121,10 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
         const int grid = (int)std::min<long long>((total + 255) / 256, 148LL * 64);
         if (dtype == FK_F64)
             fk::fk_pack_kernel<double><<<grid, 256>>>(fk_logical, (double*)t->owned_fk, N, nx, C,
-                                                     kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, cstride, row_stride);
+                                                     kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, cstride, jp, row_stride);
         else
             fk::fk_pack_kernel<float><<<grid, 256>>>(fk_logical, (float*)t->owned_fk, N, nx, C,
-                                                    kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, cstride, row_stride);
+                                                    kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS, K, cstride, jp, row_stride);
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaDeviceSynchronize();
         if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: pack kernel: %s", cudaGetErrorString(e)); }

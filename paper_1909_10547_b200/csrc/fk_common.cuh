@@ -10,7 +10,8 @@ namespace fk {
 constexpr int KIND_DIS = 0;
 constexpr int KIND_HADRONIC = 1;
 constexpr int LAYOUT_LOGICAL = 0;  // hadronic k = (i*nx + j)*C + c ; DIS k = i*nA + c   (BASELINE.json order)
-constexpr int LAYOUT_PACKED = 1;   // hadronic k = c*cstride + i*nx + j, cstride = nx*nx rounded up to 4 (zero padded) ; DIS k = c*nx + i
+constexpr int LAYOUT_PACKED = 1;   // hadronic k = c*cstride + i*jp + j, cstride = nx*jp rounded up to 4 (zero padded) ; DIS k = c*nx + i
+                                   // (jp = nx, except fp32 tables: nx rounded up to 4, so that every x-row starts on 16 bytes: TMA)
 
 // Programmatic dependent launch (PDL): the later kernels of a compute call are launched with
 // cudaLaunchAttributeProgrammaticStreamSerialization (fk_api.cu, launch_pdl).  A kernel calls pdl_trigger() first thing, so
@@ -36,7 +37,8 @@ struct TableDesc {
     long long row_stride; // elements (>= K; PACK pads it to a 16-byte multiple)
     int K;                // contraction length per datapoint: C*nx*nx (hadronic) or nA*nx (DIS)
     int N, nx, nfl, C;
-    int cstride;          // PACKED hadronic: elements per channel block (nx*nx rounded up to a multiple of 4)
+    int cstride;          // PACKED hadronic: elements per channel block (nx*jp rounded up to a multiple of 4)
+    int jp;               // PACKED hadronic: elements between consecutive x-rows i of a channel block (>= nx; the gap is zero)
     int kind, layout;
     int vec_ok;           // rows are 16-byte aligned -> 128-bit loads
     int store32;          // the table is stored in fp32 (FK_F32, FK_F32S64)
@@ -82,12 +84,12 @@ __device__ __forceinline__ void decode_k(const TableDesc& d, const uint8_t* __re
         } else {
             c = k / d.cstride;
             const int rem = k - c * d.cstride;
-            if (rem >= nx * nx) {  // zero padding at the end of a channel block: no luminosity
+            i = rem / d.jp;
+            j = rem - i * d.jp;
+            if (i >= nx || j >= nx) {  // zero padding at the end of an x-row or of a channel block: no luminosity
                 ia = ib = -1;
                 return;
             }
-            i = rem / nx;
-            j = rem - i * nx;
         }
         ia = (int)ca[c] * nx + i;
         ib = (int)cb[c] * nx + j;
@@ -108,7 +110,7 @@ __device__ __forceinline__ void decode_k(const TableDesc& d, const uint8_t* __re
 // Contraction index of (i, j, c) resp. (i, c) in the table's k-order (inverse of decode_k).
 __device__ __forceinline__ int encode_k(const TableDesc& d, int i, int j, int c) {
     if (d.kind == KIND_HADRONIC)
-        return d.layout == LAYOUT_LOGICAL ? (i * d.nx + j) * d.C + c : c * d.cstride + i * d.nx + j;
+        return d.layout == LAYOUT_LOGICAL ? (i * d.nx + j) * d.C + c : c * d.cstride + i * d.jp + j;
     return d.layout == LAYOUT_LOGICAL ? i * d.C + c : c * d.nx + i;
 }
 

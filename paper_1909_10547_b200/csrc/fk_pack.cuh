@@ -9,11 +9,11 @@
 namespace fk {
 
 // out[n][kp] = (T) in[n][klog(kp)],  kp in packed order (hadronic: channel blocks of cstride elements,
-// the tail of each block zero); pad columns [K, row_stride) = 0
+// x-rows jp apart, the tail of each x-row and of each block zero); pad columns [K, row_stride) = 0
 template <typename T>
 __global__ void __launch_bounds__(256)
 fk_pack_kernel(const double* __restrict__ in, T* __restrict__ out, int N, int nx, int C, int kind,
-               int K, int cstride, long long row_stride) {
+               int K, int cstride, int jp, long long row_stride) {
     const long long total = (long long)N * row_stride;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
          t += (long long)gridDim.x * blockDim.x) {
@@ -25,10 +25,8 @@ fk_pack_kernel(const double* __restrict__ in, T* __restrict__ out, int N, int nx
             long long klen;  // logical row length
             if (kind == KIND_HADRONIC) {
                 const int c = kp / cstride, rem = kp - c * cstride;
-                if (rem < nx * nx) {
-                    const int i = rem / nx, j = rem - i * nx;
-                    klog = (i * nx + j) * C + c;
-                }
+                const int i = rem / jp, j = rem - i * jp;
+                if (i < nx && j < nx) klog = (i * nx + j) * C + c;
                 klen = (long long)C * nx * nx;
             } else {
                 const int c = kp / nx, i = kp - c * nx;
