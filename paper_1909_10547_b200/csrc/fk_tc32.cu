@@ -80,6 +80,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int wha
         }
     }
 }
+// one lane of a converged warp (the same one every time): control flow stays warp-uniform around the single-thread
+// instructions (TMA, tcgen05.mma, tcgen05.commit), so their operands live in uniform registers
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}\n" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, int c0, int c1, uint32_t bar) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
                  "l"(tmap), "r"(bar), "r"(c0), "r"(c1)
@@ -137,7 +144,8 @@ template <bool GROUPED>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
     extern __shared__ unsigned char fk_smem_raw[];
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform: role branches do not diverge
 
     const TableDesc* dp = &p.desc;
     const uint8_t* __restrict__ cha = p.chan.a;
@@ -206,8 +214,9 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
     if (warp < 4) {
         // ============================ control warpgroup ============================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
-        if (warp == 0 && lane == 0) {
+        if (warp == 0) {
             // ---- TMA producer: the raw FK rows of (c, i) for 128 datapoints -> ring slot t % TC_RAW_STAGES
+            const bool leader = elect_one();
             const uint32_t tx = nk8 > 4 ? TC_STAGE_BYTES : TC_BOX_BYTES;
             int c = c_first, i = i_first;
             for (int t = 0; t < ntl; ++t) {
@@ -215,13 +224,17 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
                 mbar_wait(bar(BAR_FK_FREE + slot), ((t / TC_RAW_STAGES) & 1) ^ 1, 1);
                 const int k0 = c * cstride + i * jp;   // 16-byte aligned: jp and cstride are multiples of 4
                 const uint32_t dst = sm_raw + (uint32_t)slot * TC_STAGE_BYTES;
-                mbar_expect_tx(bar(BAR_FK_FULL + slot), tx);
-                tma_load_2d(dst, tmap, k0, n0, bar(BAR_FK_FULL + slot));
-                if (nk8 > 4) tma_load_2d(dst + TC_BOX_BYTES, tmap, k0 + 32, n0, bar(BAR_FK_FULL + slot));
+                if (leader) {
+                    mbar_expect_tx(bar(BAR_FK_FULL + slot), tx);
+                    tma_load_2d(dst, tmap, k0, n0, bar(BAR_FK_FULL + slot));
+                    if (nk8 > 4) tma_load_2d(dst + TC_BOX_BYTES, tmap, k0 + 32, n0, bar(BAR_FK_FULL + slot));
+                }
+                __syncwarp();
                 if (++i == nx) { i = 0; ++c; }
             }
-        } else if (warp == 1 && lane == 0) {
-            // ---- MMA issuer
+        } else if (warp == 1) {
+            // ---- MMA issuer: the whole warp walks the loop, one elected lane issues
+            const bool leader = elect_one();
             const uint32_t idesc = umma_idesc_tf32(128, NT);
             int i = i_first, cc = 0;
             bool newch = true;
@@ -236,28 +249,41 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
                 tc_fence_after();
                 const uint32_t d_acc = tmem_base + (uint32_t)buf * 128u;
                 const uint32_t a_hi = tmem_base + TC_TMEM_A + (uint32_t)abuf * 128u, a_lo = a_hi + 64u;
-                const uint32_t raw = sm_raw + (uint32_t)slot * TC_STAGE_BYTES, lo = sm_lo + (uint32_t)ls * TC_STAGE_BYTES;
-                for (int k8 = 0; k8 < nk8; ++k8) {
-                    // 8 fp32 = 32 bytes along the swizzle row; the second box holds k 32..63
-                    const uint64_t b = umma_desc_sw128(raw + (uint32_t)(k8 >> 2) * TC_BOX_BYTES) + (uint64_t)((k8 & 3) * 2);
-                    tc_mma_tf32_ts(d_acc, a_hi + 8u * (uint32_t)k8, b, idesc, k8 > 0 ? 1u : 0u);
-                    tc_mma_tf32_ts(d_acc, a_lo + 8u * (uint32_t)k8, b, idesc, 1u);
+                // 8 fp32 = 32 bytes (descriptor + 2) along the swizzle row; the second box holds k 32..63
+                const uint64_t braw = umma_desc_sw128(sm_raw + (uint32_t)slot * TC_STAGE_BYTES);
+                const uint64_t blo = umma_desc_sw128(sm_lo + (uint32_t)ls * TC_STAGE_BYTES);
+                if (leader) {
+#pragma unroll
+                    for (int k8 = 0; k8 < 8; ++k8) {
+                        if (k8 < nk8) {
+                            const uint64_t b = braw + (uint64_t)((k8 >> 2) * (TC_BOX_BYTES >> 4) + (k8 & 3) * 2);
+                            tc_mma_tf32_ts(d_acc, a_hi + 8u * (uint32_t)k8, b, idesc, k8 > 0 ? 1u : 0u);
+                            tc_mma_tf32_ts(d_acc, a_lo + 8u * (uint32_t)k8, b, idesc, 1u);
+                        }
+                    }
                 }
+                __syncwarp();
                 mbar_wait(bar(BAR_LO_FULL + ls), (t >> 1) & 1, 5);
                 tc_fence_after();
-                for (int k8 = 0; k8 < nk8; ++k8) {
-                    const uint64_t b = umma_desc_sw128(lo + (uint32_t)(k8 >> 2) * TC_BOX_BYTES) + (uint64_t)((k8 & 3) * 2);
-                    tc_mma_tf32_ts(d_acc, a_hi + 8u * (uint32_t)k8, b, idesc, 1u);
+                if (leader) {
+#pragma unroll
+                    for (int k8 = 0; k8 < 8; ++k8) {
+                        if (k8 < nk8) {
+                            const uint64_t b = blo + (uint64_t)((k8 >> 2) * (TC_BOX_BYTES >> 4) + (k8 & 3) * 2);
+                            tc_mma_tf32_ts(d_acc, a_hi + 8u * (uint32_t)k8, b, idesc, 1u);
+                        }
+                    }
+                    tc_commit(bar(BAR_FK_FREE + slot));
+                    tc_commit(bar(BAR_LO_FREE + ls));
+                    tc_commit(bar(BAR_ACC_FULL + buf));
                 }
-                tc_commit(bar(BAR_FK_FREE + slot));
-                tc_commit(bar(BAR_LO_FREE + ls));
-                tc_commit(bar(BAR_ACC_FULL + buf));
                 if (++i == nx) {   // last row of the channel: its fb operand buffer goes back to the builders
                     i = 0;
-                    tc_commit(bar(BAR_A_FREE + abuf));
+                    if (leader) tc_commit(bar(BAR_A_FREE + abuf));
                     ++cc;
                     newch = true;
                 }
+                __syncwarp();
             }
         }
     } else if (warp < 4 + TC_SPLIT_WARPS) {
