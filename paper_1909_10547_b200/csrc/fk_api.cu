@@ -584,11 +584,11 @@ int run_conv_tc32(const fk::TableDesc& d, const fk::ChannelList& ch, const float
         const long long tot = (long long)slots * p.RP;
         FK_TIMED("fk_transpose_f", s) fk::fk_transpose_f_kernel<float, float><<<(int)std::min<long long>(2048, (tot + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, p.RP);
         cudaError_t e = cudaSuccess;
-        FK_TIMED("fk_tc32_fwd", s) e = fk::tc32_fwd_launch(p, fk::tc32_ntiles(d.N) * tp.ksplit, false, s);
+        FK_TIMED("fk_tc32_fwd", s) e = fk::tc32_fwd_launch(p, fk::tc32_ntiles(d.N) * tp.ksplit, false, opt(FK_OPT_PDL) != 0, s);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward launch failed: %s", cudaGetErrorString(e));
         const long long outs = (long long)d.N * p.RP;
-        FK_TIMED("fk_gemm_reduce", s) fk::fk_gemm_reduce_kernel<float, float><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
-            gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, tp.ksplit);
+        FK_TIMED("fk_gemm_reduce", s) launch_pdl(fk::fk_gemm_reduce_kernel<float, float>, (int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s,
+                                                 gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, tp.ksplit);
         e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward reduce launch failed: %s", cudaGetErrorString(e));
         nl += 3;

@@ -91,6 +91,7 @@ __global__ void __launch_bounds__(256) fk_kdec_kernel(TableDesc d, ChannelList c
 template <typename T, typename O = double>
 __global__ void __launch_bounds__(256) fk_transpose_f_kernel(const T* __restrict__ f, O* __restrict__ fT, int slots,
                                                               int R, int r0, int RP) {
+    pdl_trigger();   // first kernel of a call: the contraction behind it may start its prologue and table loads now
     const long long total = (long long)slots * RP;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
         const int s = (int)(t / RP), c = (int)(t - (long long)s * RP);
@@ -256,6 +257,7 @@ fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
 template <typename T, typename P = double>
 __global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const P* __restrict__ gpart, T* __restrict__ sigma,
                                                               long long out_off, int N, int R, int r0, int RP, int ksplit) {
+    pdl_wait();   // the level-1 partials of the whole contraction grid (no-op in a normal launch)
     const long long total = (long long)N * RP;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
         const int n = (int)(t / RP), c = (int)(t - (long long)n * RP);

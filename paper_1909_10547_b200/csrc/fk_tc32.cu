@@ -146,6 +146,7 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
     extern __shared__ unsigned char fk_smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform: role branches do not diverge
+    pdl_trigger();   // the level-2 reduction may be scheduled under this grid's tail (it waits for the partials itself)
 
     const TableDesc* dp = &p.desc;
     const uint8_t* __restrict__ cha = p.chan.a;
@@ -315,6 +316,7 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
             if (lane == 0) mbar_arrive(bar(BAR_A_FULL + abuf));
         };
         int c = c_first, i = i_first, cc = 0;
+        pdl_wait();   // fT is written by the transpose kernel just before this launch (the table itself is not: TMA runs ahead)
         if (ntl > 0) build_a(0, c);
         bool build_next = c < c_last;   // the next channel's operand is built under the first row of this one
         const int nq = 2 * nk8;         // 16-byte chunks of a row
@@ -366,6 +368,7 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
         for (int e = 0; e < 64; ++e) acc[e] = tot[e] = 0.f;
         int c = c_first, i = i_first;
         auto load_fa = [&](int cq, int iq) { return r < RP ? __ldg(fT + ((long long)cha[cq] * nx + iq) * RP + r) : 0.f; };
+        pdl_wait();   // fT (see the builders); also orders the final gpart stores after the previous call's readers
         float fa_next = ntl > 0 ? load_fa(c, i) : 0.f;
         for (int t = 0; t < ntl; ++t) {
             const int buf = t & 1;
@@ -442,12 +445,22 @@ bool tc32_encode_tensor_map(void* out_host, const void* fk_dev, long long row_st
     return true;
 }
 
-cudaError_t tc32_fwd_launch(const Tc32Params& p, int grid, bool grouped, cudaStream_t s) {
+cudaError_t tc32_fwd_launch(const Tc32Params& p, int grid, bool grouped, bool pdl, cudaStream_t s) {
     auto kern = grouped ? fk_tc32_fwd_kernel<true> : fk_tc32_fwd_kernel<false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    kern<<<grid, TC_THREADS, TC_SMEM_BYTES, s>>>(p);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(TC_THREADS);
+    cfg.dynamicSmemBytes = TC_SMEM_BYTES;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // fk_common.cuh, pdl_wait
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, p);
 }
 
 }  // namespace fk

@@ -40,7 +40,8 @@ inline int tc32_ntiles(int N) { return (N + TC_BN - 1) / TC_BN; }
 // Writes the 128-byte tensor map of a packed fp32 table [N][row_stride] (box 32 k x 128 rows, 128-byte swizzle,
 // zero fill outside the table) to `out_host`.  false: the driver entry point is missing or refused the arguments.
 bool tc32_encode_tensor_map(void* out_host, const void* fk_dev, long long row_stride, int K, int N);
-// Launches the contraction; grid = datapoint tiles x ranges (single) or items (grouped).
-cudaError_t tc32_fwd_launch(const Tc32Params& p, int grid, bool grouped, cudaStream_t s);
+// Launches the contraction; grid = datapoint tiles x ranges (single) or items (grouped); pdl: as a programmatic
+// dependent launch behind the transpose kernel (the kernel waits for fT itself, fk_common.cuh pdl_wait).
+cudaError_t tc32_fwd_launch(const Tc32Params& p, int grid, bool grouped, bool pdl, cudaStream_t s);
 
 }  // namespace fk
