@@ -348,6 +348,10 @@ def run_config4(K, torch, peak):
         out[f"cfg4_grouped_vjp_R{R}"] = {"ms": ms, "GBps": nbytes / ms / 1e6, "frac_of_peak": nbytes / ms / 1e6 / peak,
                                          "TFLOPs": flops / ms / 1e9, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS,
                                          "launches": grp.last_launches()}
+        if R == 1:   # forward + VJP from one read of every table (fk_conv_grouped_conv_vjp)
+            ms = _bench_call(lambda: grp.conv_vjp(f_cat, g_cat, R, sig, df), stream, steps=nst, warmup=3)
+            out["cfg4_grouped_conv_vjp_one_read_R1"] = {"ms": ms, "GBps": nbytes / ms / 1e6, "frac_of_peak": nbytes / ms / 1e6 / peak,
+                                                        "step_equiv_GBps": 2 * nbytes / ms / 1e6, "launches": grp.last_launches()}
     grp.destroy()
     for t in tabs:
         t.destroy()

@@ -195,6 +195,14 @@ int fk_group_offsets(const fk_group* g, int R, int64_t* f_offsets, int64_t* sigm
 int fk_conv_grouped(fk_group* g, const void* f_cat, void* sigma_cat, int R, void* stream);
 int fk_conv_grouped_vjp(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat, int R,
                         void* stream);
+/* Forward AND VJP of the whole group from ONE read of every table, for a `g_cat` that is known before the forward
+ * pass (a loss linear in sigma: BASELINE config 4's seeded weights; the fit evaluates the
+ * convolution "and its corresponding gradient" every iteration).  Same results as fk_conv_grouped
+ * followed by fk_conv_grouped_vjp (sigma bit for bit; df within rounding: the column sums are cut into the
+ * forward's datapoint ranges).  One read applies for R <= 4 on groups of hadronic tables with nx <= 128; otherwise
+ * the call runs the two passes. */
+int fk_conv_grouped_conv_vjp(fk_group* g, const void* f_cat, const void* g_cat, void* sigma_cat, void* df_cat,
+                             int R, void* stream);
 int fk_group_last_launches(const fk_group* g);
 
 #ifdef __cplusplus

@@ -755,7 +755,7 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.fwd.r0 = r0;
-#define FK_FUSED(V, RTv) FK_TIMED("fk_fused_column", s) fk::fk_fused_column_kernel<T, V, RTv, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
+#define FK_FUSED(V, RTv) FK_TIMED("fk_fused_column", s) fk::fk_fused_column_kernel<T, V, RTv, FWD_U, false, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
         if (d.vec_ok) {
             if (rt == 1) FK_FUSED(VW, 1); else if (rt == 2) FK_FUSED(VW, 2); else FK_FUSED(VW, 4);
         } else {

@@ -246,7 +246,7 @@ struct FusedParams {
     double* G;       // [fsplit][R][K] column sums, one slice per datapoint range
 };
 
-template <typename T, int VEC, int RT, int U, typename TS = T>
+template <typename T, int VEC, int RT, int U, bool GROUPED, typename TS = T>
 __global__ void __launch_bounds__(FWD_THREADS)
 fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
     pdl_trigger();
@@ -256,17 +256,29 @@ fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
     __shared__ double red[2][FWD_WARPS][U][RT];
     __shared__ T gs[(MAX_ROWS + U) * RT];
     const FwdParams& p = q.fwd;
-    const TableDesc& d = p.desc;
+    const TableDesc* dp = &p.desc;
     const uint8_t* __restrict__ ca = p.chan.a;
     const uint8_t* __restrict__ cb = p.chan.b;
-    const int kblock = blockIdx.x % d.nchunks, split = blockIdx.x / d.nchunks;
+    int kblock, split;
+    if constexpr (GROUPED) {   // grouped: static list of (table, k-block, datapoint range) CTAs; descs carry the fused splits
+        const ColSeg sg = p.segs[blockIdx.x];
+        dp = &p.descs[sg.table];
+        ca = dp->chan_a;
+        cb = dp->chan_b;
+        kblock = sg.kblock;
+        split = sg.split;
+    } else {
+        kblock = blockIdx.x % p.desc.nchunks;
+        split = blockIdx.x / p.desc.nchunks;
+    }
+    const TableDesc& d = *dp;
     const int R = p.R;
     const int rb = (int)((long long)d.N * split / d.fsplit);
     const int re = (int)((long long)d.N * (split + 1) / d.fsplit);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     {   // g tile of this datapoint range, zero padded to a multiple of U rows
-        const T* __restrict__ g = reinterpret_cast<const T*>(q.g);
+        const T* __restrict__ g = reinterpret_cast<const T*>(q.g) + d.out_off * R;
         const int rows = re - rb, rows_pad = (rows + U - 1) / U * U;
         for (int t = threadIdx.x; t < rows_pad * RT; t += FWD_THREADS) {
             const int m = t / RT, r = t - m * RT, rr = p.r0 + r;
@@ -278,7 +290,7 @@ fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
     T L[RT][VEC];
     {
         const int fstride = d.nfl * d.nx;
-        const T* __restrict__ f = reinterpret_cast<const T*>(p.f);
+        const T* __restrict__ f = reinterpret_cast<const T*>(p.f) + d.f_off * R;
 #pragma unroll
         for (int e = 0; e < VEC; ++e) {
             int ia = 0, ib = -1;
@@ -341,9 +353,9 @@ fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
             const int n = m + u, rr = p.r0 + r;
             if (n < re && rr < R) {
                 if (d.nchunks == 1)
-                    reinterpret_cast<T*>(p.sigma)[(long long)n * R + rr] = (T)s;
+                    reinterpret_cast<T*>(p.sigma)[d.out_off * R + (long long)n * R + rr] = (T)s;
                 else
-                    p.part[((long long)n * R + rr) * d.nchunks + kblock] = s;
+                    p.part[d.part_off * R + ((long long)n * R + rr) * d.nchunks + kblock] = s;
             }
         }
     }
@@ -354,7 +366,7 @@ fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
             if (rr >= R) continue;
 #pragma unroll
             for (int e = 0; e < VEC; ++e)
-                if (k + e < d.K) q.G[((long long)split * R + rr) * d.K + k + e] = (double)cs[0][r][e] + (double)cs[1][r][e];
+                if (k + e < d.K) q.G[d.g_off * R + ((long long)split * R + rr) * d.K + k + e] = (double)cs[0][r][e] + (double)cs[1][r][e];
         }
     }
 }

@@ -38,6 +38,13 @@ struct fk_group {
     int fold_nchunk = 1;
     fk::ColSeg* d_foitems = nullptr;  // fold CTAs: {table, channel, x-row chunk}
     int nfoitems = 0;
+    // forward + VJP from one read of FK (fk_fused_column_kernel, GROUPED): the datapoint ranges of the fused CTAs
+    // (<= 64 rows) are also the slices of the column sums, so the group keeps a second set of descriptors
+    bool fused_all = true;
+    fk::TableDesc* d_descs_fused = nullptr;
+    fk::ColSeg* d_usegs = nullptr;
+    int nusegs = 0;
+    long long G_total1_fused = 0;
     double* scratch = nullptr;
     size_t scratch_elems = 0;
     int last_launches = 0;
@@ -70,6 +77,14 @@ size_t group_scratch_need(const fk_group* g, int R) {
         return ((size_t)g->ai_total + std::max(fwd, vjp)) * RP;
     }
     return std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1 + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R;
+}
+
+bool group_fused_wanted(const fk_group* g, int R) {
+    return g->fused_all && !group_gemm_wanted(g, R) && R <= 4 && opt(FK_OPT_FUSED);
+}
+// part [rows][R][nchunks] | G [fused splits][R][K] | fold partials
+size_t group_fused_scratch_need(const fk_group* g, int R) {
+    return ((size_t)g->part_total1 + (size_t)g->G_total1_fused + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R;
 }
 
 int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, cudaStream_t s) {
@@ -304,6 +319,90 @@ int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat,
     return FK_OK;
 }
 
+// forward + VJP of the whole group from ONE read of every table (g known before the forward pass, e.g.
+// config 4's seeded weights): one fused column launch per <= 4 replicas, the level-2 reduce, the one-pass fold.
+template <typename T, typename TS = T>
+int group_conv_vjp_fused_t(fk_group* g, const void* f_cat, const void* g_cat, void* sigma_cat, void* df_cat, int R, cudaStream_t s) {
+    constexpr int VW = fk::VecWidth<TS>::value;
+    int rc = group_scratch(g, group_fused_scratch_need(g, R), s);
+    if (rc) return rc;
+    double* part = g->scratch;
+    double* G = part + (size_t)g->part_total1 * R;
+    int nl = 0;
+    fk::FusedParams p;
+    memset(&p, 0, sizeof p);
+    p.fwd.descs = g->d_descs_fused;
+    p.fwd.segs = g->d_usegs;
+    p.fwd.f = f_cat;
+    p.fwd.part = part;
+    p.fwd.sigma = sigma_cat;
+    p.fwd.R = R;
+    p.g = g_cat;
+    p.G = G;
+    for (int r0 = 0; r0 < R;) {
+        const int rt = pick_rt(R - r0);
+        p.fwd.r0 = r0;
+#define FK_FUSED_G(V, RTv) FK_TIMED("fk_fused_column", s) fk::fk_fused_column_kernel<T, V, RTv, FWD_U, true, TS><<<g->nusegs, fk::FWD_THREADS, 0, s>>>(p)
+        if (g->all_vec) {
+            if (rt == 1) FK_FUSED_G(VW, 1); else if (rt == 2) FK_FUSED_G(VW, 2); else FK_FUSED_G(VW, 4);
+        } else {
+            if (rt == 1) FK_FUSED_G(1, 1); else if (rt == 2) FK_FUSED_G(1, 2); else FK_FUSED_G(1, 4);
+        }
+#undef FK_FUSED_G
+        ++nl;
+        r0 += rt;
+    }
+    if (g->part_total1 > 0) {
+        fk::ReduceParams q;
+        memset(&q, 0, sizeof q);
+        q.descs = g->d_descs_fused;
+        q.row_prefix = g->d_row_prefix;
+        q.T = g->T;
+        q.part = part;
+        q.sigma = sigma_cat;
+        q.rows = g->rows_total;
+        q.R = R;
+        const long long outs = g->rows_total * R;
+        const int grid = (int)std::min<long long>((outs + 7) / 8, (long long)sm_count() * 8);
+        FK_TIMED("fk_reduce_chunks", s) launch_pdl(fk::fk_reduce_chunks_kernel<T, true>, std::max(1, grid), 256, 0, s, q);
+        ++nl;
+    }
+    if (!ensure_dyn_smem(fk::fk_vjp_foldk_kernel<T, true>, foldk_smem(128)))
+        return fail(FK_ERR_CUDA, "grouped conv_vjp: cannot reserve %zu bytes of shared memory", foldk_smem(128));
+    fk::FoldKParams q;
+    memset(&q, 0, sizeof q);
+    q.descs = g->d_descs_fused;
+    q.items = g->d_kitems;
+    q.ai_prefix = g->d_ai_prefix;
+    q.T = g->T;
+    q.f = f_cat;
+    q.G = G;
+    q.cx_total = g->cx_total;
+    q.PA = G + (size_t)g->G_total1_fused * R;
+    q.PB = q.PA + (size_t)g->cx_total * R;
+    q.nchunk = foldk_chunks(g->nkitems);
+    q.df = df_cat;
+    q.R = R;
+    FK_TIMED("fk_vjp_foldk", s) launch_pdl(fk::fk_vjp_foldk_kernel<T, true>, dim3((unsigned)(g->nkitems * q.nchunk), R), fk::FOLDK_THREADS, foldk_smem(g->nx_max), s, q);
+    FK_TIMED("fk_vjp_foldk_final", s) launch_pdl(fk::fk_vjp_foldk_final_kernel<T, true>, dim3((unsigned)((g->ai_total + 7) / 8), R), 256, 0, s, q, g->ai_total);
+    nl += 2;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped fused forward + VJP launch failed: %s", cudaGetErrorString(e));
+    g->last_launches = nl;
+    return FK_OK;
+}
+
+template <typename T, typename TS = T>
+int group_conv_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* sigma_cat, void* df_cat, int R, cudaStream_t s) {
+    if (group_fused_wanted(g, R)) return group_conv_vjp_fused_t<T, TS>(g, f_cat, g_cat, sigma_cat, df_cat, R, s);
+    int rc = group_conv_t<T, TS>(g, f_cat, sigma_cat, R, s);   // two passes: R >= 5, DIS tables, very large x-grids
+    if (rc) return rc;
+    const int nl = g->last_launches;
+    rc = group_vjp_t<T, TS>(g, f_cat, g_cat, df_cat, R, s);
+    g->last_launches += nl;
+    return rc;
+}
+
 }  // namespace
 
 extern "C" {
@@ -340,7 +439,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     const long long want_items = (long long)std::max(1, sm_count()) * GROUP_GEMM_WAVES;
     long long kper_target = (tile_k + want_items - 1) / want_items;
     kper_target = std::max<long long>(fk::GEMM_KT * 8, (kper_target + fk::GEMM_KT - 1) / fk::GEMM_KT * fk::GEMM_KT);
-    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems, foitems, witems, kitems;
+    std::vector<fk::ColSeg> fsegs, csegs, gitems, vitems, foitems, witems, kitems, usegs;
+    std::vector<fk::TableDesc> descs_fused;
     long long group_kblocks = 0;
     for (int t = 0; t < T; ++t) group_kblocks += tables[t]->desc.nchunks;
     {
@@ -420,6 +520,17 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             for (int kb = 0; kb < d.nchunks; ++kb) csegs.push_back(fk::ColSeg{t, kb, sp, 0});
         g->tables.push_back(tb);
         g->descs.push_back(d);
+        {   // one-read forward + VJP: up to 64 datapoints per CTA; its ranges are the slices of the column sums
+            fk::TableDesc du = d;
+            du.fsplit = std::max(1, std::min(d.fsplit, (d.N + 63) / 64));
+            du.nsplit = du.fsplit;
+            du.g_off = g->G_total1_fused;
+            g->G_total1_fused += (long long)du.fsplit * du.K;
+            g->fused_all = g->fused_all && foldk_ok(du) && (du.N + du.fsplit - 1) / du.fsplit <= 64;
+            for (int sp = 0; sp < du.fsplit; ++sp)
+                for (int kb = 0; kb < du.nchunks; ++kb) usegs.push_back(fk::ColSeg{t, kb, sp, 0});
+            descs_fused.push_back(du);
+        }
     }
     if (g->rows_total >= (1LL << 31) || g->ai_total >= (1LL << 31)) {
         g->sync.destroy();
@@ -433,6 +544,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     g->nfoitems = (int)foitems.size();
     g->nwitems = (int)witems.size();
     g->nkitems = (int)kitems.size();
+    g->nusegs = (int)usegs.size();
     auto bail = [&](int code) { fk_group_destroy(g); return code; };
     cudaError_t e = cudaMalloc((void**)&g->d_descs, T * sizeof(fk::TableDesc));
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_row_prefix, (T + 1) * sizeof(int));
@@ -454,6 +566,10 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     if (e == cudaSuccess) e = cudaMemcpy(g->d_row_prefix, row_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_ai_prefix, ai_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_csegs, csegs.data(), csegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_descs_fused, T * sizeof(fk::TableDesc));
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_descs_fused, descs_fused.data(), T * sizeof(fk::TableDesc), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_usegs, usegs.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess) e = cudaMemcpy(g->d_usegs, usegs.data(), usegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_group_create: %s", cudaGetErrorString(e)); }
     int rc = group_scratch(g, std::max(group_scratch_need(g, 1), group_scratch_need(g, std::max(1, R_hint))));
     if (rc) return bail(rc);
@@ -473,6 +589,8 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_foitems) cudaFree(g->d_foitems);
     if (g->d_kitems) cudaFree(g->d_kitems);
     if (g->d_witems) cudaFree(g->d_witems);
+    if (g->d_descs_fused) cudaFree(g->d_descs_fused);
+    if (g->d_usegs) cudaFree(g->d_usegs);
     if (g->scratch) cudaFree(g->scratch);
     g->sync.destroy();
     delete g;
@@ -510,6 +628,18 @@ int fk_conv_grouped_vjp(fk_group* g, const void* f_cat, const void* g_cat, void*
     if (g->dtype == FK_F32S64) return group_vjp_t<double, float>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream);
     return g->dtype == FK_F64 ? group_vjp_t<double>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream)
                               : group_vjp_t<float>(g, f_cat, g_cat, df_cat, R, (cudaStream_t)stream);
+}
+
+int fk_conv_grouped_conv_vjp(fk_group* g, const void* f_cat, const void* g_cat, void* sigma_cat, void* df_cat, int R, void* stream) {
+    g_err.clear();
+    if (!g || !f_cat || !g_cat || !sigma_cat || !df_cat) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped_conv_vjp: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_conv_grouped_conv_vjp: R=%d", R);
+    cudaStream_t s = (cudaStream_t)stream;
+    CallGuard cg(g->sync, s);
+    if (int rc = cg.begin("fk_conv_grouped_conv_vjp")) return rc;
+    if (g->dtype == FK_F32S64) return group_conv_vjp_t<double, float>(g, f_cat, g_cat, sigma_cat, df_cat, R, s);
+    return g->dtype == FK_F64 ? group_conv_vjp_t<double>(g, f_cat, g_cat, sigma_cat, df_cat, R, s)
+                              : group_conv_vjp_t<float>(g, f_cat, g_cat, sigma_cat, df_cat, R, s);
 }
 
 int fk_group_last_launches(const fk_group* g) { return g ? g->last_launches : 0; }

@@ -33,7 +33,7 @@ SYMBOLS = (
     "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp", "fk_table_conv_vjp", "fk_chi2", "fk_table_fit_step",
     "fk_table_conv_host", "fk_table_vjp_host", "fk_table_last_launches",
     "fk_group_create", "fk_group_destroy", "fk_group_offsets", "fk_conv_grouped",
-    "fk_conv_grouped_vjp", "fk_group_last_launches",
+    "fk_conv_grouped_vjp", "fk_conv_grouped_conv_vjp", "fk_group_last_launches",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -72,6 +72,7 @@ lib.fk_group_destroy.argtypes = [_vp]
 lib.fk_group_offsets.argtypes = [_vp, _ci, _vp, _vp]
 lib.fk_conv_grouped.argtypes = [_vp, _vp, _vp, _ci, _vp]
 lib.fk_conv_grouped_vjp.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
+lib.fk_conv_grouped_conv_vjp.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _vp]
 lib.fk_group_last_launches.argtypes = [_vp]
 
 
@@ -389,6 +390,17 @@ class FkGroup:
         _check(lib.fk_conv_grouped_vjp(self.handle, _dev(f_cat, self.tdtype), _dev(g_cat, self.tdtype),
                                        _dev(df_cat, self.tdtype), R, _stream(stream)), "fk_conv_grouped_vjp")
         return df_cat
+
+    def conv_vjp(self, f_cat, g_cat, R, sigma_cat=None, df_cat=None, stream=None):
+        """Forward and VJP of the whole group from one read of every table (g known before the forward pass)."""
+        if sigma_cat is None:
+            sigma_cat = torch.empty(int(self.offsets(R)[1][-1]), dtype=self.tdtype, device=f_cat.device)
+        if df_cat is None:
+            df_cat = torch.empty_like(f_cat)
+        self._chk(R, f_cat=f_cat, sigma_cat=sigma_cat, g_cat=g_cat, df_cat=df_cat)
+        _check(lib.fk_conv_grouped_conv_vjp(self.handle, _dev(f_cat, self.tdtype), _dev(g_cat, self.tdtype), _dev(sigma_cat, self.tdtype),
+                                            _dev(df_cat, self.tdtype), R, _stream(stream)), "fk_conv_grouped_conv_vjp")
+        return sigma_cat, df_cat
 
     def last_launches(self) -> int:
         return lib.fk_group_last_launches(self.handle)

@@ -165,6 +165,17 @@ def test_config4_full_grouped(K):
             worst_d = max(worst_d, rel_err(d_t, dref[:kv], D[:kv]))
         print(f"config 4 R={Rr}: forward {worst_s:.2e} vjp {worst_d:.2e} launches {grp.last_launches()}")
         assert worst_s <= TOL64 and worst_d <= TOL64, (Rr, worst_s, worst_d)
+        if Rr == 1:
+            # forward + VJP from ONE read of the 14.8 GB (fk_conv_grouped_conv_vjp, config 4's seeded weights are known
+            # before the forward pass: SURVEY 8(f).2): same gates, sigma bit for bit the grouped forward's
+            sig1, df1 = grp.conv_vjp(f_cat, g_cat, 1)
+            assert grp.last_launches() == 4
+            assert np.array_equal(sig1.cpu().numpy(), sig)
+            df1 = df1.cpu().numpy()
+            worst_1 = max(rel_err(df1[fo[t]:fo[t + 1]].reshape(1, nfl, nx), dref[:1], D[:1])
+                          for t, ((ref, scale), (dref, D), vcols, N, nfl, nx) in enumerate(refs))
+            print(f"config 4 R=1 one read: vjp {worst_1:.2e}")
+            assert worst_1 <= TOL64
     grp.destroy()
     for t in tabs:
         t.destroy()

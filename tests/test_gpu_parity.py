@@ -402,6 +402,41 @@ def test_grouped_small_ragged(K, R, store):
     assert grp.last_launches() >= 2
 
 
+@pytest.mark.parametrize("R", [1, 2, 4, 6])
+@pytest.mark.parametrize("store", ["pack", "borrow"])
+def test_grouped_conv_vjp_one_read(K, R, store):
+    """fk_conv_grouped_conv_vjp: forward and VJP of a ragged group from one read of every table when g
+    is known before the forward pass (config 4's seeded weights).  R <= 4: the fused column kernel over the group's
+    static CTA list (3 launches + 1 per extra replica tile); R = 6: the two passes.  sigma is bit for bit the
+    grouped forward's; df meets the same 1e-13 gate against the oracle."""
+    import torch
+    shapes = synth.small_ragged_shapes(T=7)
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    cases = [synth.config4_table(t, shapes, R, params) for t in range(shapes.T)]
+    st = K.FK_STORE_PACK if store == "pack" else K.FK_STORE_BORROW
+    keep = [to_dev(c.fk) for c in cases]
+    tabs = [K.FkTable(K.FK_KIND_HADRONIC, keep[t], cases[t].pairs, cases[t].nfl, K.FK_F64, st) for t in range(shapes.T)]
+    grp = K.FkGroup(tabs, R_hint=R)
+    fo, so = grp.offsets(R)
+    f_cat = torch.cat([to_dev(c.f).reshape(-1) for c in cases])
+    rng = synth.rng_for(8, synth.T_G, 50 + R)
+    gs = [rng.standard_normal(size=(c.N, R)) for c in cases]     # a general g[n][r], not the broadcast weights
+    g_cat = torch.cat([to_dev(g).reshape(-1) for g in gs])
+    sig_d, df_d = grp.conv_vjp(f_cat, g_cat, R)
+    nl = grp.last_launches()
+    assert nl == (4 if R <= 4 else nl) and (R > 4 or nl == 4)   # fused column + reduce + fold + final
+    sig, df = sig_d.cpu().numpy(), df_d.cpu().numpy()
+    for t, c in enumerate(cases):
+        ref, scale = O.hadronic(c.fk, c.pairs, c.f)
+        dref, D = O.hadronic_vjp(c.fk, c.pairs, c.f, gs[t])
+        assert rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale) <= TOL64, t
+        assert rel_err(df[fo[t]:fo[t + 1]].reshape(R, c.nfl, c.nx), dref, np.maximum(D, 1e-300)) <= TOL64, t
+    assert np.array_equal(sig, grp.conv(f_cat, R).cpu().numpy())
+    sig2, df2 = grp.conv_vjp(f_cat, g_cat, R)
+    assert torch.equal(sig2, sig_d) and torch.equal(df2, df_d)   # bitwise repeatable
+    grp.destroy()
+
+
 @pytest.mark.parametrize("R", [2, 9])
 def test_grouped_mixed_dis_and_hadronic(K, R):
     """A 'global' group: DIS and hadronic tables in one launch; R=9 takes the
