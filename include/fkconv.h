@@ -137,6 +137,18 @@ int fk_conv_hadronic_f32(const float* fk, const int32_t* pairs, const float* f, 
 int fk_conv_hadronic_vjp_f32(const float* fk, const int32_t* pairs, const float* f, const float* g,
                              float* df, int N, int nx, int nfl, int C, int R, void* stream);
 
+/* ------------------------------------------------------------------ two-PDF (p pbar) form
+ * Eq. (1), with distinct PDFs on the two legs:
+ *     sigma[n][r] = sum_{c,i,j} f1[r][a_c][i] * f2[r][b_c][j] * FK[n][i][j][c]
+ * f1, f2  dev  [R][nfl][nx]  (f1 = first hadron, index i; f2 = second hadron, index j; reading R3)
+ * VJP: df1[r][alpha][i] = d(sum_n g sigma)/d f1[r][alpha][i], df2 likewise: two outputs, both overwritten.
+ * Runs on the single-PDF kernels over the stacked grid (f1 ; f2) with pairs (a_c, nfl + b_c): 2*nfl <= 256.
+ * fp64, logical-layout table, asynchronous on `stream`; same error conventions as fk_conv_hadronic. */
+int fk_conv_hadronic2(const double* fk, const int32_t* pairs, const double* f1, const double* f2, double* sigma,
+                      int N, int nx, int nfl, int C, int R, void* stream);
+int fk_conv_hadronic2_vjp(const double* fk, const int32_t* pairs, const double* f1, const double* f2, const double* g,
+                          double* df1, double* df2, int N, int nx, int nfl, int C, int R, void* stream);
+
 /* ------------------------------------------------------------------ resident-table path
  * What a fit uses: thousands of iterations over fixed tables, tables loaded once.
  * fk_table_create validates the index list, (store==PACK) repacks and (dtype==FK_F32) demotes the

@@ -1051,6 +1051,54 @@ int fk_profile_report(char* buf, int capacity) {
     return FK_OK;
 }
 
+// ---- two-PDF (p pbar) form: stacked flavours, then the single-PDF path (fk_pack.cuh, fk_stack2_kernel) ----
+namespace {
+int hadronic2(const char* who, bool vjp, const double* fkp, const int32_t* pairs, const double* f1, const double* f2, const double* g,
+              double* out1, double* out2, int N, int nx, int nfl, int C, int R, void* stream) {
+    g_err.clear();
+    if (!fkp || !pairs || !f1 || !f2 || !out1 || (vjp && (!g || !out2))) return fail(FK_ERR_INVALID_ARG, "%s: null pointer", who);
+    int rc = check_dims(who, FK_KIND_HADRONIC, N, nx, nfl, C, R);
+    if (rc) return rc;
+    if (2 * nfl > fk::MAX_NFL) return fail(FK_ERR_UNSUPPORTED, "%s: 2*nfl=%d > %d", who, 2 * nfl, fk::MAX_NFL);
+    std::vector<int32_t> p2(2 * (size_t)C);
+    for (int c = 0; c < C; ++c) {
+        const int a = pairs[2 * c], b = pairs[2 * c + 1];
+        if (a < 0 || a >= nfl || b < 0 || b >= nfl)
+            return fail(FK_ERR_INVALID_ARG, "%s: flavour index out of [0,%d) at channel %d: (%d,%d)", who, nfl, c, a, b);
+        p2[2 * c] = a;
+        p2[2 * c + 1] = nfl + b;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    const int slots = nfl * nx;
+    const size_t fe = 2 * (size_t)R * slots;
+    double* F = nullptr;
+    FK_CUDA(cudaMallocAsync((void**)&F, (vjp ? 2 : 1) * fe * sizeof(double), s));
+    const int grid = (int)std::min<size_t>(1024, (fe + 255) / 256);
+    fk::fk_stack2_kernel<double><<<grid, 256, 0, s>>>(f1, f2, F, R, slots);
+    if (vjp) {
+        rc = stateless<double>(who, FK_KIND_HADRONIC, true, fkp, p2.data(), F, g, F + fe, N, nx, 2 * nfl, C, R, stream);
+        if (rc == FK_OK) fk::fk_unstack2_kernel<double><<<grid, 256, 0, s>>>(F + fe, out1, out2, R, slots);
+    } else {
+        rc = stateless<double>(who, FK_KIND_HADRONIC, false, fkp, p2.data(), F, nullptr, out1, N, nx, 2 * nfl, C, R, stream);
+    }
+    const std::string keep = g_err;   // stateless() clears the message on entry only; keep it across the free
+    cudaError_t e = cudaGetLastError();
+    cudaError_t e2 = cudaFreeAsync(F, s);
+    if (rc != FK_OK) { g_err = keep; return rc; }
+    if (e != cudaSuccess || e2 != cudaSuccess) return fail(FK_ERR_CUDA, "%s: %s", who, cudaGetErrorString(e != cudaSuccess ? e : e2));
+    return FK_OK;
+}
+}  // namespace
+
+int fk_conv_hadronic2(const double* fk, const int32_t* pairs, const double* f1, const double* f2, double* sigma, int N, int nx,
+                      int nfl, int C, int R, void* stream) {
+    return hadronic2("fk_conv_hadronic2", false, fk, pairs, f1, f2, nullptr, sigma, nullptr, N, nx, nfl, C, R, stream);
+}
+int fk_conv_hadronic2_vjp(const double* fk, const int32_t* pairs, const double* f1, const double* f2, const double* g, double* df1,
+                          double* df2, int N, int nx, int nfl, int C, int R, void* stream) {
+    return hadronic2("fk_conv_hadronic2_vjp", true, fk, pairs, f1, f2, g, df1, df2, N, nx, nfl, C, R, stream);
+}
+
 int fk_conv_dis(const double* fk, const int32_t* flav, const double* f, double* sigma, int N, int nx, int nfl, int nA,
                 int R, void* stream) {
     return stateless<double>("fk_conv_dis", FK_KIND_DIS, false, fk, flav, f, nullptr, sigma, N, nx, nfl, nA, R, stream);

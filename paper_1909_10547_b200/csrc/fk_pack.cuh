@@ -39,4 +39,29 @@ fk_pack_kernel(const double* __restrict__ in, T* __restrict__ out, int N, int nx
     }
 }
 
+// Two-PDF (p pbar) form of Eq. (1) (PAPER.md:43 with distinct f, fbar): the second hadron's PDFs become
+// nfl extra flavours of ONE stacked grid F[r][2 nfl][nx] = (f1[r] ; f2[r]), and the pair (a, b) becomes (a, nfl + b):
+// the single-PDF kernels then compute sum f1[a][i] f2[b][j] FK, and their VJP returns dF = (df1 ; df2).
+template <typename T>
+__global__ void __launch_bounds__(256) fk_stack2_kernel(const T* __restrict__ f1, const T* __restrict__ f2, T* __restrict__ F,
+                                                         int R, int slots) {
+    const long long total = 2LL * R * slots;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long r = t / (2 * slots);
+        const int s = (int)(t - r * 2 * slots);
+        F[t] = s < slots ? f1[r * slots + s] : f2[r * slots + s - slots];
+    }
+}
+template <typename T>
+__global__ void __launch_bounds__(256) fk_unstack2_kernel(const T* __restrict__ dF, T* __restrict__ df1, T* __restrict__ df2,
+                                                           int R, int slots) {
+    const long long total = 2LL * R * slots;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const long long r = t / (2 * slots);
+        const int s = (int)(t - r * 2 * slots);
+        if (s < slots) df1[r * slots + s] = dF[t];
+        else df2[r * slots + s - slots] = dF[t];
+    }
+}
+
 }  // namespace fk

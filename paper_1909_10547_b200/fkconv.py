@@ -33,7 +33,7 @@ SYMBOLS = (
     "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp", "fk_table_conv_vjp", "fk_chi2", "fk_table_fit_step",
     "fk_table_conv_host", "fk_table_vjp_host", "fk_table_last_launches",
     "fk_group_create", "fk_group_destroy", "fk_group_offsets", "fk_conv_grouped",
-    "fk_conv_grouped_vjp", "fk_conv_grouped_conv_vjp", "fk_group_last_launches",
+    "fk_conv_grouped_vjp", "fk_conv_grouped_conv_vjp", "fk_group_last_launches", "fk_conv_hadronic2", "fk_conv_hadronic2_vjp",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -51,6 +51,8 @@ for _name in ("fk_conv_dis", "fk_conv_hadronic", "fk_conv_dis_f32", "fk_conv_had
     getattr(lib, _name).argtypes = [_vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
 for _name in ("fk_conv_hadronic_vjp", "fk_conv_dis_vjp", "fk_conv_hadronic_vjp_f32"):
     getattr(lib, _name).argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
+lib.fk_conv_hadronic2.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
+lib.fk_conv_hadronic2_vjp.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
 lib.fk_profile_enable.argtypes = [_ci]
 lib.fk_set_option.argtypes = [_ci, _ci]
 lib.fk_get_option.argtypes = [_ci, ctypes.POINTER(_ci)]
@@ -201,6 +203,35 @@ def fk_conv_hadronic_vjp(fk, pairs, f, g, df=None, stream=None):
     _check(fn(_dev(fk), _hostptr(pairs), _dev(f, fk.dtype), _dev(g, fk.dtype), _dev(df, fk.dtype),
               N, nx, nfl, C, R, _stream(stream)), "fk_conv_hadronic_vjp")
     return df
+
+
+def fk_conv_hadronic2(fk, pairs, f1, f2, sigma=None, stream=None):
+    """Two-PDF (p pbar) form: sigma[n][r] = sum f1[r][a_c][i] f2[r][b_c][j] FK[n][i][j][c] (fp64)."""
+    N, nx, _, C = fk.shape
+    R, nfl, _ = f1.shape
+    pairs = _idx(pairs)
+    if sigma is None:
+        sigma = torch.empty((N, R), dtype=torch.float64, device=fk.device)
+    _shape(pairs, (C, 2), "pairs"); _shape(f1, (R, nfl, nx), "f1", fk.device); _shape(f2, (R, nfl, nx), "f2", fk.device)
+    _shape(sigma, (N, R), "sigma", fk.device)
+    _check(lib.fk_conv_hadronic2(_dev(fk, torch.float64), _hostptr(pairs), _dev(f1, torch.float64), _dev(f2, torch.float64),
+                                 _dev(sigma, torch.float64), N, nx, nfl, C, R, _stream(stream)), "fk_conv_hadronic2")
+    return sigma
+
+
+def fk_conv_hadronic2_vjp(fk, pairs, f1, f2, g, df1=None, df2=None, stream=None):
+    """(df1, df2): the derivatives of sum_n g[n][r] sigma[n][r] with respect to f1 and f2."""
+    N, nx, _, C = fk.shape
+    R, nfl, _ = f1.shape
+    pairs = _idx(pairs)
+    df1 = torch.empty_like(f1) if df1 is None else df1
+    df2 = torch.empty_like(f2) if df2 is None else df2
+    _shape(pairs, (C, 2), "pairs"); _shape(f1, (R, nfl, nx), "f1", fk.device); _shape(f2, (R, nfl, nx), "f2", fk.device)
+    _shape(g, (N, R), "g", fk.device); _shape(df1, (R, nfl, nx), "df1", fk.device); _shape(df2, (R, nfl, nx), "df2", fk.device)
+    t64 = torch.float64
+    _check(lib.fk_conv_hadronic2_vjp(_dev(fk, t64), _hostptr(pairs), _dev(f1, t64), _dev(f2, t64), _dev(g, t64), _dev(df1, t64),
+                                     _dev(df2, t64), N, nx, nfl, C, R, _stream(stream)), "fk_conv_hadronic2_vjp")
+    return df1, df2
 
 
 def fk_conv_dis_vjp(fk, flav, f, g, df=None, stream=None):

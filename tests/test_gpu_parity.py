@@ -183,6 +183,53 @@ def test_conv_vjp_one_read_dis_and_fp32(K):
     assert rel_err(sig.cpu().numpy(), ref, scale) <= TOL32 and rel_err(df.cpu().numpy(), dref, D) <= TOL32
 
 
+# ------------------------------------------------------------------ two-PDF (p pbar) form
+@pytest.mark.parametrize("shape_R", [((5, 6, 4, 7), 1), ((40, 17, 14, 30), 3), ((70, 30, 14, 60), 9)])
+def test_two_pdf_form_against_the_oracle(K, shape_R):
+    """fk_conv_hadronic2 / _vjp (Eq. (1), with distinct PDFs on the two legs) against the
+    oracle's two-PDF loop.  The VJP is checked without any two-PDF derivative code on the oracle side: sigma is linear in
+    f1 for fixed f2, so df1[r][alpha][i] = sum_n g[n][r] sigma(e_{alpha,i}, f2)[n][r] exactly (e = unit grid), and the same
+    with the roles swapped for df2; the unit-grid sigmas come from the oracle.  R = 9 takes the dense contraction."""
+    (N, nx, nfl, C), R = shape_R
+    case = synth.hadronic_case(8, N, nx, C, R, nfl=nfl, sub=77 + N)
+    rng = synth.rng_for(8, synth.T_PDF, 500 + N)
+    f2 = case.f * rng.uniform(0.5, 1.5, size=case.f.shape) + 0.01 * rng.standard_normal(size=case.f.shape)
+    g = synth.rng_for(8, synth.T_G, 600 + N).standard_normal(size=(N, R))
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f, f2=f2)
+    fk_d, f1_d, f2_d, g_d = to_dev(case.fk), to_dev(case.f), to_dev(f2), to_dev(g)
+    sig = K.fk_conv_hadronic2(fk_d, case.pairs, f1_d, f2_d).cpu().numpy()
+    assert rel_err(sig, ref, scale) <= TOL64
+    # swapping the legs is a different observable unless FK is symmetric: the entry point must not symmetrise
+    swapped, _ = O.hadronic(case.fk, case.pairs, f2, f2=case.f)
+    assert np.max(np.abs(swapped - ref)) > 1e-6 * np.max(np.abs(ref))
+    df1, df2 = (t.cpu().numpy() for t in K.fk_conv_hadronic2_vjp(fk_d, case.pairs, f1_d, f2_d, g_d))
+    used_a, used_b = sorted(set(int(a) for a in case.pairs[:, 0])), sorted(set(int(b) for b in case.pairs[:, 1]))
+    for alpha in range(nfl):
+        if alpha not in used_a:
+            assert np.all(df1[:, alpha] == 0.0)
+        if alpha not in used_b:
+            assert np.all(df2[:, alpha] == 0.0)
+    picks = [(used_a[0], 0), (used_a[-1], nx - 1), (used_a[len(used_a) // 2], nx // 2)]
+    for (alpha, i) in picks:
+        e = np.zeros_like(case.f); e[:, alpha, i] = 1.0
+        s_e, sc_e = O.hadronic(case.fk, case.pairs, e, f2=f2)
+        want, D = np.sum(g * s_e, axis=0), np.sum(np.abs(g) * sc_e, axis=0)
+        assert np.max(np.abs(df1[:, alpha, i] - want) / np.maximum(D, 1e-300)) <= TOL64, (alpha, i)
+    picks = [(used_b[0], 0), (used_b[-1], nx - 1), (used_b[len(used_b) // 2], nx // 3)]
+    for (beta, j) in picks:
+        e = np.zeros_like(case.f); e[:, beta, j] = 1.0
+        s_e, sc_e = O.hadronic(case.fk, case.pairs, case.f, f2=e)
+        want, D = np.sum(g * s_e, axis=0), np.sum(np.abs(g) * sc_e, axis=0)
+        assert np.max(np.abs(df2[:, beta, j] - want) / np.maximum(D, 1e-300)) <= TOL64, (beta, j)
+    # f1 = f2 = f reduces to the single-PDF entry points: forward bit for bit (same kernel, same order), df = df1 + df2
+    s1 = K.fk_conv_hadronic2(fk_d, case.pairs, f1_d, f1_d).cpu().numpy()
+    r1, sc1 = O.hadronic(case.fk, case.pairs, case.f)
+    assert rel_err(s1, r1, sc1) <= TOL64
+    d1, d2 = (t.cpu().numpy() for t in K.fk_conv_hadronic2_vjp(fk_d, case.pairs, f1_d, f1_d, g_d))
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, g)
+    assert rel_err(d1 + d2, dref, np.maximum(D, 1e-300)) <= 2 * TOL64
+
+
 # ------------------------------------------------------------------ config 1 (DIS)
 @pytest.mark.parametrize("R", [1, 100])
 def test_config1_dis(K, R):
