@@ -263,8 +263,15 @@ def run_extras(K, torch, level, table2, case2, peak):
     ms = _bench_call(lambda: t32.vjp(f2, g2, d2), stream)
     out["cfg2_vjp_fp32_storage"] = {"ms": ms, "GBps": fkb / 2 / ms / 1e6, "frac_of_peak": fkb / 2 / ms / 1e6 / peak}
     t32.destroy()
+    # latency floors next to the microsecond-scale configs (SURVEY 8(d), L2 caveat): an empty launch, and one streaming
+    # read of the same number of bytes (cold: L2 flushed before every call), through the same C-ABI library
+    sink = torch.zeros(1, dtype=torch.float64, device="cuda")
+    out["floor_empty_kernel_launch"] = {"ms": _bench_call(lambda: K.probe_launch(0), stream, steps=50),
+                                        "ms_cold": cold(lambda: K.probe_launch(0))}
     c0 = synth.config0()
-    t0 = K.FkTable(K.FK_KIND_HADRONIC, torch.from_numpy(c0.fk).cuda(), c0.pairs, c0.nfl)
+    fk0_d = torch.from_numpy(c0.fk).cuda()
+    out["floor_read_probe_cfg0_bytes_cold"] = {"ms": cold(lambda: K.probe_launch(1, fk0_d, sink)), "bytes": c0.fk.nbytes}
+    t0 = K.FkTable(K.FK_KIND_HADRONIC, fk0_d, c0.pairs, c0.nfl)
     f0 = torch.from_numpy(c0.f).cuda(); s0 = torch.empty((c0.N, 1), dtype=torch.float64, device="cuda")
     ms = cold(lambda: t0.conv(f0, s0))
     out["cfg0_forward_cold"] = {"ms": ms, "GBps": c0.fk.nbytes / ms / 1e6, "predictions_per_s": c0.N / ms * 1e3}
@@ -272,7 +279,10 @@ def run_extras(K, torch, level, table2, case2, peak):
     out["cfg0_forward_L2warm"] = {"ms": ms, "GBps": c0.fk.nbytes / ms / 1e6}
     for R in (1, 100):
         c1 = synth.config1(R=R)
-        t1 = K.FkTable(K.FK_KIND_DIS, torch.from_numpy(c1.fk).cuda(), c1.flav, c1.nfl, R_hint=R)
+        fk1_d = torch.from_numpy(c1.fk).cuda()
+        if R == 1:
+            out["floor_read_probe_cfg1_bytes_cold"] = {"ms": cold(lambda: K.probe_launch(1, fk1_d, sink)), "bytes": c1.fk.nbytes}
+        t1 = K.FkTable(K.FK_KIND_DIS, fk1_d, c1.flav, c1.nfl, R_hint=R)
         f1 = torch.from_numpy(c1.f).cuda(); s1 = torch.empty((c1.N, R), dtype=torch.float64, device="cuda")
         ms = cold(lambda: t1.conv(f1, s1))
         out[f"cfg1_dis_R{R}_cold"] = {"ms": ms, "GBps": c1.fk.nbytes / ms / 1e6,
@@ -397,11 +407,29 @@ def run_table3(K, torch, peak):
             ts.append(e0.elapsed_time(e1))
         ms = float(np.median(ts))
         nbytes = 8.0 * (N * Kc + Kc * R + N * R)
+        # H2D-inclusive, as the paper's GPU numbers are ("the time required for the memory transfer to the
+        # GPU" is included): both operands come from pinned host memory and the result goes back, inside the timed region
+        fk_h = torch.empty(fk.shape, dtype=fk.dtype, pin_memory=True); fk_h.copy_(fk)
+        f_h = torch.empty(f.shape, dtype=f.dtype, pin_memory=True); f_h.copy_(f)
+        sig_h = torch.empty(sig.shape, dtype=sig.dtype, pin_memory=True)
+        ts = []
+        for it in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0 = time.perf_counter()
+            e0.record(stream)
+            fk.copy_(fk_h, non_blocking=True); f.copy_(f_h, non_blocking=True)
+            tab.conv(f, sig)
+            sig_h.copy_(sig, non_blocking=True)
+            e1.record(stream); e1.synchronize()
+            if it:
+                ts.append(max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3))
+        ms_h2d = float(np.median(ts))
         out.append({"K": Kc, "R": R, "N": N, "ms": ms, "GBps": nbytes / ms / 1e6, "TFLOPs": 2.0 * N * Kc * R / ms / 1e9,
+                    "ms_h2d_inclusive": ms_h2d, "h2d_GBps": 8.0 * (N * Kc + Kc * R) / ms_h2d / 1e6,
                     "launches": tab.last_launches(), "streamed": "PDF matrix" if swapped else "FK", "paper_best_s": paper_s, "paper_best": who,
-                    "paper_over_ours": paper_s * 1e3 / ms})
+                    "paper_over_ours": paper_s * 1e3 / ms, "paper_over_ours_h2d_inclusive": paper_s * 1e3 / ms_h2d})
         tab.destroy()
-        del fk, f, sig
+        del fk, f, sig, fk_h, f_h, sig_h
         torch.cuda.empty_cache()
     return out
 

@@ -109,6 +109,11 @@ int fk_profile_enable(int on);
 int fk_profile_read(double* mean_kernel_ms, int* launches);
 int fk_profile_report(char* buf, int capacity);
 
+/* Latency floors for the microsecond-scale workloads (SURVEY 8(d), L2 caveat): kind 0 launches an empty kernel; kind 1
+ * a kernel that reads `bytes` bytes of `buf` (dev, 16-byte aligned) once with 128-bit streaming loads and keeps nothing
+ * (`sink`: dev, one double, never written for finite data).  Asynchronous on `stream`; the caller times them. */
+int fk_probe_launch(int kind, const void* buf, long long bytes, double* sink, void* stream);
+
 /* ------------------------------------------------------------------ stateless entry points (fp64)
  * Eq. (1) P:43 / DIS / VJP on the caller's logical-layout device buffers.  Level-1 partials live in
  * stream-ordered scratch (cudaMallocAsync on `stream`).

@@ -33,7 +33,7 @@ SYMBOLS = (
     "fk_table_create", "fk_table_destroy", "fk_table_info", "fk_table_conv", "fk_table_vjp", "fk_table_conv_vjp", "fk_chi2", "fk_table_fit_step",
     "fk_table_conv_host", "fk_table_vjp_host", "fk_table_last_launches",
     "fk_group_create", "fk_group_destroy", "fk_group_offsets", "fk_conv_grouped",
-    "fk_conv_grouped_vjp", "fk_conv_grouped_conv_vjp", "fk_group_last_launches", "fk_conv_hadronic2", "fk_conv_hadronic2_vjp",
+    "fk_conv_grouped_vjp", "fk_conv_grouped_conv_vjp", "fk_group_last_launches", "fk_conv_hadronic2", "fk_conv_hadronic2_vjp", "fk_probe_launch",
 )
 
 if not os.path.exists(LIB_PATH):
@@ -53,6 +53,7 @@ for _name in ("fk_conv_hadronic_vjp", "fk_conv_dis_vjp", "fk_conv_hadronic_vjp_f
     getattr(lib, _name).argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
 lib.fk_conv_hadronic2.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
 lib.fk_conv_hadronic2_vjp.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
+lib.fk_probe_launch.argtypes = [_ci, _vp, ctypes.c_longlong, _vp, _vp]
 lib.fk_profile_enable.argtypes = [_ci]
 lib.fk_set_option.argtypes = [_ci, _ci]
 lib.fk_get_option.argtypes = [_ci, ctypes.POINTER(_ci)]
@@ -136,6 +137,13 @@ def get_option(option: int) -> int:
     v = _ci()
     _check(lib.fk_get_option(option, ctypes.byref(v)), "fk_get_option")
     return v.value
+
+
+def probe_launch(kind: int, buf=None, sink=None, stream=None) -> None:
+    """Latency floors: kind 0 = empty kernel, kind 1 = one streaming read of `buf` (any contiguous device tensor)."""
+    nbytes = 0 if buf is None else buf.numel() * buf.element_size()
+    _check(lib.fk_probe_launch(kind, None if buf is None else _vp(buf.data_ptr()), nbytes,
+                               None if sink is None else _vp(sink.data_ptr()), _stream(stream)), "fk_probe_launch")
 
 
 def profile_enable(on: bool) -> None:
