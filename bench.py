@@ -263,6 +263,24 @@ def run_extras(K, torch, level, table2, case2, peak):
     ms = _bench_call(lambda: t32.vjp(f2, g2, d2), stream)
     out["cfg2_vjp_fp32_storage"] = {"ms": ms, "GBps": fkb / 2 / ms / 1e6, "frac_of_peak": fkb / 2 / ms / 1e6 / peak}
     t32.destroy()
+    # element-sparse storage (FK_STORE_SPARSE): the config-2 table with 30 % of its entries zeroed (config 1's
+    # fraction) and with 60 %: bytes counted AS STORED (values + masks + headers); dense_equiv_GBps = the dense bytes / time
+    gen = torch.Generator(device="cuda"); gen.manual_seed(190910547 + 2300)
+    fk_dense = torch.from_numpy(case2.fk).cuda()
+    for zf in (0.3, 0.6):
+        fkz = fk_dense * (torch.rand(fk_dense.shape, device="cuda", generator=gen) >= zf)
+        nnz = int(torch.count_nonzero(fkz).item())
+        tsp = K.FkTable(K.FK_KIND_HADRONIC, fkz, case2.pairs, case2.nfl, K.FK_F64, K.FK_STORE_SPARSE)
+        del fkz
+        torch.cuda.empty_cache()
+        stored = 8 * nnz + case2.N * ((case2.fk[0].size + 511) // 512) * 80
+        for name, fn in (("forward", lambda: tsp.conv(f2, s2)), ("vjp", lambda: tsp.vjp(f2, g2, d2))):
+            ms = _bench_call(fn, stream)
+            out[f"cfg2_sparse{int(zf * 100)}_{name}"] = {"ms": ms, "stored_bytes": stored, "stored_over_dense": stored / fkb, "GBps": stored / ms / 1e6,
+                                                        "frac_of_peak": stored / ms / 1e6 / peak, "dense_equiv_GBps": fkb / ms / 1e6}
+        tsp.destroy()
+    del fk_dense
+    torch.cuda.empty_cache()
     # latency floors next to the microsecond-scale configs (SURVEY 8(d), L2 caveat): an empty launch, and one streaming
     # read of the same number of bytes (cold: L2 flushed before every call), through the same C-ABI library
     sink = torch.zeros(1, dtype=torch.float64, device="cuda")

@@ -65,8 +65,14 @@ enum { FK_F64 = 0, FK_F32 = 1, FK_F32S64 = 2 };
 /* table storage: BORROW keeps the caller's logical-layout buffer (no copy; it must outlive the
  * table); PACK copies into the library's device layout: channel-major, x innermost
  * ([N][C][nx*nx rounded up to 4, zero padded] resp. [N][nA][nx]), each datapoint row padded to a
- * multiple of 16 bytes, so every channel block and every row starts on a 32- resp. 16-byte boundary. */
-enum { FK_STORE_BORROW = 0, FK_STORE_PACK = 1 };
+ * multiple of 16 bytes, so every channel block and every row starts on a 32- resp. 16-byte boundary
+ * (FK_F32 hadronic tables also pad every x-row to 16 bytes: the TMA boxes of the tcgen05 path).
+ * SPARSE (FK_F64 only) stores only the NONZERO entries, in the same k-order: per datapoint and per
+ * block of 512 k a 64-byte bit mask, a 16-byte header and the packed values -- 8 bytes per nonzero + 0.16 bytes per
+ * element (72 % of the dense bytes at config 1's 30 % zeros).  fk_table_conv / _vjp / _conv_vjp / _fit_step and the
+ * _host calls take it (column kernels, <= 4 replicas per pass over the table); the grouped launch does not.
+ * fk_table_info's device_bytes reports the bytes as stored. */
+enum { FK_STORE_BORROW = 0, FK_STORE_PACK = 1, FK_STORE_SPARSE = 2 };
 
 typedef struct fk_table fk_table; /* opaque: one FK table resident in HBM + its scratch */
 typedef struct fk_group fk_group; /* opaque: a ragged set of tables with a static work list */

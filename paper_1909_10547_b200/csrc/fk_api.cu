@@ -27,6 +27,7 @@
 #include "fk_vjp.cuh"
 #include "fk_chi2.cuh"
 #include "fk_tc32.h"
+#include "fk_sparse.cuh"
 
 namespace {
 
@@ -309,7 +310,7 @@ struct GemmPlan {
 
 template <typename T>
 bool gemm_wanted(const fk::TableDesc& d, int R) {
-    if (dtype_of<T>() != FK_F64 || d.store32) return false;  // the fp32 variants stay on the column kernels (reading R18)
+    if (dtype_of<T>() != FK_F64 || d.store32 || d.sp_blk) return false;  // fp32 variants (reading R18) and sparse tables: column kernels
     if ((long long)d.nfl * d.nx >= (long long)fk::KDEC_NONE) return false;
     // packed hadronic tables take the warp-specialised kernel, which beats the <= 4-replica column passes from
     // R = 5 on; the generic cp.async kernel (DIS, logical layout) streams FK at ~2 TB/s and only wins once the
@@ -619,7 +620,7 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
     const int fgrid = pl.nkb * pl.fsplit;
     // few datapoints per range and very many k-blocks: CTAs that walk the k-blocks (fk_fwd_fewrows_kernel)
     const bool fewrows = (d.N + pl.fsplit - 1) / pl.fsplit <= FWD_U && pl.nkb >= 64 * std::max(1, sm_count()) &&
-                         d.vec_ok && opt(FK_OPT_FEWROWS);
+                         d.vec_ok && !d.sp_blk && opt(FK_OPT_FEWROWS);
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
@@ -630,6 +631,13 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
             if (rt == 1) FK_TIMED("fk_fwd_fewrows", s) fk::fk_fwd_fewrows_kernel<T, VW, 1, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
             else if (rt == 2) FK_TIMED("fk_fwd_fewrows", s) fk::fk_fwd_fewrows_kernel<T, VW, 2, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
             else FK_TIMED("fk_fwd_fewrows", s) fk::fk_fwd_fewrows_kernel<T, VW, 4, FWD_U, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            e = cudaGetLastError();
+        } else if (d.sp_blk) {
+            if constexpr (std::is_same<T, double>::value && std::is_same<TS, double>::value) {
+                if (rt == 1) FK_TIMED("fk_fwd_sparse", s) fk::fk_fwd_sparse_kernel<1, FWD_U><<<fgrid, fk::FWD_THREADS, 0, s>>>(p);
+                else if (rt == 2) FK_TIMED("fk_fwd_sparse", s) fk::fk_fwd_sparse_kernel<2, FWD_U><<<fgrid, fk::FWD_THREADS, 0, s>>>(p);
+                else FK_TIMED("fk_fwd_sparse", s) fk::fk_fwd_sparse_kernel<4, FWD_U><<<fgrid, fk::FWD_THREADS, 0, s>>>(p);
+            }
             e = cudaGetLastError();
         } else
             e = fwd_dispatch<T, false, TS>(d.vec_ok, rt, p, fgrid, s);
@@ -676,7 +684,17 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
         for (int r0 = 0; r0 < R;) {
             const int rt = pick_rt(R - r0);
             p.r0 = r0;
-            cudaError_t e = colsum_dispatch<T, false, TS>(d.vec_ok, rt, p, pl.nkb * pl.nsplit, s);
+            cudaError_t e;
+            if (d.sp_blk) {
+                if constexpr (std::is_same<T, double>::value && std::is_same<TS, double>::value) {
+                    const int cgrid = pl.nkb * pl.nsplit;
+                    if (rt == 1) FK_TIMED("fk_colsum_sparse", s) fk::fk_colsum_sparse_kernel<1, 8><<<cgrid, fk::COLSUM_THREADS, 0, s>>>(p);
+                    else if (rt == 2) FK_TIMED("fk_colsum_sparse", s) fk::fk_colsum_sparse_kernel<2, 8><<<cgrid, fk::COLSUM_THREADS, 0, s>>>(p);
+                    else FK_TIMED("fk_colsum_sparse", s) fk::fk_colsum_sparse_kernel<4, 8><<<cgrid, fk::COLSUM_THREADS, 0, s>>>(p);
+                }
+                e = cudaGetLastError();
+            } else
+                e = colsum_dispatch<T, false, TS>(d.vec_ok, rt, p, pl.nkb * pl.nsplit, s);
             if (e != cudaSuccess) return fail(FK_ERR_CUDA, "colsum kernel launch failed: %s", cudaGetErrorString(e));
             ++nl;
             r0 += rt;
@@ -724,7 +742,7 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
 // scratch: part [N][R][nchunks] | G [fsplit][R][K] | fold partials
 template <typename T>
 bool fused_ok(const fk::TableDesc& d, int R) {
-    return !gemm_wanted<T>(d, R) && foldk_ok(d) && (d.N + d.fsplit - 1) / d.fsplit <= 64 && opt(FK_OPT_FUSED);
+    return !gemm_wanted<T>(d, R) && !d.sp_blk && foldk_ok(d) && (d.N + d.fsplit - 1) / d.fsplit <= 64 && opt(FK_OPT_FUSED);
 }
 size_t fused_scratch_elems(const fk::TableDesc& d, int R) {
     return (part_elems_per_replica(d) + (size_t)d.fsplit * d.K + (1 + FOLDK_MAX_CHUNKS) * (size_t)d.C * d.nx) * R;
@@ -880,6 +898,8 @@ struct fk_table {
     uint8_t* dev_chan = nullptr;  // [2][C] for grouped launches
     uint32_t* kdec = nullptr;     // [K] k -> (slot a, slot b) codes for the R >> 1 contraction
     void* d_tmap = nullptr;       // device copy of the CUtensorMap of a packed fp32 hadronic table (fk_tc32.cu)
+    void* sp_blk = nullptr;       // FK_STORE_SPARSE (fk_sparse.cuh): index records; owned_fk holds the nonzero values
+    size_t sp_bytes = 0;          // bytes of the sparse table as stored (values + masks + headers)
     double* scratch = nullptr;    // forward partials / VJP column sums (one buffer, used by one call at a time)
     size_t scratch_elems = 0;
     void* h_stage = nullptr;      // pinned host staging for the *_host calls
@@ -1173,7 +1193,8 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
     if (!fk_logical || !index_list) return fail(FK_ERR_INVALID_ARG, "fk_table_create: null pointer");
     if (kind != FK_KIND_DIS && kind != FK_KIND_HADRONIC) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad kind %d", kind);
     if (dtype != FK_F64 && dtype != FK_F32 && dtype != FK_F32S64) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad dtype %d", dtype);
-    if (store != FK_STORE_BORROW && store != FK_STORE_PACK) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad store %d", store);
+    if (store != FK_STORE_BORROW && store != FK_STORE_PACK && store != FK_STORE_SPARSE) return fail(FK_ERR_INVALID_ARG, "fk_table_create: bad store %d", store);
+    if (store == FK_STORE_SPARSE && dtype != FK_F64) return fail(FK_ERR_UNSUPPORTED, "fk_table_create: sparse storage holds fp64 tables only");
     if (dtype != FK_F64 && store == FK_STORE_BORROW)
         return fail(FK_ERR_INVALID_ARG, "fk_table_create: an fp32 table must be packed (the logical input is fp64)");
     int rc = check_dims("fk_table_create", kind, N, nx, nfl, C, std::max(1, R_hint));
@@ -1189,9 +1210,42 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
 
     const int jp = packed_jp(kind, nx, dtype);
     const int cstride = (nx * jp + 3) / 4 * 4;  // packed hadronic channel block (fk_common.cuh)
-    const int K = kind == FK_KIND_HADRONIC ? C * (store == FK_STORE_PACK ? cstride : nx * nx) : C * nx;
+    const int K = kind == FK_KIND_HADRONIC ? C * (store != FK_STORE_BORROW ? cstride : nx * nx) : C * nx;
     auto bail = [&](int code) { fk_table_destroy(t); return code; };
-    if (store == FK_STORE_PACK) {
+    if (store == FK_STORE_SPARSE) {
+        // two passes over the logical table (one-time): masks + block counts, host scan, values + per-word prefixes
+        const int dkind = kind == FK_KIND_HADRONIC ? fk::KIND_HADRONIC : fk::KIND_DIS;
+        const int nkb = (K + fk::SP_BLOCK - 1) / fk::SP_BLOCK;
+        const long long nblk = (long long)N * nkb;
+        if (nblk >= (1LL << 31)) { bail(0); return fail(FK_ERR_UNSUPPORTED, "fk_table_create: sparse table with %lld blocks", nblk); }
+        unsigned int* d_count = nullptr;
+        cudaError_t e = cudaMalloc(&t->sp_blk, (size_t)nblk * sizeof(fk::SparseBlk));
+        if (e == cudaSuccess) e = cudaMalloc((void**)&d_count, (size_t)nblk * sizeof(unsigned int));
+        if (e != cudaSuccess) { if (d_count) cudaFree(d_count); bail(0); return fail(FK_ERR_ALLOC, "fk_table_create: sparse index: %s", cudaGetErrorString(e)); }
+        fk::fk_sparse_build_kernel<false><<<(unsigned)nblk, 256>>>(fk_logical, dkind, N, nx, C, K, cstride, jp, nkb, d_count,
+                                                                   (fk::SparseBlk*)t->sp_blk, nullptr);
+        std::vector<unsigned int> cnt((size_t)nblk);
+        e = cudaMemcpy(cnt.data(), d_count, (size_t)nblk * sizeof(unsigned int), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) { cudaFree(d_count); bail(0); return fail(FK_ERR_CUDA, "fk_table_create: sparse pass 1: %s", cudaGetErrorString(e)); }
+        // exclusive scan of the block counts on the host (one-time), written into the records' `off` field
+        std::vector<unsigned long long> off((size_t)nblk);
+        unsigned long long nnz = 0;
+        for (long long b = 0; b < nblk; ++b) { off[b] = nnz; nnz += cnt[b]; }
+        e = cudaMemcpy2D(t->sp_blk, sizeof(fk::SparseBlk), off.data(), sizeof(unsigned long long), sizeof(unsigned long long), (size_t)nblk,
+                         cudaMemcpyHostToDevice);
+        cudaFree(d_count);
+        if (e == cudaSuccess) e = cudaMalloc(&t->owned_fk, std::max<size_t>(16, (size_t)nnz * sizeof(double)));
+        if (e != cudaSuccess) { bail(0); return fail(FK_ERR_ALLOC, "fk_table_create: sparse values (%llu nonzeros): %s", nnz, cudaGetErrorString(e)); }
+        fk::fk_sparse_build_kernel<true><<<(unsigned)nblk, 256>>>(fk_logical, dkind, N, nx, C, K, cstride, jp, nkb, nullptr,
+                                                                  (fk::SparseBlk*)t->sp_blk, (double*)t->owned_fk);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: sparse pass 2: %s", cudaGetErrorString(e)); }
+        t->desc = make_desc(kind, fk::LAYOUT_PACKED, t->owned_fk, N, nx, nfl, C, ((long long)K + 1) / 2 * 2, dtype);
+        t->desc.vec_ok = 1;   // the plan's k-blocks are the 512-element sparse blocks
+        t->desc.sp_blk = t->sp_blk;
+        t->sp_bytes = (size_t)nnz * sizeof(double) + (size_t)nblk * sizeof(fk::SparseBlk);
+    } else if (store == FK_STORE_PACK) {
         const int vecw = dtype == FK_F64 ? 2 : 4;
         const long long row_stride = ((long long)K + vecw - 1) / vecw * vecw;
         const size_t bytes = (size_t)N * row_stride * dtype_size(dtype);
@@ -1220,7 +1274,7 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
     if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: channel upload: %s", cudaGetErrorString(e)); }
     t->desc.chan_a = t->dev_chan;
     t->desc.chan_b = t->dev_chan + C;
-    if (dtype == FK_F64 && (long long)nfl * nx < (long long)fk::KDEC_NONE) {
+    if (dtype == FK_F64 && store != FK_STORE_SPARSE && (long long)nfl * nx < (long long)fk::KDEC_NONE) {
         e = cudaMalloc((void**)&t->kdec, (size_t)K * sizeof(uint32_t));
         if (e == cudaSuccess) {
             fk::fk_kdec_kernel<<<std::min(1024, (K + 255) / 256), 256>>>(t->desc, t->chan, t->kdec);
@@ -1253,6 +1307,7 @@ int fk_table_destroy(fk_table* t) {
     if (t->dev_chan) cudaFree(t->dev_chan);
     if (t->kdec) cudaFree(t->kdec);
     if (t->d_tmap) cudaFree(t->d_tmap);
+    if (t->sp_blk) cudaFree(t->sp_blk);
     if (t->scratch) cudaFree(t->scratch);
     if (t->h_stage) cudaFreeHost(t->h_stage);
     if (t->d_stage) cudaFree(t->d_stage);
@@ -1271,7 +1326,7 @@ int fk_table_info(const fk_table* t, int* N, int* nx, int* nfl, int* C, int64_t*
     if (K) *K = t->desc.K;
     if (row_stride) *row_stride = t->desc.row_stride;
     if (device_bytes)
-        *device_bytes = (int64_t)((t->owned_fk ? (size_t)t->desc.N * t->desc.row_stride * dtype_size(t->dtype) : 0) +
+        *device_bytes = (int64_t)((t->sp_blk ? t->sp_bytes : t->owned_fk ? (size_t)t->desc.N * t->desc.row_stride * dtype_size(t->dtype) : 0) +
                                   t->scratch_elems * sizeof(double) + t->stage_bytes + 2 * (size_t)t->desc.C);
     return FK_OK;
 }

@@ -60,6 +60,8 @@ struct TableDesc {
     long long cx_off;        // sum of C * nx over earlier tables: first (channel, x) slot of the VJP fold partials
     // tcgen05 contraction of fp32 tables (fk_tc32.cu)
     const void* tmap;        // device copy of the table's CUtensorMap (null: the table cannot take that path)
+    // element-sparse storage (fk_sparse.cuh): fk = the nonzero values; null sp_blk: dense
+    const void* sp_blk;                   // [N][nchunks] SparseBlk: value offset, per-word prefix counts, bit masks
     int tc_ksplit, tc_kper;  // grouped launches: K ranges of the tcgen05 contraction and their length (multiple of 32)
     long long tc_gp_off;     // grouped launches: row offset of this table's tcgen05 split-K partials
 };

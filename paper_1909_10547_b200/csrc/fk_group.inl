@@ -427,6 +427,10 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             g->sync.destroy(); delete g;
             return fail(FK_ERR_INVALID_ARG, "fk_group_create: table %d lives on device %d, the current device is %d", t, tb->sync.device, g->sync.device);
         }
+        if (tb->desc.sp_blk) {
+            g->sync.destroy(); delete g;
+            return fail(FK_ERR_UNSUPPORTED, "fk_group_create: table %d uses sparse storage, which the grouped launch does not take", t);
+        }
         g->all_vec = g->all_vec && tb->desc.vec_ok;
     }
     // R >> 1 contraction: every item (128-datapoint tile x K range) costs about the same DMMA time

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libfkconv.so")
 FK_OK, FK_ERR_INVALID_ARG, FK_ERR_ALLOC, FK_ERR_CUDA, FK_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 FK_KIND_DIS, FK_KIND_HADRONIC = 0, 1
 FK_F64, FK_F32, FK_F32S64 = 0, 1, 2
-FK_STORE_BORROW, FK_STORE_PACK = 0, 1
+FK_STORE_BORROW, FK_STORE_PACK, FK_STORE_SPARSE = 0, 1, 2
 (FK_OPT_GEMM_MIN_R, FK_OPT_WARP_SPEC, FK_OPT_FOLD, FK_OPT_FOLDK, FK_OPT_FUSED, FK_OPT_FEWROWS, FK_OPT_TC32,
  FK_OPT_TC32_MIN_R, FK_OPT_PDL) = range(9)
 

@@ -183,6 +183,68 @@ def test_conv_vjp_one_read_dis_and_fp32(K):
     assert rel_err(sig.cpu().numpy(), ref, scale) <= TOL32 and rel_err(df.cpu().numpy(), dref, D) <= TOL32
 
 
+# ------------------------------------------------------------------ element-sparse storage
+@pytest.mark.parametrize("zero_frac", [0.0, 0.3, 0.9, 1.0])
+@pytest.mark.parametrize("shape_R", [((37, 23, 14, 29), 1), ((64, 50, 14, 9), 3), ((33, 8, 6, 5), 6), ((300, 30, 14, 40), 2)])
+def test_sparse_storage_hadronic(K, shape_R, zero_frac):
+    """FK_STORE_SPARSE: only the nonzero entries are stored (bit masks + packed values).  Same gates as the
+    dense table against the oracle of the same (zero-riddled) table; a zero fraction of 1.0 is the empty table (sigma = 0,
+    df = 0 exactly); the stored bytes follow the nonzero count; forward + VJP, one-read entry point, bitwise repeatable."""
+    import torch
+    (N, nx, nfl, C), R = shape_R
+    case = synth.hadronic_case(8, N, nx, C, R, nfl=nfl, sub=N + 31 * nx)
+    rng = synth.rng_for(8, synth.T_FK, 9000 + N + int(100 * zero_frac))
+    fk = case.fk * (rng.random(size=case.fk.shape) >= zero_frac)
+    if zero_frac == 0.3:   # structured zeros as well: a whole channel, a whole datapoint, a band of x-rows
+        fk[..., 0] = 0.0; fk[N // 2] = 0.0; fk[:, nx // 2:, : nx // 3, :] = 0.0
+    g = synth.rng_for(8, synth.T_G, 40 + N).standard_normal(size=(N, R))
+    ref, scale = O.hadronic(fk, case.pairs, case.f)
+    dref, D = O.hadronic_vjp(fk, case.pairs, case.f, g)
+    ts = K.FkTable(K.FK_KIND_HADRONIC, to_dev(fk), case.pairs, case.nfl, K.FK_F64, K.FK_STORE_SPARSE, R_hint=R)
+    f_d, g_d = to_dev(case.f), to_dev(g)
+    sig, df = ts.conv(f_d), ts.vjp(f_d, g_d)
+    assert rel_err(sig.cpu().numpy(), ref, scale) <= TOL64 and rel_err(df.cpu().numpy(), dref, D) <= TOL64
+    assert torch.equal(sig, ts.conv(f_d)) and torch.equal(df, ts.vjp(f_d, g_d))
+    s2, d2 = ts.conv_vjp(f_d, g_d)   # two passes on a sparse table, same results
+    assert torch.equal(s2, sig) and torch.equal(d2, df)
+    nnz = int(np.count_nonzero(fk))
+    Kp = C * ((nx * nx + 3) // 4 * 4)
+    stored = ts.info()["device_bytes"]
+    assert stored >= 8 * nnz + N * ((Kp + 511) // 512) * 80 and stored <= 8 * nnz + N * ((Kp + 511) // 512) * 80 + (1 << 26)
+    if zero_frac == 1.0:
+        assert not sig.any() and not df.any()
+    ts.destroy()
+
+
+def test_sparse_storage_dis_config1(K):
+    """BASELINE config 1 as given (30 % of the entries zeroed): the sparse table against the oracle and bit for bit
+    repeatable; exact-integer inputs equal the oracle bit for bit in any order."""
+    import torch
+    for R in (1, 5):
+        case = synth.config1(R=R)
+        ref, scale = O.dis(case.fk, case.flav, case.f)
+        dref, D = O.dis_vjp(case.fk, case.flav, case.f, case.g)
+        ts = K.FkTable(K.FK_KIND_DIS, to_dev(case.fk), case.flav, case.nfl, K.FK_F64, K.FK_STORE_SPARSE, R_hint=R)
+        f_d, g_d = to_dev(case.f), to_dev(case.g)
+        assert rel_err(ts.conv(f_d).cpu().numpy(), ref, scale) <= TOL64
+        assert rel_err(ts.vjp(f_d, g_d).cpu().numpy(), dref, D) <= TOL64
+        stored = 8 * int(np.count_nonzero(case.fk)) + case.N * ((case.nx * case.nA + 511) // 512) * 80   # values + masks + headers
+        frac = stored / case.fk.nbytes
+        print(f"config 1 sparse R={R}: stored / dense bytes = {frac:.3f}")
+        assert frac < 0.75 and stored <= ts.info()["device_bytes"] <= stored + (1 << 24)   # + scratch and staging
+        ts.destroy()
+    ic = synth.integer_hadronic_case(11, N=40, nx=17, C=12, R=2)
+    fk = ic.fk * (synth.rng_for(7, synth.T_FK, 123).random(size=ic.fk.shape) >= 0.4)
+    ref, _ = O.hadronic(fk, ic.pairs, ic.f)
+    dref, _ = O.hadronic_vjp(fk, ic.pairs, ic.f, ic.g)
+    ts = K.FkTable(K.FK_KIND_HADRONIC, to_dev(fk), ic.pairs, ic.nfl, K.FK_F64, K.FK_STORE_SPARSE)
+    assert np.array_equal(ts.conv(to_dev(ic.f)).cpu().numpy(), ref)
+    assert np.array_equal(ts.vjp(to_dev(ic.f), to_dev(ic.g)).cpu().numpy(), dref)
+    with pytest.raises(RuntimeError):
+        K.FkGroup([ts])
+    ts.destroy()
+
+
 # ------------------------------------------------------------------ two-PDF (p pbar) form
 @pytest.mark.parametrize("shape_R", [((5, 6, 4, 7), 1), ((40, 17, 14, 30), 3), ((70, 30, 14, 60), 9)])
 def test_two_pdf_form_against_the_oracle(K, shape_R):
