@@ -414,7 +414,9 @@ def run_table3(K, torch, peak):
         fk = torch.randn((rows, Kc, 1), dtype=torch.float64, device="cuda", generator=gen)
         f = torch.randn((cols, 1, Kc), dtype=torch.float64, device="cuda", generator=gen)
         sig = torch.empty((rows, cols), dtype=torch.float64, device="cuda")
-        tab = K.FkTable(K.FK_KIND_DIS, fk, flav, 1, K.FK_F64, K.FK_STORE_BORROW, R_hint=cols)
+        # rows of odd length (K = 35721) are not 16-byte aligned in place: the packed copy pads them (128-bit loads)
+        store = K.FK_STORE_PACK if (Kc % 2 and rows * Kc * 8 < 40e9) else K.FK_STORE_BORROW
+        tab = K.FkTable(K.FK_KIND_DIS, fk, flav, 1, K.FK_F64, store, R_hint=cols)
         for _ in range(2):
             tab.conv(f, sig)
         ts = []

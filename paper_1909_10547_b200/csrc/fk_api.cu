@@ -280,6 +280,13 @@ template <typename T, bool GROUPED, typename TS = T>
 cudaError_t fwd_dispatch(bool vec_ok, int rt, const fk::FwdParams& p, int grid, cudaStream_t s) {
     constexpr int VW = fk::VecWidth<TS>::value;
 #define FK_FWD(V, RTv) FK_TIMED("fk_fwd_column", s) fk::fk_fwd_column_kernel<T, V, RTv, FWD_U, GROUPED, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p)
+    if constexpr (!GROUPED && std::is_same<T, double>::value && std::is_same<TS, double>::value) {
+        if (rt == 8) {   // 5..12 replicas on tables without a dense path (DIS, logical layout): 8 per read, 4 rows in flight
+            if (vec_ok) FK_TIMED("fk_fwd_column", s) fk::fk_fwd_column_kernel<T, VW, 8, 4, false, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            else FK_TIMED("fk_fwd_column", s) fk::fk_fwd_column_kernel<T, 1, 8, 4, false, TS><<<grid, fk::FWD_THREADS, 0, s>>>(p);
+            return cudaGetLastError();
+        }
+    }
     if (vec_ok) {
         if (rt == 1) FK_FWD(VW, 1); else if (rt == 2) FK_FWD(VW, 2); else FK_FWD(VW, 4);
     } else {
@@ -622,7 +629,8 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
     const bool fewrows = (d.N + pl.fsplit - 1) / pl.fsplit <= FWD_U && pl.nkb >= 64 * std::max(1, sm_count()) &&
                          d.vec_ok && !d.sp_blk && opt(FK_OPT_FEWROWS);
     for (int r0 = 0; r0 < R;) {
-        const int rt = pick_rt(R - r0);
+        int rt = pick_rt(R - r0);
+        if (R - r0 >= 5 && !fewrows && !d.sp_blk && std::is_same<T, double>::value && std::is_same<TS, double>::value) rt = 8;
         p.r0 = r0;
         cudaError_t e;
         if (fewrows) {
@@ -643,7 +651,7 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
             e = fwd_dispatch<T, false, TS>(d.vec_ok, rt, p, fgrid, s);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "forward kernel launch failed: %s", cudaGetErrorString(e));
         ++nl;
-        r0 += rt;
+        r0 += std::min(rt, R - r0);
     }
     if (pl.nkb > 1) {
         fk::ReduceParams q;
