@@ -359,7 +359,7 @@ template <bool GROUPED>
 bool ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) {
     switch (w.RP / 8) {
 #define FK_WS_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, MAX_DYN_SMEM)) return false; \
-                                  FK_TIMED("fk_gemm_fwd_ws", s) fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, smem, s>>>(w); break
+                                  FK_TIMED("fk_gemm_fwd_ws", s) launch_pdl(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, grid, fk::WS_THREADS, smem, s, w); break
         FK_WS_CASE(2); FK_WS_CASE(4); FK_WS_CASE(6); FK_WS_CASE(8); FK_WS_CASE(10); FK_WS_CASE(12); FK_WS_CASE(14);
         default: FK_WS_CASE(16);
 #undef FK_WS_CASE
@@ -430,11 +430,11 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
             const int nfull = d.N / fk::GEMM_BM;
             if (!ws_launch<false>(w, nfull * gp.ksplit + (d.N % fk::GEMM_BM ? gp.ksplit / gp.ksub_rem : 0), fk::ws_smem_bytes(d.nx, p.RP), s))
                 return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
-        } else if (d.vec_ok) FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<2, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
-        else FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<1, false><<<mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        } else if (d.vec_ok) FK_TIMED("fk_gemm_fwd", s) launch_pdl(fk::fk_gemm_fwd_kernel<2, false>, mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s, p);
+        else FK_TIMED("fk_gemm_fwd", s) launch_pdl(fk::fk_gemm_fwd_kernel<1, false>, mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s, p);
         const long long outs = (long long)d.N * p.RP;
-        FK_TIMED("fk_gemm_reduce", s) fk::fk_gemm_reduce_kernel<double><<<(int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s>>>(
-            gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, gp.ksplit);
+        FK_TIMED("fk_gemm_reduce", s) launch_pdl(fk::fk_gemm_reduce_kernel<double>, (int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s,
+                                                 gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, gp.ksplit);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm forward launch failed: %s", cudaGetErrorString(e));
         nl += 3;

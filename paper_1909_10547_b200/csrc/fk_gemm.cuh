@@ -103,6 +103,8 @@ __global__ void __launch_bounds__(256) fk_transpose_f_kernel(const T* __restrict
 template <int VEC, bool GROUPED>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
+    pdl_trigger();
+    pdl_wait();   // fT of the transpose kernel launched just before (a programmatic dependent launch, fk_common.cuh)
     extern __shared__ __align__(128) unsigned char fk_smem[];
     double* As = reinterpret_cast<double*>(fk_smem);                  // [STAGES][BM][SA]
     double* Ls = As + GEMM_STAGES * GEMM_BM * GEMM_SA;                 // [2][KT][SB]

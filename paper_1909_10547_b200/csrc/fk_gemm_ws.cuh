@@ -89,6 +89,8 @@ __host__ __device__ inline int ws_ksub_for_rows(int rows) { return rows <= 32 ? 
 template <int NFRAG, bool GROUPED>
 __global__ void __launch_bounds__(WS_THREADS, 1)
 fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
+    pdl_trigger();
+    pdl_wait();   // fT of the transpose kernel launched just before (a programmatic dependent launch, fk_common.cuh)
     extern __shared__ __align__(128) unsigned char fk_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
