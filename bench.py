@@ -351,11 +351,12 @@ def run_config4(K, torch, peak):
     stream = torch.cuda.current_stream()
     Rmax = 100
     params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), Rmax)
-    tabs, fs, gs = [], [], []
+    tabs, tabs32, fs, gs = [], [], [], []
     for t in range(shapes.T):
         c = synth.config4_table(t, shapes, Rmax, params)
         fk_d = torch.from_numpy(c.fk).cuda()
         tabs.append(K.FkTable(K.FK_KIND_HADRONIC, fk_d, c.pairs, c.nfl, R_hint=1))
+        tabs32.append(K.FkTable(K.FK_KIND_HADRONIC, fk_d, c.pairs, c.nfl, K.FK_F32, K.FK_STORE_PACK, R_hint=1))
         del fk_d
         fs.append(c.f); gs.append(c.g)
     torch.cuda.empty_cache()
@@ -382,6 +383,18 @@ def run_config4(K, torch, peak):
                                                         "step_equiv_GBps": 2 * nbytes / ms / 1e6, "launches": grp.last_launches()}
     grp.destroy()
     for t in tabs:
+        t.destroy()
+    # fp32 variant of the group at R = 100: one grouped tcgen05 launch (3xTF32) over all 60 tables
+    grp32 = K.FkGroup(tabs32, R_hint=Rmax)
+    f32_cat = torch.cat([torch.from_numpy(np.ascontiguousarray(f[:Rmax])).reshape(-1) for f in fs]).cuda().float()
+    _, so = grp32.offsets(Rmax)
+    sig32 = torch.empty(int(so[-1]), dtype=torch.float32, device="cuda")
+    ms = _bench_call(lambda: grp32.conv(f32_cat, Rmax, sig32), stream, steps=5, warmup=3)
+    flops = 2.0 * shapes.fk_elements() * Rmax
+    out[f"cfg4_grouped_forward_R{Rmax}_fp32"] = {"ms": ms, "TFLOPs_useful": flops / ms / 1e9, "frac_of_tf32_peak": 3 * flops / ms / 1e9 / _tf32_peak(),
+                                                 "launches": grp32.last_launches(), "tolerance": 1e-5}
+    grp32.destroy()
+    for t in tabs32:
         t.destroy()
     return out
 

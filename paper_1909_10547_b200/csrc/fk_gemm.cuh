@@ -287,8 +287,8 @@ __device__ __forceinline__ int table_of(const int* __restrict__ prefix, int T, l
 }
 
 // grouped: fT_cat[global slot][c] = f_cat[f_off_t * R + (r0 + c) * slots_t + slot]
-template <typename T>
-__global__ void __launch_bounds__(256) fk_transpose_f_grouped_kernel(const T* __restrict__ f_cat, double* __restrict__ fT,
+template <typename T, typename O = double>
+__global__ void __launch_bounds__(256) fk_transpose_f_grouped_kernel(const T* __restrict__ f_cat, O* __restrict__ fT,
                                                                       const int* __restrict__ ai_prefix, int ntab,
                                                                       long long slots_total, int R, int r0, int RP) {
     const long long total = slots_total * RP;
@@ -297,16 +297,18 @@ __global__ void __launch_bounds__(256) fk_transpose_f_grouped_kernel(const T* __
         const int c = (int)(t - gs * RP), r = r0 + c;
         const int tb = table_of(ai_prefix, ntab, gs);
         const long long base = ai_prefix[tb], slots = ai_prefix[tb + 1] - base;
-        fT[t] = r < R ? (double)f_cat[base * R + (long long)r * slots + (gs - base)] : 0.0;
+        fT[t] = r < R ? (O)f_cat[base * R + (long long)r * slots + (gs - base)] : O(0);
     }
 }
 
 // grouped level 2: sigma_cat[global row][r0 + c] = sum over the K ranges of the row's table, fixed order
-template <typename T>
-__global__ void __launch_bounds__(256) fk_gemm_reduce_grouped_kernel(const double* __restrict__ gpart, T* __restrict__ sigma,
+// TC: the partials of the tcgen05 contraction (fk_tc32.cu: TableDesc::tc_gp_off, tc_ksplit), else of the DMMA one
+template <typename T, typename P = double, bool TC = false>
+__global__ void __launch_bounds__(256) fk_gemm_reduce_grouped_kernel(const P* __restrict__ gpart, T* __restrict__ sigma,
                                                                       const TableDesc* __restrict__ descs,
                                                                       const int* __restrict__ row_prefix, int ntab,
                                                                       long long rows_total, int R, int r0, int RP) {
+    pdl_wait();   // the level-1 partials of the whole contraction grid (no-op in a normal launch)
     const long long total = rows_total * RP;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
         const long long grow = t / RP;
@@ -315,13 +317,14 @@ __global__ void __launch_bounds__(256) fk_gemm_reduce_grouped_kernel(const doubl
         const int tb = table_of(row_prefix, ntab, grow);
         const TableDesc& d = descs[tb];
         const long long n = grow - row_prefix[tb];
-        const double* src = gpart + (d.gp_off + n) * RP + c;
+        const P* src = gpart + ((TC ? d.tc_gp_off : d.gp_off) + n) * RP + c;
         const long long stride = (long long)d.N * RP;
+        const int nsl = TC ? d.tc_ksplit : d.gksplit;
         double s = 0.0;
-        for (int k0 = 0; k0 < d.gksplit; k0 += 8) {  // eight loads in flight, added in index order
+        for (int k0 = 0; k0 < nsl; k0 += 8) {  // eight loads in flight, added in index order
             double w[8];
 #pragma unroll
-            for (int q = 0; q < 8; ++q) w[q] = k0 + q < d.gksplit ? src[(k0 + q) * stride] : 0.0;
+            for (int q = 0; q < 8; ++q) w[q] = k0 + q < nsl ? (double)src[(k0 + q) * stride] : 0.0;
 #pragma unroll
             for (int q = 0; q < 8; ++q) s += w[q];
         }

@@ -38,6 +38,11 @@ struct fk_group {
     int fold_nchunk = 1;
     fk::ColSeg* d_foitems = nullptr;  // fold CTAs: {table, channel, x-row chunk}
     int nfoitems = 0;
+    // fp32 variant at R >> 1: tcgen05 contraction over the group (fk_tc32.cu): items {table, first datapoint, range of (c, i) rows}
+    bool tc_all = false;
+    fk::ColSeg* d_tcitems = nullptr;
+    int ntcitems = 0;
+    long long tc_gp_rows = 0;
     // forward + VJP from one read of FK (fk_fused_column_kernel, GROUPED): the datapoint ranges of the fused CTAs
     // (<= 64 rows) are also the slices of the column sums, so the group keeps a second set of descriptors
     bool fused_all = true;
@@ -69,7 +74,13 @@ bool group_gemm_wanted(const fk_group* g, int R) {
     return g->gemm_ok && g->dtype == FK_F64 && R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : g->ws_all ? 5 : 13);
 }
 
+size_t group_tc32_scratch_need(const fk_group* g, int R);
+bool group_tc32_wanted(const fk_group* g, int R);
+
 size_t group_scratch_need(const fk_group* g, int R) {
+    if (group_tc32_wanted(g, R))   // the fp32 VJP of the same R stays on the column kernels
+        return std::max<size_t>(group_tc32_scratch_need(g, R),
+                                std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1 + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R);
     if (group_gemm_wanted(g, R)) {
         const size_t RP = fk::gemm_rp(R);
         const size_t fwd = (size_t)g->gp_rows,
@@ -77,6 +88,45 @@ size_t group_scratch_need(const fk_group* g, int R) {
         return ((size_t)g->ai_total + std::max(fwd, vjp)) * RP;
     }
     return std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1 + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R;
+}
+
+// ---- fp32 variant at R >> 1 over a group: one tcgen05 launch per pass of <= 128 replicas ----
+bool group_tc32_wanted(const fk_group* g, int R) {
+    return g->tc_all && g->dtype == FK_F32 && opt(FK_OPT_TC32) && R >= (opt(FK_OPT_TC32_MIN_R) > 0 ? opt(FK_OPT_TC32_MIN_R) : TC32_DEFAULT_MIN_R);
+}
+// scratch in doubles: fT32 [slots of the group][RPmax] floats + level-1 partials [tc_gp_rows][RPmax] floats
+size_t group_tc32_scratch_need(const fk_group* g, int R) {
+    const size_t RP = fk::tc_rp(R);
+    return (((size_t)g->ai_total * RP + 31) / 32 * 32 + (size_t)g->tc_gp_rows * RP + 1) / 2 + 64;
+}
+int group_conv_tc32(fk_group* g, const float* f_cat, float* sigma_cat, int R, cudaStream_t s) {
+    const int RPmax = fk::tc_rp(R);
+    float* fT = reinterpret_cast<float*>(g->scratch);
+    float* gpart = fT + ((size_t)g->ai_total * RPmax + 31) / 32 * 32;   // 128-byte aligned
+    int nl = 0;
+    for (int r0 = 0; r0 < R; r0 += fk::TC_MAX_RP) {
+        fk::Tc32Params p;
+        memset(&p, 0, sizeof p);
+        p.fT = fT;
+        p.gpart = gpart;
+        p.RP = fk::tc_rp(R - r0);
+        p.descs = g->d_descs;
+        p.items = g->d_tcitems;
+        const long long tf = g->ai_total * p.RP;
+        FK_TIMED("fk_transpose_f_grouped", s) fk::fk_transpose_f_grouped_kernel<float, float><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
+            f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, p.RP);
+        cudaError_t e = cudaSuccess;
+        FK_TIMED("fk_tc32_fwd", s) e = fk::tc32_fwd_launch(p, g->ntcitems, true, false, s);
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped tcgen05 forward launch failed: %s", cudaGetErrorString(e));
+        const long long outs = g->rows_total * p.RP;
+        FK_TIMED("fk_gemm_reduce_grouped", s) launch_pdl(fk::fk_gemm_reduce_grouped_kernel<float, float, true>, (int)std::min<long long>(8192, (outs + 255) / 256), 256, 0, s,
+                                                         gpart, sigma_cat, g->d_descs, g->d_row_prefix, g->T, g->rows_total, R, r0, p.RP);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped tcgen05 reduce launch failed: %s", cudaGetErrorString(e));
+        nl += 3;
+    }
+    g->last_launches = nl;
+    return FK_OK;
 }
 
 bool group_fused_wanted(const fk_group* g, int R) {
@@ -217,6 +267,9 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
     if (rc) return rc;
     if constexpr (std::is_same<T, double>::value) {
         if (group_gemm_wanted(g, R)) return group_conv_gemm(g, (const double*)f_cat, (double*)sigma_cat, R, s);
+    }
+    if constexpr (std::is_same<T, float>::value && std::is_same<TS, float>::value) {
+        if (group_tc32_wanted(g, R)) return group_conv_tc32(g, (const float*)f_cat, (float*)sigma_cat, R, s);
     }
     int nl = 0;
     fk::FwdParams p;
@@ -536,6 +589,32 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             descs_fused.push_back(du);
         }
     }
+    std::vector<fk::ColSeg> tcitems;
+    if (g->dtype == FK_F32) {   // tcgen05 items of about equal cost: 4 waves of (128-datapoint tile) x (range of (c, i) rows)
+        g->tc_all = true;
+        long long work = 0;
+        for (int t = 0; t < T; ++t) {
+            const fk::TableDesc& d = g->descs[t];
+            g->tc_all = g->tc_all && d.tmap && d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.nx <= fk::TC_MAX_NX && d.jp % 4 == 0;
+            work += (long long)fk::tc32_ntiles(d.N) * d.C * d.nx;
+        }
+        if (g->tc_all) {
+            const long long tper_target = std::max<long long>(16, (work + 4LL * std::max(1, sm_count()) - 1) / (4LL * std::max(1, sm_count())));
+            for (int t = 0; t < T; ++t) {
+                fk::TableDesc& d = g->descs[t];
+                const int Trows = d.C * d.nx;
+                int ksplit = (int)std::max<long long>(1, (Trows + tper_target - 1) / tper_target);
+                ksplit = std::max(ksplit, (Trows + fk::TC_MAX_TILES - 1) / fk::TC_MAX_TILES);
+                d.tc_kper = (Trows + ksplit - 1) / ksplit;
+                d.tc_ksplit = (Trows + d.tc_kper - 1) / d.tc_kper;
+                d.tc_gp_off = g->tc_gp_rows;
+                g->tc_gp_rows += (long long)d.tc_ksplit * d.N;
+                for (int ks = 0; ks < d.tc_ksplit; ++ks)
+                    for (int n0 = 0; n0 < d.N; n0 += fk::TC_BN) tcitems.push_back(fk::ColSeg{t, n0, ks, 0});
+            }
+        }
+    }
+    g->ntcitems = (int)tcitems.size();
     if (g->rows_total >= (1LL << 31) || g->ai_total >= (1LL << 31)) {
         g->sync.destroy();
         delete g;
@@ -570,6 +649,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     if (e == cudaSuccess) e = cudaMemcpy(g->d_row_prefix, row_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_ai_prefix, ai_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_csegs, csegs.data(), csegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && !tcitems.empty()) e = cudaMalloc((void**)&g->d_tcitems, tcitems.size() * sizeof(fk::ColSeg));
+    if (e == cudaSuccess && !tcitems.empty()) e = cudaMemcpy(g->d_tcitems, tcitems.data(), tcitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_descs_fused, T * sizeof(fk::TableDesc));
     if (e == cudaSuccess) e = cudaMemcpy(g->d_descs_fused, descs_fused.data(), T * sizeof(fk::TableDesc), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_usegs, usegs.size() * sizeof(fk::ColSeg));
@@ -593,6 +674,7 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_foitems) cudaFree(g->d_foitems);
     if (g->d_kitems) cudaFree(g->d_kitems);
     if (g->d_witems) cudaFree(g->d_witems);
+    if (g->d_tcitems) cudaFree(g->d_tcitems);
     if (g->d_descs_fused) cudaFree(g->d_descs_fused);
     if (g->d_usegs) cudaFree(g->d_usegs);
     if (g->scratch) cudaFree(g->scratch);

@@ -733,3 +733,32 @@ def test_grouped_fp32_variant(K):
         dref, D = O.hadronic_vjp(c.fk, c.pairs, c.f, c.g)
         assert rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale) <= TOL32, t
         assert rel_err(df[fo[t]:fo[t + 1]].reshape(R, c.nfl, c.nx), dref, D) <= TOL32, t
+    grp.destroy()
+
+
+@pytest.mark.parametrize("R", [20, 130])
+def test_grouped_fp32_variant_tensor_cores(K, R):
+    """The fp32 variant of a ragged group at R >> 1: ONE tcgen05 launch per pass of <= 128 replicas over static items
+    (table, 128-datapoint tile, range of (c, i) rows) of about equal cost; tables of 1..400 datapoints and x-grids from 7 to
+    50 points (partial tiles, K extents of one and two TMA boxes) against the fp64 oracle at 1e-5; equal to the
+    single-table calls bit for bit only where the plans coincide, so compared through the oracle."""
+    import torch
+    shapes = synth.RaggedShapes(np.array([1, 37, 130, 400, 64, 257], dtype=np.int64), np.array([7, 23, 50, 30, 32, 44], dtype=np.int64),
+                                np.array([1, 29, 12, 9, 20, 5], dtype=np.int64))
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    cases = [synth.config4_table(t, shapes, R, params) for t in range(shapes.T)]
+    tabs = [K.FkTable(K.FK_KIND_HADRONIC, to_dev(c.fk), c.pairs, c.nfl, K.FK_F32, R_hint=R) for c in cases]
+    grp = K.FkGroup(tabs, R_hint=R)
+    fo, so = grp.offsets(R)
+    f_cat = torch.cat([to_dev(c.f, torch.float32).reshape(-1) for c in cases])
+    sig_d = grp.conv(f_cat, R)
+    assert grp.last_launches() == 3 * ((R + 127) // 128)     # transpose, contraction, reduce per pass
+    sig = sig_d.cpu().numpy()
+    worst = 0.0
+    for t, c in enumerate(cases):
+        ref, scale = O.hadronic(c.fk, c.pairs, c.f)
+        worst = max(worst, rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale))
+    print(f"grouped tcgen05 R={R}: {worst:.2e}")
+    assert sig.dtype == np.float32 and worst <= TOL32
+    assert torch.equal(sig_d, grp.conv(f_cat, R))
+    grp.destroy()
