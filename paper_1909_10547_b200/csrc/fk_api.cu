@@ -69,6 +69,7 @@ int g_opt[FK_OPT_COUNT_] = {
     /* FK_OPT_TC32        */ 1,
     /* FK_OPT_TC32_MIN_R  */ 0,
     /* FK_OPT_PDL         */ 1,
+    /* FK_OPT_FUSE_L2     */ 1,
 };
 inline int opt(int o) { return g_opt[o]; }
 
@@ -608,7 +609,7 @@ int run_conv_tc32(const fk::TableDesc& d, const fk::ChannelList& ch, const float
 // One table, any R.  `part` holds >= part_elems_per_replica * R doubles (may be null if nchunks == 1).
 template <typename T, typename TS = T>
 int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const uint32_t* kdec,
-                    const T* f, T* sigma, int R, double* part, cudaStream_t s, int* launches) {
+                    const T* f, T* sigma, int R, double* part, cudaStream_t s, int* launches, int* cnt = nullptr) {
     int nl = 0;
     if constexpr (std::is_same<T, double>::value) {
         if (gemm_wanted<T>(d, R)) return run_conv_gemm(d, ch, kdec, f, sigma, R, part, s, launches);
@@ -628,6 +629,13 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
     // few datapoints per range and very many k-blocks: CTAs that walk the k-blocks (fk_fwd_fewrows_kernel)
     const bool fewrows = (d.N + pl.fsplit - 1) / pl.fsplit <= FWD_U && pl.nkb >= 64 * std::max(1, sm_count()) &&
                          d.vec_ok && !d.sp_blk && opt(FK_OPT_FEWROWS);
+    // resident tables whose forward grid is one wave or less (latency-bound, L2-resident: configs 0 and 1): the column
+    // kernel's last CTA per datapoint range runs the level-2 reduction itself and the second launch goes away.  On large
+    // tables the ticket's round trip at the end of EVERY CTA costs more occupancy than the launch (measured: config 2
+    // forward 0.160 -> 0.166 ms, config 4 2.16 -> 2.77 ms), so they keep the separate kernel.
+    const bool l2_in_kernel = cnt != nullptr && !fewrows && !d.sp_blk && opt(FK_OPT_FUSE_L2) &&
+                              (long long)pl.nkb * pl.fsplit <= 8LL * std::max(1, sm_count());
+    p.cnt = l2_in_kernel ? cnt : nullptr;
     for (int r0 = 0; r0 < R;) {
         int rt = pick_rt(R - r0);
         if (R - r0 >= 5 && !fewrows && !d.sp_blk && std::is_same<T, double>::value && std::is_same<TS, double>::value) rt = 8;
@@ -653,7 +661,7 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
         ++nl;
         r0 += std::min(rt, R - r0);
     }
-    if (pl.nkb > 1) {
+    if (pl.nkb > 1 && !l2_in_kernel) {
         fk::ReduceParams q;
         memset(&q, 0, sizeof q);
         q.desc = d;
@@ -906,6 +914,7 @@ struct fk_table {
     uint8_t* dev_chan = nullptr;  // [2][C] for grouped launches
     uint32_t* kdec = nullptr;     // [K] k -> (slot a, slot b) codes for the R >> 1 contraction
     void* d_tmap = nullptr;       // device copy of the CUtensorMap of a packed fp32 hadronic table (fk_tc32.cu)
+    int* l2cnt = nullptr;         // [fsplit] tickets of the forward kernel's in-kernel level-2 reduction (zero between launches)
     void* sp_blk = nullptr;       // FK_STORE_SPARSE (fk_sparse.cuh): index records; owned_fk holds the nonzero values
     size_t sp_bytes = 0;          // bytes of the sparse table as stored (values + masks + headers)
     double* scratch = nullptr;    // forward partials / VJP column sums (one buffer, used by one call at a time)
@@ -987,7 +996,7 @@ int table_conv_t(fk_table* t, const void* f, void* sigma, int R, cudaStream_t s)
     int rc = ensure_scratch(t, table_scratch_need(t, R), s);
     if (rc) return rc;
     return run_conv_single<T, TS>(t->desc, t->chan, t->plan, t->kdec, (const T*)f, (T*)sigma, R, t->scratch, s,
-                              &t->last_launches);
+                              &t->last_launches, t->l2cnt);
 }
 
 template <typename T, typename TS = T>
@@ -1276,7 +1285,10 @@ int fk_table_create(fk_table** out, int kind, const double* fk_logical, const in
     }
     make_plan(t->desc, dtype, t->plan);
 
-    cudaError_t e = cudaMalloc((void**)&t->dev_chan, 2 * (size_t)C);
+    cudaError_t e = cudaMalloc((void**)&t->l2cnt, std::max(1, t->plan.fsplit) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(t->l2cnt, 0, std::max(1, t->plan.fsplit) * sizeof(int));
+    if (e != cudaSuccess) { bail(0); return fail(FK_ERR_ALLOC, "fk_table_create: ticket counters: %s", cudaGetErrorString(e)); }
+    e = cudaMalloc((void**)&t->dev_chan, 2 * (size_t)C);
     if (e == cudaSuccess) e = cudaMemcpy(t->dev_chan, t->chan.a, C, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(t->dev_chan + C, t->chan.b, C, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { bail(0); return fail(FK_ERR_CUDA, "fk_table_create: channel upload: %s", cudaGetErrorString(e)); }
@@ -1316,6 +1328,7 @@ int fk_table_destroy(fk_table* t) {
     if (t->kdec) cudaFree(t->kdec);
     if (t->d_tmap) cudaFree(t->d_tmap);
     if (t->sp_blk) cudaFree(t->sp_blk);
+    if (t->l2cnt) cudaFree(t->l2cnt);
     if (t->scratch) cudaFree(t->scratch);
     if (t->h_stage) cudaFreeHost(t->h_stage);
     if (t->d_stage) cudaFree(t->d_stage);

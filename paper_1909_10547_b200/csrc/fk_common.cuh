@@ -48,6 +48,7 @@ struct TableDesc {
     long long f_off;         // element offset of f_t / df_t inside f_cat for R = 1 (scaled by R)
     long long out_off;       // element offset of sigma_t / g_t inside sigma_cat for R = 1 (scaled by R)
     long long part_off;      // element offset of this table's level-1 partials for R = 1 (scaled by R)
+    long long cnt_off;       // first ticket counter of this table (FwdParams::cnt), one per forward datapoint range
     long long g_off;         // element offset of this table's column sums G for R = 1 (scaled by R)
     int nchunks;             // forward: number of k-blocks (= level-1 partials per row)
     int fsplit;              // forward: number of datapoint ranges per k-block

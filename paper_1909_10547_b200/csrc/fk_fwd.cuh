@@ -30,10 +30,38 @@ struct FwdParams {
     double* part;             // level-1 partials [row][replica][k-block]
     void* sigma;              // direct output for tables with a single k-block
     int R, r0;                // replicas, first replica of this pass
+    int* cnt;                 // tickets per datapoint range (resident tables / groups; zero between launches), or null:
+                              // the CTA that completes a range also runs its level-2 reduction (no second launch)
 };
 
 constexpr int FWD_THREADS = 256;
 constexpr int FWD_WARPS = FWD_THREADS / 32;
+
+// a3 level 2 for up to 4 outputs (n, r) at once: per output the fixed order of the level-2 kernel (four lane-strided
+// chains per lane, combined pairwise, then the xor butterfly); the outputs' loads are interleaved so that a warp has up to
+// 16 of them in flight.  Partials are read past L1 (they were written by other SMs).
+template <int NO>
+__device__ __forceinline__ void reduce_chunks_rows(const double* (&src)[NO], int nch, int lane, double (&out)[NO]) {
+    double a[NO][4];
+#pragma unroll
+    for (int q = 0; q < NO; ++q) a[q][0] = a[q][1] = a[q][2] = a[q][3] = 0.0;
+    int c = lane;
+    for (; c + 96 < nch; c += 128) {
+#pragma unroll
+        for (int q = 0; q < NO; ++q) {
+            a[q][0] += __ldcg(src[q] + c);
+            a[q][1] += __ldcg(src[q] + c + 32);
+            a[q][2] += __ldcg(src[q] + c + 64);
+            a[q][3] += __ldcg(src[q] + c + 96);
+        }
+    }
+    for (; c < nch; c += 32) {
+#pragma unroll
+        for (int q = 0; q < NO; ++q) a[q][0] += __ldcg(src[q] + c);
+    }
+#pragma unroll
+    for (int q = 0; q < NO; ++q) out[q] = warp_sum((a[q][0] + a[q][1]) + (a[q][2] + a[q][3]));
+}
 
 // Folds U per-lane values (one per row) across the warp: afterwards lane l holds the warp total of
 // row l >> (5 - log2 U).  Fixed tree; a+b and b+a give the same bits, so every lane agrees.
@@ -150,6 +178,37 @@ fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
                 else
                     p.part[d.part_off * R + ((long long)n * R + rr) * d.nchunks + kblock] = s;
             }
+        }
+    }
+    // a3 level 2 without a second launch: the CTA that hands in the last k-block of its datapoint range sums the range's
+    // partials (same arithmetic and order as fk_reduce_chunks_kernel, whoever runs it: bitwise the same result)
+    if (p.cnt != nullptr && d.nchunks > 1) {
+        __shared__ int s_last;
+        __threadfence();   // this CTA's partials before its ticket
+        __syncthreads();
+        if (threadIdx.x == 0) s_last = atomicAdd(p.cnt + d.cnt_off + split, 1) == d.nchunks - 1;
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const int nout = (re - rb) * RT;
+            for (int o0 = warp * 4; o0 < nout; o0 += FWD_WARPS * 4) {
+                const double* src[4];
+                int nn[4], rq[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int o = min(o0 + q, nout - 1);
+                    nn[q] = rb + o / RT;
+                    rq[q] = min(p.r0 + o % RT, R - 1);
+                    src[q] = p.part + d.part_off * R + ((long long)nn[q] * R + rq[q]) * d.nchunks;
+                }
+                double sum[4];
+                reduce_chunks_rows<4>(src, d.nchunks, lane, sum);
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    if (lane == 0 && o0 + q < nout && p.r0 + (o0 + q) % RT < R)
+                        reinterpret_cast<T*>(p.sigma)[d.out_off * R + (long long)nn[q] * R + rq[q]] = (T)sum[q];
+            }
+            if (threadIdx.x == 0) p.cnt[d.cnt_off + split] = 0;   // ready for the next launch
         }
     }
 }
@@ -408,18 +467,10 @@ __global__ void __launch_bounds__(256) fk_reduce_chunks_kernel(const __grid_cons
         const int nch = d->nchunks;
         if (nch == 1) continue;  // written directly by the column kernel
         const double* src = p.part + d->part_off * p.R + (n * p.R + r) * nch;
-        // four lane-strided chains per lane (four loads in flight), combined pairwise, then the butterfly
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        int c = lane;
-        for (; c + 96 < nch; c += 128) {
-            a0 += src[c];
-            a1 += src[c + 32];
-            a2 += src[c + 64];
-            a3 += src[c + 96];
-        }
-        for (; c < nch; c += 32) a0 += src[c];
-        const double s = warp_sum((a0 + a1) + (a2 + a3));
-        if (lane == 0) reinterpret_cast<T*>(p.sigma)[d->out_off * p.R + n * p.R + r] = (T)s;
+        const double* srcs[1] = {src};
+        double s1[1];
+        reduce_chunks_rows<1>(srcs, nch, lane, s1);
+        if (lane == 0) reinterpret_cast<T*>(p.sigma)[d->out_off * p.R + n * p.R + r] = (T)s1[0];
     }
 }
 

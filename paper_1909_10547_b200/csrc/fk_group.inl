@@ -50,6 +50,8 @@ struct fk_group {
     fk::ColSeg* d_usegs = nullptr;
     int nusegs = 0;
     long long G_total1_fused = 0;
+    int* d_l2cnt = nullptr;   // tickets of the forward kernel's in-kernel level-2 reduction, one per (table, datapoint range)
+    long long cnt_total = 0;
     double* scratch = nullptr;
     size_t scratch_elems = 0;
     int last_launches = 0;
@@ -280,6 +282,8 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
     p.part = g->scratch;
     p.sigma = sigma_cat;
     p.R = R;
+    const bool l2_in_kernel = g->d_l2cnt != nullptr && opt(FK_OPT_FUSE_L2) && g->nfsegs <= 8 * std::max(1, sm_count());   // small groups only (fk_api.cu, run_conv_single)
+    p.cnt = l2_in_kernel ? g->d_l2cnt : nullptr;
     for (int r0 = 0; r0 < R;) {
         const int rt = pick_rt(R - r0);
         p.r0 = r0;
@@ -288,7 +292,7 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
         ++nl;
         r0 += rt;
     }
-    if (g->part_total1 > 0) {
+    if (g->part_total1 > 0 && !l2_in_kernel) {
         fk::ReduceParams q;
         memset(&q, 0, sizeof q);
         q.descs = g->d_descs;
@@ -559,6 +563,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
             ns = std::max(ns, (d.N + fk::COLSUM_MAX_ROWS - 1) / fk::COLSUM_MAX_ROWS);
             d.nsplit = std::max(1, std::min(ns, d.N));
         }
+        d.cnt_off = g->cnt_total;
+        g->cnt_total += d.fsplit;
         d.f_off = g->f_total1;
         d.out_off = g->rows_total;
         d.part_off = g->part_total1;
@@ -649,6 +655,8 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
     if (e == cudaSuccess) e = cudaMemcpy(g->d_row_prefix, row_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_ai_prefix, ai_prefix.data(), (T + 1) * sizeof(int), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(g->d_csegs, csegs.data(), csegs.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_l2cnt, (size_t)std::max<long long>(1, g->cnt_total) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(g->d_l2cnt, 0, (size_t)std::max<long long>(1, g->cnt_total) * sizeof(int));
     if (e == cudaSuccess && !tcitems.empty()) e = cudaMalloc((void**)&g->d_tcitems, tcitems.size() * sizeof(fk::ColSeg));
     if (e == cudaSuccess && !tcitems.empty()) e = cudaMemcpy(g->d_tcitems, tcitems.data(), tcitems.size() * sizeof(fk::ColSeg), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc((void**)&g->d_descs_fused, T * sizeof(fk::TableDesc));
@@ -675,6 +683,7 @@ int fk_group_destroy(fk_group* g) {
     if (g->d_kitems) cudaFree(g->d_kitems);
     if (g->d_witems) cudaFree(g->d_witems);
     if (g->d_tcitems) cudaFree(g->d_tcitems);
+    if (g->d_l2cnt) cudaFree(g->d_l2cnt);
     if (g->d_descs_fused) cudaFree(g->d_descs_fused);
     if (g->d_usegs) cudaFree(g->d_usegs);
     if (g->scratch) cudaFree(g->scratch);
