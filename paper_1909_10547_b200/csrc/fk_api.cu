@@ -195,7 +195,9 @@ void make_plan(fk::TableDesc& d, int dtype, Plan& pl) {
     pl.fsplit = std::max(1, std::min(d.N, (d.N + rows - 1) / rows));
 
     // VJP stage 1: fewer, longer ranges (every range writes K column sums that stage 2 adds up)
-    const int want = COLSUM_CTAS_PER_SM * sms;  // CTAs wanted for stage 1
+    // CTAs wanted for stage 1; a k-block of an fp32-stored table is twice as many k (1024), so the same CTA count would
+    // halve the rows per CTA and double the column-sum slices: ask for half as many
+    const int want = COLSUM_CTAS_PER_SM * sms / (dtype == FK_F64 ? 1 : 2);
     int nsplit = (want + pl.nkb - 1) / pl.nkb;
     nsplit = std::min(nsplit, std::max(1, d.N / 16));                  // >= 16 datapoints per split
     nsplit = std::max(nsplit, (d.N + fk::COLSUM_MAX_ROWS - 1) / fk::COLSUM_MAX_ROWS);

@@ -86,7 +86,7 @@ __device__ __forceinline__ double fold_rows(double (&p)[U], int lane) {
 
 // TS = storage type of the table (float for the fp32-storage variants), T = type of f, sigma and of the arithmetic
 template <typename T, int VEC, int RT, int U, bool GROUPED, typename TS = T>
-__global__ void __launch_bounds__(FWD_THREADS)
+__global__ void __launch_bounds__(FWD_THREADS, RT == 1 ? 4 : 1)   // R = 1: at most 64 registers, four CTAs per SM
 fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
     pdl_trigger();   // first kernel of a call (normal launch): lets the level-2 reduction be scheduled under this grid's last wave
     using V = Vec<TS, VEC>;
@@ -305,8 +305,9 @@ struct FusedParams {
     double* G;       // [fsplit][R][K] column sums, one slice per datapoint range
 };
 
+// (R = 1: capped at 51 registers so that five CTAs stay resident per SM; 54 cost one CTA and 6 % of the bandwidth)
 template <typename T, int VEC, int RT, int U, bool GROUPED, typename TS = T>
-__global__ void __launch_bounds__(FWD_THREADS)
+__global__ void __launch_bounds__(FWD_THREADS, RT == 1 ? (sizeof(T) == sizeof(TS) ? 5 : 4) : 1)
 fk_fused_column_kernel(const __grid_constant__ FusedParams q) {
     pdl_trigger();
     using V = Vec<TS, VEC>;

@@ -30,7 +30,7 @@ constexpr int COLSUM_THREADS = 256;
 constexpr int COLSUM_MAX_ROWS = 512;  // datapoints per split (bounds the g tile in shared memory)
 
 template <typename T, int VEC, int RT, int UNROLL, bool GROUPED, typename TS = T>
-__global__ void __launch_bounds__(COLSUM_THREADS)
+__global__ void __launch_bounds__(COLSUM_THREADS, RT == 1 ? 4 : 1)   // R = 1: at most 64 registers, four CTAs per SM
 fk_colsum_kernel(const __grid_constant__ ColsumParams p) {
     pdl_trigger();
     pdl_wait();
