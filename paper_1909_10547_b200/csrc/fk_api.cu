@@ -436,7 +436,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
         } else if (d.vec_ok) FK_TIMED("fk_gemm_fwd", s) launch_pdl(fk::fk_gemm_fwd_kernel<2, false>, mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s, p);
         else FK_TIMED("fk_gemm_fwd", s) launch_pdl(fk::fk_gemm_fwd_kernel<1, false>, mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s, p);
         const long long outs = (long long)d.N * p.RP;
-        FK_TIMED("fk_gemm_reduce", s) launch_pdl(fk::fk_gemm_reduce_kernel<double>, (int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s,
+        FK_TIMED("fk_gemm_reduce", s) launch_pdl(fk::fk_gemm_reduce_kernel<double>, (int)std::min<long long>(16384, ((gp.ksplit < fk::GEMM_REDUCE_QUAD ? 1 : 4) * outs + 255) / 256), 256, 0, s,
                                                  gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, gp.ksplit);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm forward launch failed: %s", cudaGetErrorString(e));
@@ -598,7 +598,7 @@ int run_conv_tc32(const fk::TableDesc& d, const fk::ChannelList& ch, const float
         FK_TIMED("fk_tc32_fwd", s) e = fk::tc32_fwd_launch(p, fk::tc32_ntiles(d.N) * tp.ksplit, false, opt(FK_OPT_PDL) != 0, s);
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward launch failed: %s", cudaGetErrorString(e));
         const long long outs = (long long)d.N * p.RP;
-        FK_TIMED("fk_gemm_reduce", s) launch_pdl(fk::fk_gemm_reduce_kernel<float, float>, (int)std::min<long long>(4096, (outs + 255) / 256), 256, 0, s,
+        FK_TIMED("fk_gemm_reduce", s) launch_pdl(fk::fk_gemm_reduce_kernel<float, float>, (int)std::min<long long>(16384, ((tp.ksplit < fk::GEMM_REDUCE_QUAD ? 1 : 4) * outs + 255) / 256), 256, 0, s,
                                                  gpart, sigma, d.out_off * R, d.N, R, r0, p.RP, tp.ksplit);
         e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "tcgen05 forward reduce launch failed: %s", cudaGetErrorString(e));

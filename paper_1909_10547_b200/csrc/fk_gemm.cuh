@@ -256,23 +256,45 @@ fk_gemm_fwd_kernel(const __grid_constant__ GemmFwdParams p) {
 }
 
 // level 2: sigma[n][r0 + c] = sum over K ranges, fixed order
+// level 2: sigma[n][r0 + c] = sum over K ranges, fixed order
+constexpr int GEMM_REDUCE_QUAD = 16;   // from this many K ranges on, four threads share an output
 template <typename T, typename P = double>
 __global__ void __launch_bounds__(256) fk_gemm_reduce_kernel(const P* __restrict__ gpart, T* __restrict__ sigma,
                                                               long long out_off, int N, int R, int r0, int RP, int ksplit) {
     pdl_wait();   // the level-1 partials of the whole contraction grid (no-op in a normal launch)
     const long long total = (long long)N * RP;
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
-        const int n = (int)(t / RP), c = (int)(t - (long long)n * RP);
-        if (r0 + c >= R) continue;
-        double s = 0.0;
-        for (int k0 = 0; k0 < ksplit; k0 += 8) {  // eight loads in flight, added in index order
-            double w[8];
+    if (ksplit < GEMM_REDUCE_QUAD) {   // few slices: one thread per output, all loads in flight
+        for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+            const int n = (int)(t / RP), c = (int)(t - (long long)n * RP);
+            if (r0 + c >= R) continue;
+            double w[GEMM_REDUCE_QUAD], s = 0.0;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) w[q] = k0 + q < ksplit ? (double)gpart[(long long)(k0 + q) * total + t] : 0.0;
+            for (int e = 0; e < GEMM_REDUCE_QUAD; ++e) w[e] = e < ksplit ? (double)gpart[(long long)e * total + t] : 0.0;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) s += w[q];
+            for (int e = 0; e < GEMM_REDUCE_QUAD; ++e) s += w[e];
+            sigma[out_off + (long long)n * R + r0 + c] = (T)s;
         }
-        sigma[out_off + (long long)n * R + r0 + c] = (T)s;
+        return;
+    }
+    // four threads per output: thread q adds the slices q, q + 4, ... in index order (all its loads in flight: at most 16
+    // slices per thread per round), then the quad is combined by a fixed xor butterfly -- one latency round instead of
+    // ksplit / 8
+    const int q = threadIdx.x & 3;
+    for (long long t = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 2; t < ((total + 63) & ~63LL); t += ((long long)gridDim.x * blockDim.x) >> 2) {
+        const bool live = t < total;
+        const long long tt = live ? t : total - 1;
+        double s = 0.0;
+        for (int k0 = q; k0 < ksplit; k0 += 64) {
+            double w[16];
+#pragma unroll
+            for (int e = 0; e < 16; ++e) w[e] = k0 + 4 * e < ksplit ? (double)gpart[(long long)(k0 + 4 * e) * total + tt] : 0.0;
+#pragma unroll
+            for (int e = 0; e < 16; ++e) s += w[e];
+        }
+        s += __shfl_xor_sync(0xffffffffu, s, 1);
+        s += __shfl_xor_sync(0xffffffffu, s, 2);
+        const int n = (int)(tt / RP), c = (int)(tt - (long long)n * RP);
+        if (live && q == 0 && r0 + c < R) sigma[out_off + (long long)n * R + r0 + c] = (T)s;
     }
 }
 
