@@ -7,8 +7,10 @@
 // tcgen05 has no f64 kind, so only the fp32 variant (reading R18: fp32 table, fp32 f, 1e-5 of sum|terms|)
 // can use it; a single TF32 pass misses that tolerance (1.7e-5), so every fp32 operand x is split
 // exactly into x = hi + lo, hi = x with the 13 low mantissa bits cleared (what kind::tf32 reads of an fp32 word),
-// lo = x - hi (exact in fp32), and three products are accumulated in fp32:  fb_hi FK_hi + fb_lo FK_hi + fb_hi FK_lo
-// (the dropped lo x lo term and the truncation of lo to 11 bits are each <= 2^-20 of |term|).
+// lo = x - hi (exact in fp32), and three products are accumulated in fp32:  fb_hi FK_hi + fb_lo FK + fb FK_lo.  The first
+// runs as kind::tf32; the two correction products are 2^-11 of the result, so 8-bit operands suffice for them and they run
+// as kind::f16 on bf16 roundings of fb_lo, FK, fb, FK_lo (twice the MMA rate, half the shared-memory bytes): each
+// rounding costs <= 2^-9 of a 2^-11 term, like the dropped lo x lo term <= 2^-20 of |term|.
 //
 // The contraction is done in the factored order above, which the flat GEMM view hides: the inner sum over j has
 // the SAME right-hand factor f[b_c][.][r] for every x-row i and every datapoint n of a channel, so the tensor-core operand
@@ -17,11 +19,12 @@
 //
 //   D^T[r][n] = sum_j fb[r][j] * FK[n][(c,i)][j]          one tcgen05.mma chain per (c, i) row: M = 128 replicas (TMEM lanes),
 //                                                         N = 128 datapoints, K = nx rounded up to 8
-//   A operand  fb_hi / fb_lo of channel c, [128 r][K], in TENSOR MEMORY (tcgen05.st, double buffered per channel):
-//              shared memory carries only the table;
+//   A operand  fb_hi (tf32), bf16(fb_lo), bf16(fb) of channel c, [128 r][K], in TENSOR MEMORY (tcgen05.st, double
+//              buffered per channel): shared memory carries only the table;
 //   B operand  FK rows [128 n][K] of (c, i): raw tile by TMA (cp.async.bulk.tensor, 128-byte swizzle, box 32 k x 128 n,
 //              two boxes; a box must start on 16 bytes, which is why fp32 tables are packed with x-rows padded to a
-//              multiple of 4 elements (TableDesc::jp); k beyond nx meets zero rows of fb), FK_lo by 4 splitter warps;
+//              multiple of 4 elements (TableDesc::jp); k beyond nx meets zero rows of fb), bf16(FK) and bf16(FK_lo)
+//              tiles ([128 n][64 bf16], one swizzle row each) by 4 splitter warps;
 //   epilogue   acc[n] += f[a_c][i][r] * D^T[r][n]  (tcgen05.ld, lane = replica r), two-level fp32 sums (x-rows of a channel, then channels);
 //              at the end the partial tile goes to gpart[range][n][r] (split level 1).
 // One CTA = one item (128-datapoint tile, range of (c, i) rows), warp-specialised: warp 0 TMA producer, warp 1 MMA
@@ -30,6 +33,7 @@
 #include "fk_tc32.h"
 
 #include <cuda.h>
+#include <cuda_bf16.h>
 
 #include <cstdio>
 #include <cstring>
@@ -46,8 +50,8 @@ constexpr int TC_RAW_STAGES = 3;           // TMA ring of raw FK tiles
 constexpr int TC_LO_STAGES = 2;            // FK_lo tiles
 constexpr int TC_BOX_BYTES = TC_BN * 32 * 4;      // one TMA box: 128 rows x 32 fp32 = 16 KB
 constexpr int TC_STAGE_BYTES = 2 * TC_BOX_BYTES;  // K extent <= 64: two boxes
-constexpr int TC_TMEM_COLS = 512;          // D: 2 x 128 columns; fb operand: 2 buffers x (hi 64 + lo 64)
-constexpr uint32_t TC_TMEM_A = 256;
+constexpr int TC_TMEM_COLS = 512;          // D: 2 x 128 columns; fb operand: 2 buffers x (tf32 hi 64 + bf16 lo 32 + bf16 full 32)
+constexpr uint32_t TC_TMEM_A = 256, TC_A_LO_BF = 64, TC_A_FULL_BF = 96;
 constexpr uint32_t TF32_MASK = 0xffffe000u;
 
 // ---- PTX wrappers (one instruction each) -------------------------------------------------------------------------
@@ -105,6 +109,13 @@ __device__ __forceinline__ void tc_mma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem,
         "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// D[tmem] += A[tmem] . B[smem desc]^T, kind::f16 on bf16 operands (K = 16 per instruction)
+__device__ __forceinline__ void tc_mma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n}\n" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 __device__ __forceinline__ void tc_ld16(uint32_t taddr, float (&v)[16]) {
     uint32_t r[16];
     asm volatile(
@@ -122,6 +133,13 @@ __device__ __forceinline__ void tc_st8(uint32_t taddr, const float (&v)[8]) {
                  "r"(__float_as_uint(v[5])), "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7]))
                  : "memory");
 }
+__device__ __forceinline__ void tc_st4(uint32_t taddr, const uint32_t (&v)[4]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory");
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {   // element k (even) in the low half, k + 1 in the high half
+    const __nv_bfloat162 b = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<const uint32_t*>(&b);
+}
 __device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // UMMA shared-memory descriptor, K-major operand in the 128-byte-swizzle canonical layout (rows of 128 bytes, 8-row
@@ -133,6 +151,10 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
 // UMMA instruction descriptor: D fp32, A and B tf32, both K-major, no negate / sparsity / saturate
 __host__ __device__ constexpr uint32_t umma_idesc_tf32(int M, int N) {
     return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+// the same with bf16 operands (kind::f16)
+__host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
 // barrier slots
@@ -175,7 +197,8 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
     }
     const TableDesc& d = *dp;
     const int nx = d.nx, cstride = d.cstride, jp = d.jp;
-    const int nk8 = (nx + 7) >> 3;                    // MMA steps of 8 k per (c, i) row
+    const int nk8 = (nx + 7) >> 3;                    // tf32 MMA steps of 8 k per (c, i) row
+    const int nk16 = (nk8 + 1) >> 1;                  // bf16 MMA steps of 16 k
     const int T = d.C * nx;                           // (c, i) rows of the table
     const int t0 = min(T, ks * tper), ntl = min(T, t0 + tper) - t0;
     const int rows = min(TC_BN, d.N - n0), NT = (rows + 15) & ~15;   // UMMA N
@@ -202,6 +225,11 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    // the bf16 tiles are written up to k = 8 nk8; a last k-step of 16 reads 8 more: zero them once (they meet zero rows of
+    // the fb operand, but 0 x NaN of stale shared memory would still poison the accumulator)
+    for (uint32_t o = (uint32_t)tid * 16u; o < (uint32_t)(TC_LO_STAGES * TC_STAGE_BYTES); o += TC_THREADS * 16u)
+        asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(sm_lo + o), "r"(0u) : "memory");
+    fence_async_smem();
     if (warp == 2) {   // TMEM: all 512 columns (one CTA per SM by shared memory), address written to shared memory
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sm_tmem_slot), "r"(TC_TMEM_COLS) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -236,7 +264,7 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
         } else if (warp == 1) {
             // ---- MMA issuer: the whole warp walks the loop, one elected lane issues
             const bool leader = elect_one();
-            const uint32_t idesc = umma_idesc_tf32(128, NT);
+            const uint32_t idesc = umma_idesc_tf32(128, NT), idesc_bf = umma_idesc_bf16(128, NT);
             int i = i_first, cc = 0;
             bool newch = true;
             for (int t = 0; t < ntl; ++t) {
@@ -249,17 +277,17 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
                 mbar_wait(bar(BAR_FK_FULL + slot), (t / TC_RAW_STAGES) & 1, 4);
                 tc_fence_after();
                 const uint32_t d_acc = tmem_base + (uint32_t)buf * 128u;
-                const uint32_t a_hi = tmem_base + TC_TMEM_A + (uint32_t)abuf * 128u, a_lo = a_hi + 64u;
-                // 8 fp32 = 32 bytes (descriptor + 2) along the swizzle row; the second box holds k 32..63
+                const uint32_t a_hi = tmem_base + TC_TMEM_A + (uint32_t)abuf * 128u;
+                // 8 fp32 = 16 bf16 = 32 bytes (descriptor + 2) along the swizzle row; the second fp32 box holds k 32..63
                 const uint64_t braw = umma_desc_sw128(sm_raw + (uint32_t)slot * TC_STAGE_BYTES);
-                const uint64_t blo = umma_desc_sw128(sm_lo + (uint32_t)ls * TC_STAGE_BYTES);
+                const uint64_t bfk = umma_desc_sw128(sm_lo + (uint32_t)ls * TC_STAGE_BYTES);                  // bf16(FK)
+                const uint64_t blo = umma_desc_sw128(sm_lo + (uint32_t)ls * TC_STAGE_BYTES + TC_BOX_BYTES);   // bf16(FK_lo)
                 if (leader) {
 #pragma unroll
                     for (int k8 = 0; k8 < 8; ++k8) {
                         if (k8 < nk8) {
                             const uint64_t b = braw + (uint64_t)((k8 >> 2) * (TC_BOX_BYTES >> 4) + (k8 & 3) * 2);
                             tc_mma_tf32_ts(d_acc, a_hi + 8u * (uint32_t)k8, b, idesc, k8 > 0 ? 1u : 0u);
-                            tc_mma_tf32_ts(d_acc, a_lo + 8u * (uint32_t)k8, b, idesc, 1u);
                         }
                     }
                 }
@@ -268,10 +296,10 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
                 tc_fence_after();
                 if (leader) {
 #pragma unroll
-                    for (int k8 = 0; k8 < 8; ++k8) {
-                        if (k8 < nk8) {
-                            const uint64_t b = blo + (uint64_t)((k8 >> 2) * (TC_BOX_BYTES >> 4) + (k8 & 3) * 2);
-                            tc_mma_tf32_ts(d_acc, a_hi + 8u * (uint32_t)k8, b, idesc, 1u);
+                    for (int k16 = 0; k16 < 4; ++k16) {
+                        if (k16 < nk16) {
+                            tc_mma_bf16_ts(d_acc, a_hi + TC_A_LO_BF + 8u * (uint32_t)k16, bfk + (uint64_t)(k16 * 2), idesc_bf, 1u);
+                            tc_mma_bf16_ts(d_acc, a_hi + TC_A_FULL_BF + 8u * (uint32_t)k16, blo + (uint64_t)(k16 * 2), idesc_bf, 1u);
                         }
                     }
                     tc_commit(bar(BAR_FK_FREE + slot));
@@ -299,16 +327,21 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
             tc_fence_after();
             const float* src = fT + (long long)chb[c] * nx * RP + st;
             const uint32_t a_hi = tmem_base + lane_addr + TC_TMEM_A + (uint32_t)abuf * 128u;
-            for (int j0 = 0; j0 < 8 * nk8; j0 += 8) {
-                float hi[8], lo[8];
+            for (int j0 = 0; j0 < 16 * nk16; j0 += 8) {   // the bf16 operands span whole k-steps of 16: zero beyond nx
+                float hi[8];
+                uint32_t lob[4], fullb[4];
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const float v = (j0 + e < nx && st < RP) ? __ldg(src + (long long)(j0 + e) * RP) : 0.f;
-                    hi[e] = __uint_as_float(__float_as_uint(v) & TF32_MASK);
-                    lo[e] = v - hi[e];
+                for (int e = 0; e < 8; e += 2) {
+                    const float v0 = (j0 + e < nx && st < RP) ? __ldg(src + (long long)(j0 + e) * RP) : 0.f;
+                    const float v1 = (j0 + e + 1 < nx && st < RP) ? __ldg(src + (long long)(j0 + e + 1) * RP) : 0.f;
+                    hi[e] = __uint_as_float(__float_as_uint(v0) & TF32_MASK);
+                    hi[e + 1] = __uint_as_float(__float_as_uint(v1) & TF32_MASK);
+                    lob[e >> 1] = pack_bf16(v0 - hi[e], v1 - hi[e + 1]);
+                    fullb[e >> 1] = pack_bf16(v0, v1);
                 }
                 tc_st8(a_hi + (uint32_t)j0, hi);
-                tc_st8(a_hi + 64u + (uint32_t)j0, lo);
+                tc_st4(a_hi + TC_A_LO_BF + (uint32_t)(j0 >> 1), lob);
+                tc_st4(a_hi + TC_A_FULL_BF + (uint32_t)(j0 >> 1), fullb);
             }
             tc_wait_st();
             tc_fence_before();
@@ -319,26 +352,36 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
         pdl_wait();   // fT is written by the transpose kernel just before this launch (the table itself is not: TMA runs ahead)
         if (ntl > 0) build_a(0, c);
         bool build_next = c < c_last;   // the next channel's operand is built under the first row of this one
-        const int nq = 2 * nk8;         // 16-byte chunks of a row
         for (int t = 0; t < ntl; ++t) {
             const int slot = t % TC_RAW_STAGES, ls = t & 1;
             mbar_wait(bar(BAR_LO_FREE + ls), ((t >> 1) & 1) ^ 1, 7);
             mbar_wait(bar(BAR_FK_FULL + slot), (t / TC_RAW_STAGES) & 1, 8);
             if (st < NT) {
-                // FK_lo = x - hi(x), element-wise (the swizzle is the same on both sides): logical chunk q of row st
-                // sits at 16-byte position (q & 7) ^ (st & 7) of the row's 128 bytes in box q >> 3
+                // bf16(FK) and bf16(FK_lo), FK_lo = x - tf32(x): logical fp32 chunk q of row st sits at 16-byte position
+                // (q & 7) ^ (st & 7) of the row's 128 bytes in box q >> 3; two fp32 chunks make bf16 chunk m = q / 2 at
+                // position m ^ (st & 7) of the row's 128 bytes in its tile
                 const uint32_t src = sm_raw + (uint32_t)slot * TC_STAGE_BYTES + (uint32_t)st * 128u;
                 const uint32_t dst = sm_lo + (uint32_t)ls * TC_STAGE_BYTES + (uint32_t)st * 128u;
-#pragma unroll 4
-                for (int q = 0; q < nq; ++q) {
-                    const uint32_t o = (uint32_t)(q >> 3) * TC_BOX_BYTES + (uint32_t)(((q & 7) ^ (st & 7)) << 4);
-                    float x0, x1, x2, x3;
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x0), "=f"(x1), "=f"(x2), "=f"(x3) : "r"(src + o));
-                    x0 -= __uint_as_float(__float_as_uint(x0) & TF32_MASK);
-                    x1 -= __uint_as_float(__float_as_uint(x1) & TF32_MASK);
-                    x2 -= __uint_as_float(__float_as_uint(x2) & TF32_MASK);
-                    x3 -= __uint_as_float(__float_as_uint(x3) & TF32_MASK);
-                    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst + o), "f"(x0), "f"(x1), "f"(x2), "f"(x3) : "memory");
+#pragma unroll 2
+                for (int m = 0; m < nk8; ++m) {
+                    float x[8];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int q = 2 * m + h;
+                        const uint32_t o = (uint32_t)(q >> 3) * TC_BOX_BYTES + (uint32_t)(((q & 7) ^ (st & 7)) << 4);
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x[4 * h]), "=f"(x[4 * h + 1]), "=f"(x[4 * h + 2]), "=f"(x[4 * h + 3]) : "r"(src + o));
+                    }
+                    uint32_t fb4[4], lo4[4];
+#pragma unroll
+                    for (int e = 0; e < 8; e += 2) {
+                        const float l0 = x[e] - __uint_as_float(__float_as_uint(x[e]) & TF32_MASK);
+                        const float l1 = x[e + 1] - __uint_as_float(__float_as_uint(x[e + 1]) & TF32_MASK);
+                        fb4[e >> 1] = pack_bf16(x[e], x[e + 1]);
+                        lo4[e >> 1] = pack_bf16(l0, l1);
+                    }
+                    const uint32_t od = (uint32_t)((m ^ (st & 7)) << 4);
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + od), "r"(fb4[0]), "r"(fb4[1]), "r"(fb4[2]), "r"(fb4[3]) : "memory");
+                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + TC_BOX_BYTES + od), "r"(lo4[0]), "r"(lo4[1]), "r"(lo4[2]), "r"(lo4[3]) : "memory");
                 }
             }
             fence_async_smem();   // generic-proxy stores -> visible to the tensor core (async proxy)
