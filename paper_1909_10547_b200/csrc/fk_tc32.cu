@@ -362,8 +362,9 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
                 // position m ^ (st & 7) of the row's 128 bytes in its tile
                 const uint32_t src = sm_raw + (uint32_t)slot * TC_STAGE_BYTES + (uint32_t)st * 128u;
                 const uint32_t dst = sm_lo + (uint32_t)ls * TC_STAGE_BYTES + (uint32_t)st * 128u;
-#pragma unroll 2
-                for (int m = 0; m < nk8; ++m) {
+#pragma unroll
+                for (int m = 0; m < 8; ++m) {
+                    if (m >= nk8) break;
                     float x[8];
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
