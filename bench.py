@@ -240,6 +240,14 @@ def run_extras(K, torch, level, table2, case2, peak):
     ms = _bench_call(lambda: table2.vjp(f2, g2, d2), stream)
     out["cfg2_vjp"] = {"ms": ms, "GBps": fkb / ms / 1e6, "frac_of_peak": fkb / ms / 1e6 / peak}
 
+    # the step replayed from a CUDA graph (capture of the two calls on a side stream): launch gaps removed by the driver
+    graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.graph(graph, stream=side):
+        table2.conv(f2, s2)
+        table2.vjp(f2, g2, d2)
+    ms = _bench_call(graph.replay, stream)
+    out["cfg2_step_cuda_graph"] = {"ms": ms, "GBps": 2 * fkb / ms / 1e6, "frac_of_peak": 2 * fkb / ms / 1e6 / peak}
+    del graph
     # forward + VJP from ONE read of FK (fk_table_conv_vjp: g known before the forward pass).
     # GBps counts the FK bytes that really move (once); step_equiv_GBps the two-pass step it replaces.
     ms = _bench_call(lambda: table2.conv_vjp(f2, g2, s2, d2), stream)

@@ -468,6 +468,64 @@ def test_tc32_same_sign_and_exact_small_integers(K):
     tp.destroy()
 
 
+# ------------------------------------------------------------------ CUDA graphs
+def test_calls_capture_into_a_cuda_graph(K):
+    """Every compute call is asynchronous on the caller's stream, allocates nothing once its scratch is sized and
+    synchronises nothing (include/fkconv.h): a fit iteration (forward, VJP, one-read step, grouped forward) must
+    therefore capture into a CUDA graph -- programmatic dependent launches included -- and every replay must give
+    the eager result bit for bit, also after the inputs changed in place."""
+    import torch
+    case = synth.hadronic_case(8, 96, 24, 30, 2, sub=77)
+    dis = synth.config1(R=2, N=300)
+    tp = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl, K.FK_F64, K.FK_STORE_PACK, R_hint=2)
+    td = K.FkTable(K.FK_KIND_DIS, to_dev(dis.fk), dis.flav, dis.nfl, R_hint=2)
+    t32 = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl, K.FK_F32, K.FK_STORE_PACK, R_hint=40)
+    grp = K.FkGroup([tp, td], R_hint=2)
+    f_d, g_d = to_dev(case.f), to_dev(case.g)
+    fd_d = to_dev(dis.f)
+    f40 = to_dev(np.ascontiguousarray(np.broadcast_to(case.f[:1], (40,) + case.f.shape[1:])), torch.float32)
+    f_cat = torch.cat([f_d.reshape(-1), fd_d.reshape(-1)])
+    sig, df = torch.empty((case.N, 2), dtype=torch.float64, device="cuda"), torch.empty_like(f_d)
+    sig1, df1 = torch.empty_like(sig), torch.empty_like(df)
+    sig_cat = torch.empty(int(grp.offsets(2)[1][-1]), dtype=torch.float64, device="cuda")
+    sig40 = torch.empty((case.N, 40), dtype=torch.float32, device="cuda")
+
+    def step():
+        tp.conv(f_d, sig)
+        tp.vjp(f_d, g_d, df)
+        tp.conv_vjp(f_d, g_d, sig1, df1)
+        grp.conv(f_cat, 2, sig_cat)
+        t32.conv(f40, sig40)      # the tcgen05 contraction (TMA, tensor memory) inside the graph as well
+
+    step()                        # sizes every scratch buffer outside the capture
+    torch.cuda.synchronize()
+    want = [t.clone() for t in (sig, df, sig1, df1, sig_cat, sig40)]
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.graph(graph, stream=side):
+        step()
+    for t in (sig, df, sig1, df1, sig_cat, sig40):
+        t.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    for got, ref in zip((sig, df, sig1, df1, sig_cat, sig40), want):
+        assert torch.equal(got, ref)
+    f_d.mul_(1.25)                # new inputs in place: the graph reads the same buffers
+    f_cat[: f_d.numel()] = f_d.reshape(-1)
+    graph.replay()
+    torch.cuda.synchronize()
+    ref, scale = O.hadronic(case.fk, case.pairs, case.f * 1.25)
+    assert rel_err(sig.cpu().numpy(), ref, scale) <= TOL64
+    assert torch.equal(sig, sig1) and torch.equal(sig_cat[: sig.numel()].reshape(sig.shape), sig)
+    # a handle refuses to grow its scratch inside a capture instead of allocating there
+    g2 = torch.cuda.CUDAGraph()
+    big = to_dev(np.ascontiguousarray(np.broadcast_to(case.f[:1], (64,) + case.f.shape[1:])))
+    with pytest.raises(RuntimeError):
+        with torch.cuda.graph(g2, stream=side):
+            tp.conv(big)
+    grp.destroy()
+
+
 # ------------------------------------------------------------------ host-buffer calls
 def test_host_buffer_calls(K):
     case = synth.hadronic_case(6, 48, 20, 30, 2, sub=5)
