@@ -468,6 +468,56 @@ def test_tc32_same_sign_and_exact_small_integers(K):
     tp.destroy()
 
 
+# ------------------------------------------------------------------ launch-mode options change timing, never bits
+def test_launch_options_do_not_change_results(K):
+    """FK_OPT_PDL (programmatic dependent launch of the later kernels of a call) and FK_OPT_FUSE_L2 (small tables: the
+    forward kernel's last CTA per datapoint range runs the level-2 reduction, one launch instead of two) only move
+    work in time: every result must be bit for bit the same with the option off."""
+    import torch
+    c0 = synth.config0(R=2)
+    big = synth.hadronic_case(8, 200, 30, 9, 2, nfl=14, sub=4)       # several k-blocks and several datapoint ranges
+    c32 = synth.hadronic_case(8, 129, 50, 3, 40, nfl=14, sub=9)
+    tabs = [(K.FkTable(K.FK_KIND_HADRONIC, to_dev(c.fk), c.pairs, c.nfl, K.FK_F64, K.FK_STORE_PACK, R_hint=2), c) for c in (c0, big)]
+    t32 = K.FkTable(K.FK_KIND_HADRONIC, to_dev(c32.fk), c32.pairs, c32.nfl, K.FK_F32, K.FK_STORE_PACK, R_hint=40)
+    grp = K.FkGroup([t for t, _ in tabs], R_hint=2)
+    f_cat = torch.cat([to_dev(c.f).reshape(-1) for _, c in tabs])
+
+    def run():
+        out = []
+        for t, c in tabs:
+            out.append(t.conv(to_dev(c.f)))
+            out.append(t.vjp(to_dev(c.f), to_dev(c.g)))
+            out.append(torch.tensor([t.last_launches()]))
+        out.append(grp.conv(f_cat, 2))
+        out.append(t32.conv(to_dev(c32.f, torch.float32)))
+        torch.cuda.synchronize()
+        return out
+
+    base = run()
+    ref, scale = O.hadronic(c0.fk, c0.pairs, c0.f)
+    assert rel_err(base[0].cpu().numpy(), ref, scale) <= TOL64
+    for option in (K.FK_OPT_PDL, K.FK_OPT_FUSE_L2):
+        K.set_option(option, 0)
+        try:
+            other = run()
+        finally:
+            K.set_option(option, 1)
+        for i, (a, b) in enumerate(zip(base, other)):
+            if a.numel() == 1 and a.dtype == torch.int64:
+                continue   # launch counts differ by design
+            assert torch.equal(a, b), (option, i)
+    # config 0 (one wave of CTAs) really is a single forward launch with the in-kernel reduction, and two without it
+    t0, c = tabs[0]
+    t0.conv(to_dev(c.f)); n_fused = t0.last_launches()
+    K.set_option(K.FK_OPT_FUSE_L2, 0)
+    try:
+        t0.conv(to_dev(c.f)); n_split = t0.last_launches()
+    finally:
+        K.set_option(K.FK_OPT_FUSE_L2, 1)
+    assert (n_fused, n_split) == (1, 2)
+    grp.destroy()
+
+
 # ------------------------------------------------------------------ CUDA graphs
 def test_calls_capture_into_a_cuda_graph(K):
     """Every compute call is asynchronous on the caller's stream, allocates nothing once its scratch is sized and
