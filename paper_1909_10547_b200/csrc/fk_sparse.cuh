@@ -102,12 +102,12 @@ __device__ __forceinline__ void sp_stage_index(const TableDesc& d, int nkb, int 
 // value loads back to back.
 __device__ __forceinline__ void sp_load_pair(const double* __restrict__ vals, const SparseBlk& b, int w, uint32_t wsh, uint32_t lt, int lane,
                                              bool live, double& xa, double& xb) {
-    const unsigned long long m = b.mask[w];
-    const unsigned int ma = (unsigned int)m, mb = (unsigned int)(m >> 32);
+    const uint2 m = *reinterpret_cast<const uint2*>(&b.mask[w]);   // bits l and l + 32 of this warp's word
+    const unsigned int ma = m.x, mb = m.y, lbit = lt + 1u;
     const unsigned int wp = w ? (unsigned int)(b.wpre >> wsh) & 0x1ffu : 0u;
-    const double* vp = vals + b.off + wp;
+    const double* vp = vals + (b.off + wp);
     const unsigned int ia = __popc(ma & lt), ib = __popc(ma) + __popc(mb & lt);
-    const unsigned int pa = live ? (ma >> lane) & 1u : 0u, pb = live ? (mb >> lane) & 1u : 0u;
+    const unsigned int pa = live ? ma & lbit : 0u, pb = live ? mb & lbit : 0u;
     xa = xb = 0.0;
     asm("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p ld.global.nc.L1::no_allocate.f64 %0, [%1];\n}\n" : "+d"(xa) : "l"(vp + ia), "r"(pa));
     asm("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p ld.global.nc.L1::no_allocate.f64 %0, [%1];\n}\n" : "+d"(xb) : "l"(vp + ib), "r"(pb));
@@ -166,14 +166,19 @@ fk_fwd_sparse_kernel(const __grid_constant__ FwdParams p) {
         }
         const int mrel = (m - rb) % SP_CHUNK, nlive = re - m;   // U divides SP_CHUNK: a batch never straddles chunks
         double xa[U], xb[U];
+        const SparseBlk* rec = sblk + mrel;
+        if (nlive >= U) {   // whole batch: immediate offsets, no selects
 #pragma unroll
-        for (int u = 0; u < U; ++u)
-            sp_load_pair(vals, sblk[mrel + (u < nlive ? u : 0)], warp, wsh, lt, lane, true, xa[u], xb[u]);
+            for (int u = 0; u < U; ++u) sp_load_pair(vals, rec[u], warp, wsh, lt, lane, true, xa[u], xb[u]);
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; ++u) sp_load_pair(vals, rec[u < nlive ? u : 0], warp, wsh, lt, lane, u < nlive, xa[u], xb[u]);
+        }
         double pr[RT][U];
 #pragma unroll
         for (int u = 0; u < U; ++u)
 #pragma unroll
-            for (int r = 0; r < RT; ++r) pr[r][u] = u < nlive ? fma(xb[u], L[r][1], xa[u] * L[r][0]) : 0.0;
+            for (int r = 0; r < RT; ++r) pr[r][u] = fma(xb[u], L[r][1], xa[u] * L[r][0]);
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
             const double s = fold_rows<U>(pr[r], lane);
@@ -245,9 +250,14 @@ fk_colsum_sparse_kernel(const __grid_constant__ ColsumParams p) {
         for (int m = c0; m < mend; m += U) {
             const int nlive = rows - m;
             double xa[U], xb[U];
+            const SparseBlk* rec = &sblk[cb][m - c0];
+            if (nlive >= U) {   // whole batch: immediate offsets, no selects
 #pragma unroll
-            for (int u = 0; u < U; ++u)
-                sp_load_pair(vals, sblk[cb][m - c0 + (u < nlive ? u : 0)], warp, wsh, lt, lane, u < nlive, xa[u], xb[u]);
+                for (int u = 0; u < U; ++u) sp_load_pair(vals, rec[u], warp, wsh, lt, lane, true, xa[u], xb[u]);
+            } else {
+#pragma unroll
+                for (int u = 0; u < U; ++u) sp_load_pair(vals, rec[u < nlive ? u : 0], warp, wsh, lt, lane, u < nlive, xa[u], xb[u]);
+            }
 #pragma unroll
             for (int u = 0; u < U; ++u)
 #pragma unroll
