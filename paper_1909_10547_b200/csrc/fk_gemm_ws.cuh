@@ -62,6 +62,20 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                  : "memory");
 }
 
+// The forward kernel reads the table once: its bulk copies carry an L2 evict-first policy, so that the streamed rows do not
+// push the small, re-read operands (the level-1 partial tiles that are read-modified-written at every flush, fT) out of L2
+// (config 3 forward 1.069 -> 1.057 ms).  The VJP kernel keeps the default policy (1.082 ms; 1.097 with the hint).
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s_stream(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar), "l"(pol)
+                 : "memory");
+}
+
 // Same fields as GemmFwdParams where they mean the same thing.
 struct WsFwdParams {
     TableDesc desc;        // single-table launch
@@ -161,6 +175,7 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
         if (warp != WS_CONSUMER_WARPS) return;
         const double* __restrict__ fk = reinterpret_cast<const double*>(d.fk);
+        const uint64_t pol = l2_evict_first_policy();
         const int rows_valid = min(TM, d.N - m0);
         auto issue_fb = [&](int c, int ccn) {  // f[b_c][.][.] of channel c -> buffer ccn & 1
             const int buf = ccn & 1;
@@ -193,8 +208,8 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
                 for (int q = 0; q < GEMM_BM / 32; ++q) {
                     const int row = lane + 32 * q;
                     if (row < rows_valid)
-                        bulk_g2s(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * SAv) * 8),
-                                 fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(len * 8), bar_full(stage));
+                        bulk_g2s_stream(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * SAv) * 8),
+                                        fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(len * 8), bar_full(stage), pol);
                 }
             }
             if (!next_issued) issue_fb(c + 1, cc + 1);
