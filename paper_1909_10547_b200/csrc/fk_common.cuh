@@ -118,6 +118,13 @@ __device__ __forceinline__ int encode_k(const TableDesc& d, int i, int j, int c)
 }
 
 // ---- streaming loads: FK is read once, keep it out of L1 -------------------------------------
+// L2 evict-first policy for the table stream (not volatile: one createpolicy per thread, hoisted out of the loops): the
+// small operands that ARE re-read -- level-1 partials, column sums G, f -- stay in L2 while the table passes through
+__device__ __forceinline__ uint64_t stream_policy() {
+    uint64_t pol;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
 template <typename T, int VEC> struct Vec;
 template <> struct Vec<double, 2> { double v[2]; };
 template <> struct Vec<double, 1> { double v[1]; };
@@ -126,23 +133,23 @@ template <> struct Vec<float, 1> { float v[1]; };
 
 __device__ __forceinline__ Vec<double, 2> ld_stream(const double* p, Vec<double, 2>*) {
     Vec<double, 2> r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.v[0]), "=d"(r.v[1]) : "l"(p));
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(r.v[0]), "=d"(r.v[1]) : "l"(p), "l"(stream_policy()));
     return r;
 }
 __device__ __forceinline__ Vec<double, 1> ld_stream(const double* p, Vec<double, 1>*) {
     Vec<double, 1> r;
-    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r.v[0]) : "l"(p));
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(r.v[0]) : "l"(p), "l"(stream_policy()));
     return r;
 }
 __device__ __forceinline__ Vec<float, 4> ld_stream(const float* p, Vec<float, 4>*) {
     Vec<float, 4> r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
-                 : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "l"(p));
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "l"(p), "l"(stream_policy()));
     return r;
 }
 __device__ __forceinline__ Vec<float, 1> ld_stream(const float* p, Vec<float, 1>*) {
     Vec<float, 1> r;
-    asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r.v[0]) : "l"(p));
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(r.v[0]) : "l"(p), "l"(stream_policy()));
     return r;
 }
 

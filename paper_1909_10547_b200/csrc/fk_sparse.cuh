@@ -109,8 +109,9 @@ __device__ __forceinline__ void sp_load_pair(const double* __restrict__ vals, co
     const unsigned int ia = __popc(ma & lt), ib = __popc(ma) + __popc(mb & lt);
     const unsigned int pa = live ? ma & lbit : 0u, pb = live ? mb & lbit : 0u;
     xa = xb = 0.0;
-    asm("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p ld.global.nc.L1::no_allocate.f64 %0, [%1];\n}\n" : "+d"(xa) : "l"(vp + ia), "r"(pa));
-    asm("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p ld.global.nc.L1::no_allocate.f64 %0, [%1];\n}\n" : "+d"(xb) : "l"(vp + ib), "r"(pb));
+    const uint64_t pol = stream_policy();   // L2 evict-first: the values are read once
+    asm("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %3;\n}\n" : "+d"(xa) : "l"(vp + ia), "r"(pa), "l"(pol));
+    asm("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %3;\n}\n" : "+d"(xb) : "l"(vp + ib), "r"(pb), "l"(pol));
 }
 
 // a1 + a2 + a3 level 1 over a sparse table: same CTA decomposition (k-block x datapoint range), same partials as
