@@ -370,6 +370,22 @@ bool ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) 
     return true;
 }
 
+// DIS tables (any k-order): the warp-specialised kernel whose B tile is 32 fT rows per stage (fk_gemm_dis_ws_kernel)
+bool wsd_ok(const fk::TableDesc& d, int RP) {
+    return d.kind == fk::KIND_DIS && d.vec_ok && opt(FK_OPT_WARP_SPEC) && fk::wsd_smem_bytes(RP) <= MAX_DYN_SMEM;
+}
+bool wsd_launch(const fk::WsFwdParams& w, int grid, cudaStream_t s) {
+    const size_t smem = fk::wsd_smem_bytes(w.RP);
+    switch (w.RP / 8) {
+#define FK_WSD_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_dis_ws_kernel<NFW>, MAX_DYN_SMEM)) return false; \
+                                   FK_TIMED("fk_gemm_dis_ws", s) launch_pdl(fk::fk_gemm_dis_ws_kernel<NFW>, grid, fk::WS_THREADS, smem, s, w); break
+        FK_WSD_CASE(2); FK_WSD_CASE(4); FK_WSD_CASE(6); FK_WSD_CASE(8); FK_WSD_CASE(10); FK_WSD_CASE(12); FK_WSD_CASE(14);
+        default: FK_WSD_CASE(16);
+#undef FK_WSD_CASE
+    }
+    return true;
+}
+
 // the persistent warp-specialised VJP contraction needs 16-byte aligned, 16-byte multiple row pieces
 bool wsv_ok(const fk::TableDesc& d) { return d.vec_ok && d.K % 2 == 0 && opt(FK_OPT_WARP_SPEC); }
 
@@ -395,13 +411,14 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
     double* gpart = fT + (size_t)slots * gp.RPmax;
     int nl = 0;
     const bool ws = ws_ok(d, gp.RPmax);
-    if (!kdec && !ws) {
+    const bool wsd = !ws && wsd_ok(d, gp.RPmax);
+    if (!kdec && !ws && !wsd) {
         uint32_t* kd = reinterpret_cast<uint32_t*>(gpart + (size_t)gp.ksplit * d.N * gp.RPmax);
         FK_TIMED("fk_kdec", s) fk::fk_kdec_kernel<<<std::min(1024, (d.K + 255) / 256), 256, 0, s>>>(d, ch, kd);
         ++nl;
         kdec = kd;
     }
-    if (!ws && !(ensure_dyn_smem(fk::fk_gemm_fwd_kernel<2, false>, fk::GEMM_SMEM_BYTES) &&
+    if (!ws && !wsd && !(ensure_dyn_smem(fk::fk_gemm_fwd_kernel<2, false>, fk::GEMM_SMEM_BYTES) &&
                  ensure_dyn_smem(fk::fk_gemm_fwd_kernel<1, false>, fk::GEMM_SMEM_BYTES)))
         return fail(FK_ERR_CUDA, "gemm: cannot reserve %d bytes of shared memory", fk::GEMM_SMEM_BYTES);
     const int mtiles = (d.N + fk::GEMM_BM - 1) / fk::GEMM_BM;
@@ -433,6 +450,17 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
             const int nfull = d.N / fk::GEMM_BM;
             if (!ws_launch<false>(w, nfull * gp.ksplit + (d.N % fk::GEMM_BM ? gp.ksplit / gp.ksub_rem : 0), fk::ws_smem_bytes(d.nx, p.RP), s))
                 return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
+        } else if (wsd) {
+            fk::WsFwdParams w;
+            memset(&w, 0, sizeof w);
+            w.desc = d;
+            w.chan = ch;
+            w.fT = fT;
+            w.gpart = gpart;
+            w.RP = p.RP;
+            w.ksplit = gp.ksplit;
+            w.kper = gp.kper;
+            if (!wsd_launch(w, mtiles * gp.ksplit, s)) return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
         } else if (d.vec_ok) FK_TIMED("fk_gemm_fwd", s) launch_pdl(fk::fk_gemm_fwd_kernel<2, false>, mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s, p);
         else FK_TIMED("fk_gemm_fwd", s) launch_pdl(fk::fk_gemm_fwd_kernel<1, false>, mtiles * gp.ksplit, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s, p);
         const long long outs = (long long)d.N * p.RP;

@@ -86,7 +86,7 @@ __device__ __forceinline__ double fold_rows(double (&p)[U], int lane) {
 
 // TS = storage type of the table (float for the fp32-storage variants), T = type of f, sigma and of the arithmetic
 template <typename T, int VEC, int RT, int U, bool GROUPED, typename TS = T>
-__global__ void __launch_bounds__(FWD_THREADS, RT == 1 ? 4 : RT <= 4 ? 3 : 1)   // R = 1: at most 64 registers, four CTAs per SM
+__global__ void __launch_bounds__(FWD_THREADS, RT == 1 ? 4 : RT <= 4 ? 3 : 2)   // R = 1: at most 64 registers, four CTAs per SM
 fk_fwd_column_kernel(const __grid_constant__ FwdParams p) {
     pdl_trigger();   // first kernel of a call (normal launch): lets the level-2 reduction be scheduled under this grid's last wave
     using V = Vec<TS, VEC>;

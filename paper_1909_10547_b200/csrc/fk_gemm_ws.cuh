@@ -508,3 +508,141 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
 }
 
 }  // namespace fk
+
+namespace fk {
+
+// ---------------------------------------------------------------------------------------------------
+// R >> 1 contraction for DIS tables (SURVEY 8(a) rows a4 + a5; the paper's flat operation of Table 3,
+// PAPER.md:83-100, is this with one pseudo-flavour):  Sigma[n][r] = sum_k FK[n][k] * f[r][slot(k)],
+// slot(k) = flav_c * nx + i.  The luminosity of a DIS table is a ROW of the replica-innermost copy fT, so the
+// B tile of a stage is 32 bulk copies of fT rows (any k-order: the producer decodes k); no luminosity is built and
+// the consumers run the plain DMMA loop.  Same producer / consumer split, mbarrier ring, split-K partials, periodic
+// flush and level-2 reduction as fk_gemm_fwd_ws_kernel; tiles of 128 datapoints (a partial last tile computes on
+// stale rows that are never stored).  Shared memory is zeroed once, so a k-step that reaches past the end of a K
+// range multiplies zeroed B rows with finite stale A columns.
+constexpr int WSD_STAGES = 3;
+__host__ __device__ inline size_t wsd_smem_bytes(int RP) {
+    return (size_t)WSD_STAGES * (WS_STAGE_DOUBLES + GEMM_KT * gemm_sb(RP)) * 8 + 2 * WSD_STAGES * 8;
+}
+
+template <int NFRAG>
+__global__ void __launch_bounds__(WS_THREADS, 1)
+fk_gemm_dis_ws_kernel(const __grid_constant__ WsFwdParams p) {
+    pdl_trigger();
+    extern __shared__ __align__(128) unsigned char fk_smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const TableDesc& d = p.desc;
+    const int RP = p.RP, SB = gemm_sb(RP);
+    constexpr int NFW = NFRAG / 2;
+    const int mtiles = (d.N + GEMM_BM - 1) / GEMM_BM;
+    const int m0 = ((int)blockIdx.x % mtiles) * GEMM_BM, ks = (int)blockIdx.x / mtiles;
+    const int kbeg = min(d.K, ks * p.kper), kend = min(d.K, kbeg + p.kper);
+    const int nst = (kend - kbeg + GEMM_KT - 1) / GEMM_KT;
+
+    double* As = reinterpret_cast<double*>(fk_smem);               // [STAGES][128][36]
+    double* Bs = As + WSD_STAGES * WS_STAGE_DOUBLES;                // [STAGES][32][SB]   fT rows of the stage's k
+    const uint32_t As_s = (uint32_t)__cvta_generic_to_shared(As), Bs_s = (uint32_t)__cvta_generic_to_shared(Bs);
+    const uint32_t bar0 = Bs_s + (uint32_t)(WSD_STAGES * GEMM_KT * SB * 8);
+    auto bar_full = [&](int s) { return bar0 + 8u * s; };
+    auto bar_empty = [&](int s) { return bar0 + 8u * (WSD_STAGES + s); };
+    for (int t = tid; t < WSD_STAGES * (WS_STAGE_DOUBLES + GEMM_KT * SB); t += WS_THREADS) As[t] = 0.0;
+    if (tid == 0) {
+        for (int s = 0; s < WSD_STAGES; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_empty(s), WS_CONSUMER_WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the zeros before any bulk copy lands
+    __syncthreads();
+    pdl_wait();   // fT of the transpose kernel launched just before
+
+    if (warp >= WS_CONSUMER_WARPS) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
+        if (warp != WS_CONSUMER_WARPS) return;
+        const double* __restrict__ fk = reinterpret_cast<const double*>(d.fk);
+        const uint64_t pol = l2_evict_first_policy();
+        const int rows_valid = min(GEMM_BM, d.N - m0);
+        for (int it = 0; it < nst; ++it) {
+            const int stage = it % WSD_STAGES, k0 = kbeg + it * GEMM_KT;
+            const int len = min(GEMM_KT, kend - k0), lenc = (len + 1) & ~1;   // whole 16-byte pieces: the pad element of a row is 0
+            mbar_wait(bar_empty(stage), ((it / WSD_STAGES) & 1) ^ 1);
+            // rows of fT for the k of this stage; rows past the end of the range are zeroed by this lane
+            const uint32_t brow = Bs_s + (uint32_t)((stage * GEMM_KT + lane) * SB * 8);
+            if (lane >= len)
+                for (int c = 0; c < RP; c += 2) asm volatile("st.shared.v2.f64 [%0], {%1, %1};" ::"r"(brow + (uint32_t)c * 8u), "d"(0.0) : "memory");
+            __syncwarp();
+            if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)((rows_valid * lenc + len * RP) * 8));
+            __syncwarp();
+            if (lane < len) {
+                int ia, ib;
+                decode_k(d, p.chan.a, p.chan.b, k0 + lane, ia, ib);
+                bulk_g2s(brow, p.fT + (long long)ia * RP, (uint32_t)(RP * 8), bar_full(stage));
+            }
+#pragma unroll
+            for (int q = 0; q < GEMM_BM / 32; ++q) {
+                const int row = lane + 32 * q;
+                if (row < rows_valid)
+                    bulk_g2s_stream(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * GEMM_SA) * 8),
+                                    fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(lenc * 8), bar_full(stage), pol);
+            }
+        }
+        return;
+    }
+
+    // consumers: warp tile 32 datapoints x (8 * NFW) replicas, plain DMMA loop
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
+    const int wm = warp & 3, wn = warp >> 2, cbcol = wn * NFW * 8;
+    double acc[4][NFW][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < NFW; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    double* out = p.gpart + (long long)ks * d.N * RP;
+    auto flush = [&](bool first) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int n = m0 + wm * 32 + i * 8 + (lane >> 2);
+            double2* q = reinterpret_cast<double2*>(out + (long long)n * RP + cbcol + 2 * (lane & 3));
+            double2 o[NFW];
+#pragma unroll
+            for (int j = 0; j < NFW; ++j) o[j] = (!first && n < d.N) ? q[j * 4] : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int j = 0; j < NFW; ++j) {
+                if (n < d.N) q[j * 4] = make_double2(acc[i][j][0] + o[j].x, acc[i][j][1] + o[j].y);
+                acc[i][j][0] = acc[i][j][1] = 0.0;
+            }
+        }
+    };
+    bool flushed = false;
+    for (int it = 0; it < nst; ++it) {
+        const int stage = it % WSD_STAGES;
+        const int nsteps = (min(GEMM_KT, kend - (kbeg + it * GEMM_KT)) + 3) >> 2;
+        mbar_wait(bar_full(stage), (it / WSD_STAGES) & 1);
+        const double* At = As + stage * WS_STAGE_DOUBLES + (wm * 32 + (lane >> 2)) * GEMM_SA + (lane & 3);
+        const double* Bt = Bs + (stage * GEMM_KT + (lane & 3)) * SB + cbcol + (lane >> 2);
+#pragma unroll
+        for (int s = 0; s < GEMM_KT / 4; ++s) {
+            if (s < nsteps) {
+                double a[4], b[NFW];
+#pragma unroll
+                for (int i4 = 0; i4 < 4; ++i4) a[i4] = At[i4 * 8 * GEMM_SA + s * 4];
+#pragma unroll
+                for (int j8 = 0; j8 < NFW; ++j8) b[j8] = Bt[s * 4 * SB + j8 * 8];
+#pragma unroll
+                for (int j8 = 0; j8 < NFW; ++j8)
+#pragma unroll
+                    for (int i4 = 0; i4 < 4; ++i4) dmma884(acc[i4][j8][0], acc[i4][j8][1], a[i4], b[j8]);
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty(stage));
+        if ((it + 1 + wn * (GEMM_FLUSH / 2)) % GEMM_FLUSH == 0) {
+            flush(!flushed);
+            flushed = true;
+        }
+    }
+    flush(!flushed);
+}
+
+}  // namespace fk
