@@ -346,6 +346,17 @@ def run_extras(K, torch, level, table2, case2, peak):
         out["cfg3_forward_R128_fp32_column_passes"] = {"ms": ms, "launches": t32v.last_launches()}
     finally:
         K.set_option(K.FK_OPT_TC32, 1)
+    # fp32 variant, VJP: FP64 tensor-core contraction over the fp32 table (widened in the fragment loads) + fp64 fold
+    g3s = g3.to(torch.float32); d3s = torch.empty_like(f3s)
+    ms = _bench_call(lambda: t32v.vjp(f3s, g3s, d3s), stream, steps=5, warmup=2)
+    out["cfg3_vjp_R128_fp32"] = {"ms": ms, "launches": t32v.last_launches(), "TFLOPs": flops / ms / 1e9,
+                                 "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS, "tolerance": 1e-5}
+    K.set_option(K.FK_OPT_GEMM_MIN_R, 1 << 20)
+    try:
+        ms = _bench_call(lambda: t32v.vjp(f3s, g3s, d3s), stream, steps=3, warmup=1)
+        out["cfg3_vjp_R128_fp32_column_passes"] = {"ms": ms, "launches": t32v.last_launches()}
+    finally:
+        K.set_option(K.FK_OPT_GEMM_MIN_R, 0)
     t32v.destroy()
     if level == "all":
         out.update(run_config4(K, torch, peak))

@@ -387,14 +387,15 @@ bool wsd_launch(const fk::WsFwdParams& w, int grid, cudaStream_t s) {
 }
 
 // the persistent warp-specialised VJP contraction needs 16-byte aligned, 16-byte multiple row pieces
-bool wsv_ok(const fk::TableDesc& d) { return d.vec_ok && d.K % 2 == 0 && opt(FK_OPT_WARP_SPEC); }
+// fp32-stored rows: vec_ok makes row_stride a multiple of 4, so the copies rounded up to 16 bytes stay inside the row
+bool wsv_ok(const fk::TableDesc& d) { return d.vec_ok && (d.store32 || d.K % 2 == 0) && opt(FK_OPT_WARP_SPEC); }
 
-template <bool GROUPED>
+template <bool GROUPED, typename TS = double>
 bool wsv_launch(const fk::WsVjpParams& w, cudaStream_t s) {
     const int grid = std::max(1, std::min(w.ntiles, sm_count()));
     switch (w.RP / 8) {
-#define FK_WSV_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED>, fk::WSV_SMEM_BYTES)) return false; \
-                                   FK_TIMED("fk_gemm_vjp_ws", s) fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break
+#define FK_WSV_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED, TS>, fk::WSV_SMEM_BYTES)) return false; \
+                                   FK_TIMED("fk_gemm_vjp_ws", s) fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED, TS><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break
         FK_WSV_CASE(2); FK_WSV_CASE(3); FK_WSV_CASE(4); FK_WSV_CASE(5); FK_WSV_CASE(6); FK_WSV_CASE(7); FK_WSV_CASE(8); FK_WSV_CASE(9);
         FK_WSV_CASE(10); FK_WSV_CASE(11); FK_WSV_CASE(12); FK_WSV_CASE(13); FK_WSV_CASE(14); FK_WSV_CASE(15);
         default: FK_WSV_CASE(16);
@@ -476,7 +477,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
 
 // the single-pass fold (fk_vjp_fold.cuh) serves packed hadronic tables with nx <= 64; others take the gather
 bool fold_ok(const fk::TableDesc& d) {
-    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.jp == d.nx && d.nx <= fk::FOLD_MAX_NX && opt(FK_OPT_FOLD);
+    return d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.nx <= fk::FOLD_MAX_NX && opt(FK_OPT_FOLD);
 }
 // x-row chunks per channel: the CTA count (channels x chunks) that fills whole waves best (1 CTA of 256 threads
 // per SM by registers), preferring fewer chunks (each chunk writes its own B partial)
@@ -499,13 +500,26 @@ size_t gemm_vjp_scratch_elems(const fk::TableDesc& d, int R) {
     return ((size_t)d.nfl * d.nx + (size_t)d.N + (size_t)d.K + (size_t)d.C * d.nx * (fk::FOLD_JQ + FOLD_MAX_CHUNKS)) * RPmax;
 }
 
-int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double* f, const double* g, double* df,
+// T = type of f, g and df; TS = storage type of the table (float: FK_F32 and FK_F32S64 tables, widened to double in the
+// A-fragment loads of the warp-specialised kernel).  The contraction, G and the fold are fp64 for every variant.
+// fp32-stored tables (FK_F32, FK_F32S64) at R >> 1: the same FP64 contraction over the table as it is stored (half the
+// bytes); G = FK^T g in fp64 costs the same DMMA work whatever the storage, and replaces ceil(R / 4) column passes.
+constexpr int VJP32_DEFAULT_MIN_R = 9;   // from 3 column passes of <= 4 replicas on
+bool vjp32_wanted(const fk::TableDesc& d, int R) {
+    if (!d.store32 || d.sp_blk || !wsv_ok(d)) return false;
+    if ((long long)d.nfl * d.nx >= (long long)fk::KDEC_NONE) return false;
+    return R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : VJP32_DEFAULT_MIN_R);
+}
+
+template <typename T, typename TS>
+int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const T* f, const T* g, T* df,
                  int R, double* scratch, cudaStream_t s, int* launches) {
     const int RPmax = fk::gemm_rp8(R);
     const int slots = d.nfl * d.nx;
     double* fT = scratch;
     double* gP = fT + (size_t)slots * RPmax;
     double* G = gP + (size_t)d.N * RPmax;
+    if (!std::is_same<TS, double>::value && !wsv_ok(d)) return fail(FK_ERR_UNSUPPORTED, "gemm vjp: fp32-stored table without 16-byte aligned rows");
     if (!wsv_ok(d) && !(ensure_dyn_smem(fk::fk_gemm_vjp_kernel<2, false>, fk::GEMMV_SMEM_BYTES) &&
                         ensure_dyn_smem(fk::fk_gemm_vjp_kernel<1, false>, fk::GEMMV_SMEM_BYTES)))
         return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %d bytes of shared memory", fk::GEMMV_SMEM_BYTES);
@@ -513,8 +527,8 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
         const int RP = fk::gemm_rp8(R - r0);
         const long long tf = (long long)slots * RP, tg = (long long)d.N * RP;
-        FK_TIMED("fk_transpose_f", s) fk::fk_transpose_f_kernel<double><<<(int)std::min<long long>(2048, (tf + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, RP);
-        FK_TIMED("fk_pad_g", s) fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(2048, (tg + 255) / 256), 256, 0, s>>>(g + d.out_off * R, gP, d.N, R, r0, RP);
+        FK_TIMED("fk_transpose_f", s) fk::fk_transpose_f_kernel<T, double><<<(int)std::min<long long>(2048, (tf + 255) / 256), 256, 0, s>>>(f, fT, slots, R, r0, RP);
+        FK_TIMED("fk_pad_g", s) fk::fk_pad_g_kernel<T><<<(int)std::min<long long>(2048, (tg + 255) / 256), 256, 0, s>>>(g + d.out_off * R, gP, d.N, R, r0, RP);
         fk::GemmVjpParams p;
         memset(&p, 0, sizeof p);
         p.desc = d;
@@ -532,7 +546,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             w.G = G;
             w.RP = RP;
             w.ntiles = grid;
-            if (!wsv_launch<false>(w, s)) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
+            if (!wsv_launch<false, TS>(w, s)) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
         } else if (d.vec_ok) FK_TIMED("fk_gemm_vjp", s) fk::fk_gemm_vjp_kernel<2, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         else FK_TIMED("fk_gemm_vjp", s) fk::fk_gemm_vjp_kernel<1, false><<<grid, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         if (fold_ok(d)) {
@@ -554,7 +568,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             if (!ensure_dyn_smem(fk::fk_vjp_fold_kernel<false>, MAX_DYN_SMEM) || q.nslots < 1) return fail(FK_ERR_CUDA, "gemm vjp: cannot reserve shared memory for the fold ring");
             FK_TIMED("fk_vjp_fold", s) fk::fk_vjp_fold_kernel<false><<<d.C * q.nchunk, fk::FOLD_THREADS,
                                             (size_t)q.nslots * d.nx * RP * 8 + 2 * fk::FOLD_MAX_SLOTS * 8, s>>>(q);
-            FK_TIMED("fk_vjp_fold_final", s) fk::fk_vjp_fold_final_kernel<double, false><<<slots, fk::GEMM_BN, 0, s>>>(q);
+            FK_TIMED("fk_vjp_fold_final", s) fk::fk_vjp_fold_final_kernel<T, false><<<slots, fk::GEMM_BN, 0, s>>>(q);
             ++nl;
         } else {
             fk::GatherRParams q;
@@ -567,7 +581,7 @@ int run_vjp_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const double
             q.R = R;
             q.r0 = r0;
             q.RP = RP;
-            FK_TIMED("fk_vjp_gather_r", s) fk::fk_vjp_gather_r_kernel<double, false><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
+            FK_TIMED("fk_vjp_gather_r", s) fk::fk_vjp_gather_r_kernel<T, false><<<dim3(slots, (RP + 127) / 128), 128, 0, s>>>(q);
         }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "gemm vjp launch failed: %s", cudaGetErrorString(e));
@@ -716,8 +730,10 @@ template <typename T, typename TS = T>
 int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan& pl, const T* f, const T* g, T* df,
                    int R, double* G, cudaStream_t s, int* launches) {
     int nl = 0;
-    if constexpr (std::is_same<T, double>::value) {
-        if (gemm_wanted<T>(d, R)) return run_vjp_gemm(d, ch, f, g, df, R, G, s, launches);
+    if constexpr (std::is_same<TS, double>::value) {
+        if (gemm_wanted<T>(d, R)) return run_vjp_gemm<T, TS>(d, ch, f, g, df, R, G, s, launches);
+    } else {
+        if (vjp32_wanted(d, R)) return run_vjp_gemm<T, TS>(d, ch, f, g, df, R, G, s, launches);
     }
     {
         fk::ColsumParams p;
@@ -876,7 +892,7 @@ size_t conv_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
 }
 template <typename T>
 size_t vjp_scratch_elems(const fk::TableDesc& d, int R) {
-    if (gemm_wanted<T>(d, R)) return gemm_vjp_scratch_elems(d, R);
+    if (gemm_wanted<T>(d, R) || vjp32_wanted(d, R)) return gemm_vjp_scratch_elems(d, R);
     return (G_elems_per_replica(d) + foldk_elems_per_replica(d)) * R;
 }
 

@@ -358,9 +358,13 @@ struct WsVjpParams {
 constexpr int WSV_STAGE_DOUBLES = 2 * GEMMV_NT * GEMMV_S;   // FK piece + g piece
 constexpr size_t WSV_SMEM_BYTES = (size_t)GEMMV_STAGES * WSV_STAGE_DOUBLES * 8 + 2 * GEMMV_STAGES * 8;
 
-template <int NFRAG, bool GROUPED>
+// TS = storage type of the table: float for the fp32-stored tables (FK_F32, FK_F32S64), whose pieces are copied as they are
+// (half the bytes) and widened to double when the A fragments are loaded; everything else is fp64 either way.
+template <int NFRAG, bool GROUPED, typename TS = double>
 __global__ void __launch_bounds__(WS_THREADS, 1)
 fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
+    constexpr int PS = GEMMV_S * 8 / (int)sizeof(TS);    // row pitch of the FK piece in elements (same byte pitch for both types)
+    constexpr int VEL = 16 / (int)sizeof(TS);            // elements per 16-byte piece of a bulk copy
     extern __shared__ __align__(128) unsigned char fk_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     double* Sm = reinterpret_cast<double*>(fk_smem);  // [STAGES][2][NT][S]
@@ -406,15 +410,16 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
             int kt;
             tile_of(t, d, gP, G, kt);
             const int k0 = kt * GEMMV_BK, klen = min(GEMMV_BK, d->K - k0);
-            const double* __restrict__ fk = reinterpret_cast<const double*>(d->fk) + k0;
+            const int klenc = (klen + VEL - 1) / VEL * VEL;   // whole 16-byte pieces: the pad elements of a packed row are 0
+            const TS* __restrict__ fk = reinterpret_cast<const TS*>(d->fk) + k0;
             for (int n0 = 0; n0 < d->N; n0 += GEMMV_NT, ++it) {
                 const int stage = it % GEMMV_STAGES, rows = min(GEMMV_NT, d->N - n0);
                 mbar_wait(bar_empty(stage), ((it / GEMMV_STAGES) & 1) ^ 1);
-                if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(rows * (klen + RP) * 8));
+                if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(rows * (klenc * (int)sizeof(TS) + RP * 8)));
                 __syncwarp();
                 if (lane < rows) {
                     const uint32_t dstA = Sm_s + (uint32_t)((stage * WSV_STAGE_DOUBLES + lane * GEMMV_S) * 8);
-                    bulk_g2s(dstA, fk + (long long)(n0 + lane) * d->row_stride, (uint32_t)(klen * 8), bar_full(stage));
+                    bulk_g2s(dstA, fk + (long long)(n0 + lane) * d->row_stride, (uint32_t)(klenc * (int)sizeof(TS)), bar_full(stage));
                     bulk_g2s(dstA + (uint32_t)(GEMMV_NT * GEMMV_S * 8), gP + (long long)(n0 + lane) * RP, (uint32_t)(RP * 8), bar_full(stage));
                 }
             }
@@ -464,14 +469,14 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
             const int stage = it % GEMMV_STAGES, rows = min(GEMMV_NT, d->N - n0);
             mbar_wait(bar_full(stage), (it / GEMMV_STAGES) & 1);
             // A fragment: row m = k (lane >> 2), col = datapoint (lane & 3)  ->  As[n][k]
-            const double* At = Sm + stage * WSV_STAGE_DOUBLES + (lane & 3) * GEMMV_S + wm * 32 + (lane >> 2);
+            const TS* At = reinterpret_cast<const TS*>(Sm + stage * WSV_STAGE_DOUBLES) + (lane & 3) * PS + wm * 32 + (lane >> 2);
             const double* Bt = Sm + stage * WSV_STAGE_DOUBLES + GEMMV_NT * GEMMV_S + (lane & 3) * GEMMV_S + cbcol + (lane >> 2);
             if (rows == GEMMV_NT) {
 #pragma unroll
                 for (int n4 = 0; n4 < GEMMV_NT / 4; ++n4) {
                     double a[4], b[NFW];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) a[i] = At[n4 * 4 * GEMMV_S + i * 8];
+                    for (int i = 0; i < 4; ++i) a[i] = (double)At[n4 * 4 * PS + i * 8];
 #pragma unroll
                     for (int j = 0; j < NFW; ++j) b[j] = Bt[n4 * 4 * GEMMV_S + j * 8];
 #pragma unroll
@@ -484,7 +489,7 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
                     const bool live = n4 * 4 + (lane & 3) < rows;
                     double a[4], b[NFW];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) a[i] = At[n4 * 4 * GEMMV_S + i * 8];
+                    for (int i = 0; i < 4; ++i) a[i] = (double)At[n4 * 4 * PS + i * 8];
 #pragma unroll
                     for (int j = 0; j < NFW; ++j) b[j] = live ? Bt[n4 * 4 * GEMMV_S + j * 8] : 0.0;
 #pragma unroll

@@ -104,7 +104,7 @@ fk_vjp_fold_kernel(const __grid_constant__ FoldParams p) {
         const int q = i - i0, s = q % S;
         mbar_wait(bar_empty(s), ((q / S) & 1) ^ 1);
         mbar_expect_tx(bar_full(s), row_bytes);
-        bulk_g2s(ring_s + (uint32_t)s * row_bytes, Gc + (long long)i * nx * RP, row_bytes, bar_full(s));
+        bulk_g2s(ring_s + (uint32_t)s * row_bytes, Gc + (long long)i * d.jp * RP, row_bytes, bar_full(s));   // x-rows are jp apart (fp32 tables pad them)
     };
     if (threadIdx.x == 0)
         for (int i = i0; i < min(i1, i0 + S - 1); ++i) issue(i);

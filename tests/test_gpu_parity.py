@@ -775,6 +775,57 @@ def test_fp32_storage_fp64_arithmetic(K, shape, R):
     assert rel_err(sig.cpu().numpy(), ref32, scale32) <= TOL64 and rel_err(df.cpu().numpy(), dref32, D32) <= TOL64
 
 
+# fp32-STORED tables at R >> 1: the VJP is the FP64 tensor-core contraction G = FK^T g over the table as stored (widened
+# in the fragment loads) + the fp64 fold; launches: transpose, pad, contraction, fold (+ final) per pass of <= 128
+# replicas.  FK_F32S64 (f, g, df fp64) meets the fp64 bar against the oracle of the DEMOTED table; FK_F32 (everything
+# fp32 outside the contraction) meets the fp32 bar.  x-grids that need the padded x-row pitch (13), partial tiles,
+# a pass boundary (150), DIS tables (gather instead of fold).
+@pytest.mark.parametrize("R", [9, 40, 128, 150])
+@pytest.mark.parametrize("shape", [(70, 13, 14, 17), (200, 30, 14, 9), (33, 50, 14, 3), (129, 8, 6, 5)])
+def test_fp32_stored_tables_dense_vjp(K, shape, R):
+    import torch
+    N, nx, nfl, C = shape
+    case = synth.hadronic_case(21, N, nx, C, R, nfl=nfl, sub=N * 100 + nx + R)
+    g = synth.rng_for(21, synth.T_G, R).standard_normal(size=(N, R))
+    fk32 = case.fk.astype(np.float32).astype(np.float64)
+    dref, D = O.hadronic_vjp(case.fk, case.pairs, case.f, g)
+    dref32, D32 = O.hadronic_vjp(fk32, case.pairs, case.f, g)
+    passes = (R + 127) // 128
+    f32 = torch.float32
+    for dtype, ft, tol_paper, tol_stored in ((K.FK_F32S64, torch.float64, TOL32S, TOL64), (K.FK_F32, f32, TOL32, TOL32)):
+        t = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl, dtype, K.FK_STORE_PACK, R_hint=R)
+        f_d, g_d = to_dev(case.f, ft), to_dev(g, ft)
+        df = t.vjp(f_d, g_d)
+        nl = t.last_launches()
+        assert df.dtype == ft and nl == 5 * passes, nl
+        e, es = rel_err(df.cpu().numpy(), dref, D), rel_err(df.cpu().numpy(), dref32, D32)
+        K.set_option(K.FK_OPT_GEMM_MIN_R, 1 << 20)
+        try:
+            dcol = t.vjp(f_d, g_d)
+            nl_col = t.last_launches()
+        finally:
+            K.set_option(K.FK_OPT_GEMM_MIN_R, 0)
+        ec = rel_err(dcol.cpu().numpy(), dref, D)
+        print(f"stored32 vjp {shape} R={R} dtype={dtype}: dense {e:.2e} / {es:.2e} vs demoted ({nl} launches)  column {ec:.2e} ({nl_col})")
+        assert e <= tol_paper and es <= tol_stored and ec <= tol_paper and nl_col >= nl and (R < 40 or nl_col > nl)
+        assert torch.equal(df, t.vjp(f_d, g_d))
+        t.destroy()
+
+
+def test_fp32_stored_dis_table_dense_vjp(K):
+    import torch
+    case = synth.config1(R=60, N=300)
+    g = synth.rng_for(22, synth.T_G, 60).standard_normal(size=(300, 60))
+    fk32 = case.fk.astype(np.float32).astype(np.float64)
+    dref32, D32 = O.dis_vjp(fk32, case.flav, case.f, g)
+    for dtype, ft, tol in ((K.FK_F32S64, torch.float64, TOL64), (K.FK_F32, torch.float32, TOL32)):
+        t = K.FkTable(K.FK_KIND_DIS, to_dev(case.fk), case.flav, case.nfl, dtype, K.FK_STORE_PACK, R_hint=60)
+        df = t.vjp(to_dev(case.f, ft), to_dev(g, ft))
+        assert t.last_launches() == 4, t.last_launches()
+        assert rel_err(df.cpu().numpy(), dref32, D32) <= tol
+        t.destroy()
+
+
 def test_fp32_storage_grouped_and_dis(K):
     import torch
     shapes = synth.small_ragged_shapes(T=5)
