@@ -358,6 +358,16 @@ def run_extras(K, torch, level, table2, case2, peak):
     finally:
         K.set_option(K.FK_OPT_GEMM_MIN_R, 0)
     t32v.destroy()
+    # fp32 STORAGE, fp64 everything else (FK_F32S64) at R = 128: the FP64 contractions over the table as stored
+    t32s = K.FkTable(K.FK_KIND_HADRONIC, torch.from_numpy(case2.fk).cuda(), case2.pairs, case2.nfl, K.FK_F32S64, K.FK_STORE_PACK, R_hint=R)
+    torch.cuda.empty_cache()
+    ms = _bench_call(lambda: t32s.conv(f3, s3), stream, steps=5, warmup=2)
+    out["cfg3_forward_R128_f32s64"] = {"ms": ms, "launches": t32s.last_launches(), "TFLOPs": flops / ms / 1e9,
+                                       "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS, "tolerance": 1e-7}
+    ms = _bench_call(lambda: t32s.vjp(f3, g3, d3), stream, steps=5, warmup=2)
+    out["cfg3_vjp_R128_f32s64"] = {"ms": ms, "launches": t32s.last_launches(), "TFLOPs": flops / ms / 1e9,
+                                   "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS, "tolerance": 1e-7}
+    t32s.destroy()
     if level == "all":
         out.update(run_config4(K, torch, peak))
     return out

@@ -358,16 +358,25 @@ bool ws_ok(const fk::TableDesc& d, int RP) {
 }
 
 // RP = 8 * NFRAG (fk::gemm_rp: a multiple of 16), NFRAG = 2, 4, ..., 16: one instantiation per fragment count
-template <bool GROUPED>
+template <bool GROUPED, typename TS = double>
 bool ws_launch(const fk::WsFwdParams& w, int grid, size_t smem, cudaStream_t s) {
     switch (w.RP / 8) {
-#define FK_WS_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, MAX_DYN_SMEM)) return false; \
-                                  FK_TIMED("fk_gemm_fwd_ws", s) launch_pdl(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED>, grid, fk::WS_THREADS, smem, s, w); break
+#define FK_WS_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED, TS>, MAX_DYN_SMEM)) return false; \
+                                  FK_TIMED("fk_gemm_fwd_ws", s) launch_pdl(fk::fk_gemm_fwd_ws_kernel<NFW, GROUPED, TS>, grid, fk::WS_THREADS, smem, s, w); break
         FK_WS_CASE(2); FK_WS_CASE(4); FK_WS_CASE(6); FK_WS_CASE(8); FK_WS_CASE(10); FK_WS_CASE(12); FK_WS_CASE(14);
         default: FK_WS_CASE(16);
 #undef FK_WS_CASE
     }
     return true;
+}
+
+// FK_F32S64 tables (fp32 storage, fp64 f / sigma and arithmetic) at R >> 1: the warp-specialised FP64 contraction over the
+// table as stored.  The DMMA work is that of the fp64 table; it replaces ceil(R / 4) column passes over half the bytes.
+constexpr int FWD32_DEFAULT_MIN_R = 9;
+bool fwd32_wanted(const fk::TableDesc& d, int R) {
+    if (!d.store32 || d.sp_blk || !ws_ok(d, fk::gemm_rp(R))) return false;
+    if ((long long)d.nfl * d.nx >= (long long)fk::KDEC_NONE) return false;
+    return R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : FWD32_DEFAULT_MIN_R);
 }
 
 // DIS tables (any k-order): the warp-specialised kernel whose B tile is 32 fT rows per stage (fk_gemm_dis_ws_kernel)
@@ -404,6 +413,8 @@ bool wsv_launch(const fk::WsVjpParams& w, cudaStream_t s) {
     return true;
 }
 
+// TS = storage type of the table; float (FK_F32S64) only with the warp-specialised kernel (fwd32_wanted)
+template <typename TS = double>
 int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint32_t* kdec, const double* f,
                   double* sigma, int R, double* scratch, cudaStream_t s, int* launches) {
     const GemmPlan gp = gemm_plan(d, R);
@@ -413,6 +424,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
     int nl = 0;
     const bool ws = ws_ok(d, gp.RPmax);
     const bool wsd = !ws && wsd_ok(d, gp.RPmax);
+    if (!std::is_same<TS, double>::value && !ws) return fail(FK_ERR_UNSUPPORTED, "gemm: fp32-stored table without the packed bulk-copy layout");
     if (!kdec && !ws && !wsd) {
         uint32_t* kd = reinterpret_cast<uint32_t*>(gpart + (size_t)gp.ksplit * d.N * gp.RPmax);
         FK_TIMED("fk_kdec", s) fk::fk_kdec_kernel<<<std::min(1024, (d.K + 255) / 256), 256, 0, s>>>(d, ch, kd);
@@ -449,7 +461,7 @@ int run_conv_gemm(const fk::TableDesc& d, const fk::ChannelList& ch, const uint3
             w.kper = gp.kper;
             w.ksub_rem = gp.ksub_rem;
             const int nfull = d.N / fk::GEMM_BM;
-            if (!ws_launch<false>(w, nfull * gp.ksplit + (d.N % fk::GEMM_BM ? gp.ksplit / gp.ksub_rem : 0), fk::ws_smem_bytes(d.nx, p.RP), s))
+            if (!ws_launch<false, TS>(w, nfull * gp.ksplit + (d.N % fk::GEMM_BM ? gp.ksplit / gp.ksub_rem : 0), fk::ws_smem_bytes(d.nx, p.RP), s))
                 return fail(FK_ERR_CUDA, "gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
         } else if (wsd) {
             fk::WsFwdParams w;
@@ -656,7 +668,10 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
                     const T* f, T* sigma, int R, double* part, cudaStream_t s, int* launches, int* cnt = nullptr) {
     int nl = 0;
     if constexpr (std::is_same<T, double>::value) {
-        if (gemm_wanted<T>(d, R)) return run_conv_gemm(d, ch, kdec, f, sigma, R, part, s, launches);
+        if constexpr (std::is_same<TS, float>::value) {
+            if (fwd32_wanted(d, R)) return run_conv_gemm<float>(d, ch, kdec, f, sigma, R, part, s, launches);
+        }
+        if (gemm_wanted<T>(d, R)) return run_conv_gemm<double>(d, ch, kdec, f, sigma, R, part, s, launches);
     }
     if constexpr (std::is_same<T, float>::value && std::is_same<TS, float>::value) {
         if (tc32_wanted(d, R)) return run_conv_tc32(d, ch, f, sigma, R, part, s, launches);
@@ -804,7 +819,7 @@ int run_vjp_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Plan
 // scratch: part [N][R][nchunks] | G [fsplit][R][K] | fold partials
 template <typename T>
 bool fused_ok(const fk::TableDesc& d, int R) {
-    return !gemm_wanted<T>(d, R) && !d.sp_blk && foldk_ok(d) && (d.N + d.fsplit - 1) / d.fsplit <= 64 && opt(FK_OPT_FUSED);
+    return !gemm_wanted<T>(d, R) && !vjp32_wanted(d, R) && !d.sp_blk && foldk_ok(d) && (d.N + d.fsplit - 1) / d.fsplit <= 64 && opt(FK_OPT_FUSED);
 }
 size_t fused_scratch_elems(const fk::TableDesc& d, int R) {
     return (part_elems_per_replica(d) + (size_t)d.fsplit * d.K + (1 + FOLDK_MAX_CHUNKS) * (size_t)d.C * d.nx) * R;
@@ -886,9 +901,11 @@ int run_conv_vjp_fused(const fk::TableDesc& d0, const fk::ChannelList& ch, const
 template <typename T>
 size_t conv_scratch_elems(const fk::TableDesc& d, int R, bool with_kdec) {
     if (gemm_wanted<T>(d, R)) return gemm_fwd_scratch_elems(d, R, with_kdec);
-    if (std::is_same<T, float>::value && d.tmap && d.kind == fk::KIND_HADRONIC)   // either fp32 path may be selected later
-        return std::max(part_elems_per_replica(d) * R, d.nx <= fk::TC_MAX_NX ? tc32_scratch_elems(d, R) : 0);
-    return part_elems_per_replica(d) * R;
+    size_t need = part_elems_per_replica(d) * R;
+    if (fwd32_wanted(d, R)) need = std::max(need, gemm_fwd_scratch_elems(d, R, false));   // FK_F32S64 handles size with T = float
+    if (std::is_same<T, float>::value && d.tmap && d.kind == fk::KIND_HADRONIC && d.nx <= fk::TC_MAX_NX)   // either fp32 path may be selected later
+        need = std::max(need, tc32_scratch_elems(d, R));
+    return need;
 }
 template <typename T>
 size_t vjp_scratch_elems(const fk::TableDesc& d, int R) {

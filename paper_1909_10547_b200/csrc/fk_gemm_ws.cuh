@@ -100,9 +100,12 @@ __host__ __device__ inline int ws_ksub_for_rows(int rows) { return rows <= 32 ? 
 // uneven split, as in the VJP kernel below, was measured slower for this kernel: two instruction streams of this
 // size per SM.)  The fragment count of a warp is a compile-time constant: the 4 x NF DMMAs of a k-step
 // carry no predicates, so ptxas is free to batch the fragment loads and the DMULs ahead of them.
-template <int NFRAG, bool GROUPED>
+// TS = storage type of the table: float for FK_F32S64 tables, whose tiles are copied as stored (half the bytes, the same
+// byte pitch per shared-memory row) and widened to double when the A fragments are loaded.
+template <int NFRAG, bool GROUPED, typename TS = double>
 __global__ void __launch_bounds__(WS_THREADS, 1)
 fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
+    constexpr int ESZ = (int)sizeof(TS);
     pdl_trigger();
     pdl_wait();   // fT of the transpose kernel launched just before (a programmatic dependent launch, fk_common.cuh)
     extern __shared__ __align__(128) unsigned char fk_smem[];
@@ -174,7 +177,7 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
         // 256 x 232 + 128 x 40 = 384 x 168 exactly (asking for more than the CTA owns would block forever)
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
         if (warp != WS_CONSUMER_WARPS) return;
-        const double* __restrict__ fk = reinterpret_cast<const double*>(d.fk);
+        const TS* __restrict__ fk = reinterpret_cast<const TS*>(d.fk);
         const uint64_t pol = l2_evict_first_policy();
         const int rows_valid = min(TM, d.N - m0);
         auto issue_fb = [&](int c, int ccn) {  // f[b_c][.][.] of channel c -> buffer ccn & 1
@@ -202,14 +205,14 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
                 const int len = min(KTv, se - k0);
                 const int stage = it % WS_STAGES;
                 mbar_wait(bar_empty(stage), ((it / WS_STAGES) & 1) ^ 1);
-                if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(rows_valid * len * 8));
+                if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(rows_valid * len * ESZ));
                 __syncwarp();
 #pragma unroll
                 for (int q = 0; q < GEMM_BM / 32; ++q) {
                     const int row = lane + 32 * q;
                     if (row < rows_valid)
                         bulk_g2s_stream(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * SAv) * 8),
-                                        fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(len * 8), bar_full(stage), pol);
+                                        fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(len * ESZ), bar_full(stage), pol);
                 }
             }
             if (!next_issued) issue_fb(c + 1, cc + 1);
@@ -280,13 +283,14 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
                 const int nsteps = max(0, ((min(KTc, se - k0) >> 2) - ksub + KS - 1) / KS);
                 const int stage = it % WS_STAGES;
                 mbar_wait(bar_full(stage), (it / WS_STAGES) & 1);
-                const double* At = As + stage * WS_STAGE_DOUBLES + (rb * 32 + (lane >> 2)) * SAc + ksub * 4 + (lane & 3);
+                constexpr int PSc = SAc * 8 / ESZ;   // row pitch in elements of TS
+                const TS* At = reinterpret_cast<const TS*>(As + stage * WS_STAGE_DOUBLES) + (rb * 32 + (lane >> 2)) * PSc + ksub * 4 + (lane & 3);
     #pragma unroll
                 for (int s = 0; s < GEMM_KT / 4; ++s) {
                     if (s < nsteps) {
                         double a[4], b[NFW];
     #pragma unroll
-                        for (int i4 = 0; i4 < 4; ++i4) a[i4] = At[i4 * 8 * SAc + s * kst];
+                        for (int i4 = 0; i4 < 4; ++i4) a[i4] = (double)At[i4 * 8 * PSc + s * kst];
     #pragma unroll
                         for (int j8 = 0; j8 < NFW; ++j8) b[j8] = Bt[j * SB + j8 * 8] * fa[j8];
     #pragma unroll

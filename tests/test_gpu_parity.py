@@ -809,6 +809,15 @@ def test_fp32_stored_tables_dense_vjp(K, shape, R):
         print(f"stored32 vjp {shape} R={R} dtype={dtype}: dense {e:.2e} / {es:.2e} vs demoted ({nl} launches)  column {ec:.2e} ({nl_col})")
         assert e <= tol_paper and es <= tol_stored and ec <= tol_paper and nl_col >= nl and (R < 40 or nl_col > nl)
         assert torch.equal(df, t.vjp(f_d, g_d))
+        if dtype == K.FK_F32S64:   # forward: the warp-specialised FP64 contraction over the fp32 tiles (3 launches per pass)
+            ref32, scale32 = O.hadronic(fk32, case.pairs, case.f)
+            sig = t.conv(f_d)
+            nl = t.last_launches()
+            es = rel_err(sig.cpu().numpy(), ref32, scale32)
+            print(f"stored32 fwd {shape} R={R}: dense {es:.2e} vs demoted ({nl} launches)")
+            assert nl == 3 * passes and es <= TOL64 and torch.equal(sig, t.conv(f_d))
+            s2, d2 = t.conv_vjp(f_d, g_d)
+            assert torch.equal(s2, sig) and torch.equal(d2, df)
         t.destroy()
 
 
