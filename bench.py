@@ -424,6 +424,12 @@ def run_config4(K, torch, peak):
     floor = 2 * flops / (_tf32_peak() * 1e9)   # one TF32 product + two bf16 correction products at twice the rate
     out[f"cfg4_grouped_forward_R{Rmax}_fp32"] = {"ms": ms, "TFLOPs_useful": flops / ms / 1e9, "tensor_floor_ms": floor, "frac_of_tensor_peak": floor / ms,
                                                  "launches": grp32.last_launches(), "tolerance": 1e-5}
+    # ... and its VJP: the grouped FP64 tensor-core contraction over the fp32 tables as stored + the fp64 fold
+    g32_cat = torch.cat([torch.from_numpy(np.ascontiguousarray(g[:, :Rmax])).reshape(-1) for g in gs]).cuda().float()
+    df32 = torch.empty_like(f32_cat)
+    ms = _bench_call(lambda: grp32.vjp(f32_cat, g32_cat, Rmax, df32), stream, steps=3, warmup=2)
+    out[f"cfg4_grouped_vjp_R{Rmax}_fp32"] = {"ms": ms, "TFLOPs": flops / ms / 1e9, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS,
+                                             "launches": grp32.last_launches(), "tolerance": 1e-5}
     grp32.destroy()
     for t in tabs32:
         t.destroy()

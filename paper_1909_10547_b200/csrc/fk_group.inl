@@ -27,6 +27,7 @@ struct fk_group {
     int nvitems = 0;
     long long gp_rows = 0, K_total = 0, cx_total = 0;
     bool ws_all = true;             // every table can take the warp-specialised forward contraction (fk_gemm_ws.cuh)
+    bool jp_all = true;             // no table pads its x-rows (jp == nx): the forward contraction walks k with nx
     int nx_max = 0;
     fk::ColSeg* d_witems = nullptr; // its items: {table, first datapoint, K range of the item, k sub-splits}
     int nwitems = 0;
@@ -76,20 +77,30 @@ bool group_gemm_wanted(const fk_group* g, int R) {
     return g->gemm_ok && g->dtype == FK_F64 && R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : g->ws_all ? 5 : 13);
 }
 
+// groups of fp32-STORED tables at R >> 1 (fk_api.cu, vjp32_wanted / fwd32_wanted): the FP64 contractions over the tables as stored
+bool group_vjp32_wanted(const fk_group* g, int R) {
+    return g->dtype != FK_F64 && g->wsv_all && opt(FK_OPT_WARP_SPEC) &&
+           R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : VJP32_DEFAULT_MIN_R);
+}
+bool group_fwd32_wanted(const fk_group* g, int R) {
+    return g->dtype == FK_F32S64 && g->ws_all && g->jp_all && opt(FK_OPT_WARP_SPEC) &&
+           fk::ws_smem_bytes(g->nx_max, fk::gemm_rp(R)) <= MAX_DYN_SMEM &&
+           R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : FWD32_DEFAULT_MIN_R);
+}
+
 size_t group_tc32_scratch_need(const fk_group* g, int R);
 bool group_tc32_wanted(const fk_group* g, int R);
 
 size_t group_scratch_need(const fk_group* g, int R) {
-    if (group_tc32_wanted(g, R))   // the fp32 VJP of the same R stays on the column kernels
-        return std::max<size_t>(group_tc32_scratch_need(g, R),
-                                std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1 + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R);
-    if (group_gemm_wanted(g, R)) {
-        const size_t RP = fk::gemm_rp(R);
-        const size_t fwd = (size_t)g->gp_rows,
-                     vjp = (size_t)g->rows_total + (size_t)g->K_total + (size_t)g->cx_total * (fk::FOLD_JQ + g->fold_nchunk);
-        return ((size_t)g->ai_total + std::max(fwd, vjp)) * RP;
-    }
-    return std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1 + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R;
+    const size_t RP = fk::gemm_rp(R);
+    const size_t gemm_fwd = ((size_t)g->ai_total + (size_t)g->gp_rows) * RP,
+                 gemm_vjp = ((size_t)g->ai_total + (size_t)g->rows_total + (size_t)g->K_total + (size_t)g->cx_total * (fk::FOLD_JQ + g->fold_nchunk)) * RP;
+    if (group_gemm_wanted(g, R)) return std::max(gemm_fwd, gemm_vjp);
+    size_t need = std::max<size_t>((size_t)g->part_total1, (size_t)g->G_total1 + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R;
+    if (group_tc32_wanted(g, R)) need = std::max(need, group_tc32_scratch_need(g, R));
+    if (group_fwd32_wanted(g, R)) need = std::max(need, gemm_fwd);
+    if (group_vjp32_wanted(g, R)) need = std::max(need, gemm_vjp);
+    return need;
 }
 
 // ---- fp32 variant at R >> 1 over a group: one tcgen05 launch per pass of <= 128 replicas ----
@@ -139,6 +150,8 @@ size_t group_fused_scratch_need(const fk_group* g, int R) {
     return ((size_t)g->part_total1 + (size_t)g->G_total1_fused + (1 + FOLDK_MAX_CHUNKS) * (size_t)g->cx_total) * R;
 }
 
+// TS = storage type of the tables (float: FK_F32S64 groups, warp-specialised kernel only)
+template <typename TS = double>
 int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, cudaStream_t s) {
     const int RPmax = fk::gemm_rp(R);
     double* fT = g->scratch;
@@ -168,9 +181,10 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
             w.RP = p.RP;
             w.descs = g->d_descs;
             w.items = g->d_witems;
-            if (!ws_launch<true>(w, g->nwitems, ws_smem, s))
+            if (!ws_launch<true, TS>(w, g->nwitems, ws_smem, s))
                 return fail(FK_ERR_CUDA, "grouped gemm: cannot reserve %zu bytes of shared memory", MAX_DYN_SMEM);
-        } else if (g->all_vec) FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<2, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
+        } else if (!std::is_same<TS, double>::value) return fail(FK_ERR_UNSUPPORTED, "grouped gemm: fp32-stored tables without the packed bulk-copy layout");
+        else if (g->all_vec) FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<2, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         else FK_TIMED("fk_gemm_fwd", s) fk::fk_gemm_fwd_kernel<1, true><<<g->ngitems, fk::GEMM_THREADS, fk::GEMM_SMEM_BYTES, s>>>(p);
         const long long outs = g->rows_total * p.RP;
         FK_TIMED("fk_gemm_reduce_grouped", s) fk::fk_gemm_reduce_grouped_kernel<double><<<(int)std::min<long long>(8192, (outs + 255) / 256), 256, 0, s>>>(
@@ -183,7 +197,10 @@ int group_conv_gemm(fk_group* g, const double* f_cat, double* sigma_cat, int R, 
     return FK_OK;
 }
 
-int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double* df_cat, int R, cudaStream_t s) {
+// T = type of f, g, df; TS = storage type of the tables (fk_api.cu, run_vjp_gemm)
+template <typename T = double, typename TS = double>
+int group_vjp_gemm(fk_group* g, const T* f_cat, const T* g_cat, T* df_cat, int R, cudaStream_t s) {
+    if (!std::is_same<TS, double>::value && !g->wsv_all) return fail(FK_ERR_UNSUPPORTED, "grouped gemm vjp: fp32-stored tables without 16-byte aligned rows");
     const int RPmax = fk::gemm_rp8(R);
     double* fT = g->scratch;
     double* gP = fT + (size_t)g->ai_total * RPmax;
@@ -194,10 +211,10 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
     for (int r0 = 0; r0 < R; r0 += fk::GEMM_BN) {
         const int RP = fk::gemm_rp8(R - r0);
         const long long tf = g->ai_total * RP, tg = g->rows_total * RP;
-        FK_TIMED("fk_transpose_f_grouped", s) fk::fk_transpose_f_grouped_kernel<double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
+        FK_TIMED("fk_transpose_f_grouped", s) fk::fk_transpose_f_grouped_kernel<T, double><<<(int)std::min<long long>(4096, (tf + 255) / 256), 256, 0, s>>>(
             f_cat, fT, g->d_ai_prefix, g->T, g->ai_total, R, r0, RP);
         // g_cat is [global row][R]: the single-table kernel pads all tables at once
-        FK_TIMED("fk_pad_g", s) fk::fk_pad_g_kernel<double><<<(int)std::min<long long>(4096, (tg + 255) / 256), 256, 0, s>>>(g_cat, gP, (int)g->rows_total, R, r0, RP);
+        FK_TIMED("fk_pad_g", s) fk::fk_pad_g_kernel<T><<<(int)std::min<long long>(4096, (tg + 255) / 256), 256, 0, s>>>(g_cat, gP, (int)g->rows_total, R, r0, RP);
         fk::GemmVjpParams p;
         memset(&p, 0, sizeof p);
         p.gP = gP;
@@ -216,7 +233,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             w.ntiles = g->nvitems;
             w.descs = g->d_descs;
             w.items = g->d_vitems;
-            if (!wsv_launch<true>(w, s)) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
+            if (!wsv_launch<true, TS>(w, s)) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve %zu bytes of shared memory", fk::WSV_SMEM_BYTES);
         } else if (g->all_vec) FK_TIMED("fk_gemm_vjp", s) fk::fk_gemm_vjp_kernel<2, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         else FK_TIMED("fk_gemm_vjp", s) fk::fk_gemm_vjp_kernel<1, true><<<g->nvitems, fk::GEMM_THREADS, fk::GEMMV_SMEM_BYTES, s>>>(p);
         if (g->fold_all) {
@@ -239,7 +256,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             if (!ensure_dyn_smem(fk::fk_vjp_fold_kernel<true>, MAX_DYN_SMEM) || q.nslots < 1) return fail(FK_ERR_CUDA, "grouped gemm vjp: cannot reserve shared memory for the fold ring");
             FK_TIMED("fk_vjp_fold", s) fk::fk_vjp_fold_kernel<true><<<g->nfoitems, fk::FOLD_THREADS,
                                            (size_t)q.nslots * g->nx_max * RP * 8 + 2 * fk::FOLD_MAX_SLOTS * 8, s>>>(q);
-            FK_TIMED("fk_vjp_fold_final", s) fk::fk_vjp_fold_final_kernel<double, true><<<(unsigned)g->ai_total, fk::GEMM_BN, 0, s>>>(q);
+            FK_TIMED("fk_vjp_fold_final", s) fk::fk_vjp_fold_final_kernel<T, true><<<(unsigned)g->ai_total, fk::GEMM_BN, 0, s>>>(q);
             ++nl;
         } else {
             fk::GatherRParams q;
@@ -253,7 +270,7 @@ int group_vjp_gemm(fk_group* g, const double* f_cat, const double* g_cat, double
             q.descs = g->d_descs;
             q.ai_prefix = g->d_ai_prefix;
             q.T = g->T;
-            FK_TIMED("fk_vjp_gather_r", s) fk::fk_vjp_gather_r_kernel<double, true><<<dim3((unsigned)g->ai_total, (RP + 127) / 128), 128, 0, s>>>(q);
+            FK_TIMED("fk_vjp_gather_r", s) fk::fk_vjp_gather_r_kernel<T, true><<<dim3((unsigned)g->ai_total, (RP + 127) / 128), 128, 0, s>>>(q);
         }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail(FK_ERR_CUDA, "grouped gemm vjp launch failed: %s", cudaGetErrorString(e));
@@ -268,7 +285,10 @@ int group_conv_t(fk_group* g, const void* f_cat, void* sigma_cat, int R, cudaStr
     int rc = group_scratch(g, group_scratch_need(g, R), s);
     if (rc) return rc;
     if constexpr (std::is_same<T, double>::value) {
-        if (group_gemm_wanted(g, R)) return group_conv_gemm(g, (const double*)f_cat, (double*)sigma_cat, R, s);
+        if constexpr (std::is_same<TS, float>::value) {
+            if (group_fwd32_wanted(g, R)) return group_conv_gemm<float>(g, (const double*)f_cat, (double*)sigma_cat, R, s);
+        }
+        if (group_gemm_wanted(g, R)) return group_conv_gemm<double>(g, (const double*)f_cat, (double*)sigma_cat, R, s);
     }
     if constexpr (std::is_same<T, float>::value && std::is_same<TS, float>::value) {
         if (group_tc32_wanted(g, R)) return group_conv_tc32(g, (const float*)f_cat, (float*)sigma_cat, R, s);
@@ -317,9 +337,11 @@ template <typename T, typename TS = T>
 int group_vjp_t(fk_group* g, const void* f_cat, const void* g_cat, void* df_cat, int R, cudaStream_t s) {
     int rc = group_scratch(g, group_scratch_need(g, R), s);
     if (rc) return rc;
-    if constexpr (std::is_same<T, double>::value) {
+    if constexpr (std::is_same<TS, double>::value) {
         if (group_gemm_wanted(g, R))
-            return group_vjp_gemm(g, (const double*)f_cat, (const double*)g_cat, (double*)df_cat, R, s);
+            return group_vjp_gemm<double, double>(g, (const double*)f_cat, (const double*)g_cat, (double*)df_cat, R, s);
+    } else {
+        if (group_vjp32_wanted(g, R)) return group_vjp_gemm<T, TS>(g, (const T*)f_cat, (const T*)g_cat, (T*)df_cat, R, s);
     }
     int nl = 0;
     fk::ColsumParams p;
@@ -531,6 +553,7 @@ int fk_group_create(fk_group** out, fk_table* const* tables, int T, int R_hint) 
                 for (int ks = 0; ks < d.gksplit / ksub_rem; ++ks) witems.push_back(fk::ColSeg{t, nfull * fk::GEMM_BM, ks, ksub_rem});
             }
             g->ws_all = g->ws_all && d.kind == fk::KIND_HADRONIC && d.layout == fk::LAYOUT_PACKED && d.vec_ok;
+            g->jp_all = g->jp_all && d.jp == d.nx;
             g->nx_max = std::max(g->nx_max, d.nx);
             d.gp_off = g->gp_rows;
             d.k_off = g->K_total;

@@ -930,3 +930,46 @@ def test_grouped_fp32_variant_tensor_cores(K, R):
     assert sig.dtype == np.float32 and worst <= TOL32
     assert torch.equal(sig_d, grp.conv(f_cat, R))
     grp.destroy()
+
+
+@pytest.mark.parametrize("R", [20, 130])
+def test_grouped_fp32_stored_tables_dense_paths(K, R):
+    """Groups of fp32-STORED tables at R >> 1: FK_F32S64 runs both FP64 contractions over the tables as stored (3 and 5
+    launches per pass of <= 128 replicas) and meets the fp64 bar against the oracle of the DEMOTED tables; FK_F32 takes
+    the same VJP (fp32 f, g, df) at the fp32 bar.  Ragged: 1..400 datapoints, x-grids 7..50 (padded x-rows for FK_F32)."""
+    import torch
+    shapes = synth.RaggedShapes(np.array([1, 37, 130, 400, 64, 257], dtype=np.int64), np.array([7, 23, 50, 30, 32, 44], dtype=np.int64),
+                                np.array([1, 29, 12, 9, 20, 5], dtype=np.int64))
+    params = synth.pdf_params(synth.rng_for(4, synth.T_PDF), R)
+    cases = [synth.config4_table(t, shapes, R, params) for t in range(shapes.T)]
+    gs = [synth.rng_for(23, synth.T_G, t).standard_normal(size=(c.N, R)) for t, c in enumerate(cases)]
+    passes = (R + 127) // 128
+    for dtype, ft, tol in ((K.FK_F32S64, torch.float64, TOL64), (K.FK_F32, torch.float32, TOL32)):
+        tabs = [K.FkTable(K.FK_KIND_HADRONIC, to_dev(c.fk), c.pairs, c.nfl, dtype, R_hint=R) for c in cases]
+        grp = K.FkGroup(tabs, R_hint=R)
+        fo, so = grp.offsets(R)
+        f_cat = torch.cat([to_dev(c.f, ft).reshape(-1) for c in cases])
+        g_cat = torch.cat([to_dev(g, ft).reshape(-1) for g in gs])
+        df_d = grp.vjp(f_cat, g_cat, R)
+        assert grp.last_launches() == 5 * passes, grp.last_launches()
+        df = df_d.cpu().numpy()
+        worst = 0.0
+        for t, c in enumerate(cases):
+            fk32 = c.fk.astype(np.float32).astype(np.float64)
+            dref, D = O.hadronic_vjp(fk32, c.pairs, c.f, gs[t])
+            worst = max(worst, rel_err(df[fo[t]:fo[t + 1]].reshape(c.f.shape), dref, D))
+        print(f"grouped stored32 vjp R={R} dtype={dtype}: {worst:.2e} vs demoted")
+        assert worst <= tol and torch.equal(df_d, grp.vjp(f_cat, g_cat, R))
+        if dtype == K.FK_F32S64:
+            sig_d = grp.conv(f_cat, R)
+            assert grp.last_launches() == 3 * passes, grp.last_launches()
+            sig = sig_d.cpu().numpy()
+            worst = 0.0
+            for t, c in enumerate(cases):
+                ref, scale = O.hadronic(c.fk.astype(np.float32).astype(np.float64), c.pairs, c.f)
+                worst = max(worst, rel_err(sig[so[t]:so[t + 1]].reshape(c.N, R), ref, scale))
+            print(f"grouped stored32 fwd R={R}: {worst:.2e} vs demoted")
+            assert worst <= TOL64 and torch.equal(sig_d, grp.conv(f_cat, R))
+            s2, d2 = grp.conv_vjp(f_cat, g_cat, R)
+            assert torch.equal(s2, sig_d) and torch.equal(d2, df_d)
+        grp.destroy()
