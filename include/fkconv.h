@@ -140,6 +140,28 @@ int fk_conv_hadronic_vjp(const double* fk, const int32_t* pairs, const double* f
 int fk_conv_dis_vjp(const double* fk, const int32_t* flav, const double* f, const double* g,
                     double* df, int N, int nx, int nfl, int nA, int R, void* stream);
 
+/* ------------------------------------------------------------------ allocation-free forward (fp64)
+ * fk_conv_hadronic (Eq. (1); same arguments, layout and results) for callers that cannot allocate device
+ * memory: code under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The level-1 partials
+ * (and, for R >= 5, the replica-innermost copy of f, the split-K partials and the k -> PDF-slot codes of the dense
+ * contraction) live in ONE file-scope `static __device__` array of FK_STATIC_SCRATCH_BYTES bytes inside the library:
+ * every GPU that loads the library holds that array until the process exits.  The call makes no cudaMalloc /
+ * cudaMallocAsync / cudaFree and calls no allocating library routine; on its first call per device it looks the array's
+ * device address up (cudaGetSymbolAddress, with that device current).
+ *   - sizes whose scratch exceeds the array: FK_ERR_UNSUPPORTED, nothing launched; fk_last_error_string() names the
+ *     bytes needed and the limit.  The need is 8 * N * ceil(nx*nx*C / 512) * R bytes for R <= 12 (k-blocks of 512;
+ *     nothing when nx*nx*C <= 512); from R = 13 on (the dense contraction) about 8 * R16 * (nfl*nx + N * ksplit) +
+ *     4 * nx*nx*C with R16 = min(128, R rounded up to 16) and ksplit ~ SMs / ceil(N / 128).  Config 2 (N = 512,
+ *     nx = 50, C = 100: 2 MB per replica, 21 MB at R >= 128) fits for every R, and so does every table of config 4.
+ *   - every call on a device SHARES the array, which keeps the previous call's contents: the call clears the part that
+ *     must start at zero (the tickets of the in-kernel level-2 reduction) on `stream` itself; everything else is written
+ *     before it is read.  Two calls that overlap on the GPU (different streams, or different host threads on one device)
+ *     RACE on the array and give wrong results silently: serialise them (one stream, or an event between them).
+ *   - asynchronous on `stream`, no synchronisation; same error conventions as fk_conv_hadronic. */
+#define FK_STATIC_SCRATCH_BYTES (32u << 20)
+int fk_conv_hadronic_static(const double* fk, const int32_t* pairs, const double* f, double* sigma,
+                            int N, int nx, int nfl, int C, int R, void* stream);
+
 /* fp32 variant (reading R18): float storage and float FMA with short chains, the
  * cross-thread stages in double, float results.  Same argument meaning as above. */
 int fk_conv_dis_f32(const float* fk, const int32_t* flav, const float* f, float* sigma,

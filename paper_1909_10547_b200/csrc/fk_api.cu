@@ -1240,6 +1240,66 @@ int fk_conv_hadronic(const double* fk, const int32_t* pairs, const double* f, do
     return stateless<double>("fk_conv_hadronic", FK_KIND_HADRONIC, false, fk, pairs, f, nullptr, sigma, N, nx, nfl, C, R,
                              stream);
 }
+// ---- allocation-free forward (include/fkconv.h, fk_conv_hadronic_static) -------------------------------------------
+// The scratch of the forward path in a file-scope device array.  In HOST code the name below is a host-side stand-in, not
+// a device address: only static_scratch_ptr() may touch it, and kernels get the address cudaGetSymbolAddress returned.
+static __device__ __align__(256) unsigned char fk_static_scratch[FK_STATIC_SCRATCH_BYTES];
+namespace {
+constexpr size_t STATIC_TICKET_BYTES = 4096;   // [1024] tickets of the in-kernel level-2 reduction, ahead of the doubles
+constexpr int STATIC_MAX_DEVICES = 64;
+
+// device address of the array on the CURRENT device: looked up once per device, with that device current
+int static_scratch_ptr(const char* who, unsigned char** out) {
+    static std::mutex mu;
+    static unsigned char* ptr[STATIC_MAX_DEVICES] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "%s: no CUDA device (%s)", who, cudaGetErrorString(e));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(FK_ERR_UNSUPPORTED, "%s: device ordinal %d beyond %d", who, dev, STATIC_MAX_DEVICES - 1);
+    std::lock_guard<std::mutex> lk(mu);
+    if (!ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, fk_static_scratch);
+        if (e != cudaSuccess || !p) return fail(FK_ERR_CUDA, "%s: cudaGetSymbolAddress failed on device %d: %s", who, dev, cudaGetErrorString(e));
+        ptr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = ptr[dev];
+    return FK_OK;
+}
+}  // namespace
+
+int fk_conv_hadronic_static(const double* fkp, const int32_t* pairs, const double* f, double* sigma, int N, int nx, int nfl,
+                            int C, int R, void* stream) {
+    const char* who = "fk_conv_hadronic_static";
+    g_err.clear();
+    if (!fkp || !pairs || !f || !sigma) return fail(FK_ERR_INVALID_ARG, "%s: null pointer", who);
+    int rc = check_dims(who, FK_KIND_HADRONIC, N, nx, nfl, C, R);
+    if (rc) return rc;
+    if ((uintptr_t)fkp % sizeof(double) || (uintptr_t)f % sizeof(double) || (uintptr_t)sigma % sizeof(double))
+        return fail(FK_ERR_INVALID_ARG, "%s: misaligned pointer", who);
+    fk::ChannelList ch;
+    rc = fill_channels(who, FK_KIND_HADRONIC, pairs, nfl, C, ch);
+    if (rc) return rc;
+    fk::TableDesc d = make_desc(FK_KIND_HADRONIC, fk::LAYOUT_LOGICAL, fkp, N, nx, nfl, C, 0, FK_F64);
+    Plan pl;
+    make_plan(d, FK_F64, pl);
+    const size_t need = conv_scratch_elems<double>(d, R, true) * sizeof(double) + STATIC_TICKET_BYTES;
+    if (need > (size_t)FK_STATIC_SCRATCH_BYTES)
+        return fail(FK_ERR_UNSUPPORTED, "%s: N=%d nx=%d C=%d R=%d needs %zu bytes of scratch, the static array holds %zu "
+                                        "(FK_STATIC_SCRATCH_BYTES): use fk_conv_hadronic or a resident table", who, N, nx, C, R, need,
+                    (size_t)FK_STATIC_SCRATCH_BYTES);
+    unsigned char* base = nullptr;
+    rc = static_scratch_ptr(who, &base);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    int* cnt = nullptr;
+    if ((size_t)pl.fsplit * sizeof(int) <= STATIC_TICKET_BYTES) {   // the tickets must start at zero whatever the last call left
+        cnt = reinterpret_cast<int*>(base);
+        FK_CUDA(cudaMemsetAsync(cnt, 0, (size_t)pl.fsplit * sizeof(int), s));
+    }
+    return run_conv_single<double>(d, ch, pl, nullptr, f, sigma, R, reinterpret_cast<double*>(base + STATIC_TICKET_BYTES), s, nullptr, cnt);
+}
+
 int fk_conv_hadronic_vjp(const double* fk, const int32_t* pairs, const double* f, const double* g, double* df, int N,
                          int nx, int nfl, int C, int R, void* stream) {
     return stateless<double>("fk_conv_hadronic_vjp", FK_KIND_HADRONIC, true, fk, pairs, f, g, df, N, nx, nfl, C, R,

@@ -34,7 +34,9 @@ SYMBOLS = (
     "fk_table_conv_host", "fk_table_vjp_host", "fk_table_last_launches",
     "fk_group_create", "fk_group_destroy", "fk_group_offsets", "fk_conv_grouped",
     "fk_conv_grouped_vjp", "fk_conv_grouped_conv_vjp", "fk_group_last_launches", "fk_conv_hadronic2", "fk_conv_hadronic2_vjp", "fk_probe_launch",
+    "fk_conv_hadronic_static",
 )
+FK_STATIC_SCRATCH_BYTES = 32 << 20   # include/fkconv.h
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(
@@ -47,7 +49,7 @@ for _name in SYMBOLS:
 lib.fk_last_error_string.restype = ctypes.c_char_p
 
 _vp, _ci = ctypes.c_void_p, ctypes.c_int
-for _name in ("fk_conv_dis", "fk_conv_hadronic", "fk_conv_dis_f32", "fk_conv_hadronic_f32"):
+for _name in ("fk_conv_dis", "fk_conv_hadronic", "fk_conv_dis_f32", "fk_conv_hadronic_f32", "fk_conv_hadronic_static"):
     getattr(lib, _name).argtypes = [_vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
 for _name in ("fk_conv_hadronic_vjp", "fk_conv_dis_vjp", "fk_conv_hadronic_vjp_f32"):
     getattr(lib, _name).argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _ci, _ci, _vp]
@@ -181,6 +183,21 @@ def fk_conv_hadronic(fk, pairs, f, sigma=None, stream=None):
     fn = lib.fk_conv_hadronic if fk.dtype == torch.float64 else lib.fk_conv_hadronic_f32
     _check(fn(_dev(fk), _hostptr(pairs), _dev(f, fk.dtype), _dev(sigma, fk.dtype), N, nx, nfl, C, R,
               _stream(stream)), "fk_conv_hadronic")
+    return sigma
+
+
+def fk_conv_hadronic_static(fk, pairs, f, sigma, stream=None):
+    """fk_conv_hadronic (fp64) without any device allocation inside the library: the scratch is a static device array of
+    FK_STATIC_SCRATCH_BYTES (include/fkconv.h).  The caller passes the output; larger problems raise FkError
+    (FK_ERR_UNSUPPORTED); calls that overlap on the GPU race on the shared array."""
+    N, nx, _, C = fk.shape
+    R, nfl, _ = f.shape
+    pairs = _idx(pairs)
+    if fk.dtype != torch.float64:
+        raise TypeError("fk_conv_hadronic_static: fp64 only")
+    _shape(pairs, (C, 2), "pairs"); _shape(f, (R, nfl, nx), "f", fk.device); _shape(sigma, (N, R), "sigma", fk.device)
+    _check(lib.fk_conv_hadronic_static(_dev(fk), _hostptr(pairs), _dev(f, fk.dtype), _dev(sigma, fk.dtype), N, nx, nfl, C, R,
+                                       _stream(stream)), "fk_conv_hadronic_static")
     return sigma
 
 
