@@ -84,6 +84,12 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int wha
         }
     }
 }
+#ifdef FK_TC32_TIMING
+// debug build only: cycles spent in a wait, added to `acc`
+#define FK_TWAIT(ACC, ...) do { const long long t0_ = clock64(); mbar_wait(__VA_ARGS__); ACC += clock64() - t0_; } while (0)
+#else
+#define FK_TWAIT(ACC, ...) mbar_wait(__VA_ARGS__)
+#endif
 // one lane of a converged warp (the same one every time): control flow stays warp-uniform around the single-thread
 // instructions (TMA, tcgen05.mma, tcgen05.commit), so their operands live in uniform registers
 __device__ __forceinline__ bool elect_one() {
@@ -169,6 +175,13 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform: role branches do not diverge
     pdl_trigger();   // the level-2 reduction may be scheduled under this grid's tail (it waits for the partials itself)
+#ifdef FK_TC32_TIMING
+    long long tw[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const long long t_start = clock64();
+#else
+    long long tw[1];   // unused: FK_TWAIT ignores it
+    (void)tw;
+#endif
 
     const TableDesc* dp = &p.desc;
     const uint8_t* __restrict__ cha = p.chan.a;
@@ -250,7 +263,7 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
             int c = c_first, i = i_first;
             for (int t = 0; t < ntl; ++t) {
                 const int slot = t % TC_RAW_STAGES;
-                mbar_wait(bar(BAR_FK_FREE + slot), ((t / TC_RAW_STAGES) & 1) ^ 1, 1);
+                FK_TWAIT(tw[6], bar(BAR_FK_FREE + slot), ((t / TC_RAW_STAGES) & 1) ^ 1, 1);
                 const int k0 = c * cstride + i * jp;   // 16-byte aligned: jp and cstride are multiples of 4
                 const uint32_t dst = sm_raw + (uint32_t)slot * TC_STAGE_BYTES;
                 if (leader) {
@@ -273,8 +286,8 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
                     mbar_wait(bar(BAR_A_FULL + abuf), (cc >> 1) & 1, 2);
                     newch = false;
                 }
-                mbar_wait(bar(BAR_ACC_FREE + buf), ((t >> 1) & 1) ^ 1, 3);
-                mbar_wait(bar(BAR_FK_FULL + slot), (t / TC_RAW_STAGES) & 1, 4);
+                FK_TWAIT(tw[0], bar(BAR_ACC_FREE + buf), ((t >> 1) & 1) ^ 1, 3);
+                FK_TWAIT(tw[1], bar(BAR_FK_FULL + slot), (t / TC_RAW_STAGES) & 1, 4);
                 tc_fence_after();
                 const uint32_t d_acc = tmem_base + (uint32_t)buf * 128u;
                 const uint32_t a_hi = tmem_base + TC_TMEM_A + (uint32_t)abuf * 128u;
@@ -292,7 +305,7 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
                     }
                 }
                 __syncwarp();
-                mbar_wait(bar(BAR_LO_FULL + ls), (t >> 1) & 1, 5);
+                FK_TWAIT(tw[2], bar(BAR_LO_FULL + ls), (t >> 1) & 1, 5);
                 tc_fence_after();
                 if (leader) {
 #pragma unroll
@@ -354,40 +367,59 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
         bool build_next = c < c_last;   // the next channel's operand is built under the first row of this one
         for (int t = 0; t < ntl; ++t) {
             const int slot = t % TC_RAW_STAGES, ls = t & 1;
-            mbar_wait(bar(BAR_LO_FREE + ls), ((t >> 1) & 1) ^ 1, 7);
-            mbar_wait(bar(BAR_FK_FULL + slot), (t / TC_RAW_STAGES) & 1, 8);
+            FK_TWAIT(tw[3], bar(BAR_LO_FREE + ls), ((t >> 1) & 1) ^ 1, 7);
+            FK_TWAIT(tw[4], bar(BAR_FK_FULL + slot), (t / TC_RAW_STAGES) & 1, 8);
+#ifdef FK_TC32_TIMING
+            const long long ts0 = clock64();
+#endif
             if (st < NT) {
                 // bf16(FK) and bf16(FK_lo), FK_lo = x - tf32(x): logical fp32 chunk q of row st sits at 16-byte position
                 // (q & 7) ^ (st & 7) of the row's 128 bytes in box q >> 3; two fp32 chunks make bf16 chunk m = q / 2 at
                 // position m ^ (st & 7) of the row's 128 bytes in its tile
                 const uint32_t src = sm_raw + (uint32_t)slot * TC_STAGE_BYTES + (uint32_t)st * 128u;
                 const uint32_t dst = sm_lo + (uint32_t)ls * TC_STAGE_BYTES + (uint32_t)st * 128u;
+                // all loads of the row first (volatile asm keeps program order: loads interleaved with the stores of the
+                // previous chunk would make every chunk wait out a full shared-memory round trip under the tensor core's own
+                // traffic), then the arithmetic and the stores
+                float x[8][8];
 #pragma unroll
                 for (int m = 0; m < 8; ++m) {
-                    if (m >= nk8) break;
-                    float x[8];
+                    if (m < nk8) {
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const int q = 2 * m + h;
-                        const uint32_t o = (uint32_t)(q >> 3) * TC_BOX_BYTES + (uint32_t)(((q & 7) ^ (st & 7)) << 4);
-                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x[4 * h]), "=f"(x[4 * h + 1]), "=f"(x[4 * h + 2]), "=f"(x[4 * h + 3]) : "r"(src + o));
+                        for (int h = 0; h < 2; ++h) {
+                            const int q = 2 * m + h;
+                            const uint32_t o = (uint32_t)(q >> 3) * TC_BOX_BYTES + (uint32_t)(((q & 7) ^ (st & 7)) << 4);
+                            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x[m][4 * h]), "=f"(x[m][4 * h + 1]), "=f"(x[m][4 * h + 2]), "=f"(x[m][4 * h + 3]) : "r"(src + o));
+                        }
                     }
-                    uint32_t fb4[4], lo4[4];
+                }
 #pragma unroll
-                    for (int e = 0; e < 8; e += 2) {
-                        const float l0 = x[e] - __uint_as_float(__float_as_uint(x[e]) & TF32_MASK);
-                        const float l1 = x[e + 1] - __uint_as_float(__float_as_uint(x[e + 1]) & TF32_MASK);
-                        fb4[e >> 1] = pack_bf16(x[e], x[e + 1]);
-                        lo4[e >> 1] = pack_bf16(l0, l1);
+                for (int m = 0; m < 8; ++m) {
+                    if (m < nk8) {
+                        uint32_t fb4[4], lo4[4];
+#pragma unroll
+                        for (int e = 0; e < 8; e += 2) {
+                            const float l0 = x[m][e] - __uint_as_float(__float_as_uint(x[m][e]) & TF32_MASK);
+                            const float l1 = x[m][e + 1] - __uint_as_float(__float_as_uint(x[m][e + 1]) & TF32_MASK);
+                            fb4[e >> 1] = pack_bf16(x[m][e], x[m][e + 1]);
+                            lo4[e >> 1] = pack_bf16(l0, l1);
+                        }
+                        const uint32_t od = (uint32_t)((m ^ (st & 7)) << 4);
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + od), "r"(fb4[0]), "r"(fb4[1]), "r"(fb4[2]), "r"(fb4[3]) : "memory");
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + TC_BOX_BYTES + od), "r"(lo4[0]), "r"(lo4[1]), "r"(lo4[2]), "r"(lo4[3]) : "memory");
                     }
-                    const uint32_t od = (uint32_t)((m ^ (st & 7)) << 4);
-                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + od), "r"(fb4[0]), "r"(fb4[1]), "r"(fb4[2]), "r"(fb4[3]) : "memory");
-                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst + TC_BOX_BYTES + od), "r"(lo4[0]), "r"(lo4[1]), "r"(lo4[2]), "r"(lo4[3]) : "memory");
                 }
             }
+#ifdef FK_TC32_TIMING
+            const long long ts1 = clock64();
+#endif
             fence_async_smem();   // generic-proxy stores -> visible to the tensor core (async proxy)
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(BAR_LO_FULL + ls));
+#ifdef FK_TC32_TIMING
+            tw[7] += ts1 - ts0;
+            tw[5] += clock64() - ts1;
+#endif
             if (build_next) {
                 build_a(cc + 1, c + 1);
                 build_next = false;
@@ -420,7 +452,7 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
             const bool chan_end = ++i == nx;
             if (chan_end) { i = 0; ++c; }
             if (t + 1 < ntl) fa_next = load_fa(c, i);
-            mbar_wait(bar(BAR_ACC_FULL + buf), (t >> 1) & 1, 9);
+            FK_TWAIT(tw[5], bar(BAR_ACC_FULL + buf), (t >> 1) & 1, 9);
             tc_fence_after();
             if (live) {
                 const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 128 + h * 64);
@@ -450,6 +482,11 @@ fk_tc32_fwd_kernel(const __grid_constant__ Tc32Params p) {
                 if (h * 64 + e < rows) out[(long long)e * RP] = tot[e];
         }
     }
+#ifdef FK_TC32_TIMING
+    if (blockIdx.x == 5 && lane == 0 && (warp == 0 || warp == 1 || warp == 4 || warp == 8))
+        printf("tc32 timing block %d warp %d: total %lld | issuer waits ACC_FREE %lld FK_FULL %lld LO_FULL %lld | splitter waits LO_FREE %lld FK_FULL %lld | "
+               "epilogue waits ACC_FULL (splitter: fence+arrive) %lld | tma waits FK_FREE %lld | splitter work %lld\n", (int)blockIdx.x, warp, clock64() - t_start, tw[0], tw[1], tw[2], tw[3], tw[4], tw[5], tw[6], tw[7]);
+#endif
     tc_fence_before();
     __syncthreads();
     if (warp == 2) {
