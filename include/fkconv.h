@@ -221,6 +221,11 @@ int fk_table_fit_step(fk_table* t, const double* f, const double* data, const do
 int fk_table_conv_host(fk_table* t, const void* f_host, void* sigma_host, int R, void* stream);
 int fk_table_vjp_host(fk_table* t, const void* f_host, const void* g_host, void* df_host, int R,
                       void* stream);
+/* fk_table_conv_vjp with HOST buffers: f and g go up in ONE copy, sigma and df come back in ONE copy, one wait; the call
+ * returns after both results have landed in host memory.  Same dispatch as fk_table_conv_vjp (forward + VJP from one read
+ * of FK when that path applies; FK_OPT_FUSED = 0 makes it the two passes). */
+int fk_table_conv_vjp_host(fk_table* t, const void* f_host, const void* g_host, void* sigma_host, void* df_host, int R,
+                           void* stream);
 /* Kernel launches issued by the last conv / vjp call on this table (for bench.py's gpu_launches). */
 int fk_table_last_launches(const fk_table* t);
 

@@ -1601,6 +1601,34 @@ int fk_table_vjp_host(fk_table* t, const void* f_host, const void* g_host, void*
     return FK_OK;
 }
 
+int fk_table_conv_vjp_host(fk_table* t, const void* f_host, const void* g_host, void* sigma_host, void* df_host, int R, void* stream) {
+    g_err.clear();
+    if (!t || !f_host || !g_host || !sigma_host || !df_host) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp_host: null pointer");
+    if (R <= 0) return fail(FK_ERR_INVALID_ARG, "fk_table_conv_vjp_host: R=%d", R);
+    const size_t es = io_size(t->dtype);
+    const size_t fb = (size_t)R * t->desc.nfl * t->desc.nx * es, gb = (size_t)t->desc.N * R * es;
+    const size_t fb_al = (fb + 255) / 256 * 256, gb_al = (gb + 255) / 256 * 256;
+    cudaStream_t s = (cudaStream_t)stream;
+    CallGuard cg(t->sync, s);
+    if (int rc0 = cg.begin("fk_table_conv_vjp_host")) return rc0;
+    int rc = ensure_stage(t, 2 * fb_al + 2 * gb_al);   // f | g | sigma | df, one copy in, one copy out
+    if (rc) return rc;
+    char* h = (char*)t->h_stage; char* d = (char*)t->d_stage;
+    memcpy(h, f_host, fb);
+    memcpy(h + fb_al, g_host, gb);
+    FK_CUDA(cudaMemcpyAsync(d, h, fb_al + gb, cudaMemcpyHostToDevice, s));
+    char* d_sig = d + fb_al + gb_al; char* d_df = d_sig + gb_al;
+    if (t->dtype == FK_F32S64) rc = table_conv_vjp_t<double, float>(t, d, d + fb_al, d_sig, d_df, R, s);
+    else rc = t->dtype == FK_F64 ? table_conv_vjp_t<double>(t, d, d + fb_al, d_sig, d_df, R, s)
+                                 : table_conv_vjp_t<float>(t, d, d + fb_al, d_sig, d_df, R, s);
+    if (rc) return rc;
+    FK_CUDA(cudaMemcpyAsync(h + fb_al + gb_al, d_sig, gb_al + fb, cudaMemcpyDeviceToHost, s));
+    FK_CUDA(cudaStreamSynchronize(s));
+    memcpy(sigma_host, h + fb_al + gb_al, gb);
+    memcpy(df_host, h + fb_al + 2 * gb_al, fb);
+    return FK_OK;
+}
+
 int fk_table_last_launches(const fk_table* t) { return t ? t->last_launches : 0; }
 
 }  // extern "C"

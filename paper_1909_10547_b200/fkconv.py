@@ -34,7 +34,7 @@ SYMBOLS = (
     "fk_table_conv_host", "fk_table_vjp_host", "fk_table_last_launches",
     "fk_group_create", "fk_group_destroy", "fk_group_offsets", "fk_conv_grouped",
     "fk_conv_grouped_vjp", "fk_conv_grouped_conv_vjp", "fk_group_last_launches", "fk_conv_hadronic2", "fk_conv_hadronic2_vjp", "fk_probe_launch",
-    "fk_conv_hadronic_static",
+    "fk_conv_hadronic_static", "fk_table_conv_vjp_host",
 )
 FK_STATIC_SCRATCH_BYTES = 32 << 20   # include/fkconv.h
 
@@ -71,6 +71,7 @@ lib.fk_table_fit_step.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _ci, _
 lib.fk_table_conv_vjp.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _vp]
 lib.fk_table_conv_host.argtypes = [_vp, _vp, _vp, _ci, _vp]
 lib.fk_table_vjp_host.argtypes = [_vp, _vp, _vp, _vp, _ci, _vp]
+lib.fk_table_conv_vjp_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _vp]
 lib.fk_table_last_launches.argtypes = [_vp]
 lib.fk_group_create.argtypes = [ctypes.POINTER(_vp), ctypes.POINTER(_vp), _ci, _ci]
 lib.fk_group_destroy.argtypes = [_vp]
@@ -384,6 +385,15 @@ class FkTable:
         dp = _host(df_host, self.ndtype, (R, self.nfl, self.nx), "df_host")
         _check(lib.fk_table_vjp_host(self.handle, fp, gp, dp, R, _stream(stream)), "fk_table_vjp_host")
         return df_host
+
+    def conv_vjp_host(self, f_host: np.ndarray, g_host: np.ndarray, sigma_host: np.ndarray, df_host: np.ndarray, stream=None):
+        R = f_host.shape[0]
+        fp = _host(f_host, self.ndtype, (R, self.nfl, self.nx), "f_host")
+        gp = _host(g_host, self.ndtype, (self.N, R), "g_host")
+        sp = _host(sigma_host, self.ndtype, (self.N, R), "sigma_host")
+        dp = _host(df_host, self.ndtype, (R, self.nfl, self.nx), "df_host")
+        _check(lib.fk_table_conv_vjp_host(self.handle, fp, gp, sp, dp, R, _stream(stream)), "fk_table_conv_vjp_host")
+        return sigma_host, df_host
 
     def last_launches(self) -> int:
         return lib.fk_table_last_launches(self.handle)

@@ -588,6 +588,21 @@ def test_host_buffer_calls(K):
     assert rel_err(sig, ref, scale) <= TOL64
     assert rel_err(df, dref, D) <= TOL64
     assert tp.last_launches() >= 2
+    # forward + VJP in one host call (one copy in, one copy out, one wait): the one-read path, then the two passes
+    for fused in (1, 0):
+        K.set_option(K.FK_OPT_FUSED, fused)
+        try:
+            sig2 = np.full((case.N, case.R), np.nan); df2 = np.full_like(case.f, np.nan)
+            tp.conv_vjp_host(case.f, case.g, sig2, df2)
+        finally:
+            K.set_option(K.FK_OPT_FUSED, 1)
+        assert rel_err(sig2, ref, scale) <= TOL64 and rel_err(df2, dref, D) <= TOL64
+        if not fused:
+            assert np.array_equal(sig2, sig) and np.array_equal(df2, df)    # the same kernels as the two calls
+    t32 = K.FkTable(K.FK_KIND_HADRONIC, to_dev(case.fk), case.pairs, case.nfl, K.FK_F32, K.FK_STORE_PACK)
+    sig3 = np.empty((case.N, case.R), dtype=np.float32); df3 = np.empty(case.f.shape, dtype=np.float32)
+    t32.conv_vjp_host(case.f.astype(np.float32), case.g.astype(np.float32), sig3, df3)
+    assert rel_err(sig3, ref, scale) <= TOL32 and rel_err(df3, dref, D) <= TOL32
 
 
 # ------------------------------------------------------------------ grouped ragged launch
