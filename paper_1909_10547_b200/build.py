@@ -19,7 +19,7 @@ OBJDIR = os.path.join(HERE, "build")   # object files (git-ignored)
 # translation units -> the files each one includes (a unit is recompiled when one of them changes)
 UNITS = {
     "fk_api.cu": ["fk_api.cu", "fk_group.inl", "fk_common.cuh", "fk_fwd.cuh", "fk_vjp.cuh", "fk_gemm.cuh", "fk_gemm_ws.cuh",
-                  "fk_vjp_fold.cuh", "fk_chi2.cuh", "fk_pack.cuh", "fk_tc32.h", "fk_sparse.cuh"],
+                  "fk_vjp_fold.cuh", "fk_chi2.cuh", "fk_pack.cuh", "fk_tc32.h", "fk_sparse.cuh", "fk_dis_direct.cuh"],
     "fk_tc32.cu": ["fk_tc32.cu", "fk_tc32.h", "fk_common.cuh"],
 }
 

@@ -28,6 +28,7 @@
 #include "fk_chi2.cuh"
 #include "fk_tc32.h"
 #include "fk_sparse.cuh"
+#include "fk_dis_direct.cuh"
 
 namespace {
 
@@ -70,6 +71,7 @@ int g_opt[FK_OPT_COUNT_] = {
     /* FK_OPT_TC32_MIN_R  */ 0,
     /* FK_OPT_PDL         */ 1,
     /* FK_OPT_FUSE_L2     */ 1,
+    /* FK_OPT_DIS_DIRECT  */ 1,
 };
 inline int opt(int o) { return g_opt[o]; }
 
@@ -395,6 +397,37 @@ bool wsd_launch(const fk::WsFwdParams& w, int grid, cudaStream_t s) {
     return true;
 }
 
+// Small packed DIS tables at R >> 1 (config 1 at R = 100): one launch, no transposed copy of f, no split-K partials
+// (fk_dis_direct.cuh).  "Small" = the table stays in L2 while every column group of CTAs reads it, and the grid is a few
+// waves at most; larger tables keep the split-K kernel, which reads FK once with 128-datapoint tiles.
+bool dis_direct_wanted(const fk::TableDesc& d, int R, const void* f) {
+    if (d.kind != fk::KIND_DIS || d.layout != fk::LAYOUT_PACKED || !d.vec_ok || d.store32 || d.sp_blk || !opt(FK_OPT_DIS_DIRECT)) return false;
+    if (d.nx % 2 || d.K > fk::DD_MAX_K || d.K != d.C * d.nx || (reinterpret_cast<uintptr_t>(f) & 15)) return false;   // 16-byte pieces of f
+    if (R > 512 || (long long)d.N * d.K * 8 > (64LL << 20) || fk::dd_smem_bytes(d.K, 2) > MAX_DYN_SMEM) return false;
+    return R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : 13);
+}
+
+int run_conv_dis_direct(const fk::TableDesc& d, const fk::ChannelList& ch, const double* f, double* sigma, int R, cudaStream_t s, int* launches) {
+    fk::DisDirectParams p;
+    memset(&p, 0, sizeof p);
+    p.desc = d;
+    p.chan = ch;
+    p.f = f;
+    p.sigma = sigma;
+    p.R = R;
+    p.nfrag = (R + 7) / 8;
+    p.ncs = (p.nfrag + fk::DD_NFC - 1) / fk::DD_NFC;
+    p.stages = fk::dd_smem_bytes(d.K, fk::DD_STAGES) <= MAX_DYN_SMEM ? fk::DD_STAGES : 2;
+    const size_t smem = fk::dd_smem_bytes(d.K, p.stages);
+    if (!ensure_dyn_smem(fk::fk_dis_direct_kernel, smem)) return fail(FK_ERR_CUDA, "dis direct: cannot reserve %zu bytes of shared memory", smem);
+    const dim3 grid((d.N + fk::DD_TM - 1) / fk::DD_TM, p.ncs);
+    FK_TIMED("fk_dis_direct", s) fk::fk_dis_direct_kernel<<<grid, fk::DD_THREADS, smem, s>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(FK_ERR_CUDA, "dis direct launch failed: %s", cudaGetErrorString(e));
+    if (launches) *launches = 1;
+    return FK_OK;
+}
+
 // the persistent warp-specialised VJP contraction needs 16-byte aligned, 16-byte multiple row pieces
 // fp32-stored rows: vec_ok makes row_stride a multiple of 4, so the copies rounded up to 16 bytes stay inside the row
 bool wsv_ok(const fk::TableDesc& d) { return d.vec_ok && (d.store32 || d.K % 2 == 0) && opt(FK_OPT_WARP_SPEC); }
@@ -670,6 +703,9 @@ int run_conv_single(const fk::TableDesc& d, const fk::ChannelList& ch, const Pla
     if constexpr (std::is_same<T, double>::value) {
         if constexpr (std::is_same<TS, float>::value) {
             if (fwd32_wanted(d, R)) return run_conv_gemm<float>(d, ch, kdec, f, sigma, R, part, s, launches);
+        }
+        if constexpr (std::is_same<TS, double>::value) {
+            if (dis_direct_wanted(d, R, f)) return run_conv_dis_direct(d, ch, f, sigma, R, s, launches);
         }
         if (gemm_wanted<T>(d, R)) return run_conv_gemm<double>(d, ch, kdec, f, sigma, R, part, s, launches);
     }

@@ -33,6 +33,7 @@ constexpr int WS_THREADS = (WS_CONSUMER_WARPS + 4) * 32;  // + the producer's wa
                                                           // reallocation (setmaxnreg) works on whole warpgroups.
                                                           // (9 warps would not help: registers are per scheduler,
                                                           // 3 warps on one of them still cap a thread at 170.)
+constexpr int WS_PRODUCER_WARPS = 4;
 constexpr int WS_STAGES = 3;
 constexpr int WS_STAGE_DOUBLES = GEMM_BM * GEMM_SA;        // FK tile [128][36]
 constexpr int WS_NBAR = 2 * WS_STAGES + 4;                 // full[S], empty[S], fb_full[2], fb_empty[2]
@@ -160,7 +161,7 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
     auto bar_fbempty = [&](int b) { return bar0 + 8u * (2 * WS_STAGES + 2 + b); };
     if (tid == 0) {
         for (int s = 0; s < WS_STAGES; ++s) {
-            mbar_init(bar_full(s), 1);
+            mbar_init(bar_full(s), WS_PRODUCER_WARPS);   // one arrive.expect_tx per producer warp
             mbar_init(bar_empty(s), WS_CONSUMER_WARPS);
         }
         for (int b = 0; b < 2; ++b) {
@@ -176,11 +177,17 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
         // 384 threads cap the kernel at 168 registers; the producer warpgroup hands its share to the consumers:
         // 256 x 232 + 128 x 40 = 384 x 168 exactly (asking for more than the CTA owns would block forever)
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
-        if (warp != WS_CONSUMER_WARPS) return;
+        // All four warps of the producer warpgroup issue copies: a bulk copy costs its warp ~57 cycles of issue whatever
+        // its size (measured, profiles/r02_bulk_copy_issue.md), so ONE warp needs 7 300 cycles for the 128 row pieces
+        // of a stage that the consumers finish in 8 192 -- any hiccup of the producer then stalls the tensor pipe.  Warp pw
+        // takes the datapoints 32*pw .. 32*pw + 31 of every stage and arrives on the stage's barrier with its own byte count.
+        const int pw = warp - WS_CONSUMER_WARPS;
         const TS* __restrict__ fk = reinterpret_cast<const TS*>(d.fk);
         const uint64_t pol = l2_evict_first_policy();
         const int rows_valid = min(TM, d.N - m0);
-        auto issue_fb = [&](int c, int ccn) {  // f[b_c][.][.] of channel c -> buffer ccn & 1
+        const int my_rows = max(0, min(32, rows_valid - 32 * pw));
+        auto issue_fb = [&](int c, int ccn) {  // f[b_c][.][.] of channel c -> buffer ccn & 1 (producer warp 0)
+            if (pw != 0) return;
             const int buf = ccn & 1;
             mbar_wait(bar_fbempty(buf), ((ccn >> 1) & 1) ^ 1);
             if (lane == 0) mbar_expect_tx(bar_fbfull(buf), (uint32_t)(nx * RP * 8));
@@ -205,15 +212,12 @@ fk_gemm_fwd_ws_kernel(const __grid_constant__ WsFwdParams p) {
                 const int len = min(KTv, se - k0);
                 const int stage = it % WS_STAGES;
                 mbar_wait(bar_empty(stage), ((it / WS_STAGES) & 1) ^ 1);
-                if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(rows_valid * len * ESZ));
+                if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)(my_rows * len * ESZ));
                 __syncwarp();
-#pragma unroll
-                for (int q = 0; q < GEMM_BM / 32; ++q) {
-                    const int row = lane + 32 * q;
-                    if (row < rows_valid)
-                        bulk_g2s_stream(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * SAv) * 8),
-                                        fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(len * ESZ), bar_full(stage), pol);
-                }
+                const int row = lane + 32 * pw;
+                if (lane < my_rows)
+                    bulk_g2s_stream(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * SAv) * 8),
+                                    fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(len * ESZ), bar_full(stage), pol);
             }
             if (!next_issued) issue_fb(c + 1, cc + 1);
         }
@@ -557,7 +561,7 @@ fk_gemm_dis_ws_kernel(const __grid_constant__ WsFwdParams p) {
     for (int t = tid; t < WSD_STAGES * (WS_STAGE_DOUBLES + GEMM_KT * SB); t += WS_THREADS) As[t] = 0.0;
     if (tid == 0) {
         for (int s = 0; s < WSD_STAGES; ++s) {
-            mbar_init(bar_full(s), 1);
+            mbar_init(bar_full(s), WS_PRODUCER_WARPS);   // one arrive.expect_tx per producer warp
             mbar_init(bar_empty(s), WS_CONSUMER_WARPS);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -568,33 +572,33 @@ fk_gemm_dis_ws_kernel(const __grid_constant__ WsFwdParams p) {
 
     if (warp >= WS_CONSUMER_WARPS) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;" ::: "memory");
-        if (warp != WS_CONSUMER_WARPS) return;
+        // four producer warps (a bulk copy costs its warp ~57 cycles of issue, fk_gemm_fwd_ws_kernel): warp pw copies the
+        // datapoints 32*pw .. 32*pw + 31 of the FK tile, warp 0 also the 32 fT rows of the stage
+        const int pw = warp - WS_CONSUMER_WARPS;
         const double* __restrict__ fk = reinterpret_cast<const double*>(d.fk);
         const uint64_t pol = l2_evict_first_policy();
         const int rows_valid = min(GEMM_BM, d.N - m0);
+        const int my_rows = max(0, min(32, rows_valid - 32 * pw));
         for (int it = 0; it < nst; ++it) {
             const int stage = it % WSD_STAGES, k0 = kbeg + it * GEMM_KT;
             const int len = min(GEMM_KT, kend - k0), lenc = (len + 1) & ~1;   // whole 16-byte pieces: the pad element of a row is 0
             mbar_wait(bar_empty(stage), ((it / WSD_STAGES) & 1) ^ 1);
             // rows of fT for the k of this stage; rows past the end of the range are zeroed by this lane
             const uint32_t brow = Bs_s + (uint32_t)((stage * GEMM_KT + lane) * SB * 8);
-            if (lane >= len)
+            if (pw == 0 && lane >= len)
                 for (int c = 0; c < RP; c += 2) asm volatile("st.shared.v2.f64 [%0], {%1, %1};" ::"r"(brow + (uint32_t)c * 8u), "d"(0.0) : "memory");
             __syncwarp();
-            if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)((rows_valid * lenc + len * RP) * 8));
+            if (lane == 0) mbar_expect_tx(bar_full(stage), (uint32_t)((my_rows * lenc + (pw == 0 ? len * RP : 0)) * 8));
             __syncwarp();
-            if (lane < len) {
+            if (pw == 0 && lane < len) {
                 int ia, ib;
                 decode_k(d, p.chan.a, p.chan.b, k0 + lane, ia, ib);
                 bulk_g2s(brow, p.fT + (long long)ia * RP, (uint32_t)(RP * 8), bar_full(stage));
             }
-#pragma unroll
-            for (int q = 0; q < GEMM_BM / 32; ++q) {
-                const int row = lane + 32 * q;
-                if (row < rows_valid)
-                    bulk_g2s_stream(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * GEMM_SA) * 8),
-                                    fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(lenc * 8), bar_full(stage), pol);
-            }
+            const int row = lane + 32 * pw;
+            if (lane < my_rows)
+                bulk_g2s_stream(As_s + (uint32_t)((stage * WS_STAGE_DOUBLES + row * GEMM_SA) * 8),
+                                fk + (long long)(m0 + row) * d.row_stride + k0, (uint32_t)(lenc * 8), bar_full(stage), pol);
         }
         return;
     }

@@ -23,7 +23,7 @@ FK_KIND_DIS, FK_KIND_HADRONIC = 0, 1
 FK_F64, FK_F32, FK_F32S64 = 0, 1, 2
 FK_STORE_BORROW, FK_STORE_PACK, FK_STORE_SPARSE = 0, 1, 2
 (FK_OPT_GEMM_MIN_R, FK_OPT_WARP_SPEC, FK_OPT_FOLD, FK_OPT_FOLDK, FK_OPT_FUSED, FK_OPT_FEWROWS, FK_OPT_TC32,
- FK_OPT_TC32_MIN_R, FK_OPT_PDL, FK_OPT_FUSE_L2) = range(10)
+ FK_OPT_TC32_MIN_R, FK_OPT_PDL, FK_OPT_FUSE_L2, FK_OPT_DIS_DIRECT) = range(11)
 
 # every symbol include/fkconv.h declares
 SYMBOLS = (

@@ -307,6 +307,35 @@ def test_config1_dis(K, R):
         assert rel_err(d.cpu().numpy(), dref, D) <= TOL64, name
 
 
+@pytest.mark.parametrize("shape", [(1, 2, 1, 13), (63, 20, 3, 16), (64, 50, 9, 17), (65, 36, 14, 40), (200, 50, 9, 100),
+                                   (130, 50, 10, 130), (2048, 50, 9, 100), (77, 8, 5, 300)])
+def test_dis_direct_small_tables(K, shape):
+    """Small packed DIS tables at R >= 13 (config 1 at R = 100) run in ONE launch (fk_dis_direct_kernel: both operands by bulk
+    copies, no transposed f, no split-K partials).  Against the oracle, and against the general R >> 1 path that
+    FK_OPT_DIS_DIRECT = 0 selects: ragged datapoint tiles, replica counts that are not multiples of 8 or 32, partial last
+    k-stage, K up to 500."""
+    N, nx, nA, R = shape
+    rng = synth.rng_for(11, synth.T_FK, N * 1000 + R)
+    fk = rng.standard_normal(size=(N, nx, nA))
+    flav = synth.draw_flavours(synth.rng_for(11, synth.T_PAIRS, nA), nA)
+    f = synth.pdf_grid(synth.pdf_params(synth.rng_for(11, synth.T_PDF, R), R), nx)
+    ref, scale = O.dis(fk, flav, f)
+    t = K.FkTable(K.FK_KIND_DIS, to_dev(fk), flav, synth.NFL, K.FK_F64, K.FK_STORE_PACK, R_hint=R)
+    f_d = to_dev(f)
+    s1 = t.conv(f_d).cpu().numpy()
+    assert t.last_launches() == 1
+    assert rel_err(s1, ref, scale) <= TOL64
+    assert np.array_equal(s1, t.conv(f_d).cpu().numpy())   # repeatable bit for bit
+    K.set_option(K.FK_OPT_DIS_DIRECT, 0)
+    try:
+        s0 = t.conv(f_d).cpu().numpy()
+        assert t.last_launches() > 1
+    finally:
+        K.set_option(K.FK_OPT_DIS_DIRECT, 1)
+    assert rel_err(s0, ref, scale) <= TOL64
+    t.destroy()
+
+
 @pytest.mark.parametrize("shape_R", [((8, 3571, 1), 1), ((8, 3571, 1), 7), ((100, 1021, 1), 3), ((33, 2048, 1), 40),
                                      ((8, 5_000_000, 1), 1), ((5, 4_900_001, 1), 3)])  # the last two: fk_fwd_fewrows_kernel
 def test_flat_matrix_view_of_table3(K, shape_R):
