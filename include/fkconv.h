@@ -98,7 +98,7 @@ enum {
     FK_OPT_TC32_MIN_R = 7, /* [0] smallest R that takes it; 0 = built-in */
     FK_OPT_PDL = 8,        /* [1] later kernels of a call use programmatic dependent launch (0: plain stream order) */
     FK_OPT_FUSE_L2 = 9,    /* [1] resident tables / groups whose forward grid is at most one wave: the forward kernel's last CTA per datapoint range runs the level-2 reduction (0: always a separate launch) */
-    FK_OPT_DIS_DIRECT = 10, /* [1] small packed DIS tables (K <= 512, <= 64 MB) at R >= 13: one launch without a transposed copy of f or split-K partials (0: the general R >> 1 path) */
+    FK_OPT_DIS_DIRECT = 10, /* [80] smallest R (>= 13) at which small packed DIS tables (K <= 512, nx even, <= 64 MB) run in one launch without a transposed copy of f or split-K partials; 0: never (the general R >> 1 path) */
     FK_OPT_COUNT_ = 11
 };
 int fk_set_option(int option, int value);

@@ -71,7 +71,7 @@ int g_opt[FK_OPT_COUNT_] = {
     /* FK_OPT_TC32_MIN_R  */ 0,
     /* FK_OPT_PDL         */ 1,
     /* FK_OPT_FUSE_L2     */ 1,
-    /* FK_OPT_DIS_DIRECT  */ 1,
+    /* FK_OPT_DIS_DIRECT  */ 80,  // smallest R that takes fk_dis_direct_kernel (0 = never): its time barely depends on R, the split-K chain's does
 };
 inline int opt(int o) { return g_opt[o]; }
 
@@ -403,8 +403,8 @@ bool wsd_launch(const fk::WsFwdParams& w, int grid, cudaStream_t s) {
 bool dis_direct_wanted(const fk::TableDesc& d, int R, const void* f) {
     if (d.kind != fk::KIND_DIS || d.layout != fk::LAYOUT_PACKED || !d.vec_ok || d.store32 || d.sp_blk || !opt(FK_OPT_DIS_DIRECT)) return false;
     if (d.nx % 2 || d.K > fk::DD_MAX_K || d.K != d.C * d.nx || (reinterpret_cast<uintptr_t>(f) & 15)) return false;   // 16-byte pieces of f
-    if (R > 512 || (long long)d.N * d.K * 8 > (64LL << 20) || fk::dd_smem_bytes(d.K, 2) > MAX_DYN_SMEM) return false;
-    return R >= (opt(FK_OPT_GEMM_MIN_R) > 0 ? opt(FK_OPT_GEMM_MIN_R) : 13);
+    if (R > 512 || (long long)d.N * d.K * 8 > (64LL << 20) || fk::dd_smem_bytes(d.K, 2) > MAX_DYN_SMEM - fk::DD_STATIC_SMEM) return false;
+    return R >= std::max(13, opt(FK_OPT_DIS_DIRECT));   // never below the dense threshold of DIS tables
 }
 
 int run_conv_dis_direct(const fk::TableDesc& d, const fk::ChannelList& ch, const double* f, double* sigma, int R, cudaStream_t s, int* launches) {
@@ -417,7 +417,7 @@ int run_conv_dis_direct(const fk::TableDesc& d, const fk::ChannelList& ch, const
     p.R = R;
     p.nfrag = (R + 7) / 8;
     p.ncs = (p.nfrag + fk::DD_NFC - 1) / fk::DD_NFC;
-    p.stages = fk::dd_smem_bytes(d.K, fk::DD_STAGES) <= MAX_DYN_SMEM ? fk::DD_STAGES : 2;
+    p.stages = fk::dd_smem_bytes(d.K, fk::DD_STAGES) <= MAX_DYN_SMEM - fk::DD_STATIC_SMEM ? fk::DD_STAGES : 2;
     const size_t smem = fk::dd_smem_bytes(d.K, p.stages);
     if (!ensure_dyn_smem(fk::fk_dis_direct_kernel, smem)) return fail(FK_ERR_CUDA, "dis direct: cannot reserve %zu bytes of shared memory", smem);
     const dim3 grid((d.N + fk::DD_TM - 1) / fk::DD_TM, p.ncs);

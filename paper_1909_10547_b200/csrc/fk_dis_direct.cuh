@@ -8,8 +8,8 @@
 // Here both operands are K-MAJOR as they lie in memory -- a row of the table, and for one replica the run
 // f[r][flav_c][0..nx) of every active flavour c -- so both go to shared memory by bulk async copies with no
 // transposed copy of f:  the B tile Bs[col][k] of a CTA's replica columns is copied once (nA pieces of nx doubles per
-// replica), the A tile streams through a ring of [64 datapoints][64 k] stages (four producer warps: the issue cost of a
-// bulk copy is per warp, profiles/r02_bulk_copy_issue.md).  Four consumer warps hold 16 datapoints
+// replica; runs of consecutive flavours merged), the A tile streams through a ring of [64 datapoints][64 k] stages (four
+// producer warps: the issue cost of a bulk copy is per warp, profiles/r02_bulk_copy_issue.md).  Four consumer warps hold 16 datapoints
 // x (<= 4) 8-replica fragments each and run the plain DMMA loop over the whole K, so there is no split-K and the
 // accumulators go straight to sigma.  K <= 512 keeps every accumulation chain within the 512 FMAs the tolerance
 // derivation assumes.  Bitwise repeatable: fixed k order per output.
@@ -30,9 +30,12 @@ constexpr int DD_CONSUMERS = 4;
 constexpr int DD_PRODUCERS = 4;            // a bulk copy costs its warp ~57 cycles of issue: ~800 pieces per CTA need four warps
 constexpr int DD_THREADS = (DD_CONSUMERS + DD_PRODUCERS) * 32;
 constexpr int DD_MAX_K = 512;
+constexpr size_t DD_STATIC_SMEM = 2048;    // the kernel's static shared memory (run list), rounded up
 
-// row pitch of the B tile: >= K rounded up to 4, pitch mod 16 == 4
-__host__ __device__ inline int dd_pitch_b(int K) { return (((K + 3) / 4 * 4) + 11) / 16 * 16 + 4; }
+// row pitch of the B tile: K rounded up to 16 (the consumers walk whole groups of 4 MMA k-steps; the tail is zero) + 4,
+// so that pitch mod 16 == 4 (conflict-free fragment loads)
+constexpr int DD_KG = 16;                 // k per group of 4 MMA k-steps
+__host__ __device__ inline int dd_pitch_b(int K) { return (K + DD_KG - 1) / DD_KG * DD_KG + 4; }
 __host__ __device__ inline size_t dd_smem_bytes(int K, int stages) {
     return (size_t)(stages * DD_TM * DD_SA + DD_NFC * 8 * dd_pitch_b(K)) * 8 + (2 * DD_STAGES + 1) * 8;
 }
@@ -65,9 +68,24 @@ fk_dis_direct_kernel(const __grid_constant__ DisDirectParams p) {
     auto bar_full = [&](int s) { return bar0 + 8u * s; };
     auto bar_empty = [&](int s) { return bar0 + 8u * (DD_STAGES + s); };
     const uint32_t bar_b = bar0 + 8u * (2 * DD_STAGES);
-    // zeros once: the k past the end of K in the last MMA k-step of a row, and whatever a short last stage leaves
+    // zeros once: the k past the end of K in the last group of k-steps, the B rows past this CTA's columns, the rows of a
+    // partial datapoint tile, whatever a short last stage leaves
     for (int t = tid; t < NS * DD_TM * DD_SA + DD_NFC * 8 * PB; t += DD_THREADS) As[t] = 0.0;
+    // runs of consecutive flavours in the (usually sorted) active list: their nx-runs of f are contiguous both in f and
+    // in the B tile, so a run is ONE copy (config 1: 5 runs for 9 flavours)
+    __shared__ short run_c0[MAX_NFL], run_len[MAX_NFL];
+    __shared__ int nruns_s;
     if (tid == 0) {
+        int nr = 0;
+        for (int c = 0; c < d.C;) {
+            int e = c + 1;
+            while (e < d.C && (int)p.chan.a[e] == (int)p.chan.a[e - 1] + 1) ++e;
+            run_c0[nr] = (short)c;
+            run_len[nr] = (short)(e - c);
+            ++nr;
+            c = e;
+        }
+        nruns_s = nr;
         for (int s = 0; s < NS; ++s) {
             mbar_init(bar_full(s), DD_PRODUCERS);   // one arrive.expect_tx per producer warp
             mbar_init(bar_empty(s), DD_CONSUMERS);
@@ -77,6 +95,7 @@ fk_dis_direct_kernel(const __grid_constant__ DisDirectParams p) {
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the zeros before any bulk copy lands
     __syncthreads();
+    const int rows_valid = min(DD_TM, d.N - m0);
 
     if (warp >= DD_CONSUMERS) {
         // ================================ producer warps ================================
@@ -84,7 +103,6 @@ fk_dis_direct_kernel(const __grid_constant__ DisDirectParams p) {
         const int pw = warp - DD_CONSUMERS;
         constexpr int RPW = DD_TM / DD_PRODUCERS;
         const double* __restrict__ fk = reinterpret_cast<const double*>(d.fk);
-        const int rows_valid = min(DD_TM, d.N - m0);
         const int my_rows = max(0, min(RPW, rows_valid - RPW * pw));
         auto issue_a = [&](int it) {
             const int stage = it % NS, k0 = it * DD_KT;
@@ -97,24 +115,24 @@ fk_dis_direct_kernel(const __grid_constant__ DisDirectParams p) {
                 bulk_g2s(As_s + (uint32_t)((stage * DD_TM * DD_SA + row * DD_SA) * 8), fk + (long long)(m0 + row) * d.row_stride + k0,
                          (uint32_t)(lenc * 8), bar_full(stage));
         };
-        // the table does not depend on the call before this one: its first stages go out before the wait
-        const int pre = min(nst, NS);
-        for (int it = 0; it < pre; ++it) issue_a(it);
+        // the table does not depend on the call before this one: its first stage goes out before the wait
+        issue_a(0);
         pdl_wait();   // f may have been written by the kernel before this one in the stream
-        // B tile: for every replica column of this CTA, the nx-run of every active flavour
-        const int slots = d.nfl * nx, C = d.C, npieces = ncols * C;
-        const int mine = npieces > pw * 32 + lane ? (npieces - pw * 32 - lane + 32 * DD_PRODUCERS - 1) / (32 * DD_PRODUCERS) : 0;
-        int warp_pieces = mine;
+        // B tile: for every replica column of this CTA, the f-run of every run of active flavours
+        const int slots = d.nfl * nx, nruns = nruns_s, npieces = ncols * nruns;
+        int my_bytes = 0;
+        for (int q = pw * 32 + lane; q < npieces; q += 32 * DD_PRODUCERS) my_bytes += (int)run_len[q % nruns] * nx * 8;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) warp_pieces += __shfl_xor_sync(0xffffffffu, warp_pieces, o);
-        if (lane == 0) mbar_expect_tx(bar_b, (uint32_t)(warp_pieces * nx * 8));
+        for (int o = 16; o > 0; o >>= 1) my_bytes += __shfl_xor_sync(0xffffffffu, my_bytes, o);
+        if (lane == 0) mbar_expect_tx(bar_b, (uint32_t)my_bytes);
         __syncwarp();
         for (int q = pw * 32 + lane; q < npieces; q += 32 * DD_PRODUCERS) {
-            const int col = q / C, c = q - col * C;
+            const int col = q / nruns, run = q - col * nruns, c = run_c0[run];
             const int r = min(rbase + col, p.R - 1);   // columns past R repeat the last replica (never stored)
-            bulk_g2s(Bs_s + (uint32_t)((col * PB + c * nx) * 8), p.f + (long long)r * slots + (int)p.chan.a[c] * nx, (uint32_t)(nx * 8), bar_b);
+            bulk_g2s(Bs_s + (uint32_t)((col * PB + c * nx) * 8), p.f + (long long)r * slots + (int)p.chan.a[c] * nx,
+                     (uint32_t)((int)run_len[run] * nx * 8), bar_b);
         }
-        for (int it = pre; it < nst; ++it) issue_a(it);
+        for (int it = 1; it < nst; ++it) issue_a(it);
         return;
     }
 
@@ -125,28 +143,32 @@ fk_dis_direct_kernel(const __grid_constant__ DisDirectParams p) {
 #pragma unroll
         for (int j = 0; j < DD_NFC; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     mbar_wait(bar_b, 0);
+    // Whole groups of 4 MMA k-steps with all 24 fragment loads ahead of the 32 DMMAs and no branch in between (one warp
+    // per scheduler: every exposed shared-memory latency is idle tensor time).  All DD_NFC fragments are computed whatever
+    // nf is: the rows of Bs past this CTA's columns are zero, and the slowest CTA (nf = DD_NFC) sets the time of the call.
     const double* Bt = Bs + (lane >> 2) * PB + (lane & 3);
     for (int it = 0; it < nst; ++it) {
         const int stage = it % NS, k0 = it * DD_KT;
-        const int nsteps = (min(DD_KT, K - k0) + 3) >> 2;
+        const int ngroups = (min(DD_KT, K - k0) + DD_KG - 1) / DD_KG;
         mbar_wait(bar_full(stage), (it / NS) & 1);
         const double* At = As + stage * DD_TM * DD_SA + (warp * 16 + (lane >> 2)) * DD_SA + (lane & 3);
         const double* Btk = Bt + k0;
+        for (int g = 0; g < ngroups; ++g) {
+            double a[4][2], b[4][DD_NFC];
 #pragma unroll
-        for (int s = 0; s < DD_KT / 4; ++s) {
-            if (s < nsteps) {
-                double a[2], b[DD_NFC];
-                a[0] = At[s * 4];
-                a[1] = At[8 * DD_SA + s * 4];
+            for (int s = 0; s < 4; ++s) {
+                a[s][0] = At[g * DD_KG + s * 4];
+                a[s][1] = At[8 * DD_SA + g * DD_KG + s * 4];
 #pragma unroll
-                for (int j = 0; j < DD_NFC; ++j) b[j] = j < nf ? Btk[j * 8 * PB + s * 4] : 0.0;
-#pragma unroll
-                for (int j = 0; j < DD_NFC; ++j)
-                    if (j < nf) {
-                        dmma884(acc[0][j][0], acc[0][j][1], a[0], b[j]);
-                        dmma884(acc[1][j][0], acc[1][j][1], a[1], b[j]);
-                    }
+                for (int j = 0; j < DD_NFC; ++j) b[s][j] = Btk[j * 8 * PB + g * DD_KG + s * 4];
             }
+#pragma unroll
+            for (int s = 0; s < 4; ++s)
+#pragma unroll
+                for (int j = 0; j < DD_NFC; ++j) {
+                    dmma884(acc[0][j][0], acc[0][j][1], a[s][0], b[s][j]);
+                    dmma884(acc[1][j][0], acc[1][j][1], a[s][1], b[s][j]);
+                }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty(stage));

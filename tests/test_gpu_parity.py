@@ -322,17 +322,21 @@ def test_dis_direct_small_tables(K, shape):
     ref, scale = O.dis(fk, flav, f)
     t = K.FkTable(K.FK_KIND_DIS, to_dev(fk), flav, synth.NFL, K.FK_F64, K.FK_STORE_PACK, R_hint=R)
     f_d = to_dev(f)
-    s1 = t.conv(f_d).cpu().numpy()
-    assert t.last_launches() == 1
-    assert rel_err(s1, ref, scale) <= TOL64
-    assert np.array_equal(s1, t.conv(f_d).cpu().numpy())   # repeatable bit for bit
-    K.set_option(K.FK_OPT_DIS_DIRECT, 0)
+    default = K.get_option(K.FK_OPT_DIS_DIRECT)   # smallest R that takes the path (80: where it starts to win)
     try:
+        K.set_option(K.FK_OPT_DIS_DIRECT, 13)
+        s1 = t.conv(f_d).cpu().numpy()
+        assert t.last_launches() == 1
+        assert np.array_equal(s1, t.conv(f_d).cpu().numpy())   # repeatable bit for bit
+        K.set_option(K.FK_OPT_DIS_DIRECT, 0)
         s0 = t.conv(f_d).cpu().numpy()
         assert t.last_launches() > 1
     finally:
-        K.set_option(K.FK_OPT_DIS_DIRECT, 1)
+        K.set_option(K.FK_OPT_DIS_DIRECT, default)
+    assert rel_err(s1, ref, scale) <= TOL64
     assert rel_err(s0, ref, scale) <= TOL64
+    t.conv(f_d)
+    assert (t.last_launches() == 1) == (R >= default)
     t.destroy()
 
 
