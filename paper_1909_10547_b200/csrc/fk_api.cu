@@ -12,6 +12,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <queue>
 #include <mutex>
 #include <new>
 #include <string>
@@ -433,8 +434,20 @@ int run_conv_dis_direct(const fk::TableDesc& d, const fk::ChannelList& ch, const
 bool wsv_ok(const fk::TableDesc& d) { return d.vec_ok && (d.store32 || d.K % 2 == 0) && opt(FK_OPT_WARP_SPEC); }
 
 template <bool GROUPED, typename TS = double>
-bool wsv_launch(const fk::WsVjpParams& w, cudaStream_t s) {
-    const int grid = std::max(1, std::min(w.ntiles, sm_count()));
+bool wsv_launch(const fk::WsVjpParams& w0, cudaStream_t s) {
+    fk::WsVjpParams w = w0;
+    const int sms = std::max(1, sm_count());
+    if (!GROUPED) {
+        // the tiles left over after the last full round of the persistent grid become 2 or 4 column parts each when that
+        // still fits one round: the last round then lasts a half or a quarter of a tile (config 3: 30 of 1954 tiles -> 120 parts)
+        const int tiles = w.ntiles, nfrag = w.RP / 8;
+        w.nwhole = tiles / sms * sms;
+        const int left = tiles - w.nwhole;
+        w.nparts = (left > 0 && nfrag % 8 == 0 && 4 * left <= sms) ? 4 : (left > 0 && nfrag % 4 == 0 && 2 * left <= sms) ? 2 : 1;
+        if (w.nparts == 1) w.nwhole = tiles;
+        w.ntiles = w.nwhole + (tiles - w.nwhole) * w.nparts;
+    }
+    const int grid = std::max(1, std::min(w.ntiles, sms));
     switch (w.RP / 8) {
 #define FK_WSV_CASE(NFW) case NFW: if (!ensure_dyn_smem(fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED, TS>, fk::WSV_SMEM_BYTES)) return false; \
                                    FK_TIMED("fk_gemm_vjp_ws", s) fk::fk_gemm_vjp_ws_kernel<NFW, GROUPED, TS><<<grid, fk::WS_THREADS, fk::WSV_SMEM_BYTES, s>>>(w); break

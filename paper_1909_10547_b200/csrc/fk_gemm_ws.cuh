@@ -358,7 +358,10 @@ struct WsVjpParams {
     TableDesc desc;     // single-table launch
     const double* gP;   // [N][RP]: g of this pass, replica innermost, zero padded (grouped: + out_off * RP)
     double* G;          // [K][RP] column sums (grouped: + k_off * RP)
-    int RP, ntiles;     // ntiles: 128-k tiles (single) or items (grouped) of the launch
+    int RP, ntiles;     // ntiles: work items of the launch: 128-k tiles (single-table: + the column parts of the tail tiles) or grouped items
+    int nwhole, nparts; // single-table launch: items [0, nwhole) are whole tiles; item nwhole + s is column part s % nparts of tile
+                        // nwhole + s / nparts.  The tiles left over after the last full round of the persistent grid are cut
+                        // into 2 or 4 column parts (disjoint outputs, nothing to add up): the last round lasts 1/2 or 1/4 tile.
     const TableDesc* descs;  // grouped launch
     const ColSeg* items;     // grouped launch {table, kblock = 128-k tile}
 };
@@ -392,7 +395,8 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
     __syncthreads();
     const int RP = p.RP;
 
-    auto tile_of = [&](int t, const TableDesc*& d, const double*& gP, double*& G, int& kt) {
+    auto tile_of = [&](int t, const TableDesc*& d, const double*& gP, double*& G, int& kt, int& part) {
+        part = -1;   // whole tile
         if constexpr (GROUPED) {
             const ColSeg it = p.items[t];
             d = &p.descs[it.table];
@@ -404,6 +408,11 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
             gP = p.gP;
             G = p.G;
             kt = t;
+            if (t >= p.nwhole) {
+                const int sidx = t - p.nwhole;
+                kt = p.nwhole + sidx / p.nparts;
+                part = sidx % p.nparts;
+            }
         }
     };
 
@@ -415,8 +424,8 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
             const TableDesc* d;
             const double* gP;
             double* G;
-            int kt;
-            tile_of(t, d, gP, G, kt);
+            int kt, part;
+            tile_of(t, d, gP, G, kt, part);
             const int k0 = kt * GEMMV_BK, klen = min(GEMMV_BK, d->K - k0);
             const int klenc = (klen + VEL - 1) / VEL * VEL;   // whole 16-byte pieces: the pad elements of a packed row are 0
             const TS* __restrict__ fk = reinterpret_cast<const TS*>(d->fk) + k0;
@@ -437,17 +446,11 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
 
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;" ::: "memory");
     constexpr int NFW0 = (NFRAG + 1) / 2, NFW1 = NFRAG / 2;
-    auto consume = [&](auto nf_tag) {
-    constexpr int NFW = decltype(nf_tag)::value;  // fragments of this warp's column
     const int wm = warp & 3, wn = warp >> 2;
-    const int cbcol = wn * NFW0 * 8;
     int it = 0;
-    for (int t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
-        const TableDesc* d;
-        const double* gP;
-        double* G;
-        int kt;
-        tile_of(t, d, gP, G, kt);
+    // one tile (or one column part of a tile): this warp's 32 k x (8 * NFW) replica columns from column cbcol on
+    auto run_tile = [&](auto nf_tag, const int cbcol, const TableDesc* d, double* G, const int kt) {
+        constexpr int NFW = decltype(nf_tag)::value;  // fragments of this warp
         double acc[4][NFW][2];
 #pragma unroll
         for (int i = 0; i < 4; ++i)
@@ -514,11 +517,31 @@ fk_gemm_vjp_ws_kernel(const __grid_constant__ WsVjpParams p) {
             }
         }
         flushG(!flushed);
-    }
     };
-    if (warp < 4) consume(std::integral_constant<int, NFW0>{});
-    else consume(std::integral_constant<int, NFW1>{});
+    for (int t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
+        const TableDesc* d;
+        const double* gP;
+        double* G;
+        int kt, part;
+        tile_of(t, d, gP, G, kt, part);
+        if (part < 0) {
+            if (wn == 0) run_tile(std::integral_constant<int, NFW0>{}, 0, d, G, kt);
+            else run_tile(std::integral_constant<int, NFW1>{}, NFW0 * 8, d, G, kt);
+        } else if constexpr (!GROUPED && NFRAG % 4 == 0) {
+            // column part of a tail tile: NFRAG / nparts fragments, half of them per warp column
+            if constexpr (NFRAG % 8 == 0) {
+                if (p.nparts == 4) {
+                    constexpr int Q = NFRAG / 8;
+                    run_tile(std::integral_constant<int, Q>{}, (part * 2 + wn) * Q * 8, d, G, kt);
+                    continue;
+                }
+            }
+            constexpr int H = NFRAG / 4;
+            run_tile(std::integral_constant<int, H>{}, (part * 2 + wn) * H * 8, d, G, kt);
+        }
+    }
 }
+
 
 }  // namespace fk
 
