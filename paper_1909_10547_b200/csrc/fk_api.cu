@@ -12,7 +12,6 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
-#include <queue>
 #include <mutex>
 #include <new>
 #include <string>
